@@ -1,0 +1,188 @@
+/*
+ * pakr.h -- C ABI of the B200-native (sm_100a) PAKR hot path.
+ *
+ * One thing lives behind this header: the batched tree-expansion iteration of PAKR
+ * (Alg. 1 lines 5-17; implementation notes PAPER.md:136-144) run in a
+ * device-resident loop inside AO-x cost-bounded replanning (Alg. 1 lines 1-4, 18).
+ * Every step (sampling, nearest neighbour, propagation, validity, prune, insert, goal, path
+ * extraction, the replan loop) runs in CUDA kernels; there is no CPU fallback.
+ *
+ * Conventions
+ *   - "HOST" / "DEVICE" says where a pointer must point.  The library never frees or keeps a
+ *     caller pointer beyond the call, except the planner object it returns.
+ *   - All bulk device memory is the caller's workspace (DEVICE, 256-byte aligned, at least
+ *     pakr_workspace_bytes()).  The library owns only the small planner object.
+ *   - Calls on one planner must not overlap (one stream at a time).  pakr_plan and
+ *     pakr_expand_step enqueue on `cuda_stream` (a cudaStream_t passed as void*); pakr_plan
+ *     synchronises that stream before filling HOST outputs, pakr_expand_step does not.
+ *   - No call throws; every failure is a pakr_status and pakr_last_error() text.
+ *   - Notation follows BASELINE.json: B sampled states per iteration, K controls per sampled
+ *     state, B*K children per iteration (the paper's "batch B", "B/A samples", "A controls",
+ *     PAPER.md:95-106,:142).
+ *
+ * Device tree layout ("four contiguous buffers" + a scalar count), fp32, node-major:
+ *   states [cap][Dp]  Dp = state_dim rounded up to a multiple of 4 (pad lanes are 0)
+ *   actions[cap][4]   control that produced node i from parents[i] (pad lanes 0); node 0: zeros
+ *   parents[cap]      int32, parents[0] = -1, parents[i] < i
+ *   costs  [cap]      cost-to-come
+ */
+#ifndef PAKR_H
+#define PAKR_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pakr_planner pakr_planner; /* opaque, owned by the library */
+
+typedef enum {
+  PAKR_OK = 0,
+  PAKR_ERR_INVALID_ARG = 1,
+  PAKR_ERR_UNSUPPORTED = 2,
+  PAKR_ERR_WORKSPACE_TOO_SMALL = 3,
+  PAKR_ERR_BUFFER_TOO_SMALL = 4,
+  PAKR_ERR_CUDA = 5
+} pakr_status;
+
+enum { PAKR_DYN_DOUBLE_INTEGRATOR = 0, PAKR_DYN_UNICYCLE2 = 1, PAKR_DYN_QUADROTOR = 2 };
+enum { PAKR_INT_EULER = 0, PAKR_INT_RK4 = 1 };
+enum { PAKR_OBS_CIRCLE2D = 0, PAKR_OBS_AABB = 1, PAKR_OBS_ZCYLINDER = 2 };
+enum { PAKR_COST_DURATION = 0, PAKR_COST_PATH_LENGTH = 1 };
+enum { PAKR_DIM_REAL = 0, PAKR_DIM_ANGLE = 1 };
+enum { PAKR_NO_SOLUTION = 0, PAKR_SOLVED = 1 }; /* "no solution" is not an error */
+
+/* child flag bits written by pakr_expand_step (Alg. 1 l.10-14) */
+enum {
+  PAKR_F_VALID = 1,     /* in bounds and collision free at every step-end state */
+  PAKR_F_INBOUNDS = 2,  /* every step-end state inside the state box                           */
+  PAKR_F_COLLFREE = 4,  /* every step-end position outside every obstacle                      */
+  PAKR_F_NOTPRUNED = 8, /* c_new + h(x_new) < c_best (Alg. 1 l.11)                             */
+  PAKR_F_GOAL = 16,     /* kept and x_new in X_goal (Alg. 1 l.14)                              */
+  PAKR_F_INSERTED = 32  /* appended to the tree (Alg. 1 l.13)                                  */
+};
+
+/* Problem statement (dynamics f, x_init, X_goal, U, cost J) plus the propagation
+ * settings of PAPER.md:144 (fixed dt, T steps per edge).  All arrays HOST, copied at create. */
+typedef struct {
+  int32_t dynamics_id; /* PAKR_DYN_*: double integrator [p, pdot], second-order
+                          unicycle [x,y,theta,v,omega], quadrotor [p, v, (phi,theta,
+                          psi) ZYX, (p,q,r)] with control (T, tau) (BASELINE.json config 4) */
+  int32_t integrator;  /* PAKR_INT_*: forward Euler or classical RK4 */
+  int32_t state_dim, control_dim, pos_dim; /* must match dynamics_id: DI (2*pos_dim, pos_dim,
+                          2|3), unicycle (5,2,2), quadrotor (12,4,3) */
+  const float* dyn_params; int32_t n_dyn_params; /* quadrotor: m, Ixx, Iyy, Izz, g; else 0 */
+  const float* state_lo; const float* state_hi;  /* [D]; +-INF = unbounded; box-tested every step */
+  const uint8_t* dim_kind; /* [D] PAKR_DIM_*; angle dims (unicycle theta, quadrotor psi) are wrapped
+                          to [-pi,pi) and never bounds-tested; must match the dynamics */
+  const float* nn_weight;  /* [D] >= 0, d^2 = sum_d w_d delta_d^2; 0 drops a dim */
+  const float* control_lo; const float* control_hi; /* [m] */
+  int32_t obstacle_type;   /* PAKR_OBS_*: circle/cylinder rows (cx, cy, r); box rows (lo[pos_dim],
+                          hi[pos_dim]).  Closed sets, point robot. */
+  const float* obstacles; int32_t n_obstacles;   /* n_obstacles <= 1024 */
+  const float* start;       /* [D] x_init */
+  const float* goal_center; /* [pos_dim] */
+  float goal_radius;        /* X_goal = closed position ball ... */
+  int32_t goal_angle_dim; float goal_angle, goal_angle_tol; /* ... and |wrap(x[dim]-angle)| <= tol; -1 = none */
+  float dt; int32_t steps_per_edge; /* every edge is exactly steps_per_edge steps of dt */
+  int32_t cost_mode;      /* PAKR_COST_DURATION (J = T) or PAKR_COST_PATH_LENGTH */
+  float heuristic_speed;  /* h(x) = max(0, |p - goal| - r) / heuristic_speed; +INF => h = 0 */
+} pakr_problem;
+
+/* Validates and copies the problem; selects the compiled kernel variant; binds `cuda_device`.
+ * INVALID_ARG: NULL, dims that do not match the dynamics, lo > hi, NaN, weight < 0, a sampled
+ * real dim (weight > 0) with an infinite bound, dt <= 0, steps < 1.  UNSUPPORTED: unknown ids,
+ * dim_kind not the dynamics' own.  CUDA: device not usable (no sm_100 device). */
+pakr_status pakr_create(const pakr_problem* problem, int cuda_device, pakr_planner** out);
+void pakr_destroy(pakr_planner* planner);
+/* Text of the last failure on this planner ("" if none); valid until the next call on it.
+ * pakr_last_error(NULL) returns the text of the last failed pakr_create in this thread. */
+const char* pakr_last_error(const pakr_planner* planner);
+
+/* Bytes of DEVICE workspace pakr_plan / pakr_expand_step need for (B, K, tree_capacity);
+ * 0 if an argument is invalid (B < 1, K < 1, K > 4096, B*K > 2^24, capacity < 2 or > 2^30). */
+size_t pakr_workspace_bytes(const pakr_planner* planner, int32_t B, int32_t K, int64_t tree_capacity);
+
+/* Where pakr_plan keeps its tree inside the workspace (byte offsets), so a caller can read the
+ * tree of the last replan after pakr_plan returns (tests check the tree invariants on it). */
+typedef struct {
+  size_t states_off, actions_off, parents_off, costs_off; /* layouts as in the header comment */
+  int32_t state_stride, action_stride;                    /* Dp, 4 */
+} pakr_tree_layout;
+pakr_status pakr_get_tree_layout(const pakr_planner* planner, int32_t B, int32_t K,
+                                 int64_t tree_capacity, pakr_tree_layout* out);
+
+typedef struct {
+  uint64_t seed;          /* Philox key; draws are keyed by (seed, replan, iteration, sample, branch) */
+  int32_t B, K;
+  int64_t tree_capacity;  /* nodes */
+  int32_t n_replans;      /* AO-x restarts (Alg. 1 l.3); 1 = plain parallel RRT; <= 4096 */
+  double time_budget_ms;  /* > 0: stop at the first iteration boundary past the budget (device
+                             %globaltimer; non-deterministic); <= 0: none (deterministic) */
+  int64_t max_iters_per_replan; /* 0 = default max(32, capacity / (B*K)) */
+} pakr_plan_opts;
+
+#define PAKR_MAX_REPLAN_STATS 64
+typedef struct {
+  int64_t iterations;      /* inner-loop trips over all replans */
+  int64_t children;        /* = iterations * B * K propagated and checked ("expanded nodes") */
+  int64_t inserted;        /* nodes appended over all replans */
+  int32_t replans_run, replans_solved;
+  int32_t termination;     /* 0 all replans run, 1 time budget */
+  double first_solution_ms;/* device time from kernel start to the end of the first solved replan; -1 if none */
+  double device_ms;        /* device time of the whole loop (%globaltimer) */
+  /* first PAKR_MAX_REPLAN_STATS replans: */
+  float replan_cost[PAKR_MAX_REPLAN_STATS];   /* c_best after the replan (+INF before any solution) */
+  int32_t replan_nodes[PAKR_MAX_REPLAN_STATS];/* tree size at its end */
+  int32_t replan_iters[PAKR_MAX_REPLAN_STATS];
+  double replan_end_ms[PAKR_MAX_REPLAN_STATS];/* device time at its end */
+} pakr_stats;
+
+typedef struct {
+  /* caller-allocated HOST buffers; any may be NULL if not wanted */
+  int32_t* path_nodes;    /* [path_capacity] node ids root -> goal (ids in the solving replan's tree) */
+  float* path_states;     /* [path_capacity][state_dim] */
+  float* path_controls;   /* [path_capacity-1][control_dim]; control i is held for steps_per_edge*dt */
+  int32_t path_capacity;  /* in  */
+  int32_t path_len;       /* out: nodes on the best path (L+1), 0 if none */
+  double cost;            /* out: c_best, +INF if none */
+  int32_t outcome;        /* out: PAKR_SOLVED / PAKR_NO_SOLUTION */
+  int32_t final_tree_nodes; /* out: size of the tree left in the workspace (the last replan's) */
+  pakr_stats stats;       /* out */
+} pakr_result;
+
+/* Alg. 1 whole: AO-x loop around the batched expansion, one persistent cooperative kernel, no
+ * host round trip per iteration.  Returns the best path found (sigma*, Alg. 1 l.18).
+ * BUFFER_TOO_SMALL: path longer than path_capacity (path_len = needed length, cost/outcome
+ * still set).  WORKSPACE_TOO_SMALL / INVALID_ARG: nothing launched. */
+pakr_status pakr_plan(pakr_planner* planner, const pakr_plan_opts* opts, void* d_workspace,
+                      size_t workspace_bytes, void* cuda_stream, pakr_result* out);
+
+/* One trip of Alg. 1 l.6-17 on caller-visible DEVICE buffers (test hook; same kernels). */
+typedef struct {
+  uint64_t seed; uint32_t replan, iteration;
+  int32_t B, K; int64_t tree_capacity;
+  float c_best;                 /* +INF = no bound yet */
+  /* tree, DEVICE, layouts as in the header comment; in/out */
+  float* states; float* actions; int32_t* parents; float* costs;
+  int32_t* n_nodes;             /* DEVICE scalar, in/out */
+  /* optional DEVICE debug outputs, each may be NULL */
+  float* x_rand;                /* [B][Dp] */
+  int32_t* nn_idx;              /* [B] */
+  float* nn_d2;                 /* [B] */
+  float* child_state;           /* [B*K][Dp]; angle dims wrapped */
+  float* child_ctrl;            /* [B*K][4] */
+  float* child_cost;            /* [B*K] */
+  int32_t* child_flags;         /* [B*K] PAKR_F_* */
+  int32_t* n_inserted;          /* scalar */
+  int32_t* goal_node;           /* scalar, -1 if no goal child was inserted */
+  float* new_c_best;            /* scalar */
+} pakr_step_args;
+
+pakr_status pakr_expand_step(pakr_planner* planner, const pakr_step_args* args, void* d_workspace,
+                             size_t workspace_bytes, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PAKR_H */

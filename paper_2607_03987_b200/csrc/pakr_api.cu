@@ -1,0 +1,404 @@
+// pakr_api.cu -- host side of the C ABI declared in include/pakr.h.
+// Validates the problem, carves the caller's workspace, launches the persistent cooperative
+// kernel of pakr_kernel.cuh and copies the small result block back.  No compute happens here.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/pakr.h"
+#include "pakr_kernel.cuh"
+
+using namespace pakr;
+
+struct pakr_planner {
+  int device = 0;
+  int dyn = 0, obs = 0;     // DynKind, ObsKind
+  int D = 0, M = 0, PD = 0, DP = 0;
+  DevProblem pb{};
+  float* d_obstacles = nullptr;
+  int num_sms = 0, blocks_per_sm = 0;
+  size_t smem_bytes = 0;
+  const void* kernel = nullptr;
+  void* h_pinned = nullptr;  // Ctrl + path staging
+  std::string err;
+};
+
+static thread_local std::string g_create_err;
+
+namespace {
+
+constexpr size_t kAlign = 256;
+size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+struct Layout {
+  size_t states, actions, parents, costs, nn_key, unit_count, scr_state, scr_ctrl, scr_cost, scr_parent,
+      scr_flags, ctrl, path_rev, path_nodes, path_states, path_controls, total;
+};
+
+Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap) {
+  Layout L{};
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+  const size_t BK = (size_t)B * K, U = (BK + 31) / 32, slots = U * 32;
+  L.states = take((size_t)cap * pl->DP * 4);
+  L.actions = take((size_t)cap * 16);
+  L.parents = take((size_t)cap * 4);
+  L.costs = take((size_t)cap * 4);
+  L.nn_key = take((size_t)B * 8);
+  L.unit_count = take(U * 4);
+  L.scr_state = take(slots * pl->DP * 4);
+  L.scr_ctrl = take(slots * 16);
+  L.scr_cost = take(slots * 4);
+  L.scr_parent = take(slots * 4);
+  L.scr_flags = take(slots * 4);
+  L.ctrl = take(sizeof(Ctrl));
+  L.path_rev = take((size_t)kPathMax * 4);
+  L.path_nodes = take((size_t)kPathMax * 4);
+  L.path_states = take((size_t)kPathMax * kMaxD * 4);
+  L.path_controls = take((size_t)kPathMax * kMaxM * 4);
+  L.total = o;
+  return L;
+}
+
+bool sizes_ok(int64_t B, int64_t K, int64_t cap) {
+  return B >= 1 && K >= 1 && K <= 4096 && B * K <= (1ll << 24) && cap >= 2 && cap <= (1ll << 30);
+}
+
+template <int DYN, int OBS> const void* kernel_ptr() { return (const void*)&pakr_loop_kernel<DYN, OBS>; }
+
+const void* select_kernel(int dyn, int obs) {
+  switch (dyn * 2 + obs) {
+    case DYN_DI2 * 2 + OBS_CIRCLE: return kernel_ptr<DYN_DI2, OBS_CIRCLE>();
+    case DYN_DI2 * 2 + OBS_BOX: return kernel_ptr<DYN_DI2, OBS_BOX>();
+    case DYN_DI3 * 2 + OBS_CIRCLE: return kernel_ptr<DYN_DI3, OBS_CIRCLE>();
+    case DYN_DI3 * 2 + OBS_BOX: return kernel_ptr<DYN_DI3, OBS_BOX>();
+    case DYN_UNI2 * 2 + OBS_CIRCLE: return kernel_ptr<DYN_UNI2, OBS_CIRCLE>();
+    case DYN_UNI2 * 2 + OBS_BOX: return kernel_ptr<DYN_UNI2, OBS_BOX>();
+    case DYN_QUAD * 2 + OBS_CIRCLE: return kernel_ptr<DYN_QUAD, OBS_CIRCLE>();
+    case DYN_QUAD * 2 + OBS_BOX: return kernel_ptr<DYN_QUAD, OBS_BOX>();
+  }
+  return nullptr;
+}
+
+size_t tile_floats(int DP) { return (size_t)(DP == 4 ? 256 : DP == 8 ? 128 : 64) * DP; }
+
+size_t smem_for(const pakr_planner* pl) {
+  const int os = pl->obs == OBS_CIRCLE ? 4 : 8;
+  return kWarps * 2 * tile_floats(pl->DP) * 4 + kWarps * 2 * 8 + (kThreads + kWarps + 8) * 4 +
+         (size_t)pl->pb.n_obs * os * 4 + 16;
+}
+
+pakr_status fail(pakr_planner* pl, pakr_status st, const std::string& msg) {
+  if (pl) pl->err = msg;
+  else g_create_err = msg;
+  return st;
+}
+
+#define CUDA_TRY(pl, expr)                                                                       \
+  do {                                                                                           \
+    cudaError_t e_ = (expr);                                                                     \
+    if (e_ != cudaSuccess)                                                                       \
+      return fail(pl, PAKR_ERR_CUDA, std::string(#expr) + ": " + cudaGetErrorString(e_));        \
+  } while (0)
+
+}  // namespace
+
+extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_planner** out) {
+  if (out) *out = nullptr;
+  if (!p || !out) return fail(nullptr, PAKR_ERR_INVALID_ARG, "null problem or out pointer");
+  if (!p->state_lo || !p->state_hi || !p->dim_kind || !p->nn_weight || !p->control_lo || !p->control_hi ||
+      !p->start || !p->goal_center)
+    return fail(nullptr, PAKR_ERR_INVALID_ARG, "null array in problem");
+  int dyn = -1;
+  if (p->dynamics_id == PAKR_DYN_DOUBLE_INTEGRATOR) {
+    if (p->pos_dim == 2 && p->state_dim == 4 && p->control_dim == 2) dyn = DYN_DI2;
+    else if (p->pos_dim == 3 && p->state_dim == 6 && p->control_dim == 3) dyn = DYN_DI3;
+    else return fail(nullptr, PAKR_ERR_INVALID_ARG, "double integrator needs (D,m,pos)=(4,2,2) or (6,3,3)");
+  } else if (p->dynamics_id == PAKR_DYN_UNICYCLE2) {
+    if (p->pos_dim != 2 || p->state_dim != 5 || p->control_dim != 2)
+      return fail(nullptr, PAKR_ERR_INVALID_ARG, "unicycle2 needs (D,m,pos)=(5,2,2)");
+    dyn = DYN_UNI2;
+  } else if (p->dynamics_id == PAKR_DYN_QUADROTOR) {
+    if (p->pos_dim != 3 || p->state_dim != 12 || p->control_dim != 4)
+      return fail(nullptr, PAKR_ERR_INVALID_ARG, "quadrotor needs (D,m,pos)=(12,4,3)");
+    if (p->n_dyn_params < 5 || !p->dyn_params)
+      return fail(nullptr, PAKR_ERR_INVALID_ARG, "quadrotor needs dyn_params m,Ixx,Iyy,Izz,g");
+    for (int i = 0; i < 4; ++i)
+      if (!(p->dyn_params[i] > 0.0f)) return fail(nullptr, PAKR_ERR_INVALID_ARG, "mass/inertia must be > 0");
+    dyn = DYN_QUAD;
+  } else {
+    return fail(nullptr, PAKR_ERR_UNSUPPORTED, "unknown dynamics_id");
+  }
+  if (p->integrator != PAKR_INT_EULER && p->integrator != PAKR_INT_RK4)
+    return fail(nullptr, PAKR_ERR_UNSUPPORTED, "unknown integrator");
+  if (p->cost_mode != PAKR_COST_DURATION && p->cost_mode != PAKR_COST_PATH_LENGTH)
+    return fail(nullptr, PAKR_ERR_UNSUPPORTED, "unknown cost_mode");
+  int obs = -1;
+  if (p->obstacle_type == PAKR_OBS_CIRCLE2D || p->obstacle_type == PAKR_OBS_ZCYLINDER) obs = OBS_CIRCLE;
+  else if (p->obstacle_type == PAKR_OBS_AABB) obs = OBS_BOX;
+  else return fail(nullptr, PAKR_ERR_UNSUPPORTED, "unknown obstacle_type");
+  if (p->n_obstacles < 0 || p->n_obstacles > 1024 || (p->n_obstacles > 0 && !p->obstacles))
+    return fail(nullptr, PAKR_ERR_INVALID_ARG, "n_obstacles must be in [0,1024] with a non-null array");
+  const int D = p->state_dim, M = p->control_dim, PD = p->pos_dim;
+  const int angle = dyn == DYN_UNI2 ? 2 : dyn == DYN_QUAD ? 8 : -1;
+  for (int d = 0; d < D; ++d) {
+    const bool is_angle = p->dim_kind[d] == PAKR_DIM_ANGLE;
+    if (p->dim_kind[d] > 1 || is_angle != (d == angle))
+      return fail(nullptr, PAKR_ERR_UNSUPPORTED, "dim_kind must mark exactly the dynamics' own angle dim");
+    if (std::isnan(p->state_lo[d]) || std::isnan(p->state_hi[d]) || std::isnan(p->nn_weight[d]) ||
+        std::isnan(p->start[d]))
+      return fail(nullptr, PAKR_ERR_INVALID_ARG, "NaN in state bounds, weights or start");
+    if (p->state_lo[d] > p->state_hi[d]) return fail(nullptr, PAKR_ERR_INVALID_ARG, "state_lo > state_hi");
+    if (p->nn_weight[d] < 0.0f) return fail(nullptr, PAKR_ERR_INVALID_ARG, "nn_weight < 0");
+    if (!is_angle && p->nn_weight[d] > 0.0f && (std::isinf(p->state_lo[d]) || std::isinf(p->state_hi[d])))
+      return fail(nullptr, PAKR_ERR_INVALID_ARG, "a sampled dim (weight > 0) needs finite bounds");
+  }
+  for (int j = 0; j < M; ++j) {
+    if (!std::isfinite(p->control_lo[j]) || !std::isfinite(p->control_hi[j]) || p->control_lo[j] > p->control_hi[j])
+      return fail(nullptr, PAKR_ERR_INVALID_ARG, "control bounds must be finite with lo <= hi");
+  }
+  if (!(p->dt > 0.0f) || !std::isfinite(p->dt) || p->steps_per_edge < 1)
+    return fail(nullptr, PAKR_ERR_INVALID_ARG, "dt must be > 0 and steps_per_edge >= 1");
+  if (!(p->goal_radius >= 0.0f) || !(p->heuristic_speed > 0.0f))
+    return fail(nullptr, PAKR_ERR_INVALID_ARG, "goal_radius >= 0 and heuristic_speed > 0 required");
+  if (p->goal_angle_dim != -1 && p->goal_angle_dim != angle)
+    return fail(nullptr, PAKR_ERR_INVALID_ARG, "goal_angle_dim must be -1 or the dynamics' angle dim");
+
+  auto* pl = new pakr_planner();
+  pl->device = cuda_device;
+  pl->dyn = dyn; pl->obs = obs; pl->D = D; pl->M = M; pl->PD = PD;
+  pl->DP = (D + 3) / 4 * 4;
+  DevProblem& pb = pl->pb;
+  std::memset(&pb, 0, sizeof(pb));
+  bool unit = true;
+  for (int d = 0; d < kMaxD; ++d) { pb.lo[d] = -INFINITY; pb.hi[d] = INFINITY; }
+  for (int d = 0; d < D; ++d) {
+    pb.lo[d] = p->state_lo[d]; pb.hi[d] = p->state_hi[d]; pb.w[d] = p->nn_weight[d]; pb.start[d] = p->start[d];
+    if (pb.w[d] != 1.0f) unit = false;
+    if (d == angle) { pb.samp_lo[d] = -kPiF; pb.samp_span[d] = kPiF - (-kPiF); }
+    else if (std::isfinite(pb.lo[d]) && std::isfinite(pb.hi[d])) { pb.samp_lo[d] = pb.lo[d]; pb.samp_span[d] = pb.hi[d] - pb.lo[d]; }
+    else { pb.samp_lo[d] = 0.0f; pb.samp_span[d] = 0.0f; }
+  }
+  for (int j = 0; j < M; ++j) { pb.ulo[j] = p->control_lo[j]; pb.uhi[j] = p->control_hi[j]; pb.uspan[j] = pb.uhi[j] - pb.ulo[j]; }
+  for (int a = 0; a < PD; ++a) pb.goal[a] = p->goal_center[a];
+  pb.goal_r = p->goal_radius; pb.goal_angle = p->goal_angle; pb.goal_angle_tol = p->goal_angle_tol;
+  pb.goal_angle_dim = p->goal_angle_dim;
+  for (int i = 0; i < 8 && i < p->n_dyn_params; ++i) pb.dyn[i] = p->dyn_params[i];
+  pb.dt = p->dt; pb.S = p->steps_per_edge; pb.integrator = p->integrator; pb.cost_mode = p->cost_mode;
+  pb.inv_hspeed = std::isinf(p->heuristic_speed) ? 0.0f : 1.0f / p->heuristic_speed;
+  pb.unit_weights = unit ? 1 : 0;
+  pb.n_obs = p->n_obstacles;
+
+  // obstacle table in the kernel's shared-memory row format
+  const int os = obs == OBS_CIRCLE ? 4 : 8;
+  std::vector<float> rows((size_t)std::max(1, p->n_obstacles) * os, 0.0f);
+  for (int o = 0; o < p->n_obstacles; ++o) {
+    if (obs == OBS_CIRCLE) {
+      const float* c = p->obstacles + (size_t)o * 3;
+      rows[(size_t)o * 4 + 0] = c[0]; rows[(size_t)o * 4 + 1] = c[1]; rows[(size_t)o * 4 + 2] = c[2] * c[2];
+    } else {
+      const float* lo = p->obstacles + (size_t)o * 2 * PD;
+      const float* hi = lo + PD;
+      float* r = &rows[(size_t)o * 8];
+      r[0] = lo[0]; r[1] = lo[1]; r[2] = PD == 3 ? lo[2] : -INFINITY; r[3] = 0;
+      r[4] = hi[0]; r[5] = hi[1]; r[6] = PD == 3 ? hi[2] : INFINITY; r[7] = 0;
+    }
+  }
+  auto bail = [&](pakr_status st, const std::string& m) { g_create_err = m; pakr_destroy(pl); return st; };
+  cudaError_t e = cudaSetDevice(cuda_device);
+  if (e != cudaSuccess) return bail(PAKR_ERR_CUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(e));
+  cudaDeviceProp prop;
+  e = cudaGetDeviceProperties(&prop, cuda_device);
+  if (e != cudaSuccess) return bail(PAKR_ERR_CUDA, std::string("cudaGetDeviceProperties: ") + cudaGetErrorString(e));
+  if (prop.major != 10) return bail(PAKR_ERR_CUDA, "this library is built for sm_100a only");
+  if (!prop.cooperativeLaunch) return bail(PAKR_ERR_CUDA, "device lacks cooperative launch");
+  pl->num_sms = prop.multiProcessorCount;
+  e = cudaMalloc(&pl->d_obstacles, rows.size() * 4);
+  if (e != cudaSuccess) return bail(PAKR_ERR_CUDA, std::string("cudaMalloc: ") + cudaGetErrorString(e));
+  e = cudaMemcpy(pl->d_obstacles, rows.data(), rows.size() * 4, cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) return bail(PAKR_ERR_CUDA, std::string("cudaMemcpy: ") + cudaGetErrorString(e));
+  pb.obstacles = pl->d_obstacles;
+  pl->kernel = select_kernel(dyn, obs);
+  pl->smem_bytes = smem_for(pl);
+  e = cudaFuncSetAttribute(pl->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes);
+  if (e != cudaSuccess) return bail(PAKR_ERR_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&pl->blocks_per_sm, pl->kernel, kThreads, pl->smem_bytes);
+  if (e != cudaSuccess || pl->blocks_per_sm < 1)
+    return bail(PAKR_ERR_CUDA, "kernel does not fit on an SM (occupancy 0)");
+  e = cudaMallocHost(&pl->h_pinned, sizeof(Ctrl) + (size_t)kPathMax * (4 + kMaxD * 4 + kMaxM * 4));
+  if (e != cudaSuccess) return bail(PAKR_ERR_CUDA, std::string("cudaMallocHost: ") + cudaGetErrorString(e));
+  *out = pl;
+  return PAKR_OK;
+}
+
+extern "C" void pakr_destroy(pakr_planner* pl) {
+  if (!pl) return;
+  if (pl->d_obstacles) cudaFree(pl->d_obstacles);
+  if (pl->h_pinned) cudaFreeHost(pl->h_pinned);
+  delete pl;
+}
+
+extern "C" const char* pakr_last_error(const pakr_planner* pl) { return pl ? pl->err.c_str() : g_create_err.c_str(); }
+
+extern "C" size_t pakr_workspace_bytes(const pakr_planner* pl, int32_t B, int32_t K, int64_t cap) {
+  if (!pl || !sizes_ok(B, K, cap)) return 0;
+  return make_layout(pl, B, K, cap).total;
+}
+
+extern "C" pakr_status pakr_get_tree_layout(const pakr_planner* pl, int32_t B, int32_t K, int64_t cap,
+                                            pakr_tree_layout* out) {
+  if (!pl || !out || !sizes_ok(B, K, cap)) return PAKR_ERR_INVALID_ARG;
+  const Layout L = make_layout(pl, B, K, cap);
+  out->states_off = L.states; out->actions_off = L.actions; out->parents_off = L.parents; out->costs_off = L.costs;
+  out->state_stride = pl->DP; out->action_stride = 4;
+  return PAKR_OK;
+}
+
+namespace {
+
+void fill_common(const pakr_planner* pl, Params& P, const Layout& L, char* ws, int B, int K, int64_t cap) {
+  std::memset(&P, 0, sizeof(P));
+  P.pb = pl->pb;
+  P.nn_key = reinterpret_cast<unsigned long long*>(ws + L.nn_key);
+  P.unit_count = reinterpret_cast<unsigned*>(ws + L.unit_count);
+  P.scr_state = reinterpret_cast<float*>(ws + L.scr_state);
+  P.scr_ctrl = reinterpret_cast<float*>(ws + L.scr_ctrl);
+  P.scr_cost = reinterpret_cast<float*>(ws + L.scr_cost);
+  P.scr_parent = reinterpret_cast<int*>(ws + L.scr_parent);
+  P.scr_flags = reinterpret_cast<int*>(ws + L.scr_flags);
+  P.ctrl = reinterpret_cast<Ctrl*>(ws + L.ctrl);
+  P.path_nodes_rev = reinterpret_cast<int*>(ws + L.path_rev);
+  P.path_nodes = reinterpret_cast<int*>(ws + L.path_nodes);
+  P.path_states = reinterpret_cast<float*>(ws + L.path_states);
+  P.path_controls = reinterpret_cast<float*>(ws + L.path_controls);
+  P.B = B; P.K = K; P.cap = (int)cap;
+}
+
+// memset of the control words + one cooperative launch; everything on `stream`
+pakr_status launch(pakr_planner* pl, Params& P, cudaStream_t stream) {
+  CUDA_TRY(pl, cudaSetDevice(pl->device));
+  CUDA_TRY(pl, cudaMemsetAsync(P.nn_key, 0xFF, (size_t)P.B * 8, stream));
+  CUDA_TRY(pl, cudaMemsetAsync(P.ctrl, 0, sizeof(Ctrl), stream));
+  CUDA_TRY(pl, cudaMemsetAsync(P.ctrl, 0xFF, 16, stream));  // goal_key[2] = none
+  void* args[] = {&P};
+  const dim3 grid(pl->num_sms * pl->blocks_per_sm), block(kThreads);
+  CUDA_TRY(pl, cudaLaunchCooperativeKernel(pl->kernel, grid, block, args, pl->smem_bytes, stream));
+  return PAKR_OK;
+}
+
+}  // namespace
+
+extern "C" pakr_status pakr_plan(pakr_planner* pl, const pakr_plan_opts* o, void* d_ws, size_t ws_bytes,
+                                 void* cuda_stream, pakr_result* out) {
+  if (!pl) return PAKR_ERR_INVALID_ARG;
+  if (!o || !out || !d_ws) return fail(pl, PAKR_ERR_INVALID_ARG, "null opts, result or workspace");
+  if (!sizes_ok(o->B, o->K, o->tree_capacity) || o->n_replans < 1 || o->n_replans > 4096 ||
+      o->max_iters_per_replan < 0 || o->max_iters_per_replan > (1ll << 30) || out->path_capacity < 0)
+    return fail(pl, PAKR_ERR_INVALID_ARG, "B, K, tree_capacity, n_replans or max_iters out of range");
+  if (reinterpret_cast<uintptr_t>(d_ws) % kAlign) return fail(pl, PAKR_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+  const Layout L = make_layout(pl, o->B, o->K, o->tree_capacity);
+  if (ws_bytes < L.total) return fail(pl, PAKR_ERR_WORKSPACE_TOO_SMALL, "workspace smaller than pakr_workspace_bytes()");
+  cudaStream_t stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+  char* ws = static_cast<char*>(d_ws);
+  Params P;
+  fill_common(pl, P, L, ws, o->B, o->K, o->tree_capacity);
+  P.states = reinterpret_cast<float*>(ws + L.states);
+  P.actions = reinterpret_cast<float*>(ws + L.actions);
+  P.parents = reinterpret_cast<int*>(ws + L.parents);
+  P.costs = reinterpret_cast<float*>(ws + L.costs);
+  P.seed = o->seed;
+  P.n_replans = o->n_replans;
+  const int64_t BK = (int64_t)o->B * o->K;
+  int64_t mi = o->max_iters_per_replan > 0 ? o->max_iters_per_replan : std::max<int64_t>(32, o->tree_capacity / BK);
+  P.max_iters = (int)mi;
+  P.budget_ns = o->time_budget_ms > 0 ? (unsigned long long)(o->time_budget_ms * 1e6) : 0ull;
+  P.r0 = 0; P.it0 = 0;
+  P.c_best0 = INFINITY;
+  P.early_exit = 1;
+  // Alg. 1 l.4: root node (x_init, no action, parent -1, cost 0); rewritten never, read by every replan
+  float root[kMaxD + kMaxM + 2] = {0};
+  for (int d = 0; d < pl->D; ++d) root[d] = pl->pb.start[d];
+  const int minus1 = -1;
+  CUDA_TRY(pl, cudaSetDevice(pl->device));
+  CUDA_TRY(pl, cudaMemcpyAsync(P.states, root, (size_t)pl->DP * 4, cudaMemcpyHostToDevice, stream));
+  CUDA_TRY(pl, cudaMemsetAsync(P.actions, 0, 16, stream));
+  CUDA_TRY(pl, cudaMemcpyAsync(P.parents, &minus1, 4, cudaMemcpyHostToDevice, stream));
+  CUDA_TRY(pl, cudaMemsetAsync(P.costs, 0, 4, stream));
+  pakr_status st = launch(pl, P, stream);
+  if (st != PAKR_OK) return st;
+  Ctrl* hc = static_cast<Ctrl*>(pl->h_pinned);
+  CUDA_TRY(pl, cudaMemcpyAsync(hc, P.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, stream));
+  CUDA_TRY(pl, cudaStreamSynchronize(stream));
+  // results
+  pakr_stats& s = out->stats;
+  std::memset(&s, 0, sizeof(s));
+  s.iterations = hc->iterations;
+  s.children = hc->iterations * BK;
+  s.inserted = hc->inserted;
+  s.replans_run = hc->replans_run;
+  s.replans_solved = hc->replans_solved;
+  s.termination = hc->termination;
+  s.first_solution_ms = hc->replans_solved > 0 ? (double)(hc->t_first_ns - hc->t_start_ns) * 1e-6 : -1.0;
+  s.device_ms = (double)(hc->t_end_ns - hc->t_start_ns) * 1e-6;
+  for (int i = 0; i < kStatsMax && i < hc->replans_run; ++i) {
+    s.replan_cost[i] = hc->replan_cost[i];
+    s.replan_nodes[i] = hc->replan_nodes[i];
+    s.replan_iters[i] = hc->replan_iters[i];
+    s.replan_end_ms[i] = (double)(hc->replan_end_ns[i] - hc->t_start_ns) * 1e-6;
+  }
+  out->final_tree_nodes = hc->n_nodes;
+  out->outcome = hc->solved ? PAKR_SOLVED : PAKR_NO_SOLUTION;
+  out->cost = hc->solved ? (double)hc->best_cost : (double)INFINITY;
+  out->path_len = hc->solved ? hc->path_len : 0;
+  if (!hc->solved) return PAKR_OK;
+  if (hc->path_len > kPathMax || hc->path_len > out->path_capacity) {
+    if (out->path_nodes || out->path_states || out->path_controls || hc->path_len > kPathMax)
+      return fail(pl, PAKR_ERR_BUFFER_TOO_SMALL, "path longer than path_capacity");
+    return PAKR_OK;
+  }
+  const int Lp = hc->path_len;
+  char* stage = static_cast<char*>(pl->h_pinned) + sizeof(Ctrl);
+  int* h_nodes = reinterpret_cast<int*>(stage);
+  float* h_states = reinterpret_cast<float*>(stage + (size_t)kPathMax * 4);
+  float* h_ctrls = h_states + (size_t)kPathMax * kMaxD;
+  if (out->path_nodes) CUDA_TRY(pl, cudaMemcpyAsync(h_nodes, P.path_nodes, (size_t)Lp * 4, cudaMemcpyDeviceToHost, stream));
+  if (out->path_states) CUDA_TRY(pl, cudaMemcpyAsync(h_states, P.path_states, (size_t)Lp * pl->D * 4, cudaMemcpyDeviceToHost, stream));
+  if (out->path_controls && Lp > 1)
+    CUDA_TRY(pl, cudaMemcpyAsync(h_ctrls, P.path_controls, (size_t)(Lp - 1) * pl->M * 4, cudaMemcpyDeviceToHost, stream));
+  CUDA_TRY(pl, cudaStreamSynchronize(stream));
+  if (out->path_nodes) std::memcpy(out->path_nodes, h_nodes, (size_t)Lp * 4);
+  if (out->path_states) std::memcpy(out->path_states, h_states, (size_t)Lp * pl->D * 4);
+  if (out->path_controls && Lp > 1) std::memcpy(out->path_controls, h_ctrls, (size_t)(Lp - 1) * pl->M * 4);
+  return PAKR_OK;
+}
+
+extern "C" pakr_status pakr_expand_step(pakr_planner* pl, const pakr_step_args* a, void* d_ws, size_t ws_bytes,
+                                        void* cuda_stream) {
+  if (!pl) return PAKR_ERR_INVALID_ARG;
+  if (!a || !d_ws) return fail(pl, PAKR_ERR_INVALID_ARG, "null args or workspace");
+  if (!sizes_ok(a->B, a->K, a->tree_capacity)) return fail(pl, PAKR_ERR_INVALID_ARG, "B, K or tree_capacity out of range");
+  if (!a->states || !a->actions || !a->parents || !a->costs || !a->n_nodes)
+    return fail(pl, PAKR_ERR_INVALID_ARG, "null tree pointer");
+  if (std::isnan(a->c_best)) return fail(pl, PAKR_ERR_INVALID_ARG, "c_best is NaN");
+  if (reinterpret_cast<uintptr_t>(d_ws) % kAlign || reinterpret_cast<uintptr_t>(a->states) % 16 ||
+      reinterpret_cast<uintptr_t>(a->actions) % 16)
+    return fail(pl, PAKR_ERR_INVALID_ARG, "workspace must be 256-byte, states/actions 16-byte aligned");
+  const Layout L = make_layout(pl, a->B, a->K, a->tree_capacity);
+  if (ws_bytes < L.total) return fail(pl, PAKR_ERR_WORKSPACE_TOO_SMALL, "workspace smaller than pakr_workspace_bytes()");
+  Params P;
+  fill_common(pl, P, L, static_cast<char*>(d_ws), a->B, a->K, a->tree_capacity);
+  P.states = a->states; P.actions = a->actions; P.parents = a->parents; P.costs = a->costs;
+  P.seed = a->seed;
+  P.n_replans = 1; P.max_iters = 1; P.budget_ns = 0;
+  P.r0 = (int)a->replan; P.it0 = (int)a->iteration;
+  P.c_best0 = a->c_best;
+  P.early_exit = 0;
+  P.n_nodes_io = a->n_nodes;
+  P.dbg_x_rand = a->x_rand; P.dbg_nn_idx = a->nn_idx; P.dbg_nn_d2 = a->nn_d2;
+  P.dbg_child_state = a->child_state; P.dbg_child_ctrl = a->child_ctrl; P.dbg_child_cost = a->child_cost;
+  P.dbg_child_flags = a->child_flags; P.dbg_n_inserted = a->n_inserted; P.dbg_goal_node = a->goal_node;
+  P.dbg_new_c_best = a->new_c_best;
+  return launch(pl, P, reinterpret_cast<cudaStream_t>(cuda_stream));
+}

@@ -1,0 +1,509 @@
+// pakr_kernel.cuh -- the persistent cooperative kernel that runs Alg. 1 on device.
+//
+// One launch = the whole AO-x loop (or one iteration for pakr_expand_step).  Per iteration:
+//   phase A  NN scan        (Alg. 1 l.6-7)   warps own 32*Q queries in registers, tree tiles are
+//                                             streamed into shared memory by TMA bulk copies
+//   -- grid sync --
+//   phase B  propagate      (Alg. 1 l.8-12)  one lane per child, state in registers, obstacles in
+//                                             shared memory, per-warp ballot compaction
+//   -- grid sync --
+//   phase C  insert + goal  (Alg. 1 l.13-15) ordered prefix over the per-warp counts, coalesced
+//                                             append at the tree tail, goal winner by atomicMin
+//   -- grid sync --
+// Loop state (n, c_best, replan, iteration) is replicated in registers of every thread and
+// recomputed from the same global values, so no broadcast step is needed.
+#pragma once
+#include <cooperative_groups.h>
+
+#include "pakr_device.cuh"
+
+namespace pakr {
+namespace cg = cooperative_groups;
+
+constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+constexpr int kQ = 4;            // queries per lane in the NN scan
+constexpr int kPathMax = 8192;   // longest path the device buffers hold
+constexpr int kStatsMax = 64;
+constexpr unsigned long long kKeyNone = ~0ull;
+
+struct Ctrl {  // device control block (in the workspace)
+  unsigned long long goal_key[2];
+  unsigned long long t_start_ns, t_first_ns, t_end_ns;
+  long long iterations, inserted;
+  int n_nodes, stop;
+  int path_len, solved;
+  float best_cost;
+  int replans_run, replans_solved, termination;
+  float replan_cost[kStatsMax];
+  int replan_nodes[kStatsMax];
+  int replan_iters[kStatsMax];
+  unsigned long long replan_end_ns[kStatsMax];
+};
+
+struct Params {
+  DevProblem pb;
+  // tree
+  float* states; float* actions; int* parents; float* costs;
+  // per-iteration work buffers
+  unsigned long long* nn_key;  // [B]   (d2 bits << 32) | node, combined with atomicMin
+  unsigned* unit_count;        // [ceil(B*K/32)] survivors per warp unit
+  float* scr_state; float* scr_ctrl; float* scr_cost; int* scr_parent; int* scr_flags;
+  Ctrl* ctrl;
+  int* path_nodes_rev; int* path_nodes; float* path_states; float* path_controls;
+  // loop
+  unsigned long long seed;
+  int B, K;
+  int cap;
+  int n_replans;
+  int max_iters;
+  unsigned long long budget_ns;  // 0 = none
+  int r0, it0;
+  float c_best0;
+  int early_exit;
+  int* n_nodes_io;               // expand_step: tree size in/out (else NULL: start from the root)
+  // expand_step debug outputs (NULL in pakr_plan)
+  float* dbg_x_rand; int* dbg_nn_idx; float* dbg_nn_d2; float* dbg_child_state; float* dbg_child_ctrl;
+  float* dbg_child_cost; int* dbg_child_flags; int* dbg_n_inserted; int* dbg_goal_node;
+  float* dbg_new_c_best;
+};
+
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+}
+// TMA 1-D bulk copy global -> shared, completion counted on an mbarrier (SASS: UBLKCP).
+__device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+          smem_u32(dst)),
+      "l"(src), "r"(bytes), "r"(smem_u32(bar))
+      : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
+template <int DYN> struct TileCfg {  // nodes per TMA tile: <= 4 KB per buffer
+  static constexpr int DP = DynTraits<DYN>::DP;
+  static constexpr int TILE = (DP == 4) ? 256 : (DP == 8) ? 128 : 64;
+  static constexpr int TILE_FLOATS = TILE * DP;
+};
+
+// squared weighted distance between a query (registers) and a node (shared memory row p)
+template <int DYN, bool UNIT_W>
+__device__ __forceinline__ float dist2(const DevProblem& pb, const float (&q)[DynTraits<DYN>::D],
+                                       const float (&p)[DynTraits<DYN>::DP]) {
+  constexpr int D = DynTraits<DYN>::D;
+  float acc = 0.0f;
+#pragma unroll
+  for (int d = 0; d < D; ++d) {
+    const float delta = (d == DynTraits<DYN>::ANGLE) ? angle_absdiff(q[d], p[d]) : (q[d] - p[d]);
+    if (UNIT_W) acc = fmaf(delta, delta, acc);
+    else acc = fmaf(delta * pb.w[d], delta, acc);
+  }
+  return acc;
+}
+
+// ---- phase A: nearest neighbour over the frozen snapshot [0, n) (Alg. 1 l.6-7) ----
+template <int DYN, bool UNIT_W>
+__device__ __forceinline__ void nn_phase(const Params& P, int n, uint32_t r, uint32_t it, float* sm_tile,
+                                         uint64_t* sm_bar, uint32_t& par0, uint32_t& par1) {
+  constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
+  constexpr int TILE = TileCfg<DYN>::TILE, TF = TileCfg<DYN>::TILE_FLOATS;
+  const int lane = threadIdx.x & 31;
+  const int W = gridDim.x * kWarps;
+  const int gw = blockIdx.x * kWarps + (threadIdx.x >> 5);
+  const int G = (P.B + 32 * kQ - 1) / (32 * kQ);  // query groups
+  int R = W / G;                                  // node ranges per group
+  if (R < 1) R = 1;
+  int len = (n + R - 1) / R;
+  if (len < 32) len = 32;
+  const int Reff = (n + len - 1) / len;
+  const int U = G * Reff;
+  for (int u = gw; u < U; u += W) {
+    const int g = u / Reff, rr = u - g * Reff;
+    const int beg = rr * len;
+    const int end = min(n, beg + len);
+    float q[kQ][D];
+    float best[kQ];
+    int bidx[kQ];
+#pragma unroll
+    for (int j = 0; j < kQ; ++j) {
+      const int s = g * 32 * kQ + j * 32 + lane;
+      sample_state<D>(P.pb, P.seed, r, it, (uint32_t)s, q[j]);
+      best[j] = __int_as_float(0x7f800000);
+      bidx[j] = 0x7fffffff;
+      if (P.dbg_x_rand && rr == 0 && s < P.B) {
+#pragma unroll
+        for (int d = 0; d < DP; ++d) P.dbg_x_rand[(size_t)s * DP + d] = d < D ? q[j][d] : 0.0f;
+      }
+    }
+    const int ntiles = (end - beg + TILE - 1) / TILE;
+    const float* src = P.states + (size_t)beg * DP;
+    if (lane == 0) {
+      const uint32_t bytes = (uint32_t)min(TILE, end - beg) * DP * 4;
+      mbar_expect_tx(&sm_bar[0], bytes);
+      tma_load_1d(sm_tile, src, bytes, &sm_bar[0]);
+    }
+    for (int t = 0; t < ntiles; ++t) {
+      const int cnt = min(TILE, end - beg - t * TILE);
+      if (t + 1 < ntiles && lane == 0) {  // prefetch the next tile into the other buffer
+        const int b = (t + 1) & 1;
+        const uint32_t bytes = (uint32_t)min(TILE, end - beg - (t + 1) * TILE) * DP * 4;
+        mbar_expect_tx(&sm_bar[b], bytes);
+        tma_load_1d(sm_tile + b * TF, src + (size_t)(t + 1) * TF, bytes, &sm_bar[b]);
+      }
+      if (t & 1) { mbar_wait(&sm_bar[1], par1); par1 ^= 1; }
+      else { mbar_wait(&sm_bar[0], par0); par0 ^= 1; }
+      const float4* tp = reinterpret_cast<const float4*>(sm_tile + (t & 1) * TF);
+      const int base = beg + t * TILE;
+#pragma unroll 2
+      for (int i = 0; i < cnt; ++i) {
+        float p[DP];
+#pragma unroll
+        for (int v = 0; v < DP / 4; ++v) {
+          const float4 a = tp[i * (DP / 4) + v];  // warp-uniform address: broadcast
+          p[4 * v] = a.x; p[4 * v + 1] = a.y; p[4 * v + 2] = a.z; p[4 * v + 3] = a.w;
+        }
+#pragma unroll
+        for (int j = 0; j < kQ; ++j) {
+          const float d2 = dist2<DYN, UNIT_W>(P.pb, q[j], p);
+          if (d2 < best[j]) { best[j] = d2; bidx[j] = base + i; }  // strict <: lowest index wins
+        }
+      }
+      __syncwarp();  // every lane is done with this buffer before lane 0 refills it
+    }
+#pragma unroll
+    for (int j = 0; j < kQ; ++j) {
+      const int s = g * 32 * kQ + j * 32 + lane;
+      if (s < P.B && bidx[j] != 0x7fffffff) {
+        const unsigned long long key =
+            ((unsigned long long)__float_as_uint(best[j]) << 32) | (unsigned)bidx[j];
+        atomicMin(&P.nn_key[s], key);  // d2 >= 0: uint order == float order; ties -> lowest node
+      }
+    }
+  }
+}
+
+// ---- phase B: controls, propagation, validity, prune, goal flag, per-warp compaction ------------
+template <int DYN, int OBS>
+__device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t it, float c_best,
+                                           const float* sm_obs) {
+  using T = DynTraits<DYN>;
+  constexpr int D = T::D, M = T::M, DP = T::DP, PD = T::PD;
+  const DevProblem& pb = P.pb;
+  const int lane = threadIdx.x & 31;
+  const int W = gridDim.x * kWarps;
+  const int gw = blockIdx.x * kWarps + (threadIdx.x >> 5);
+  const int BK = P.B * P.K;
+  const int U = (BK + 31) / 32;
+  for (int u = gw; u < U; u += W) {
+    const int c = u * 32 + lane;
+    const bool active = c < BK;
+    const int s = active ? c / P.K : 0;
+    const int k = active ? c - s * P.K : 0;
+    const unsigned long long key = __ldcg(&P.nn_key[s]);
+    const int parent = (int)(unsigned)(key & 0xffffffffu);
+    if (active && k == 0) {
+      if (P.dbg_nn_idx) P.dbg_nn_idx[s] = parent;
+      if (P.dbg_nn_d2) P.dbg_nn_d2[s] = __uint_as_float((unsigned)(key >> 32));
+    }
+    float x[D], ctl[M];
+    {
+      const float4* sp = reinterpret_cast<const float4*>(P.states + (size_t)parent * DP);
+      float tmp[DP];
+#pragma unroll
+      for (int v = 0; v < DP / 4; ++v) {
+        const float4 a = __ldcg(sp + v);
+        tmp[4 * v] = a.x; tmp[4 * v + 1] = a.y; tmp[4 * v + 2] = a.z; tmp[4 * v + 3] = a.w;
+      }
+#pragma unroll
+      for (int d = 0; d < D; ++d) x[d] = tmp[d];
+    }
+    const float parent_cost = __ldcg(&P.costs[parent]);
+    sample_control<M>(pb, P.seed, r, it, (uint32_t)s, (uint32_t)k, ctl);
+    bool inb = active, cf = active;
+    float length = 0.0f;
+    for (int j = 0; j < pb.S; ++j) {
+      float px[PD];
+#pragma unroll
+      for (int a = 0; a < PD; ++a) px[a] = x[a];
+      dyn_step<DYN>(pb, x, ctl);
+      if (pb.cost_mode == 1) {
+        float seg = 0.0f;
+#pragma unroll
+        for (int a = 0; a < PD; ++a) seg = fmaf(x[a] - px[a], x[a] - px[a], seg);
+        length += sqrtf(seg);
+      }
+      inb = inb && in_bounds<DYN>(pb, x);
+      cf = cf && collision_free<OBS, PD>(sm_obs, pb.n_obs, x, 0, 1);
+      if (P.early_exit && !__any_sync(0xffffffffu, inb && cf)) break;
+    }
+    if (T::ANGLE >= 0) x[T::ANGLE >= 0 ? T::ANGLE : 0] = wrap_pi(x[T::ANGLE >= 0 ? T::ANGLE : 0]);
+    const float edge = (pb.cost_mode == 1) ? length : (float)pb.S * pb.dt;
+    const float c_new = parent_cost + edge;
+    const float gd = goal_dist<PD>(pb, x);
+    const float h = fmaxf(0.0f, gd - pb.goal_r) * pb.inv_hspeed;
+    const bool notpruned = (c_new + h) < c_best;
+    bool ing = gd <= pb.goal_r;
+    if (pb.goal_angle_dim >= 0) ing = ing && (fabsf(wrap_pi(x[T::ANGLE >= 0 ? T::ANGLE : 0] - pb.goal_angle)) <= pb.goal_angle_tol);
+    const bool valid = inb && cf;
+    const bool keep = valid && notpruned;
+    int flags = (valid ? 1 : 0) | (inb ? 2 : 0) | (cf ? 4 : 0) | (notpruned ? 8 : 0) | ((keep && ing) ? 16 : 0);
+    const unsigned bal = __ballot_sync(0xffffffffu, keep);
+    const int rank = __popc(bal & ((1u << lane) - 1u));
+    if (lane == 0) P.unit_count[u] = __popc(bal);
+    float4 cv = make_float4(0.f, 0.f, 0.f, 0.f);
+    {
+      float t4[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+      for (int j = 0; j < M; ++j) t4[j] = ctl[j];
+      cv = make_float4(t4[0], t4[1], t4[2], t4[3]);
+    }
+    float xs[DP];
+#pragma unroll
+    for (int d = 0; d < DP; ++d) xs[d] = d < D ? x[d] : 0.0f;
+    if (keep) {
+      const size_t slot = (size_t)u * 32 + rank;
+      float4* dst = reinterpret_cast<float4*>(P.scr_state + slot * DP);
+#pragma unroll
+      for (int v = 0; v < DP / 4; ++v) __stcg(dst + v, make_float4(xs[4 * v], xs[4 * v + 1], xs[4 * v + 2], xs[4 * v + 3]));
+      __stcg(reinterpret_cast<float4*>(P.scr_ctrl) + slot, cv);
+      __stcg(&P.scr_cost[slot], c_new);
+      __stcg(&P.scr_parent[slot], parent);
+      __stcg(&P.scr_flags[slot], flags | (lane << 8));
+    }
+    if (active && P.dbg_child_flags) {
+      P.dbg_child_flags[c] = flags;
+      if (P.dbg_child_cost) P.dbg_child_cost[c] = c_new;
+      if (P.dbg_child_ctrl) reinterpret_cast<float4*>(P.dbg_child_ctrl)[c] = cv;
+      if (P.dbg_child_state) {
+#pragma unroll
+        for (int d = 0; d < DP; ++d) P.dbg_child_state[(size_t)c * DP + d] = xs[d];
+      }
+    }
+  }
+}
+
+// ---- phase C: ordered insert at the tree tail, goal winner (Alg. 1 l.13-15; P19, P20) ----
+// Returns the number of survivors of this iteration (identical in every thread of the grid).
+template <int DYN>
+__device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, int* sm_pref) {
+  using T = DynTraits<DYN>;
+  constexpr int DP = T::DP;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int W = gridDim.x * kWarps;
+  const int gw = blockIdx.x * kWarps + warp;
+  const int BK = P.B * P.K;
+  const int U = (BK + 31) / 32;
+  // exclusive prefix of the per-unit counts at chunk granularity, redundantly in every CTA
+  const int cpt = (U + kThreads - 1) / kThreads;  // units per thread-chunk
+  int mine = 0;
+  for (int v = threadIdx.x * cpt; v < min(U, (threadIdx.x + 1) * cpt); ++v) mine += (int)__ldcg(&P.unit_count[v]);
+  int incl = mine;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int t = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += t;
+  }
+  __syncthreads();  // sm_pref reuse across iterations
+  if (lane == 31) sm_pref[kThreads + warp] = incl;
+  __syncthreads();
+  int wbase = 0, total = 0;
+#pragma unroll
+  for (int w = 0; w < kWarps; ++w) {
+    const int t = sm_pref[kThreads + w];
+    if (w < warp) wbase += t;
+    total += t;
+  }
+  sm_pref[threadIdx.x] = wbase + incl - mine;
+  __syncthreads();
+  const int room = P.cap - n;
+  for (int u = gw; u < U; u += W) {
+    const int ch = u / cpt;
+    int part = 0;
+    for (int v = ch * cpt + lane; v < u; v += 32) part += (int)__ldcg(&P.unit_count[v]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+    const int off = sm_pref[ch] + part;
+    const int cnt = (int)__ldcg(&P.unit_count[u]);
+    const int pos = off + lane;
+    if (lane < cnt && pos < room) {
+      const size_t slot = (size_t)u * 32 + lane;
+      const int node = n + pos;
+      const float4* src = reinterpret_cast<const float4*>(P.scr_state + slot * DP);
+      float4* dst = reinterpret_cast<float4*>(P.states + (size_t)node * DP);
+#pragma unroll
+      for (int v = 0; v < DP / 4; ++v) dst[v] = __ldcg(src + v);
+      reinterpret_cast<float4*>(P.actions)[node] = __ldcg(reinterpret_cast<const float4*>(P.scr_ctrl) + slot);
+      const float cost = __ldcg(&P.scr_cost[slot]);
+      P.costs[node] = cost;
+      P.parents[node] = __ldcg(&P.scr_parent[slot]);
+      const int fl = __ldcg(&P.scr_flags[slot]);
+      if (fl & 16)  // goal child: min cost, ties -> lowest node id == lowest child index
+        atomicMin(&P.ctrl->goal_key[gslot], ((unsigned long long)__float_as_uint(cost) << 32) | (unsigned)node);
+      if (P.dbg_child_flags) P.dbg_child_flags[u * 32 + (fl >> 8)] |= 32;
+    }
+  }
+  // reset the NN keys for the next iteration
+  for (int s = blockIdx.x * kThreads + threadIdx.x; s < P.B; s += gridDim.x * kThreads) P.nn_key[s] = kKeyNone;
+  return total;
+}
+
+// Alg. 1 l.16 ExtractPath: warp 0 of block 0 walks parents, then copies in parallel.
+template <int DYN>
+__device__ __forceinline__ void extract_path(const Params& P, int goal_node) {
+  using T = DynTraits<DYN>;
+  const int lane = threadIdx.x & 31;
+  int len = 0;
+  if (lane == 0) {
+    for (int i = goal_node; i >= 0; i = __ldcg(&P.parents[i])) {
+      if (len < kPathMax) P.path_nodes_rev[kPathMax - 1 - len] = i;
+      ++len;
+    }
+    P.ctrl->path_len = len;
+  }
+  len = __shfl_sync(0xffffffffu, len, 0);
+  if (len > kPathMax) return;
+  __syncwarp();
+  for (int i = lane; i < len; i += 32) {
+    const int node = P.path_nodes_rev[kPathMax - len + i];
+    P.path_nodes[i] = node;
+    for (int d = 0; d < T::D; ++d) P.path_states[(size_t)i * T::D + d] = __ldcg(&P.states[(size_t)node * T::DP + d]);
+    if (i > 0)
+      for (int j = 0; j < T::M; ++j) P.path_controls[(size_t)(i - 1) * T::M + j] = __ldcg(&P.actions[(size_t)node * 4 + j]);
+  }
+}
+
+template <int DYN, int OBS>
+__global__ void __launch_bounds__(kThreads, 2) pakr_loop_kernel(const __grid_constant__ Params P) {
+  using T = DynTraits<DYN>;
+  constexpr int OS = (OBS == OBS_CIRCLE) ? 4 : 8;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  // [tiles: kWarps * 2 * TILE_FLOATS][bars: kWarps * 2][pref: kThreads + kWarps][obstacles]
+  float* sm_tiles = reinterpret_cast<float*>(smem_raw);
+  uint64_t* sm_bars = reinterpret_cast<uint64_t*>(sm_tiles + kWarps * 2 * TileCfg<DYN>::TILE_FLOATS);
+  int* sm_pref = reinterpret_cast<int*>(sm_bars + kWarps * 2);
+  float* sm_obs = reinterpret_cast<float*>(sm_pref + kThreads + kWarps + 8);
+  cg::grid_group grid = cg::this_grid();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const bool leader = (blockIdx.x == 0 && threadIdx.x == 0);
+
+  for (int i = threadIdx.x; i < P.pb.n_obs * OS; i += kThreads) sm_obs[i] = P.pb.obstacles[i];
+  if (lane == 0) {
+    mbar_init(&sm_bars[warp * 2], 1);
+    mbar_init(&sm_bars[warp * 2 + 1], 1);
+  }
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  fence_proxy_async();
+  __syncthreads();
+  float* my_tile = sm_tiles + warp * 2 * TileCfg<DYN>::TILE_FLOATS;
+  uint64_t* my_bar = sm_bars + warp * 2;
+  uint32_t par0 = 0, par1 = 0;
+
+  unsigned long long t_start = 0;
+  if (leader) { t_start = globaltimer_ns(); P.ctrl->t_start_ns = t_start; }
+
+  float c_best = P.c_best0;
+  int n = P.n_nodes_io ? __ldcg(P.n_nodes_io) : 1;
+  int solved_any = 0, replans_solved = 0, replans_run = 0, termination = 0;
+  long long iterations = 0, inserted = 0;
+  bool stop = false;
+
+  for (int r = P.r0; r < P.r0 + P.n_replans && !stop; ++r) {
+    if (!P.n_nodes_io) n = 1;  // Alg. 1 l.4: node 0 = (x_init, 0, -1, 0) is written once by the host
+    int it = P.it0;
+    int iters = 0;
+    int goal_node = -1;
+    for (;;) {
+      // phase A
+      if (P.pb.unit_weights) nn_phase<DYN, true>(P, n, (uint32_t)r, (uint32_t)it, my_tile, my_bar, par0, par1);
+      else nn_phase<DYN, false>(P, n, (uint32_t)r, (uint32_t)it, my_tile, my_bar, par0, par1);
+      grid.sync();
+      // phase B
+      prop_phase<DYN, OBS>(P, (uint32_t)r, (uint32_t)it, c_best, sm_obs);
+      // goal-key slots alternate over the whole launch (not per replan): the other slot was last
+      // read before the previous grid sync and is next written after the following one
+      const int slot = (int)(iterations & 1);
+      if (leader) P.ctrl->goal_key[slot ^ 1] = kKeyNone;
+      grid.sync();
+      // phase C
+      const int total = insert_phase<DYN>(P, n, slot, sm_pref);
+      const int added = min(total, P.cap - n);
+      if (leader && P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) P.ctrl->stop = 1;
+      __threadfence();
+      fence_proxy_async();  // tree rows written with st.global are read next by TMA (async proxy)
+      grid.sync();
+      fence_proxy_async();
+      n += added;
+      inserted += added;
+      ++iterations;
+      ++iters;
+      const unsigned long long gk = __ldcg(&P.ctrl->goal_key[slot]);
+      stop = __ldcg(&P.ctrl->stop) != 0;
+      ++it;
+      if (gk != kKeyNone) {  // Alg. 1 l.14-17
+        c_best = __uint_as_float((unsigned)(gk >> 32));
+        goal_node = (int)(unsigned)(gk & 0xffffffffu);
+        break;
+      }
+      if (n >= P.cap || iters >= P.max_iters || stop) break;
+    }
+    ++replans_run;
+    if (goal_node >= 0) {
+      ++replans_solved;
+      solved_any = 1;
+      if (blockIdx.x == 0 && warp == 0) extract_path<DYN>(P, goal_node);
+    }
+    if (leader) {
+      const unsigned long long now = globaltimer_ns();
+      if (goal_node >= 0 && replans_solved == 1) P.ctrl->t_first_ns = now;
+      const int ri = r - P.r0;
+      if (ri < kStatsMax) {
+        P.ctrl->replan_cost[ri] = c_best;
+        P.ctrl->replan_nodes[ri] = n;
+        P.ctrl->replan_iters[ri] = iters;
+        P.ctrl->replan_end_ns[ri] = now;
+      }
+      if (P.dbg_goal_node) *P.dbg_goal_node = goal_node;
+    }
+    if (stop) termination = 1;
+  }
+  if (leader) {
+    Ctrl* c = P.ctrl;
+    c->t_end_ns = globaltimer_ns();
+    c->iterations = iterations;
+    c->inserted = inserted;
+    c->n_nodes = n;
+    c->solved = solved_any;
+    c->best_cost = c_best;
+    c->replans_run = replans_run;
+    c->replans_solved = replans_solved;
+    c->termination = termination;
+    if (P.n_nodes_io) *P.n_nodes_io = n;
+    if (P.dbg_n_inserted) *P.dbg_n_inserted = (int)inserted;
+    if (P.dbg_new_c_best) *P.dbg_new_c_best = c_best;
+  }
+}
+
+}  // namespace pakr
