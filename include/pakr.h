@@ -127,6 +127,7 @@ typedef struct {
   int64_t iterations;      /* inner-loop trips over all replans */
   int64_t children;        /* = iterations * B * K propagated and checked ("expanded nodes") */
   int64_t inserted;        /* nodes appended over all replans */
+  int64_t nn_pairs;        /* sum over iterations of B * n: (query, node) distance evaluations */
   int32_t replans_run, replans_solved;
   int32_t termination;     /* 0 all replans run, 1 time budget */
   double first_solution_ms;/* device time from kernel start to the end of the first solved replan; -1 if none */

@@ -337,6 +337,7 @@ extern "C" pakr_status pakr_plan(pakr_planner* pl, const pakr_plan_opts* o, void
   s.iterations = hc->iterations;
   s.children = hc->iterations * BK;
   s.inserted = hc->inserted;
+  s.nn_pairs = hc->nn_pairs;
   s.replans_run = hc->replans_run;
   s.replans_solved = hc->replans_solved;
   s.termination = hc->termination;

@@ -104,9 +104,10 @@ __device__ __forceinline__ float wrap_pi(float a) {  // -> [-pi, pi)
   if (w < -kPiF) w += kTwoPiF;
   return w;
 }
-// |wrap(a - b)| for a, b in [-pi, pi]: pi - | pi - |a-b| |  (two adds with abs modifiers)
+// |wrap(a - b)| for a, b in [-pi, pi]: min(|a-b|, 2pi - |a-b|); exact whenever no wrap happens
 __device__ __forceinline__ float angle_absdiff(float a, float b) {
-  return kPiF - fabsf(kPiF - fabsf(a - b));
+  const float d = fabsf(a - b);
+  return fminf(d, kTwoPiF - d);
 }
 
 // ---- dynamics xdot = f(x, u) -----------------------------------------------------------------

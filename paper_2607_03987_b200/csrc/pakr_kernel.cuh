@@ -30,7 +30,7 @@ constexpr unsigned long long kKeyNone = ~0ull;
 struct Ctrl {  // device control block (in the workspace)
   unsigned long long goal_key[2];
   unsigned long long t_start_ns, t_first_ns, t_end_ns;
-  long long iterations, inserted;
+  long long iterations, inserted, nn_pairs;
   int n_nodes, stop;
   int path_len, solved;
   float best_cost;
@@ -427,7 +427,7 @@ __global__ void __launch_bounds__(kThreads, 2) pakr_loop_kernel(const __grid_con
   float c_best = P.c_best0;
   int n = P.n_nodes_io ? __ldcg(P.n_nodes_io) : 1;
   int solved_any = 0, replans_solved = 0, replans_run = 0, termination = 0;
-  long long iterations = 0, inserted = 0;
+  long long iterations = 0, inserted = 0, nn_pairs = 0;
   bool stop = false;
 
   for (int r = P.r0; r < P.r0 + P.n_replans && !stop; ++r) {
@@ -455,6 +455,7 @@ __global__ void __launch_bounds__(kThreads, 2) pakr_loop_kernel(const __grid_con
       fence_proxy_async();  // tree rows written with st.global are read next by TMA (async proxy)
       grid.sync();
       fence_proxy_async();
+      nn_pairs += (long long)P.B * n;  // (query, node) pairs the scan of this iteration evaluated
       n += added;
       inserted += added;
       ++iterations;
@@ -494,6 +495,7 @@ __global__ void __launch_bounds__(kThreads, 2) pakr_loop_kernel(const __grid_con
     c->t_end_ns = globaltimer_ns();
     c->iterations = iterations;
     c->inserted = inserted;
+    c->nn_pairs = nn_pairs;
     c->n_nodes = n;
     c->solved = solved_any;
     c->best_cost = c_best;

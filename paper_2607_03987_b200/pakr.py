@@ -77,7 +77,7 @@ class _PlanOpts(C.Structure):
 
 
 class _Stats(C.Structure):
-    _fields_ = [("iterations", C.c_int64), ("children", C.c_int64), ("inserted", C.c_int64),
+    _fields_ = [("iterations", C.c_int64), ("children", C.c_int64), ("inserted", C.c_int64), ("nn_pairs", C.c_int64),
                 ("replans_run", C.c_int32), ("replans_solved", C.c_int32), ("termination", C.c_int32),
                 ("first_solution_ms", C.c_double), ("device_ms", C.c_double),
                 ("replan_cost", C.c_float * MAX_REPLAN_STATS), ("replan_nodes", C.c_int32 * MAX_REPLAN_STATS),
@@ -219,7 +219,7 @@ class Planner:
         return dict(outcome=int(res.outcome), cost=float(res.cost), path_len=L, path_nodes=nodes[:L].copy(),
                     path_states=states[:L].copy(), path_controls=ctrls[:max(L - 1, 0)].copy(),
                     final_tree_nodes=int(res.final_tree_nodes), iterations=int(s.iterations), children=int(s.children),
-                    inserted=int(s.inserted), replans_run=int(s.replans_run), replans_solved=int(s.replans_solved),
+                    inserted=int(s.inserted), nn_pairs=int(s.nn_pairs), replans_run=int(s.replans_run), replans_solved=int(s.replans_solved),
                     termination=int(s.termination), first_solution_ms=float(s.first_solution_ms),
                     device_ms=float(s.device_ms), replan_cost=np.array(s.replan_cost[:R], np.float32),
                     replan_nodes=np.array(s.replan_nodes[:R], np.int64), replan_iters=np.array(s.replan_iters[:R], np.int64),

@@ -1,0 +1,92 @@
+"""CPU-side checks of the boundary: libpakr.so builds for sm_100a, loads without a GPU and exports
+every function include/pakr.h declares; the ctypes structs match the header's field order; the
+workload generator is deterministic and keeps start/goal clear of obstacles (P30)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2607_03987_b200 import workloads as wl
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared_functions():
+    text = open(os.path.join(ROOT, "include", "pakr.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(pakr_[a-z_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    from paper_2607_03987_b200 import pakr
+    names = _declared_functions()
+    assert set(names) == set(pakr.EXPORTS), names
+    L = ctypes.CDLL(pakr.build())
+    for n in names:
+        assert hasattr(L, n), n
+
+
+def test_sass_is_sm100a_with_tma():
+    """The built library carries sm_100a SASS and the NN scan's bulk copies are TMA (UBLKCP)."""
+    from paper_2607_03987_b200 import pakr
+    import subprocess
+    so = pakr.build()
+    out = subprocess.run(["/usr/local/cuda/bin/cuobjdump", "-sass", so], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+    assert "UBLKCP" in out
+
+
+def test_struct_field_order_matches_header():
+    from paper_2607_03987_b200 import pakr
+    text = open(os.path.join(ROOT, "include", "pakr.h")).read()
+    body = re.search(r"typedef struct \{(.*?)\} pakr_problem;", text, flags=re.S).group(1)
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    fields = []
+    for decl in body.split(";"):
+        decl = decl.strip()
+        if not decl:
+            continue
+        names = re.sub(r"^(const\s+)?\w+\s*\*?", "", decl, count=1)
+        fields += [n.strip(" *") for n in names.split(",")]
+    assert fields == [f[0] for f in pakr._Problem._fields_]
+
+
+def test_create_without_gpu_fails_loudly():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    from paper_2607_03987_b200 import pakr
+    p, _ = wl.config1()
+    with pytest.raises(pakr.PakrError):
+        pakr.Planner(p)
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C5"])
+def test_workloads_deterministic_and_clear(name):
+    a, cfg = wl.CONFIGS[name]()
+    b, _ = wl.CONFIGS[name]()
+    np.testing.assert_array_equal(a.obstacles, b.obstacles)
+    assert a.obstacles.dtype == np.float32 and a.start.dtype == np.float32
+    ps, g = a.start[:a.pos_dim].astype(np.float64), a.goal_center.astype(np.float64)
+    if a.obstacle_type == wl.OBS_AABB:
+        lo, hi = a.obstacles[:, :a.pos_dim], a.obstacles[:, a.pos_dim:]
+        for q, clear in ((ps, 0.5), (g, 0.5 + a.goal_radius)):
+            d = np.linalg.norm(np.maximum(np.maximum(lo - q, q - hi), 0), axis=1)
+            assert d.min() > clear - 1e-6
+        assert np.all(hi - lo >= 0.5 - 1e-6) and np.all(hi - lo <= 2.0 + 1e-6)
+    else:
+        for q, clear in ((ps[:2], 0.5), (g[:2], 0.5 + a.goal_radius)):
+            d = np.linalg.norm(a.obstacles[:, :2] - q, axis=1) - a.obstacles[:, 2]
+            assert d.min() > clear - 1e-6
+    expected = {"C1": 8, "C2": 32, "C3": 64, "C4": 128, "C5": 128}[name]
+    assert a.n_obstacles == expected
+    assert cfg.B >= 1 and cfg.K >= 1
+
+
+def test_random_tree_invariants():
+    p, _ = wl.config3()
+    t = wl.random_tree(p, 500, seed=1)
+    assert t["parents"][0] == -1 and np.all(t["parents"][1:] < np.arange(1, 500))
+    np.testing.assert_array_equal(t["states"][0], p.start)

@@ -1,0 +1,190 @@
+"""GPU parity of one expansion iteration (pakr_expand_step through the C ABI) against the oracle.
+
+Teacher forcing (SURVEY.md 8(c) "T"): both sides start from the same tree snapshot and the same
+(seed, replan, iteration) and must agree element by element under north_star's tolerances
+(tests/parity_util.py).
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+
+from paper_2607_03987_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pakr():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2607_03987_b200 import pakr as mod
+    mod.lib()  # fails loudly if the extension is missing
+    return mod
+
+
+_CASES = [
+    # config, n_tree, B, K
+    ("C1", 1, 256, 4),
+    ("C1", 31, 100, 3),
+    ("C1", 33, 129, 1),
+    ("C1", 4097, 256, 4),
+    ("C2", 32, 64, 8),
+    ("C2", 4095, 300, 5),
+    ("C2", 20000, 1024, 8),
+    ("C3", 4096, 257, 7),
+    ("C3", 9000, 512, 8),
+    ("C4", 2500, 384, 16),
+    ("C4", 12345, 200, 9),
+    ("C5", 7777, 256, 16),
+]
+
+
+@pytest.mark.parametrize("name,n0,B,K", _CASES)
+def test_step_matches_oracle(pakr, orc, name, n0, B, K):
+    from parity_util import check_iteration, run_both
+    p, _ = wl.CONFIGS[name]()
+    pl = pakr.Planner(p)
+    op = orc.OracleProblem(p)
+    host = wl.random_tree(p, n0, seed=n0 + B)
+    cap = n0 + B * K
+    out, after, ref, _ = run_both(pl, orc, op, p, host, seed=11, r=2, it=5, B=B, K=K, cap=cap)
+    st = check_iteration(orc, op, p, host, out, after, ref, B, K, cap)
+    assert st["nn_equal"] > 0.99
+    pl.close()
+
+
+def test_step_duplicates_and_ties(pakr, orc):
+    """Duplicate nodes: the lowest index must win in every NN variant / tile split (P6, P26)."""
+    from parity_util import check_iteration, run_both
+    p, _ = wl.config2()
+    pl = pakr.Planner(p)
+    op = orc.OracleProblem(p)
+    host = wl.random_tree(p, 6000, seed=3)
+    host["states"][3000:] = host["states"][:3000]  # every node appears twice
+    out, after, ref, _ = run_both(pl, orc, op, p, host, seed=1, r=0, it=0, B=512, K=2)
+    np.testing.assert_array_equal(out["nn_idx"], ref["nn_idx"])
+    assert out["nn_idx"].max() < 3000
+    check_iteration(orc, op, p, host, out, after, ref, 512, 2, 6000 + 1024)
+    pl.close()
+
+
+def test_step_query_equals_node_and_zero_weight(pakr, orc):
+    from parity_util import check_iteration, run_both
+    p, _ = wl.config4()
+    w = p.nn_weight.copy()
+    w[3:] = 0.0  # NN over position only (PAPER.md:286 subset of dims)
+    p = dataclasses.replace(p, nn_weight=w)
+    pl = pakr.Planner(p)
+    op = orc.OracleProblem(p)
+    host = wl.random_tree(p, 5000, seed=4)
+    # plant the exact sampled states of the first queries as nodes: their NN is that node, d2 == 0
+    for s in range(8):
+        host["states"][1000 + s] = op.sample_state(21, 0, 3, s).astype(np.float32)
+    out, after, ref, _ = run_both(pl, orc, op, p, host, seed=21, r=0, it=3, B=128, K=4)
+    np.testing.assert_array_equal(out["nn_idx"][:8], 1000 + np.arange(8))
+    assert np.all(out["nn_d2"][:8] == 0.0)
+    check_iteration(orc, op, p, host, out, after, ref, 128, 4, 5000 + 512)
+    pl.close()
+
+
+def test_step_prune_goal_and_overflow(pakr, orc):
+    """Finite c_best prunes; goal children are inserted and the winner is the cheapest, lowest index;
+    a full tree takes only the first cap - n survivors (P16, P19, P20)."""
+    from parity_util import check_iteration, run_both
+    p, _ = wl.config1()
+    p = dataclasses.replace(p, obstacles=p.obstacles[:2], goal_radius=2.5)
+    pl = pakr.Planner(p)
+    op = orc.OracleProblem(p)
+    n0 = 400
+    rng = np.random.default_rng(0)
+    host = wl.random_tree(p, n0, seed=9)
+    host["states"][1:, :2] = rng.uniform(7.0, 9.8, size=(n0 - 1, 2)).astype(np.float32)
+    host["states"][1:, 2:] = rng.uniform(-0.5, 0.5, size=(n0 - 1, 2)).astype(np.float32)
+    B, K = 256, 4
+    for c_best, cap in ((float("inf"), n0 + B * K), (4.0, n0 + B * K), (float("inf"), n0 + 37), (0.0, n0 + B * K)):
+        out, after, ref, _ = run_both(pl, orc, op, p, host, seed=5, r=1, it=0, B=B, K=K, c_best=c_best, cap=cap)
+        st = check_iteration(orc, op, p, host, out, after, ref, B, K, cap)
+        if c_best == float("inf") and cap > n0 + 37:
+            assert st["n_goal"] > 3 and out["goal_node"] >= n0
+        if c_best == 0.0:
+            assert st["n_inserted"] == 0 and after["n"] == n0
+        if cap == n0 + 37:
+            assert after["n"] == cap
+    pl.close()
+
+
+def test_step_path_length_cost_mode(pakr, orc):
+    from parity_util import check_iteration, run_both
+    p, _ = wl.config2()
+    p = dataclasses.replace(p, cost_mode=wl.COST_PATH_LENGTH, heuristic_speed=1.0)
+    pl = pakr.Planner(p)
+    op = orc.OracleProblem(p)
+    host = wl.random_tree(p, 3000, seed=2)
+    out, after, ref, _ = run_both(pl, orc, op, p, host, seed=8, r=0, it=1, B=256, K=4, c_best=30.0)
+    check_iteration(orc, op, p, host, out, after, ref, 256, 4, 3000 + 1024)
+    pl.close()
+
+
+def test_teacher_forced_run_c2(pakr, orc):
+    """Grow a tree with the GPU from the root; at sampled iterations hand the GPU's snapshot to the
+    oracle and compare that one iteration."""
+    from parity_util import check_iteration
+    import torch
+    p, _ = wl.config2()
+    pl = pakr.Planner(p)
+    op = orc.OracleProblem(p)
+    B, K, cap = 256, 8, 60000
+    tree = pl.new_tree(cap)
+    D, m = p.state_dim, p.control_dim
+    for it in range(14):
+        n0 = int(tree["n_nodes"][0].item())
+        snap = dict(states=tree["states"][:n0, :D].cpu().numpy(), actions=tree["actions"][:n0, :m].cpu().numpy(),
+                    parents=tree["parents"][:n0].cpu().numpy(), costs=tree["costs"][:n0].cpu().numpy())
+        out = pl.expand_step(tree, 3, 0, it, B, K)
+        if it in (0, 1, 5, 13):
+            n1 = int(tree["n_nodes"][0].item())
+            after = dict(states=tree["states"][:n1, :D].cpu().numpy(), actions=tree["actions"][:n1, :m].cpu().numpy(),
+                         parents=tree["parents"][:n1].cpu().numpy(), costs=tree["costs"][:n1].cpu().numpy(), n=n1)
+            ot = orc.OracleTree(op, cap)
+            ot.load(snap["states"], snap["actions"], snap["parents"], snap["costs"])
+            ref = orc.expand_iteration(op, ot, 3, 0, it, B, K)
+            check_iteration(orc, op, p, snap, out, after, ref, B, K, cap)
+    assert int(tree["n_nodes"][0].item()) > 2000
+    pl.close()
+
+
+def test_full_size_c2_sampled(pakr, orc):
+    """BASELINE config C2 at full B, K in the bench launch configuration on a large tree: NN checked
+    on sampled queries (oracle one by one), children of those queries checked exactly."""
+    p, cfg = wl.config2()
+    pl = pakr.Planner(p)
+    op = orc.OracleProblem(p)
+    n0 = 300000
+    host = wl.random_tree(p, n0, seed=77)
+    B, K = cfg.B, cfg.K
+    tree = pl.new_tree(n0 + B * K, host)
+    out = pl.expand_step(tree, 0, 0, 40, B, K)
+    tree64 = host["states"].astype(np.float64)
+    rng = np.random.default_rng(1)
+    for s in rng.choice(B, 24, replace=False):
+        q = op.sample_state(0, 0, 40, int(s))
+        np.testing.assert_array_equal(out["x_rand"][s].astype(np.float64), q)
+        i, d2 = op.nearest(tree64, q)
+        if out["nn_idx"][s] != i:
+            assert op.dist2(q, tree64[out["nn_idx"][s]]) <= (1 + 1e-6) * d2
+        for k in (0, K - 1):
+            c = s * K + k
+            u = op.sample_control(0, 0, 40, int(s), k)
+            np.testing.assert_array_equal(out["child_ctrl"][c].astype(np.float64), u)
+            x, fl, fb, mm, ec = op.propagate(tree64[out["nn_idx"][s]], u)
+            if mm > 1e-5:
+                assert (out["child_flags"][c] & 1) == (fl & 1)
+            if fl & 1 and out["child_flags"][c] & 1:
+                assert np.abs(out["child_state"][c] - x).max() < 1e-4
+    # properties that hold at any size
+    assert out["nn_idx"].min() >= 0 and out["nn_idx"].max() < n0
+    keep = (out["child_flags"] & 9) == 9
+    assert out["n_inserted"] == int(keep.sum()) == int(tree["n_nodes"][0].item()) - n0
+    pl.close()
