@@ -226,6 +226,8 @@ def main():
             "best_cost_at_100ms_median": statistics.median(best100),
             "final_cost_median": statistics.median(r["cost"] for r in results),
             "iterations_per_step": float(np.mean([r["iterations"] for r in results])),
+            "phase_share": {k: sum(r["phase_ms"][i] for r in results) / sum(kern_ms)
+                            for i, k in enumerate(("nn", "propagate", "insert"))},
             "inserted_nodes_per_s": sum(r["inserted"] for r in results) / (sum(dev_ms) * 1e-3),
             "solved": sum(r["outcome"] for r in results),
         }

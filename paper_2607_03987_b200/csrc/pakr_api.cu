@@ -41,7 +41,7 @@ Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap) {
   Layout L{};
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
-  const size_t BK = (size_t)B * K, U = (BK + 31) / 32, slots = U * 32;
+  const size_t BK = (size_t)B * K, U = BK, slots = BK + 32;  // phase-B warp units hold 1..32 children
   L.states = take((size_t)cap * pl->DP * 4);
   L.actions = take((size_t)cap * 16);
   L.parents = take((size_t)cap * 4);
@@ -284,6 +284,11 @@ pakr_status launch(pakr_planner* pl, Params& P, cudaStream_t stream) {
   CUDA_TRY(pl, cudaMemsetAsync(P.ctrl, 0xFF, 16, stream));  // goal_key[2] = none
   void* args[] = {&P};
   const dim3 grid(pl->num_sms * pl->blocks_per_sm), block(kThreads);
+  // lanes per child in phase B: as many as fill the grid, at most one obstacle-share per lane
+  const long long lanes_total = (long long)grid.x * kThreads, BK = (long long)P.B * P.K;
+  int lanes = 1;
+  while (lanes < 32 && BK * lanes * 2 <= lanes_total && lanes < P.pb.n_obs) lanes *= 2;
+  P.lanes = lanes;
   CUDA_TRY(pl, cudaLaunchCooperativeKernel(pl->kernel, grid, block, args, pl->smem_bytes, stream));
   return PAKR_OK;
 }
@@ -338,6 +343,7 @@ extern "C" pakr_status pakr_plan(pakr_planner* pl, const pakr_plan_opts* o, void
   s.children = hc->iterations * BK;
   s.inserted = hc->inserted;
   s.nn_pairs = hc->nn_pairs;
+  for (int i = 0; i < 3; ++i) s.phase_ms[i] = (double)hc->phase_ns[i] * 1e-6;
   s.replans_run = hc->replans_run;
   s.replans_solved = hc->replans_solved;
   s.termination = hc->termination;

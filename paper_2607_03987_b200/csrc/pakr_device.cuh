@@ -183,44 +183,67 @@ __device__ __forceinline__ void dyn_step(const DevProblem& pb, float (&x)[DynTra
 }
 
 // ---- validity ("validity checked at each step"; P10-P13) ----------------
+// Both tests return a margin whose SIGN is exact (a difference of two fp32 values has the exact
+// sign), so "margin >= 0" / "margin > 0" decide exactly like the comparisons they replace, while
+// the min/max trees keep the per-step dependency chain short and free of predicate registers.
+
+// >= 0 iff lo <= x <= hi on every non-angle dim (closed box, P12)
 template <int DYN>
-__device__ __forceinline__ bool in_bounds(const DevProblem& pb, const float (&x)[DynTraits<DYN>::D]) {
-  bool ok = true;
+__device__ __forceinline__ float bounds_margin(const DevProblem& pb, const float (&x)[DynTraits<DYN>::D]) {
+  float m0 = __int_as_float(0x7f800000), m1 = m0;
 #pragma unroll
   for (int d = 0; d < DynTraits<DYN>::D; ++d)
-    if (d != DynTraits<DYN>::ANGLE) ok = ok && (x[d] >= pb.lo[d]) && (x[d] <= pb.hi[d]);
-  return ok;
+    if (d != DynTraits<DYN>::ANGLE) {
+      m0 = fminf(m0, x[d] - pb.lo[d]);
+      m1 = fminf(m1, pb.hi[d] - x[d]);
+    }
+  return fminf(m0, m1);
 }
 
-template <int OBS, int PD> struct ObsStride { static constexpr int value = (OBS == OBS_CIRCLE) ? 4 : 8; };
-
 // obstacles in shared memory: circle rows (cx, cy, r*r, pad); box rows (lo[3], pad, hi[3], pad)
-// (2D boxes carry lo/hi z = -inf/+inf).  Closed sets.  Lanes of a child group may each take a
-// strided subset (first, step).
+// (2D boxes carry lo/hi z = -inf/+inf).  > 0 iff the position is outside every obstacle of the
+// strided subset first, first+step, ... (closed sets, P11).  circle: |p-c|^2 - r^2; box: max over
+// axes of max(lo - p, p - hi).
 template <int OBS, int PD>
-__device__ __forceinline__ bool collision_free(const float* __restrict__ sm_obs, int n_obs,
-                                               const float* pos, int first, int step) {
-  bool hit = false;
+__device__ __forceinline__ float obstacle_margin(const float* __restrict__ sm_obs, int n_obs,
+                                                 const float* pos, int first, int step) {
+  const float4* o4 = reinterpret_cast<const float4*>(sm_obs);
+  float m0 = __int_as_float(0x7f800000), m1 = m0;
   if constexpr (OBS == OBS_CIRCLE) {
-    const float4* o4 = reinterpret_cast<const float4*>(sm_obs);
+    int o = first;
 #pragma unroll 4
-    for (int o = first; o < n_obs; o += step) {
-      const float4 c = o4[o];
-      const float dx = pos[0] - c.x, dy = pos[1] - c.y;
-      hit = hit || (fmaf(dx, dx, dy * dy) <= c.z);
+    for (; o + step < n_obs; o += 2 * step) {
+      const float4 a = o4[o], b = o4[o + step];
+      const float ax = pos[0] - a.x, ay = pos[1] - a.y, bx = pos[0] - b.x, by = pos[1] - b.y;
+      m0 = fminf(m0, fmaf(ax, ax, ay * ay) - a.z);
+      m1 = fminf(m1, fmaf(bx, bx, by * by) - b.z);
+    }
+    if (o < n_obs) {
+      const float4 a = o4[o];
+      const float ax = pos[0] - a.x, ay = pos[1] - a.y;
+      m0 = fminf(m0, fmaf(ax, ax, ay * ay) - a.z);
     }
   } else {
-    const float4* o4 = reinterpret_cast<const float4*>(sm_obs);
     const float pz = (PD == 3) ? pos[2] : 0.0f;
+    int o = first;
 #pragma unroll 4
-    for (int o = first; o < n_obs; o += step) {
-      const float4 lo = o4[2 * o], hi = o4[2 * o + 1];
-      const bool in = (pos[0] >= lo.x) && (pos[0] <= hi.x) && (pos[1] >= lo.y) && (pos[1] <= hi.y) &&
-                      (pz >= lo.z) && (pz <= hi.z);
-      hit = hit || in;
+    for (; o + step < n_obs; o += 2 * step) {
+      const float4 alo = o4[2 * o], ahi = o4[2 * o + 1], blo = o4[2 * (o + step)], bhi = o4[2 * (o + step) + 1];
+      const float ma = fmaxf(fmaxf(fmaxf(alo.x - pos[0], pos[0] - ahi.x), fmaxf(alo.y - pos[1], pos[1] - ahi.y)),
+                             fmaxf(alo.z - pz, pz - ahi.z));
+      const float mb = fmaxf(fmaxf(fmaxf(blo.x - pos[0], pos[0] - bhi.x), fmaxf(blo.y - pos[1], pos[1] - bhi.y)),
+                             fmaxf(blo.z - pz, pz - bhi.z));
+      m0 = fminf(m0, ma);
+      m1 = fminf(m1, mb);
+    }
+    if (o < n_obs) {
+      const float4 alo = o4[2 * o], ahi = o4[2 * o + 1];
+      const float ma = fmaxf(fmaxf(fmaxf(alo.x - pos[0], pos[0] - ahi.x), fmaxf(alo.y - pos[1], pos[1] - ahi.y)),
+                             fmaxf(alo.z - pz, pz - ahi.z));
+      m0 = fminf(m0, ma);
     }
   }
-  return !hit;
+  return fminf(m0, m1);
 }
 
 template <int PD>

@@ -31,6 +31,7 @@ struct Ctrl {  // device control block (in the workspace)
   unsigned long long goal_key[2];
   unsigned long long t_start_ns, t_first_ns, t_end_ns;
   long long iterations, inserted, nn_pairs;
+  unsigned long long phase_ns[3];  // leader's time in NN / propagate / insert incl. the grid sync after each
   int n_nodes, stop;
   int path_len, solved;
   float best_cost;
@@ -61,6 +62,7 @@ struct Params {
   int r0, it0;
   float c_best0;
   int early_exit;
+  int lanes;                     // lanes per child in phase B: 1, 2, 4, 8, 16 or 32
   int* n_nodes_io;               // expand_step: tree size in/out (else NULL: start from the root)
   // expand_step debug outputs (NULL in pakr_plan)
   float* dbg_x_rand; int* dbg_nn_idx; float* dbg_nn_d2; float* dbg_child_state; float* dbg_child_ctrl;
@@ -206,25 +208,34 @@ __device__ __forceinline__ void nn_phase(const Params& P, int n, uint32_t r, uin
 }
 
 // ---- phase B: controls, propagation, validity, prune, goal flag, per-warp compaction ------------
-template <int DYN, int OBS>
+// L lanes share one child: each integrates the same edge (replicated, registers only) and tests a
+// strided 1/L of the obstacles; the group's verdict is one ballot.  L is chosen per launch so that
+// B*K*L lanes just fill the grid: few children => short per-step latency chains instead of idle SMs.
+template <int L> struct GroupMask { static constexpr unsigned value = 0xffffffffu / ((1u << L) - 1u); };
+template <> struct GroupMask<32> { static constexpr unsigned value = 1u; };
+
+template <int DYN, int OBS, int L>
 __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t it, float c_best,
                                            const float* sm_obs) {
   using T = DynTraits<DYN>;
   constexpr int D = T::D, M = T::M, DP = T::DP, PD = T::PD;
+  constexpr int CPW = 32 / L;                      // children per warp
+  constexpr unsigned GM = GroupMask<L>::value;     // bit at the first lane of every group
   const DevProblem& pb = P.pb;
   const int lane = threadIdx.x & 31;
+  const int sub = lane % L, ci = lane / L;
   const int W = gridDim.x * kWarps;
   const int gw = blockIdx.x * kWarps + (threadIdx.x >> 5);
   const int BK = P.B * P.K;
-  const int U = (BK + 31) / 32;
+  const int U = (BK + CPW - 1) / CPW;
   for (int u = gw; u < U; u += W) {
-    const int c = u * 32 + lane;
+    const int c = u * CPW + ci;
     const bool active = c < BK;
     const int s = active ? c / P.K : 0;
     const int k = active ? c - s * P.K : 0;
     const unsigned long long key = __ldcg(&P.nn_key[s]);
     const int parent = (int)(unsigned)(key & 0xffffffffu);
-    if (active && k == 0) {
+    if (active && k == 0 && sub == 0) {
       if (P.dbg_nn_idx) P.dbg_nn_idx[s] = parent;
       if (P.dbg_nn_d2) P.dbg_nn_d2[s] = __uint_as_float((unsigned)(key >> 32));
     }
@@ -242,7 +253,10 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
     }
     const float parent_cost = __ldcg(&P.costs[parent]);
     sample_control<M>(pb, P.seed, r, it, (uint32_t)s, (uint32_t)k, ctl);
-    bool inb = active, cf = active;
+    // margins: > 0 means still valid.  bm: state box (same in every lane of the group); om: this
+    // lane's share of the obstacles.  Inactive lanes start dead.
+    float bm = active ? __int_as_float(0x7f800000) : -1.0f;
+    float om = bm;
     float length = 0.0f;
     for (int j = 0; j < pb.S; ++j) {
       float px[PD];
@@ -255,10 +269,23 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
         for (int a = 0; a < PD; ++a) seg = fmaf(x[a] - px[a], x[a] - px[a], seg);
         length += sqrtf(seg);
       }
-      inb = inb && in_bounds<DYN>(pb, x);
-      cf = cf && collision_free<OBS, PD>(sm_obs, pb.n_obs, x, 0, 1);
-      if (P.early_exit && !__any_sync(0xffffffffu, inb && cf)) break;
+      bm = fminf(bm, bounds_margin<DYN>(pb, x));
+      om = fminf(om, obstacle_margin<OBS, PD>(sm_obs, pb.n_obs, x, sub, L));
+      if (P.early_exit) {  // leave once every child of the warp is dead
+        unsigned dead = __ballot_sync(0xffffffffu, !(bm >= 0.0f) || !(om > 0.0f));
+#pragma unroll
+        for (int sh = 1; sh < L; sh <<= 1) dead |= dead >> sh;
+        if ((dead & GM) == GM) break;
+      }
     }
+    bool finite = true;
+#pragma unroll
+    for (int d = 0; d < D; ++d) finite = finite & (fabsf(x[d]) <= 3.4e38f);
+    const bool inb = (bm >= 0.0f) & finite;  // closed box (P12); a non-finite state is out of bounds
+    unsigned hitm = __ballot_sync(0xffffffffu, !(om > 0.0f));  // closed obstacles (P11)
+#pragma unroll
+    for (int sh = 1; sh < L; sh <<= 1) hitm |= hitm >> sh;
+    const bool cf = !((hitm >> (ci * L)) & 1u);
     if (T::ANGLE >= 0) x[T::ANGLE >= 0 ? T::ANGLE : 0] = wrap_pi(x[T::ANGLE >= 0 ? T::ANGLE : 0]);
     const float edge = (pb.cost_mode == 1) ? length : (float)pb.S * pb.dt;
     const float c_new = parent_cost + edge;
@@ -268,8 +295,8 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
     bool ing = gd <= pb.goal_r;
     if (pb.goal_angle_dim >= 0) ing = ing && (fabsf(wrap_pi(x[T::ANGLE >= 0 ? T::ANGLE : 0] - pb.goal_angle)) <= pb.goal_angle_tol);
     const bool valid = inb && cf;
-    const bool keep = valid && notpruned;
-    int flags = (valid ? 1 : 0) | (inb ? 2 : 0) | (cf ? 4 : 0) | (notpruned ? 8 : 0) | ((keep && ing) ? 16 : 0);
+    const bool keep = valid && notpruned && sub == 0;  // one lane speaks for the child
+    int flags = (valid ? 1 : 0) | (inb ? 2 : 0) | (cf ? 4 : 0) | (notpruned ? 8 : 0) | ((valid && notpruned && ing) ? 16 : 0);
     const unsigned bal = __ballot_sync(0xffffffffu, keep);
     const int rank = __popc(bal & ((1u << lane) - 1u));
     if (lane == 0) P.unit_count[u] = __popc(bal);
@@ -284,16 +311,16 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
 #pragma unroll
     for (int d = 0; d < DP; ++d) xs[d] = d < D ? x[d] : 0.0f;
     if (keep) {
-      const size_t slot = (size_t)u * 32 + rank;
+      const size_t slot = (size_t)u * CPW + rank;
       float4* dst = reinterpret_cast<float4*>(P.scr_state + slot * DP);
 #pragma unroll
       for (int v = 0; v < DP / 4; ++v) __stcg(dst + v, make_float4(xs[4 * v], xs[4 * v + 1], xs[4 * v + 2], xs[4 * v + 3]));
       __stcg(reinterpret_cast<float4*>(P.scr_ctrl) + slot, cv);
       __stcg(&P.scr_cost[slot], c_new);
       __stcg(&P.scr_parent[slot], parent);
-      __stcg(&P.scr_flags[slot], flags | (lane << 8));
+      __stcg(&P.scr_flags[slot], flags | (ci << 8));
     }
-    if (active && P.dbg_child_flags) {
+    if (active && sub == 0 && P.dbg_child_flags) {
       P.dbg_child_flags[c] = flags;
       if (P.dbg_child_cost) P.dbg_child_cost[c] = c_new;
       if (P.dbg_child_ctrl) reinterpret_cast<float4*>(P.dbg_child_ctrl)[c] = cv;
@@ -308,14 +335,14 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
 // ---- phase C: ordered insert at the tree tail, goal winner (Alg. 1 l.13-15; P19, P20) ----
 // Returns the number of survivors of this iteration (identical in every thread of the grid).
 template <int DYN>
-__device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, int* sm_pref) {
+__device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, int cpw, int* sm_pref) {
   using T = DynTraits<DYN>;
   constexpr int DP = T::DP;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int W = gridDim.x * kWarps;
   const int gw = blockIdx.x * kWarps + warp;
   const int BK = P.B * P.K;
-  const int U = (BK + 31) / 32;
+  const int U = (BK + cpw - 1) / cpw;  // warp units of phase B (cpw children each)
   // exclusive prefix of the per-unit counts at chunk granularity, redundantly in every CTA
   const int cpt = (U + kThreads - 1) / kThreads;  // units per thread-chunk
   int mine = 0;
@@ -349,7 +376,7 @@ __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, i
     const int cnt = (int)__ldcg(&P.unit_count[u]);
     const int pos = off + lane;
     if (lane < cnt && pos < room) {
-      const size_t slot = (size_t)u * 32 + lane;
+      const size_t slot = (size_t)u * cpw + lane;
       const int node = n + pos;
       const float4* src = reinterpret_cast<const float4*>(P.scr_state + slot * DP);
       float4* dst = reinterpret_cast<float4*>(P.states + (size_t)node * DP);
@@ -362,7 +389,7 @@ __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, i
       const int fl = __ldcg(&P.scr_flags[slot]);
       if (fl & 16)  // goal child: min cost, ties -> lowest node id == lowest child index
         atomicMin(&P.ctrl->goal_key[gslot], ((unsigned long long)__float_as_uint(cost) << 32) | (unsigned)node);
-      if (P.dbg_child_flags) P.dbg_child_flags[u * 32 + (fl >> 8)] |= 32;
+      if (P.dbg_child_flags) P.dbg_child_flags[u * cpw + (fl >> 8)] |= 32;
     }
   }
   // reset the NN keys for the next iteration
@@ -428,6 +455,7 @@ __global__ void __launch_bounds__(kThreads, 2) pakr_loop_kernel(const __grid_con
   int n = P.n_nodes_io ? __ldcg(P.n_nodes_io) : 1;
   int solved_any = 0, replans_solved = 0, replans_run = 0, termination = 0;
   long long iterations = 0, inserted = 0, nn_pairs = 0;
+  unsigned long long ph0 = 0, ph1 = 0, ph2 = 0, tp = t_start;
   bool stop = false;
 
   for (int r = P.r0; r < P.r0 + P.n_replans && !stop; ++r) {
@@ -440,20 +468,30 @@ __global__ void __launch_bounds__(kThreads, 2) pakr_loop_kernel(const __grid_con
       if (P.pb.unit_weights) nn_phase<DYN, true>(P, n, (uint32_t)r, (uint32_t)it, my_tile, my_bar, par0, par1);
       else nn_phase<DYN, false>(P, n, (uint32_t)r, (uint32_t)it, my_tile, my_bar, par0, par1);
       grid.sync();
+      if (leader) { const unsigned long long t = globaltimer_ns(); ph0 += t - tp; tp = t; }
       // phase B
-      prop_phase<DYN, OBS>(P, (uint32_t)r, (uint32_t)it, c_best, sm_obs);
+      switch (P.lanes) {
+        case 2: prop_phase<DYN, OBS, 2>(P, (uint32_t)r, (uint32_t)it, c_best, sm_obs); break;
+        case 4: prop_phase<DYN, OBS, 4>(P, (uint32_t)r, (uint32_t)it, c_best, sm_obs); break;
+        case 8: prop_phase<DYN, OBS, 8>(P, (uint32_t)r, (uint32_t)it, c_best, sm_obs); break;
+        case 16: prop_phase<DYN, OBS, 16>(P, (uint32_t)r, (uint32_t)it, c_best, sm_obs); break;
+        case 32: prop_phase<DYN, OBS, 32>(P, (uint32_t)r, (uint32_t)it, c_best, sm_obs); break;
+        default: prop_phase<DYN, OBS, 1>(P, (uint32_t)r, (uint32_t)it, c_best, sm_obs); break;
+      }
       // goal-key slots alternate over the whole launch (not per replan): the other slot was last
       // read before the previous grid sync and is next written after the following one
       const int slot = (int)(iterations & 1);
       if (leader) P.ctrl->goal_key[slot ^ 1] = kKeyNone;
       grid.sync();
+      if (leader) { const unsigned long long t = globaltimer_ns(); ph1 += t - tp; tp = t; }
       // phase C
-      const int total = insert_phase<DYN>(P, n, slot, sm_pref);
+      const int total = insert_phase<DYN>(P, n, slot, 32 / P.lanes, sm_pref);
       const int added = min(total, P.cap - n);
       if (leader && P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) P.ctrl->stop = 1;
       __threadfence();
       fence_proxy_async();  // tree rows written with st.global are read next by TMA (async proxy)
       grid.sync();
+      if (leader) { const unsigned long long t = globaltimer_ns(); ph2 += t - tp; tp = t; }
       fence_proxy_async();
       nn_pairs += (long long)P.B * n;  // (query, node) pairs the scan of this iteration evaluated
       n += added;
@@ -496,6 +534,7 @@ __global__ void __launch_bounds__(kThreads, 2) pakr_loop_kernel(const __grid_con
     c->iterations = iterations;
     c->inserted = inserted;
     c->nn_pairs = nn_pairs;
+    c->phase_ns[0] = ph0; c->phase_ns[1] = ph1; c->phase_ns[2] = ph2;
     c->n_nodes = n;
     c->solved = solved_any;
     c->best_cost = c_best;

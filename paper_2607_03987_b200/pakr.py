@@ -79,7 +79,7 @@ class _PlanOpts(C.Structure):
 class _Stats(C.Structure):
     _fields_ = [("iterations", C.c_int64), ("children", C.c_int64), ("inserted", C.c_int64), ("nn_pairs", C.c_int64),
                 ("replans_run", C.c_int32), ("replans_solved", C.c_int32), ("termination", C.c_int32),
-                ("first_solution_ms", C.c_double), ("device_ms", C.c_double),
+                ("first_solution_ms", C.c_double), ("device_ms", C.c_double), ("phase_ms", C.c_double * 3),
                 ("replan_cost", C.c_float * MAX_REPLAN_STATS), ("replan_nodes", C.c_int32 * MAX_REPLAN_STATS),
                 ("replan_iters", C.c_int32 * MAX_REPLAN_STATS), ("replan_end_ms", C.c_double * MAX_REPLAN_STATS)]
 
@@ -221,7 +221,7 @@ class Planner:
                     final_tree_nodes=int(res.final_tree_nodes), iterations=int(s.iterations), children=int(s.children),
                     inserted=int(s.inserted), nn_pairs=int(s.nn_pairs), replans_run=int(s.replans_run), replans_solved=int(s.replans_solved),
                     termination=int(s.termination), first_solution_ms=float(s.first_solution_ms),
-                    device_ms=float(s.device_ms), replan_cost=np.array(s.replan_cost[:R], np.float32),
+                    device_ms=float(s.device_ms), phase_ms=[float(v) for v in s.phase_ms], replan_cost=np.array(s.replan_cost[:R], np.float32),
                     replan_nodes=np.array(s.replan_nodes[:R], np.int64), replan_iters=np.array(s.replan_iters[:R], np.int64),
                     replan_end_ms=np.array(s.replan_end_ms[:R], np.float64))
 
