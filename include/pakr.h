@@ -132,7 +132,8 @@ typedef struct {
   int32_t termination;     /* 0 all replans run, 1 time budget */
   double first_solution_ms;/* device time from kernel start to the end of the first solved replan; -1 if none */
   double device_ms;        /* device time of the whole loop (%globaltimer) */
-  double phase_ms[3];      /* block 0's time in NN / propagate / insert, each incl. the grid sync after it */
+  double phase_ms[3];      /* CTA 0's time in: NN scan of the newly appended rows / propagate (with the next
+                              iteration's NN look-ahead scan beside it) / insert; each incl. its grid barrier */
   /* first PAKR_MAX_REPLAN_STATS replans: */
   float replan_cost[PAKR_MAX_REPLAN_STATS];   /* c_best after the replan (+INF before any solution) */
   int32_t replan_nodes[PAKR_MAX_REPLAN_STATS];/* tree size at its end */

@@ -1,6 +1,7 @@
 // pakr_api.cu -- host side of the C ABI declared in include/pakr.h.
 // Validates the problem, carves the caller's workspace, launches the persistent cooperative
 // kernel of pakr_kernel.cuh and copies the small result block back.  No compute happens here.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -18,6 +19,8 @@ struct pakr_planner {
   int D = 0, M = 0, PD = 0, DP = 0;
   DevProblem pb{};
   float* d_obstacles = nullptr;
+  uint32_t* d_grid_cells = nullptr;
+  uint16_t* d_grid_list = nullptr;
   int num_sms = 0, blocks_per_sm = 0;
   size_t smem_bytes = 0;
   const void* kernel = nullptr;
@@ -46,7 +49,7 @@ Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap) {
   L.actions = take((size_t)cap * 16);
   L.parents = take((size_t)cap * 4);
   L.costs = take((size_t)cap * 4);
-  L.nn_key = take((size_t)B * 8);
+  L.nn_key = take((size_t)B * 16);  // two iterations in flight
   L.unit_count = take(U * 4);
   L.scr_state = take(slots * pl->DP * 4);
   L.scr_ctrl = take(slots * 16);
@@ -87,7 +90,76 @@ size_t tile_floats(int DP) { return (size_t)(DP == 4 ? 256 : DP == 8 ? 128 : 64)
 size_t smem_for(const pakr_planner* pl) {
   const int os = pl->obs == OBS_CIRCLE ? 4 : 8;
   return kWarps * 2 * tile_floats(pl->DP) * 4 + kWarps * 2 * 8 + (kThreads + kWarps + 8) * 4 +
-         (size_t)pl->pb.n_obs * os * 4 + 16;
+         (size_t)((pl->pb.n_obs * os + 3) & ~3) * 4 + (size_t)pl->pb.g_cells * 4 + (size_t)pl->pb.g_list * 2 + 16;
+}
+
+// Obstacle broad phase: a uniform grid over the position box with a CSR list of obstacle ids per cell.
+// An obstacle is registered in every cell its bounding box, inflated by a thousandth of a cell, touches,
+// using the same clamp(floor((x - org) * inv)) the kernel applies to a position; that function is monotone
+// per axis, so a position inside an obstacle always lands in a cell that lists it (exact culling).
+struct HostGrid {
+  bool on = false;
+  int dim[3] = {1, 1, 1};
+  float org[3] = {0, 0, 0}, inv[3] = {0, 0, 0};
+  std::vector<uint32_t> cells;
+  std::vector<uint16_t> list;
+};
+
+HostGrid build_grid(const pakr_problem* p, int obs_kind) {
+  HostGrid g;
+  const int gd = obs_kind == OBS_CIRCLE ? 2 : p->pos_dim;
+  if (p->n_obstacles < 4) return g;  // nothing to cull
+  for (int a = 0; a < gd; ++a)
+    if (!std::isfinite(p->state_lo[a]) || !std::isfinite(p->state_hi[a]) || !(p->state_hi[a] > p->state_lo[a])) return g;
+  for (int res = (gd == 2 ? 32 : 16); res >= 4; res /= 2) {
+    float cell[3];
+    for (int a = 0; a < 3; ++a) g.dim[a] = 1;
+    for (int a = 0; a < gd; ++a) {
+      g.dim[a] = res;
+      g.org[a] = p->state_lo[a];
+      cell[a] = (p->state_hi[a] - p->state_lo[a]) / (float)res;
+      g.inv[a] = 1.0f / cell[a];
+    }
+    auto cell_of = [&](float x, int a) {
+      const float f = std::floor((x - g.org[a]) * g.inv[a]);
+      int c = f >= 2.0e9f ? 2000000000 : f <= -2.0e9f ? -2000000000 : (int)f;
+      return std::min(std::max(c, 0), g.dim[a] - 1);
+    };
+    const int ncells = g.dim[0] * g.dim[1] * g.dim[2];
+    std::vector<std::vector<uint16_t>> per(ncells);
+    for (int o = 0; o < p->n_obstacles; ++o) {
+      int c0[3] = {0, 0, 0}, c1[3] = {0, 0, 0};
+      for (int a = 0; a < gd; ++a) {
+        float lo, hi;
+        if (obs_kind == OBS_CIRCLE) {
+          const float* c = p->obstacles + (size_t)o * 3;
+          lo = c[a] - std::fabs(c[2]); hi = c[a] + std::fabs(c[2]);
+        } else {
+          lo = p->obstacles[(size_t)o * 2 * p->pos_dim + a];
+          hi = p->obstacles[(size_t)o * 2 * p->pos_dim + p->pos_dim + a];
+        }
+        const float pad = 1e-3f * cell[a] + 1e-5f * (std::fabs(lo) + std::fabs(hi));
+        c0[a] = cell_of(lo - pad, a);
+        c1[a] = cell_of(hi + pad, a);
+      }
+      for (int z = c0[2]; z <= c1[2]; ++z)
+        for (int y = c0[1]; y <= c1[1]; ++y)
+          for (int x = c0[0]; x <= c1[0]; ++x) per[x + g.dim[0] * (y + g.dim[1] * z)].push_back((uint16_t)o);
+    }
+    size_t total = 0, worst = 0;
+    for (auto& v : per) { total += v.size(); worst = std::max(worst, v.size()); }
+    if (worst > 255 || total > 24576) continue;  // coarser grid
+    g.cells.resize(ncells);
+    g.list.clear();
+    for (int c = 0; c < ncells; ++c) {
+      g.cells[c] = ((uint32_t)g.list.size() << 8) | (uint32_t)per[c].size();
+      g.list.insert(g.list.end(), per[c].begin(), per[c].end());
+    }
+    if (g.list.empty()) g.list.push_back(0);
+    g.on = true;
+    return g;
+  }
+  return g;
 }
 
 pakr_status fail(pakr_planner* pl, pakr_status st, const std::string& msg) {
@@ -142,6 +214,11 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
   if (p->n_obstacles < 0 || p->n_obstacles > 1024 || (p->n_obstacles > 0 && !p->obstacles))
     return fail(nullptr, PAKR_ERR_INVALID_ARG, "n_obstacles must be in [0,1024] with a non-null array");
   const int D = p->state_dim, M = p->control_dim, PD = p->pos_dim;
+  {
+    const int per = (obs == OBS_CIRCLE) ? 3 : 2 * PD;
+    for (int i = 0; i < p->n_obstacles * per; ++i)
+      if (!std::isfinite(p->obstacles[i])) return fail(nullptr, PAKR_ERR_INVALID_ARG, "obstacle coordinates must be finite");
+  }
   const int angle = dyn == DYN_UNI2 ? 2 : dyn == DYN_QUAD ? 8 : -1;
   for (int d = 0; d < D; ++d) {
     const bool is_angle = p->dim_kind[d] == PAKR_DIM_ANGLE;
@@ -220,6 +297,22 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
   e = cudaMemcpy(pl->d_obstacles, rows.data(), rows.size() * 4, cudaMemcpyHostToDevice);
   if (e != cudaSuccess) return bail(PAKR_ERR_CUDA, std::string("cudaMemcpy: ") + cudaGetErrorString(e));
   pb.obstacles = pl->d_obstacles;
+  {
+    const HostGrid g = build_grid(p, obs);
+    pb.grid_on = g.on ? 1 : 0;
+    if (g.on) {
+      for (int a = 0; a < 3; ++a) { pb.gdim[a] = g.dim[a]; pb.gorg[a] = g.org[a]; pb.ginv[a] = g.inv[a]; }
+      pb.g_cells = (int)g.cells.size();
+      pb.g_list = (int)g.list.size();
+      e = cudaMalloc(&pl->d_grid_cells, g.cells.size() * 4);
+      if (e == cudaSuccess) e = cudaMalloc(&pl->d_grid_list, g.list.size() * 2);
+      if (e == cudaSuccess) e = cudaMemcpy(pl->d_grid_cells, g.cells.data(), g.cells.size() * 4, cudaMemcpyHostToDevice);
+      if (e == cudaSuccess) e = cudaMemcpy(pl->d_grid_list, g.list.data(), g.list.size() * 2, cudaMemcpyHostToDevice);
+      if (e != cudaSuccess) return bail(PAKR_ERR_CUDA, std::string("obstacle grid upload: ") + cudaGetErrorString(e));
+      pb.grid_cells = pl->d_grid_cells;
+      pb.grid_list = pl->d_grid_list;
+    }
+  }
   pl->kernel = select_kernel(dyn, obs);
   pl->smem_bytes = smem_for(pl);
   e = cudaFuncSetAttribute(pl->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes);
@@ -236,6 +329,8 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
 extern "C" void pakr_destroy(pakr_planner* pl) {
   if (!pl) return;
   if (pl->d_obstacles) cudaFree(pl->d_obstacles);
+  if (pl->d_grid_cells) cudaFree(pl->d_grid_cells);
+  if (pl->d_grid_list) cudaFree(pl->d_grid_list);
   if (pl->h_pinned) cudaFreeHost(pl->h_pinned);
   delete pl;
 }
@@ -279,16 +374,11 @@ void fill_common(const pakr_planner* pl, Params& P, const Layout& L, char* ws, i
 // memset of the control words + one cooperative launch; everything on `stream`
 pakr_status launch(pakr_planner* pl, Params& P, cudaStream_t stream) {
   CUDA_TRY(pl, cudaSetDevice(pl->device));
-  CUDA_TRY(pl, cudaMemsetAsync(P.nn_key, 0xFF, (size_t)P.B * 8, stream));
+  CUDA_TRY(pl, cudaMemsetAsync(P.nn_key, 0xFF, (size_t)P.B * 16, stream));
   CUDA_TRY(pl, cudaMemsetAsync(P.ctrl, 0, sizeof(Ctrl), stream));
   CUDA_TRY(pl, cudaMemsetAsync(P.ctrl, 0xFF, 16, stream));  // goal_key[2] = none
   void* args[] = {&P};
   const dim3 grid(pl->num_sms * pl->blocks_per_sm), block(kThreads);
-  // lanes per child in phase B: as many as fill the grid, at most one obstacle-share per lane
-  const long long lanes_total = (long long)grid.x * kThreads, BK = (long long)P.B * P.K;
-  int lanes = 1;
-  while (lanes < 32 && BK * lanes * 2 <= lanes_total && lanes < P.pb.n_obs) lanes *= 2;
-  P.lanes = lanes;
   CUDA_TRY(pl, cudaLaunchCooperativeKernel(pl->kernel, grid, block, args, pl->smem_bytes, stream));
   return PAKR_OK;
 }

@@ -44,6 +44,13 @@ struct DevProblem {
   int unit_weights;                    // all w == 1: skip the weight multiply in the NN scan
   int n_obs;
   const float* obstacles;              // DEVICE, rows of OBS_STRIDE floats
+  // obstacle broad phase: uniform grid over the position box, CSR lists of obstacle ids per cell
+  int grid_on;                         // 0: test every obstacle
+  int gdim[3];                         // cells per axis (gdim[2] == 1 for circle / cylinder fields)
+  float gorg[3], ginv[3];              // cell(x) = clamp(floor((x - gorg) * ginv), 0, gdim - 1)
+  int g_cells, g_list;                 // number of cells, total list entries
+  const uint32_t* grid_cells;          // DEVICE [g_cells]: (list offset << 8) | count
+  const uint16_t* grid_list;           // DEVICE [g_list] obstacle ids
 };
 
 // ---- Philox4x32-10 ---------------------------------------------------------------------------
@@ -244,6 +251,47 @@ __device__ __forceinline__ float obstacle_margin(const float* __restrict__ sm_ob
     }
   }
   return fminf(m0, m1);
+}
+
+// Margin of one obstacle (same formulas as obstacle_margin above).
+template <int OBS, int PD>
+__device__ __forceinline__ float one_obstacle_margin(const float4* __restrict__ o4, int o, const float* pos) {
+  if constexpr (OBS == OBS_CIRCLE) {
+    const float4 a = o4[o];
+    const float ax = pos[0] - a.x, ay = pos[1] - a.y;
+    return fmaf(ax, ax, ay * ay) - a.z;
+  } else {
+    const float pz = (PD == 3) ? pos[2] : 0.0f;
+    const float4 alo = o4[2 * o], ahi = o4[2 * o + 1];
+    return fmaxf(fmaxf(fmaxf(alo.x - pos[0], pos[0] - ahi.x), fmaxf(alo.y - pos[1], pos[1] - ahi.y)),
+                 fmaxf(alo.z - pz, pz - ahi.z));
+  }
+}
+
+// Broad phase (exact): only the obstacles registered in the grid cell of `pos` can contain it, because the
+// host registers an obstacle in every cell its (slightly inflated) bounding box touches and cell() is
+// monotone per axis; positions outside the box clamp into the border cells, whose lists hold everything
+// that sticks out of the box.  The SIGN of the returned margin equals that of the full scan.
+template <int OBS, int PD>
+__device__ __forceinline__ float obstacle_margin_grid(const DevProblem& pb, const uint32_t* __restrict__ sm_cells,
+                                                      const uint16_t* __restrict__ sm_list,
+                                                      const float* __restrict__ sm_obs, const float* pos) {
+  constexpr int GD = (OBS == OBS_CIRCLE) ? 2 : PD;  // circles / vertical cylinders: xy grid
+  int cell = 0, mul = 1;
+#pragma unroll
+  for (int a = 0; a < GD; ++a) {
+    int c = __float2int_rd((pos[a] - pb.gorg[a]) * pb.ginv[a]);
+    c = min(max(c, 0), pb.gdim[a] - 1);
+    cell += c * mul;
+    mul *= pb.gdim[a];
+  }
+  const uint32_t hdr = sm_cells[cell];
+  const int cnt = (int)(hdr & 0xffu);
+  const uint16_t* lst = sm_list + (hdr >> 8);
+  const float4* o4 = reinterpret_cast<const float4*>(sm_obs);
+  float m = __int_as_float(0x7f800000);
+  for (int k = 0; k < cnt; ++k) m = fminf(m, one_obstacle_margin<OBS, PD>(o4, (int)lst[k], pos));
+  return m;
 }
 
 template <int PD>

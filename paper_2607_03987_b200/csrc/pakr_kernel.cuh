@@ -1,15 +1,20 @@
 // pakr_kernel.cuh -- the persistent cooperative kernel that runs Alg. 1 on device.
 //
-// One launch = the whole AO-x loop (or one iteration for pakr_expand_step).  Per iteration:
-//   phase A  NN scan        (Alg. 1 l.6-7)   warps own 32*Q queries in registers, tree tiles are
+// One launch = the whole AO-x loop (or one iteration for pakr_expand_step).  Per iteration i:
+//   phase A' NN tail scan   (Alg. 1 l.6-7)   finishes NN(i) over the nodes appended by iteration i-1;
+//                                             warps own 32*Q queries in registers, tree tiles are
 //                                             streamed into shared memory by TMA bulk copies
 //   -- grid sync --
-//   phase B  propagate      (Alg. 1 l.8-12)  one lane per child, state in registers, obstacles in
-//                                             shared memory, per-warp ballot compaction
+//   phase X  propagate(i)   (Alg. 1 l.8-12)  one lane per child, state in registers, obstacles and
+//                                             their broad-phase grid in shared memory, ballot compaction
+//          + NN(i+1) over the frozen snapshot [0, n_i) on the warps that have no child unit
+//            (speculative: dropped when iteration i ends the replan)
 //   -- grid sync --
 //   phase C  insert + goal  (Alg. 1 l.13-15) ordered prefix over the per-warp counts, coalesced
 //                                             append at the tree tail, goal winner by atomicMin
 //   -- grid sync --
+// NN(i+1) = min(scan of [0, n_i) done in X(i), scan of [n_i, n_{i+1}) done in A'(i+1)): the snapshot a
+// batch sees is exactly the tree after the previous batch's inserts.
 // Loop state (n, c_best, replan, iteration) is replicated in registers of every thread and
 // recomputed from the same global values, so no broadcast step is needed.
 #pragma once
@@ -47,7 +52,7 @@ struct Params {
   // tree
   float* states; float* actions; int* parents; float* costs;
   // per-iteration work buffers
-  unsigned long long* nn_key;  // [B]   (d2 bits << 32) | node, combined with atomicMin
+  unsigned long long* nn_key;  // [2][B] (d2 bits << 32) | node, combined with atomicMin; two iterations in flight
   unsigned* unit_count;        // [ceil(B*K/32)] survivors per warp unit
   float* scr_state; float* scr_ctrl; float* scr_cost; int* scr_parent; int* scr_flags;
   Ctrl* ctrl;
@@ -62,7 +67,6 @@ struct Params {
   int r0, it0;
   float c_best0;
   int early_exit;
-  int lanes;                     // lanes per child in phase B: 1, 2, 4, 8, 16 or 32
   int* n_nodes_io;               // expand_step: tree size in/out (else NULL: start from the root)
   // expand_step debug outputs (NULL in pakr_plan)
   float* dbg_x_rand; int* dbg_nn_idx; float* dbg_nn_d2; float* dbg_child_state; float* dbg_child_ctrl;
@@ -126,15 +130,20 @@ __device__ __forceinline__ float dist2(const DevProblem& pb, const float (&q)[Dy
   return acc;
 }
 
-// ---- phase A: nearest neighbour over the frozen snapshot [0, n) (Alg. 1 l.6-7) ----
+// ---- NN scan of tree rows [nbeg, nend) for the queries of iteration `it` (Alg. 1 l.6-7) ----
+// Warps vw = 0..vcount-1 take part (vw < 0: this warp sits out).  Partial minima are merged into
+// key[s] with a 64-bit atomicMin, so any split of the rows over warps / phases gives the same result.
 template <int DYN, bool UNIT_W>
-__device__ __forceinline__ void nn_phase(const Params& P, int n, uint32_t r, uint32_t it, float* sm_tile,
+__device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, uint32_t r, uint32_t it,
+                                         unsigned long long* key, int vw, int vcount, float* sm_tile,
                                          uint64_t* sm_bar, uint32_t& par0, uint32_t& par1) {
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
   constexpr int TILE = TileCfg<DYN>::TILE, TF = TileCfg<DYN>::TILE_FLOATS;
   const int lane = threadIdx.x & 31;
-  const int W = gridDim.x * kWarps;
-  const int gw = blockIdx.x * kWarps + (threadIdx.x >> 5);
+  const int n = nend - nbeg;
+  if (vw < 0 || n <= 0) return;
+  const int W = vcount;
+  const int gw = vw;
   const int G = (P.B + 32 * kQ - 1) / (32 * kQ);  // query groups
   int R = W / G;                                  // node ranges per group
   if (R < 1) R = 1;
@@ -144,8 +153,8 @@ __device__ __forceinline__ void nn_phase(const Params& P, int n, uint32_t r, uin
   const int U = G * Reff;
   for (int u = gw; u < U; u += W) {
     const int g = u / Reff, rr = u - g * Reff;
-    const int beg = rr * len;
-    const int end = min(n, beg + len);
+    const int beg = nbeg + rr * len;
+    const int end = min(nend, beg + len);
     float q[kQ][D];
     float best[kQ];
     int bidx[kQ];
@@ -155,7 +164,7 @@ __device__ __forceinline__ void nn_phase(const Params& P, int n, uint32_t r, uin
       sample_state<D>(P.pb, P.seed, r, it, (uint32_t)s, q[j]);
       best[j] = __int_as_float(0x7f800000);
       bidx[j] = 0x7fffffff;
-      if (P.dbg_x_rand && rr == 0 && s < P.B) {
+      if (P.dbg_x_rand && rr == 0 && nbeg == 0 && s < P.B) {
 #pragma unroll
         for (int d = 0; d < DP; ++d) P.dbg_x_rand[(size_t)s * DP + d] = d < D ? q[j][d] : 0.0f;
       }
@@ -199,45 +208,42 @@ __device__ __forceinline__ void nn_phase(const Params& P, int n, uint32_t r, uin
     for (int j = 0; j < kQ; ++j) {
       const int s = g * 32 * kQ + j * 32 + lane;
       if (s < P.B && bidx[j] != 0x7fffffff) {
-        const unsigned long long key =
+        const unsigned long long kv =
             ((unsigned long long)__float_as_uint(best[j]) << 32) | (unsigned)bidx[j];
-        atomicMin(&P.nn_key[s], key);  // d2 >= 0: uint order == float order; ties -> lowest node
+        atomicMin(&key[s], kv);  // d2 >= 0: uint order == float order; ties -> lowest node
       }
     }
   }
 }
 
-// ---- phase B: controls, propagation, validity, prune, goal flag, per-warp compaction ------------
-// L lanes share one child: each integrates the same edge (replicated, registers only) and tests a
-// strided 1/L of the obstacles; the group's verdict is one ballot.  L is chosen per launch so that
-// B*K*L lanes just fill the grid: few children => short per-step latency chains instead of idle SMs.
-template <int L> struct GroupMask { static constexpr unsigned value = 0xffffffffu / ((1u << L) - 1u); };
-template <> struct GroupMask<32> { static constexpr unsigned value = 1u; };
-
-template <int DYN, int OBS, int L>
+// ---- propagate: controls, RK4 edge, validity, prune, goal flag, per-warp compaction (Alg. 1 l.8-12) ----
+// One lane per child, state in registers for the whole edge.  Warp unit u = children [32u, 32u+32) is taken
+// by the warp whose prop-order index pw == u (mod W); pw runs across CTAs first, so few children spread
+// over all SMs.  Survivors go to the scratch rows of the unit, packed by ballot rank.
+template <int DYN, int OBS>
 __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t it, float c_best,
-                                           const float* sm_obs) {
+                                           const unsigned long long* key, bool root_only, int pw, int W,
+                                           const float* sm_obs, const uint32_t* sm_cells,
+                                           const uint16_t* sm_list) {
   using T = DynTraits<DYN>;
   constexpr int D = T::D, M = T::M, DP = T::DP, PD = T::PD;
-  constexpr int CPW = 32 / L;                      // children per warp
-  constexpr unsigned GM = GroupMask<L>::value;     // bit at the first lane of every group
   const DevProblem& pb = P.pb;
   const int lane = threadIdx.x & 31;
-  const int sub = lane % L, ci = lane / L;
-  const int W = gridDim.x * kWarps;
-  const int gw = blockIdx.x * kWarps + (threadIdx.x >> 5);
   const int BK = P.B * P.K;
-  const int U = (BK + CPW - 1) / CPW;
-  for (int u = gw; u < U; u += W) {
-    const int c = u * CPW + ci;
+  const int U = (BK + 31) / 32;
+  for (int u = pw; u < U; u += W) {
+    const int c = u * 32 + lane;
     const bool active = c < BK;
     const int s = active ? c / P.K : 0;
     const int k = active ? c - s * P.K : 0;
-    const unsigned long long key = __ldcg(&P.nn_key[s]);
-    const int parent = (int)(unsigned)(key & 0xffffffffu);
-    if (active && k == 0 && sub == 0) {
-      if (P.dbg_nn_idx) P.dbg_nn_idx[s] = parent;
-      if (P.dbg_nn_d2) P.dbg_nn_d2[s] = __uint_as_float((unsigned)(key >> 32));
+    int parent = 0;
+    if (!root_only) {
+      const unsigned long long kv = __ldcg(&key[s]);
+      parent = (int)(unsigned)(kv & 0xffffffffu);
+      if (active && k == 0) {
+        if (P.dbg_nn_idx) P.dbg_nn_idx[s] = parent;
+        if (P.dbg_nn_d2) P.dbg_nn_d2[s] = __uint_as_float((unsigned)(kv >> 32));
+      }
     }
     float x[D], ctl[M];
     {
@@ -253,8 +259,7 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
     }
     const float parent_cost = __ldcg(&P.costs[parent]);
     sample_control<M>(pb, P.seed, r, it, (uint32_t)s, (uint32_t)k, ctl);
-    // margins: > 0 means still valid.  bm: state box (same in every lane of the group); om: this
-    // lane's share of the obstacles.  Inactive lanes start dead.
+    // margins: bm >= 0 / om > 0 mean still valid.  Inactive lanes start dead.
     float bm = active ? __int_as_float(0x7f800000) : -1.0f;
     float om = bm;
     float length = 0.0f;
@@ -270,22 +275,15 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
         length += sqrtf(seg);
       }
       bm = fminf(bm, bounds_margin<DYN>(pb, x));
-      om = fminf(om, obstacle_margin<OBS, PD>(sm_obs, pb.n_obs, x, sub, L));
-      if (P.early_exit) {  // leave once every child of the warp is dead
-        unsigned dead = __ballot_sync(0xffffffffu, !(bm >= 0.0f) || !(om > 0.0f));
-#pragma unroll
-        for (int sh = 1; sh < L; sh <<= 1) dead |= dead >> sh;
-        if ((dead & GM) == GM) break;
-      }
+      if (pb.grid_on) om = fminf(om, obstacle_margin_grid<OBS, PD>(pb, sm_cells, sm_list, sm_obs, x));
+      else om = fminf(om, obstacle_margin<OBS, PD>(sm_obs, pb.n_obs, x, 0, 1));
+      if (P.early_exit && __all_sync(0xffffffffu, !(bm >= 0.0f) || !(om > 0.0f))) break;  // whole warp dead
     }
     bool finite = true;
 #pragma unroll
     for (int d = 0; d < D; ++d) finite = finite & (fabsf(x[d]) <= 3.4e38f);
     const bool inb = (bm >= 0.0f) & finite;  // closed box (P12); a non-finite state is out of bounds
-    unsigned hitm = __ballot_sync(0xffffffffu, !(om > 0.0f));  // closed obstacles (P11)
-#pragma unroll
-    for (int sh = 1; sh < L; sh <<= 1) hitm |= hitm >> sh;
-    const bool cf = !((hitm >> (ci * L)) & 1u);
+    const bool cf = om > 0.0f;               // closed obstacles (P11)
     if (T::ANGLE >= 0) x[T::ANGLE >= 0 ? T::ANGLE : 0] = wrap_pi(x[T::ANGLE >= 0 ? T::ANGLE : 0]);
     const float edge = (pb.cost_mode == 1) ? length : (float)pb.S * pb.dt;
     const float c_new = parent_cost + edge;
@@ -295,12 +293,12 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
     bool ing = gd <= pb.goal_r;
     if (pb.goal_angle_dim >= 0) ing = ing && (fabsf(wrap_pi(x[T::ANGLE >= 0 ? T::ANGLE : 0] - pb.goal_angle)) <= pb.goal_angle_tol);
     const bool valid = inb && cf;
-    const bool keep = valid && notpruned && sub == 0;  // one lane speaks for the child
-    int flags = (valid ? 1 : 0) | (inb ? 2 : 0) | (cf ? 4 : 0) | (notpruned ? 8 : 0) | ((valid && notpruned && ing) ? 16 : 0);
+    const bool keep = valid && notpruned;
+    const int flags = (valid ? 1 : 0) | (inb ? 2 : 0) | (cf ? 4 : 0) | (notpruned ? 8 : 0) | ((keep && ing) ? 16 : 0);
     const unsigned bal = __ballot_sync(0xffffffffu, keep);
     const int rank = __popc(bal & ((1u << lane) - 1u));
     if (lane == 0) P.unit_count[u] = __popc(bal);
-    float4 cv = make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 cv;
     {
       float t4[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
@@ -311,16 +309,16 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
 #pragma unroll
     for (int d = 0; d < DP; ++d) xs[d] = d < D ? x[d] : 0.0f;
     if (keep) {
-      const size_t slot = (size_t)u * CPW + rank;
+      const size_t slot = (size_t)u * 32 + rank;
       float4* dst = reinterpret_cast<float4*>(P.scr_state + slot * DP);
 #pragma unroll
       for (int v = 0; v < DP / 4; ++v) __stcg(dst + v, make_float4(xs[4 * v], xs[4 * v + 1], xs[4 * v + 2], xs[4 * v + 3]));
       __stcg(reinterpret_cast<float4*>(P.scr_ctrl) + slot, cv);
       __stcg(&P.scr_cost[slot], c_new);
       __stcg(&P.scr_parent[slot], parent);
-      __stcg(&P.scr_flags[slot], flags | (ci << 8));
+      __stcg(&P.scr_flags[slot], flags | (lane << 8));
     }
-    if (active && sub == 0 && P.dbg_child_flags) {
+    if (active && P.dbg_child_flags) {
       P.dbg_child_flags[c] = flags;
       if (P.dbg_child_cost) P.dbg_child_cost[c] = c_new;
       if (P.dbg_child_ctrl) reinterpret_cast<float4*>(P.dbg_child_ctrl)[c] = cv;
@@ -335,14 +333,16 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
 // ---- phase C: ordered insert at the tree tail, goal winner (Alg. 1 l.13-15; P19, P20) ----
 // Returns the number of survivors of this iteration (identical in every thread of the grid).
 template <int DYN>
-__device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, int cpw, int* sm_pref) {
+__device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, unsigned long long* key_done,
+                                            int* sm_pref) {
   using T = DynTraits<DYN>;
   constexpr int DP = T::DP;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int W = gridDim.x * kWarps;
   const int gw = blockIdx.x * kWarps + warp;
   const int BK = P.B * P.K;
-  const int U = (BK + cpw - 1) / cpw;  // warp units of phase B (cpw children each)
+  constexpr int cpw = 32;
+  const int U = (BK + cpw - 1) / cpw;  // warp units of the propagate phase (32 children each)
   // exclusive prefix of the per-unit counts at chunk granularity, redundantly in every CTA
   const int cpt = (U + kThreads - 1) / kThreads;  // units per thread-chunk
   int mine = 0;
@@ -392,8 +392,8 @@ __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, i
       if (P.dbg_child_flags) P.dbg_child_flags[u * cpw + (fl >> 8)] |= 32;
     }
   }
-  // reset the NN keys for the next iteration
-  for (int s = blockIdx.x * kThreads + threadIdx.x; s < P.B; s += gridDim.x * kThreads) P.nn_key[s] = kKeyNone;
+  // the NN keys this iteration consumed are free again: reset them for iteration i+2
+  for (int s = blockIdx.x * kThreads + threadIdx.x; s < P.B; s += gridDim.x * kThreads) key_done[s] = kKeyNone;
   return total;
 }
 
@@ -427,16 +427,22 @@ __global__ void __launch_bounds__(kThreads, 2) pakr_loop_kernel(const __grid_con
   using T = DynTraits<DYN>;
   constexpr int OS = (OBS == OBS_CIRCLE) ? 4 : 8;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  // [tiles: kWarps * 2 * TILE_FLOATS][bars: kWarps * 2][pref: kThreads + kWarps][obstacles]
+  // [tiles: kWarps * 2 * TILE_FLOATS][bars: kWarps * 2][pref: kThreads + kWarps + 8][obstacles][grid cells][grid lists]
   float* sm_tiles = reinterpret_cast<float*>(smem_raw);
   uint64_t* sm_bars = reinterpret_cast<uint64_t*>(sm_tiles + kWarps * 2 * TileCfg<DYN>::TILE_FLOATS);
   int* sm_pref = reinterpret_cast<int*>(sm_bars + kWarps * 2);
   float* sm_obs = reinterpret_cast<float*>(sm_pref + kThreads + kWarps + 8);
+  uint32_t* sm_cells = reinterpret_cast<uint32_t*>(sm_obs + ((P.pb.n_obs * OS + 3) & ~3));
+  uint16_t* sm_list = reinterpret_cast<uint16_t*>(sm_cells + P.pb.g_cells);
   cg::grid_group grid = cg::this_grid();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const bool leader = (blockIdx.x == 0 && threadIdx.x == 0);
 
   for (int i = threadIdx.x; i < P.pb.n_obs * OS; i += kThreads) sm_obs[i] = P.pb.obstacles[i];
+  if (P.pb.grid_on) {
+    for (int i = threadIdx.x; i < P.pb.g_cells; i += kThreads) sm_cells[i] = P.pb.grid_cells[i];
+    for (int i = threadIdx.x; i < P.pb.g_list; i += kThreads) sm_list[i] = P.pb.grid_list[i];
+  }
   if (lane == 0) {
     mbar_init(&sm_bars[warp * 2], 1);
     mbar_init(&sm_bars[warp * 2 + 1], 1);
@@ -448,6 +454,18 @@ __global__ void __launch_bounds__(kThreads, 2) pakr_loop_kernel(const __grid_con
   uint64_t* my_bar = sm_bars + warp * 2;
   uint32_t par0 = 0, par1 = 0;
 
+  // Warp roles.  pw orders the warps across CTAs first (warp 0 of every CTA, then warp 1, ...): propagate unit
+  // u runs on the warp with pw == u (mod W).  When the children need fewer than half of the warps, the others
+  // run the look-ahead NN scan meanwhile; otherwise every warp does both, one after the other.
+  const int W = gridDim.x * kWarps;
+  const int pw = warp * gridDim.x + blockIdx.x;
+  const int U_prop = (P.B * P.K + 31) / 32;
+  const bool split = U_prop * 2 <= W;
+  const int x_vw = split ? pw - U_prop : pw;  // < 0: propagate-only warp
+  const int x_cnt = split ? W - U_prop : W;
+  unsigned long long* const key0 = P.nn_key;
+  unsigned long long* const key1 = P.nn_key + P.B;
+
   unsigned long long t_start = 0;
   if (leader) { t_start = globaltimer_ns(); P.ctrl->t_start_ns = t_start; }
 
@@ -457,26 +475,32 @@ __global__ void __launch_bounds__(kThreads, 2) pakr_loop_kernel(const __grid_con
   long long iterations = 0, inserted = 0, nn_pairs = 0;
   unsigned long long ph0 = 0, ph1 = 0, ph2 = 0, tp = t_start;
   bool stop = false;
+  int cur = 0;  // key buffer of the current iteration
 
   for (int r = P.r0; r < P.r0 + P.n_replans && !stop; ++r) {
     if (!P.n_nodes_io) n = 1;  // Alg. 1 l.4: node 0 = (x_init, 0, -1, 0) is written once by the host
     int it = P.it0;
     int iters = 0;
     int goal_node = -1;
+    int n_scanned = 0;  // NN(it) already covers tree rows [0, n_scanned)
     for (;;) {
-      // phase A
-      if (P.pb.unit_weights) nn_phase<DYN, true>(P, n, (uint32_t)r, (uint32_t)it, my_tile, my_bar, par0, par1);
-      else nn_phase<DYN, false>(P, n, (uint32_t)r, (uint32_t)it, my_tile, my_bar, par0, par1);
-      grid.sync();
+      unsigned long long* const kcur = cur ? key1 : key0;
+      unsigned long long* const knext = cur ? key0 : key1;
+      // a fresh tree is the root alone: every query's nearest node is node 0, no scan needed
+      const bool root_only = (n == 1) && !P.n_nodes_io;
+      // phase A': rows appended since the look-ahead scan
+      if (!root_only && n_scanned < n) {
+        if (P.pb.unit_weights) nn_phase<DYN, true>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, pw, W, my_tile, my_bar, par0, par1);
+        else nn_phase<DYN, false>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, pw, W, my_tile, my_bar, par0, par1);
+        grid.sync();
+      }
       if (leader) { const unsigned long long t = globaltimer_ns(); ph0 += t - tp; tp = t; }
-      // phase B
-      switch (P.lanes) {
-        case 2: prop_phase<DYN, OBS, 2>(P, (uint32_t)r, (uint32_t)it, c_best, sm_obs); break;
-        case 4: prop_phase<DYN, OBS, 4>(P, (uint32_t)r, (uint32_t)it, c_best, sm_obs); break;
-        case 8: prop_phase<DYN, OBS, 8>(P, (uint32_t)r, (uint32_t)it, c_best, sm_obs); break;
-        case 16: prop_phase<DYN, OBS, 16>(P, (uint32_t)r, (uint32_t)it, c_best, sm_obs); break;
-        case 32: prop_phase<DYN, OBS, 32>(P, (uint32_t)r, (uint32_t)it, c_best, sm_obs); break;
-        default: prop_phase<DYN, OBS, 1>(P, (uint32_t)r, (uint32_t)it, c_best, sm_obs); break;
+      // phase X: propagate(it) and, meanwhile, NN(it+1) over the frozen snapshot [0, n)
+      const bool ahead = (iters + 1 < P.max_iters);
+      prop_phase<DYN, OBS>(P, (uint32_t)r, (uint32_t)it, c_best, kcur, root_only, pw, W, sm_obs, sm_cells, sm_list);
+      if (ahead) {
+        if (P.pb.unit_weights) nn_phase<DYN, true>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vw, x_cnt, my_tile, my_bar, par0, par1);
+        else nn_phase<DYN, false>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vw, x_cnt, my_tile, my_bar, par0, par1);
       }
       // goal-key slots alternate over the whole launch (not per replan): the other slot was last
       // read before the previous grid sync and is next written after the following one
@@ -485,7 +509,7 @@ __global__ void __launch_bounds__(kThreads, 2) pakr_loop_kernel(const __grid_con
       grid.sync();
       if (leader) { const unsigned long long t = globaltimer_ns(); ph1 += t - tp; tp = t; }
       // phase C
-      const int total = insert_phase<DYN>(P, n, slot, 32 / P.lanes, sm_pref);
+      const int total = insert_phase<DYN>(P, n, slot, kcur, sm_pref);
       const int added = min(total, P.cap - n);
       if (leader && P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) P.ctrl->stop = 1;
       __threadfence();
@@ -493,11 +517,13 @@ __global__ void __launch_bounds__(kThreads, 2) pakr_loop_kernel(const __grid_con
       grid.sync();
       if (leader) { const unsigned long long t = globaltimer_ns(); ph2 += t - tp; tp = t; }
       fence_proxy_async();
-      nn_pairs += (long long)P.B * n;  // (query, node) pairs the scan of this iteration evaluated
+      nn_pairs += (long long)P.B * n;  // (query, node) pairs of this iteration's NN
+      n_scanned = ahead ? n : 0;
       n += added;
       inserted += added;
       ++iterations;
       ++iters;
+      cur ^= 1;
       const unsigned long long gk = __ldcg(&P.ctrl->goal_key[slot]);
       stop = __ldcg(&P.ctrl->stop) != 0;
       ++it;
