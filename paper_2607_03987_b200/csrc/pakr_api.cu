@@ -152,8 +152,13 @@ HostGrid build_grid(const pakr_problem* p, int obs_kind) {
     g.cells.resize(ncells);
     g.list.clear();
     for (int c = 0; c < ncells; ++c) {
-      g.cells[c] = ((uint32_t)g.list.size() << 8) | (uint32_t)per[c].size();
-      g.list.insert(g.list.end(), per[c].begin(), per[c].end());
+      const uint32_t cnt = (uint32_t)per[c].size();
+      if (cnt <= 2) {  // ids inline (n_obstacles <= 1024 fits 12 bits)
+        g.cells[c] = cnt | (cnt > 0 ? (uint32_t)per[c][0] << 8 : 0u) | (cnt > 1 ? (uint32_t)per[c][1] << 20 : 0u);
+      } else {
+        g.cells[c] = ((uint32_t)g.list.size() << 8) | cnt;
+        g.list.insert(g.list.end(), per[c].begin(), per[c].end());
+      }
     }
     if (g.list.empty()) g.list.push_back(0);
     g.on = true;
@@ -434,6 +439,7 @@ extern "C" pakr_status pakr_plan(pakr_planner* pl, const pakr_plan_opts* o, void
   s.inserted = hc->inserted;
   s.nn_pairs = hc->nn_pairs;
   for (int i = 0; i < 3; ++i) s.phase_ms[i] = (double)hc->phase_ns[i] * 1e-6;
+  for (int i = 0; i < 16; ++i) s.probe_cycles[i] = (int64_t)hc->probe[i];
   s.replans_run = hc->replans_run;
   s.replans_solved = hc->replans_solved;
   s.termination = hc->termination;

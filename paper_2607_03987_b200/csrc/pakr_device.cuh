@@ -49,7 +49,7 @@ struct DevProblem {
   int gdim[3];                         // cells per axis (gdim[2] == 1 for circle / cylinder fields)
   float gorg[3], ginv[3];              // cell(x) = clamp(floor((x - gorg) * ginv), 0, gdim - 1)
   int g_cells, g_list;                 // number of cells, total list entries
-  const uint32_t* grid_cells;          // DEVICE [g_cells]: (list offset << 8) | count
+  const uint32_t* grid_cells;          // DEVICE [g_cells]: cell words, see cell_margin()
   const uint16_t* grid_list;           // DEVICE [g_list] obstacle ids
 };
 
@@ -271,11 +271,10 @@ __device__ __forceinline__ float one_obstacle_margin(const float4* __restrict__ 
 // Broad phase (exact): only the obstacles registered in the grid cell of `pos` can contain it, because the
 // host registers an obstacle in every cell its (slightly inflated) bounding box touches and cell() is
 // monotone per axis; positions outside the box clamp into the border cells, whose lists hold everything
-// that sticks out of the box.  The SIGN of the returned margin equals that of the full scan.
+// that sticks out of the box.  The SIGN of the resulting margin equals that of the full scan.
+// Cell word: bits 0-7 count; count <= 2: ids inline in bits 8-19 and 20-31; else bits 8-31 = list offset.
 template <int OBS, int PD>
-__device__ __forceinline__ float obstacle_margin_grid(const DevProblem& pb, const uint32_t* __restrict__ sm_cells,
-                                                      const uint16_t* __restrict__ sm_list,
-                                                      const float* __restrict__ sm_obs, const float* pos) {
+__device__ __forceinline__ int grid_cell(const DevProblem& pb, const float* pos) {
   constexpr int GD = (OBS == OBS_CIRCLE) ? 2 : PD;  // circles / vertical cylinders: xy grid
   int cell = 0, mul = 1;
 #pragma unroll
@@ -285,11 +284,22 @@ __device__ __forceinline__ float obstacle_margin_grid(const DevProblem& pb, cons
     cell += c * mul;
     mul *= pb.gdim[a];
   }
-  const uint32_t hdr = sm_cells[cell];
-  const int cnt = (int)(hdr & 0xffu);
-  const uint16_t* lst = sm_list + (hdr >> 8);
+  return cell;
+}
+
+template <int OBS, int PD>
+__device__ __forceinline__ float cell_margin(uint32_t hdr, const uint16_t* __restrict__ sm_list,
+                                             const float* __restrict__ sm_obs, const float* pos) {
   const float4* o4 = reinterpret_cast<const float4*>(sm_obs);
+  const int cnt = (int)(hdr & 0xffu);
   float m = __int_as_float(0x7f800000);
+  if (cnt == 0) return m;
+  if (cnt <= 2) {
+    m = one_obstacle_margin<OBS, PD>(o4, (int)((hdr >> 8) & 0xfffu), pos);
+    if (cnt == 2) m = fminf(m, one_obstacle_margin<OBS, PD>(o4, (int)(hdr >> 20), pos));
+    return m;
+  }
+  const uint16_t* lst = sm_list + (hdr >> 8);
   for (int k = 0; k < cnt; ++k) m = fminf(m, one_obstacle_margin<OBS, PD>(o4, (int)lst[k], pos));
   return m;
 }

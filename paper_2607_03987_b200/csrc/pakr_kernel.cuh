@@ -37,6 +37,7 @@ struct Ctrl {  // device control block (in the workspace)
   unsigned long long t_start_ns, t_first_ns, t_end_ns;
   long long iterations, inserted, nn_pairs;
   unsigned long long phase_ns[3];  // leader's time in NN / propagate / insert incl. the grid sync after each
+  unsigned long long probe[16];    // -DPAKR_PROBE: SM cycles of thread 0 of CTA 0 between probe points
   int n_nodes, stop;
   int path_len, solved;
   float best_cost;
@@ -79,6 +80,30 @@ __device__ __forceinline__ unsigned long long globaltimer_ns() {
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
   return t;
 }
+#ifdef PAKR_PROBE
+#define PROBE(P, i)                                                                   \
+  do {                                                                                \
+    if (blockIdx.x == 0 && threadIdx.x == 0) {                                        \
+      const long long t_ = clock64();                                                 \
+      atomicAdd(&(P).ctrl->probe[i], (unsigned long long)(t_ - g_probe_prev));        \
+      g_probe_prev = t_;                                                              \
+    }                                                                                 \
+  } while (0)
+#define PROBE_DEP(v)                                                                                 \
+  do {                                                                                               \
+    float d_;                                                                                        \
+    asm volatile("shfl.sync.idx.b32 %0, %1, 0, 31, 0xffffffff;" : "=f"(d_) : "f"((float)(v)));       \
+  } while (0)
+#define PROBE_DECL long long g_probe_prev = clock64()
+#define PROBE_ARG , long long& g_probe_prev
+#define PROBE_PASS , g_probe_prev
+#else
+#define PROBE(P, i) do {} while (0)
+#define PROBE_DEP(v) do {} while (0)
+#define PROBE_DECL
+#define PROBE_ARG
+#define PROBE_PASS
+#endif
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return (uint32_t)__cvta_generic_to_shared(p);
 }
@@ -136,7 +161,7 @@ __device__ __forceinline__ float dist2(const DevProblem& pb, const float (&q)[Dy
 template <int DYN, bool UNIT_W>
 __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, uint32_t r, uint32_t it,
                                          unsigned long long* key, int vw, int vcount, float* sm_tile,
-                                         uint64_t* sm_bar, uint32_t& par0, uint32_t& par1) {
+                                         uint64_t* sm_bar, uint32_t& par0, uint32_t& par1 PROBE_ARG) {
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
   constexpr int TILE = TileCfg<DYN>::TILE, TF = TileCfg<DYN>::TILE_FLOATS;
   const int lane = threadIdx.x & 31;
@@ -169,6 +194,8 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
         for (int d = 0; d < DP; ++d) P.dbg_x_rand[(size_t)s * DP + d] = d < D ? q[j][d] : 0.0f;
       }
     }
+    PROBE_DEP(q[0][0]);
+    PROBE(P, 0);
     const int ntiles = (end - beg + TILE - 1) / TILE;
     const float* src = P.states + (size_t)beg * DP;
     if (lane == 0) {
@@ -186,6 +213,7 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
       }
       if (t & 1) { mbar_wait(&sm_bar[1], par1); par1 ^= 1; }
       else { mbar_wait(&sm_bar[0], par0); par0 ^= 1; }
+      if (t == 0) PROBE(P, 1);
       const float4* tp = reinterpret_cast<const float4*>(sm_tile + (t & 1) * TF);
       const int base = beg + t * TILE;
 #pragma unroll 2
@@ -204,6 +232,8 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
       }
       __syncwarp();  // every lane is done with this buffer before lane 0 refills it
     }
+    PROBE_DEP(best[0]);
+    PROBE(P, 2);
 #pragma unroll
     for (int j = 0; j < kQ; ++j) {
       const int s = g * 32 * kQ + j * 32 + lane;
@@ -224,7 +254,7 @@ template <int DYN, int OBS>
 __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t it, float c_best,
                                            const unsigned long long* key, bool root_only, int pw, int W,
                                            const float* sm_obs, const uint32_t* sm_cells,
-                                           const uint16_t* sm_list) {
+                                           const uint16_t* sm_list PROBE_ARG) {
   using T = DynTraits<DYN>;
   constexpr int D = T::D, M = T::M, DP = T::DP, PD = T::PD;
   const DevProblem& pb = P.pb;
@@ -259,26 +289,51 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
     }
     const float parent_cost = __ldcg(&P.costs[parent]);
     sample_control<M>(pb, P.seed, r, it, (uint32_t)s, (uint32_t)k, ctl);
+    PROBE_DEP(ctl[0]);
+    PROBE(P, 5);
+    PROBE_DEP(x[0] + parent_cost);
+    PROBE(P, 6);
     // margins: bm >= 0 / om > 0 mean still valid.  Inactive lanes start dead.
     float bm = active ? __int_as_float(0x7f800000) : -1.0f;
     float om = bm;
     float length = 0.0f;
-    for (int j = 0; j < pb.S; ++j) {
-      float px[PD];
+    // Steps are taken in chunks of kChunk: the integration chain runs ahead and the obstacle tests of the
+    // chunk's step-end positions (dependent shared-memory lookups) are issued together.
+    constexpr int kChunk = 4;
+    for (int j0 = 0; j0 < pb.S; j0 += kChunk) {
+      float pos[kChunk][PD];
 #pragma unroll
-      for (int a = 0; a < PD; ++a) px[a] = x[a];
-      dyn_step<DYN>(pb, x, ctl);
-      if (pb.cost_mode == 1) {
-        float seg = 0.0f;
+      for (int cj = 0; cj < kChunk; ++cj) {
+        if (j0 + cj < pb.S) {
+          float px[PD];
 #pragma unroll
-        for (int a = 0; a < PD; ++a) seg = fmaf(x[a] - px[a], x[a] - px[a], seg);
-        length += sqrtf(seg);
+          for (int a = 0; a < PD; ++a) px[a] = x[a];
+          dyn_step<DYN>(pb, x, ctl);
+          if (pb.cost_mode == 1) {
+            float seg = 0.0f;
+#pragma unroll
+            for (int a = 0; a < PD; ++a) seg = fmaf(x[a] - px[a], x[a] - px[a], seg);
+            length += sqrtf(seg);
+          }
+          bm = fminf(bm, bounds_margin<DYN>(pb, x));
+        }
+#pragma unroll
+        for (int a = 0; a < PD; ++a) pos[cj][a] = x[a];  // past the last step: a repeat of it (harmless)
       }
-      bm = fminf(bm, bounds_margin<DYN>(pb, x));
-      if (pb.grid_on) om = fminf(om, obstacle_margin_grid<OBS, PD>(pb, sm_cells, sm_list, sm_obs, x));
-      else om = fminf(om, obstacle_margin<OBS, PD>(sm_obs, pb.n_obs, x, 0, 1));
+      if (pb.grid_on) {
+        uint32_t hdr[kChunk];
+#pragma unroll
+        for (int cj = 0; cj < kChunk; ++cj) hdr[cj] = sm_cells[grid_cell<OBS, PD>(pb, pos[cj])];
+#pragma unroll
+        for (int cj = 0; cj < kChunk; ++cj) om = fminf(om, cell_margin<OBS, PD>(hdr[cj], sm_list, sm_obs, pos[cj]));
+      } else {
+#pragma unroll
+        for (int cj = 0; cj < kChunk; ++cj) om = fminf(om, obstacle_margin<OBS, PD>(sm_obs, pb.n_obs, pos[cj], 0, 1));
+      }
       if (P.early_exit && __all_sync(0xffffffffu, !(bm >= 0.0f) || !(om > 0.0f))) break;  // whole warp dead
     }
+    PROBE_DEP(bm + om);
+    PROBE(P, 7);
     bool finite = true;
 #pragma unroll
     for (int d = 0; d < D; ++d) finite = finite & (fabsf(x[d]) <= 3.4e38f);
@@ -318,6 +373,7 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
       __stcg(&P.scr_parent[slot], parent);
       __stcg(&P.scr_flags[slot], flags | (lane << 8));
     }
+    PROBE(P, 8);
     if (active && P.dbg_child_flags) {
       P.dbg_child_flags[c] = flags;
       if (P.dbg_child_cost) P.dbg_child_cost[c] = c_new;
@@ -334,7 +390,7 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
 // Returns the number of survivors of this iteration (identical in every thread of the grid).
 template <int DYN>
 __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, unsigned long long* key_done,
-                                            int* sm_pref) {
+                                            int* sm_pref PROBE_ARG) {
   using T = DynTraits<DYN>;
   constexpr int DP = T::DP;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -365,6 +421,7 @@ __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, u
   }
   sm_pref[threadIdx.x] = wbase + incl - mine;
   __syncthreads();
+  PROBE(P, 10);
   const int room = P.cap - n;
   for (int u = gw; u < U; u += W) {
     const int ch = u / cpt;
@@ -392,6 +449,7 @@ __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, u
       if (P.dbg_child_flags) P.dbg_child_flags[u * cpw + (fl >> 8)] |= 32;
     }
   }
+  PROBE(P, 11);
   // the NN keys this iteration consumed are free again: reset them for iteration i+2
   for (int s = blockIdx.x * kThreads + threadIdx.x; s < P.B; s += gridDim.x * kThreads) key_done[s] = kKeyNone;
   return total;
@@ -466,6 +524,7 @@ __global__ void __launch_bounds__(kThreads, 2) pakr_loop_kernel(const __grid_con
   unsigned long long* const key0 = P.nn_key;
   unsigned long long* const key1 = P.nn_key + P.B;
 
+  PROBE_DECL;
   unsigned long long t_start = 0;
   if (leader) { t_start = globaltimer_ns(); P.ctrl->t_start_ns = t_start; }
 
@@ -490,31 +549,40 @@ __global__ void __launch_bounds__(kThreads, 2) pakr_loop_kernel(const __grid_con
       const bool root_only = (n == 1) && !P.n_nodes_io;
       // phase A': rows appended since the look-ahead scan
       if (!root_only && n_scanned < n) {
-        if (P.pb.unit_weights) nn_phase<DYN, true>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, pw, W, my_tile, my_bar, par0, par1);
-        else nn_phase<DYN, false>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, pw, W, my_tile, my_bar, par0, par1);
+        if (P.pb.unit_weights) nn_phase<DYN, true>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, pw, W, my_tile, my_bar, par0, par1 PROBE_PASS);
+        else nn_phase<DYN, false>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, pw, W, my_tile, my_bar, par0, par1 PROBE_PASS);
+        PROBE(P, 3);
         grid.sync();
       }
+      PROBE(P, 4);
       if (leader) { const unsigned long long t = globaltimer_ns(); ph0 += t - tp; tp = t; }
       // phase X: propagate(it) and, meanwhile, NN(it+1) over the frozen snapshot [0, n)
+#ifdef PAKR_EXP_NOAHEAD
+      const bool ahead = false;
+#else
       const bool ahead = (iters + 1 < P.max_iters);
-      prop_phase<DYN, OBS>(P, (uint32_t)r, (uint32_t)it, c_best, kcur, root_only, pw, W, sm_obs, sm_cells, sm_list);
+#endif
+      prop_phase<DYN, OBS>(P, (uint32_t)r, (uint32_t)it, c_best, kcur, root_only, pw, W, sm_obs, sm_cells, sm_list PROBE_PASS);
       if (ahead) {
-        if (P.pb.unit_weights) nn_phase<DYN, true>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vw, x_cnt, my_tile, my_bar, par0, par1);
-        else nn_phase<DYN, false>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vw, x_cnt, my_tile, my_bar, par0, par1);
+        if (P.pb.unit_weights) nn_phase<DYN, true>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vw, x_cnt, my_tile, my_bar, par0, par1 PROBE_PASS);
+        else nn_phase<DYN, false>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vw, x_cnt, my_tile, my_bar, par0, par1 PROBE_PASS);
       }
       // goal-key slots alternate over the whole launch (not per replan): the other slot was last
       // read before the previous grid sync and is next written after the following one
       const int slot = (int)(iterations & 1);
       if (leader) P.ctrl->goal_key[slot ^ 1] = kKeyNone;
       grid.sync();
+      PROBE(P, 9);
       if (leader) { const unsigned long long t = globaltimer_ns(); ph1 += t - tp; tp = t; }
       // phase C
-      const int total = insert_phase<DYN>(P, n, slot, kcur, sm_pref);
+      const int total = insert_phase<DYN>(P, n, slot, kcur, sm_pref PROBE_PASS);
       const int added = min(total, P.cap - n);
       if (leader && P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) P.ctrl->stop = 1;
       __threadfence();
       fence_proxy_async();  // tree rows written with st.global are read next by TMA (async proxy)
+      PROBE(P, 12);
       grid.sync();
+      PROBE(P, 13);
       if (leader) { const unsigned long long t = globaltimer_ns(); ph2 += t - tp; tp = t; }
       fence_proxy_async();
       nn_pairs += (long long)P.B * n;  // (query, node) pairs of this iteration's NN

@@ -81,7 +81,8 @@ class _Stats(C.Structure):
                 ("replans_run", C.c_int32), ("replans_solved", C.c_int32), ("termination", C.c_int32),
                 ("first_solution_ms", C.c_double), ("device_ms", C.c_double), ("phase_ms", C.c_double * 3),
                 ("replan_cost", C.c_float * MAX_REPLAN_STATS), ("replan_nodes", C.c_int32 * MAX_REPLAN_STATS),
-                ("replan_iters", C.c_int32 * MAX_REPLAN_STATS), ("replan_end_ms", C.c_double * MAX_REPLAN_STATS)]
+                ("replan_iters", C.c_int32 * MAX_REPLAN_STATS), ("replan_end_ms", C.c_double * MAX_REPLAN_STATS),
+                ("probe_cycles", C.c_int64 * 16)]
 
 
 class _Result(C.Structure):
@@ -223,7 +224,8 @@ class Planner:
                     termination=int(s.termination), first_solution_ms=float(s.first_solution_ms),
                     device_ms=float(s.device_ms), phase_ms=[float(v) for v in s.phase_ms], replan_cost=np.array(s.replan_cost[:R], np.float32),
                     replan_nodes=np.array(s.replan_nodes[:R], np.int64), replan_iters=np.array(s.replan_iters[:R], np.int64),
-                    replan_end_ms=np.array(s.replan_end_ms[:R], np.float64))
+                    replan_end_ms=np.array(s.replan_end_ms[:R], np.float64),
+                    probe_cycles=[int(v) for v in s.probe_cycles])
 
     def read_tree(self, B: int, K: int, tree_capacity: int, n: int) -> dict:
         """Copies the first n nodes of the tree pakr_plan left in the workspace to numpy."""
