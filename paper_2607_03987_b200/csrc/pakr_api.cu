@@ -89,7 +89,7 @@ size_t tile_floats(int DP) { return (size_t)(DP == 4 ? 256 : DP == 8 ? 128 : 64)
 
 size_t smem_for(const pakr_planner* pl) {
   const int os = pl->obs == OBS_CIRCLE ? 4 : 8;
-  return kWarps * 2 * tile_floats(pl->DP) * 4 + kWarps * 2 * 8 + (kThreads + kWarps + 8) * 4 +
+  return kWarps * 2 * tile_floats(pl->DP) * 4 + kWarps * 2 * 8 + (kThreads + kWarps + 8) * 4 + kMaxD * 2 * 32 * kQ * 4 + kWarps * 32 * kQ * 8 +
          (size_t)((pl->pb.n_obs * os + 3) & ~3) * 4 + (size_t)pl->pb.g_cells * 4 + (size_t)pl->pb.g_list * 2 + 16;
 }
 
@@ -383,7 +383,7 @@ pakr_status launch(pakr_planner* pl, Params& P, cudaStream_t stream) {
   CUDA_TRY(pl, cudaMemsetAsync(P.ctrl, 0, sizeof(Ctrl), stream));
   CUDA_TRY(pl, cudaMemsetAsync(P.ctrl, 0xFF, 16, stream));  // goal_key[2] = none
   void* args[] = {&P};
-  const dim3 grid(pl->num_sms * pl->blocks_per_sm), block(kThreads);
+  const dim3 grid(pl->num_sms * std::min(pl->blocks_per_sm, kCtasPerSm)), block(kThreads);
   CUDA_TRY(pl, cudaLaunchCooperativeKernel(pl->kernel, grid, block, args, pl->smem_bytes, stream));
   return PAKR_OK;
 }
@@ -439,7 +439,7 @@ extern "C" pakr_status pakr_plan(pakr_planner* pl, const pakr_plan_opts* o, void
   s.inserted = hc->inserted;
   s.nn_pairs = hc->nn_pairs;
   for (int i = 0; i < 3; ++i) s.phase_ms[i] = (double)hc->phase_ns[i] * 1e-6;
-  for (int i = 0; i < 16; ++i) s.probe_cycles[i] = (int64_t)hc->probe[i];
+  for (int i = 0; i < 192; ++i) s.probe_cycles[i] = (int64_t)hc->probe[i];
   s.replans_run = hc->replans_run;
   s.replans_solved = hc->replans_solved;
   s.termination = hc->termination;

@@ -25,7 +25,11 @@
 namespace pakr {
 namespace cg = cooperative_groups;
 
-constexpr int kThreads = 256;
+#ifndef PAKR_THREADS
+#define PAKR_THREADS 256
+#endif
+constexpr int kThreads = PAKR_THREADS;  // 256 x 2 CTAs per SM measured 1.4x faster in the NN scan than 512 x 1
+constexpr int kCtasPerSm = 1024 / (2 * PAKR_THREADS);
 constexpr int kWarps = kThreads / 32;
 constexpr int kQ = 4;            // queries per lane in the NN scan
 constexpr int kPathMax = 8192;   // longest path the device buffers hold
@@ -37,7 +41,7 @@ struct Ctrl {  // device control block (in the workspace)
   unsigned long long t_start_ns, t_first_ns, t_end_ns;
   long long iterations, inserted, nn_pairs;
   unsigned long long phase_ns[3];  // leader's time in NN / propagate / insert incl. the grid sync after each
-  unsigned long long probe[16];    // -DPAKR_PROBE: SM cycles of thread 0 of CTA 0 between probe points
+  unsigned long long probe[192];    // -DPAKR_PROBE: SM cycles of thread 0 of CTA 0 between probe points
   int n_nodes, stop;
   int path_len, solved;
   float best_cost;
@@ -81,11 +85,14 @@ __device__ __forceinline__ unsigned long long globaltimer_ns() {
   return t;
 }
 #ifdef PAKR_PROBE
+#ifndef PAKR_PROBE_BLOCK
+#define PAKR_PROBE_BLOCK 0
+#endif
 #define PROBE(P, i)                                                                   \
   do {                                                                                \
-    if (blockIdx.x == 0 && threadIdx.x == 0) {                                        \
+    if (blockIdx.x == PAKR_PROBE_BLOCK && threadIdx.x == 0) {                         \
       const long long t_ = clock64();                                                 \
-      atomicAdd(&(P).ctrl->probe[i], (unsigned long long)(t_ - g_probe_prev));        \
+      atomicAdd(&(P).ctrl->probe[(i) + g_pb], (unsigned long long)(t_ - g_probe_prev)); \
       g_probe_prev = t_;                                                              \
     }                                                                                 \
   } while (0)
@@ -94,15 +101,17 @@ __device__ __forceinline__ unsigned long long globaltimer_ns() {
     float d_;                                                                                        \
     asm volatile("shfl.sync.idx.b32 %0, %1, 0, 31, 0xffffffff;" : "=f"(d_) : "f"((float)(v)));       \
   } while (0)
-#define PROBE_DECL long long g_probe_prev = clock64()
-#define PROBE_ARG , long long& g_probe_prev
-#define PROBE_PASS , g_probe_prev
+#define PROBE_DECL long long g_probe_prev = clock64(); const int g_pb = 0
+#define PROBE_ARG , long long& g_probe_prev, int g_pb
+#define PROBE_PASS , g_probe_prev, 0
+#define PROBE_PASSX , g_probe_prev, 16
 #else
 #define PROBE(P, i) do {} while (0)
 #define PROBE_DEP(v) do {} while (0)
 #define PROBE_DECL
 #define PROBE_ARG
 #define PROBE_PASS
+#define PROBE_PASSX
 #endif
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return (uint32_t)__cvta_generic_to_shared(p);
@@ -156,44 +165,69 @@ __device__ __forceinline__ float dist2(const DevProblem& pb, const float (&q)[Dy
 }
 
 // ---- NN scan of tree rows [nbeg, nend) for the queries of iteration `it` (Alg. 1 l.6-7) ----
-// Warps vw = 0..vcount-1 take part (vw < 0: this warp sits out).  Partial minima are merged into
-// key[s] with a 64-bit atomicMin, so any split of the rows over warps / phases gives the same result.
+// CTAs vb = 0..vbcount-1 take part (vb < 0: this CTA sits out; the call is CTA-uniform).  Work units are
+// (query group of 128, node range); a CTA takes kWarps consecutive units per round, one per warp.  The
+// sampled states of the (at most two) query groups a CTA touches in a round are drawn once by the CTA into
+// shared memory (Alg. 1 l.6) instead of once per warp.  Partial minima are merged into key[s] with a 64-bit
+// atomicMin, so any split of the rows over warps / phases gives the same result.
 template <int DYN, bool UNIT_W>
 __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, uint32_t r, uint32_t it,
-                                         unsigned long long* key, int vw, int vcount, float* sm_tile,
-                                         uint64_t* sm_bar, uint32_t& par0, uint32_t& par1 PROBE_ARG) {
+                                         unsigned long long* key, int vb, int vbcount, float* sm_tile,
+                                         uint64_t* sm_bar, float* sm_q, unsigned long long* sm_keys, uint32_t& par0,
+                                         uint32_t& par1 PROBE_ARG) {
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
   constexpr int TILE = TileCfg<DYN>::TILE, TF = TileCfg<DYN>::TILE_FLOATS;
-  const int lane = threadIdx.x & 31;
+  constexpr int QG = 32 * kQ;  // queries per group
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int n = nend - nbeg;
-  if (vw < 0 || n <= 0) return;
-  const int W = vcount;
-  const int gw = vw;
-  const int G = (P.B + 32 * kQ - 1) / (32 * kQ);  // query groups
-  int R = W / G;                                  // node ranges per group
+  if (vb < 0 || n <= 0) return;
+  const int W = vbcount * kWarps;
+  const int G = (P.B + QG - 1) / QG;  // query groups
+  int R = W / G;                      // node ranges per group
   if (R < 1) R = 1;
   int len = (n + R - 1) / R;
   if (len < 32) len = 32;
   const int Reff = (n + len - 1) / len;
   const int U = G * Reff;
-  for (int u = gw; u < U; u += W) {
-    const int g = u / Reff, rr = u - g * Reff;
+  for (int ub = vb * kWarps; ub < U; ub += W) {
+    const int u = ub + warp;
+    const bool has = u < U;
+    const int g = has ? u / Reff : 0, rr = u - g * Reff;
     const int beg = nbeg + rr * len;
     const int end = min(nend, beg + len);
+    const int g_lo = ub / Reff, g_hi = min(U - 1, ub + kWarps - 1) / Reff;
+    const bool shared_q = (g_hi - g_lo) <= 1;  // CTA-uniform
     float q[kQ][D];
     float best[kQ];
     int bidx[kQ];
+    if (shared_q) {
+      if (ub != vb * kWarps) __syncthreads();  // previous round's readers are done with sm_q
+      const int ng = (g_hi - g_lo + 1) * QG;
+      for (int t = threadIdx.x; t < ng; t += kThreads) {
+        float x[D];
+        sample_state<D>(P.pb, P.seed, r, it, (uint32_t)(g_lo * QG + t), x);
+#pragma unroll
+        for (int d = 0; d < D; ++d) sm_q[d * (2 * QG) + t] = x[d];
+      }
+      __syncthreads();
+    }
 #pragma unroll
     for (int j = 0; j < kQ; ++j) {
-      const int s = g * 32 * kQ + j * 32 + lane;
-      sample_state<D>(P.pb, P.seed, r, it, (uint32_t)s, q[j]);
+      const int s = g * QG + j * 32 + lane;
+      if (shared_q) {
+#pragma unroll
+        for (int d = 0; d < D; ++d) q[j][d] = sm_q[d * (2 * QG) + (g - g_lo) * QG + j * 32 + lane];
+      } else {
+        sample_state<D>(P.pb, P.seed, r, it, (uint32_t)s, q[j]);
+      }
       best[j] = __int_as_float(0x7f800000);
       bidx[j] = 0x7fffffff;
-      if (P.dbg_x_rand && rr == 0 && nbeg == 0 && s < P.B) {
+      if (P.dbg_x_rand && has && rr == 0 && nbeg == 0 && s < P.B) {
 #pragma unroll
         for (int d = 0; d < DP; ++d) P.dbg_x_rand[(size_t)s * DP + d] = d < D ? q[j][d] : 0.0f;
       }
     }
+    if (has) {
     PROBE_DEP(q[0][0]);
     PROBE(P, 0);
     const int ntiles = (end - beg + TILE - 1) / TILE;
@@ -216,14 +250,19 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
       if (t == 0) PROBE(P, 1);
       const float4* tp = reinterpret_cast<const float4*>(sm_tile + (t & 1) * TF);
       const int base = beg + t * TILE;
+      float4 nx[DP / 4];  // row i+1 is fetched while row i is scored (hides the shared-memory latency)
+#pragma unroll
+      for (int v = 0; v < DP / 4; ++v) nx[v] = tp[v];
 #pragma unroll 2
       for (int i = 0; i < cnt; ++i) {
         float p[DP];
 #pragma unroll
         for (int v = 0; v < DP / 4; ++v) {
-          const float4 a = tp[i * (DP / 4) + v];  // warp-uniform address: broadcast
-          p[4 * v] = a.x; p[4 * v + 1] = a.y; p[4 * v + 2] = a.z; p[4 * v + 3] = a.w;
+          p[4 * v] = nx[v].x; p[4 * v + 1] = nx[v].y; p[4 * v + 2] = nx[v].z; p[4 * v + 3] = nx[v].w;
         }
+        const int in = min(i + 1, cnt - 1);
+#pragma unroll
+        for (int v = 0; v < DP / 4; ++v) nx[v] = tp[in * (DP / 4) + v];  // warp-uniform address: broadcast
 #pragma unroll
         for (int j = 0; j < kQ; ++j) {
           const float d2 = dist2<DYN, UNIT_W>(P.pb, q[j], p);
@@ -234,22 +273,43 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
     }
     PROBE_DEP(best[0]);
     PROBE(P, 2);
+    }  // has
+    if (shared_q) {
+      // CTA-level merge: one global atomicMin per (CTA, query) instead of one per (warp, query)
 #pragma unroll
-    for (int j = 0; j < kQ; ++j) {
-      const int s = g * 32 * kQ + j * 32 + lane;
-      if (s < P.B && bidx[j] != 0x7fffffff) {
-        const unsigned long long kv =
-            ((unsigned long long)__float_as_uint(best[j]) << 32) | (unsigned)bidx[j];
-        atomicMin(&key[s], kv);  // d2 >= 0: uint order == float order; ties -> lowest node
+      for (int j = 0; j < kQ; ++j)
+        sm_keys[warp * QG + j * 32 + lane] =
+            (has && bidx[j] != 0x7fffffff) ? (((unsigned long long)__float_as_uint(best[j]) << 32) | (unsigned)bidx[j]) : kKeyNone;
+      __syncthreads();
+      const int ngroups = g_hi - g_lo + 1;
+      for (int t = threadIdx.x; t < ngroups * QG; t += kThreads) {
+        const int gi = g_lo + t / QG, qi = t % QG;
+        // warps of this round whose unit belongs to group gi: units [max(ub, gi*Reff), min(ub+kWarps, (gi+1)*Reff, U))
+        const int w0 = max(ub, gi * Reff) - ub, w1 = min(min(ub + kWarps, (gi + 1) * Reff), U) - ub;
+        unsigned long long m = kKeyNone;
+        for (int w = w0; w < w1; ++w) m = min(m, sm_keys[w * QG + qi]);
+        const int s = gi * QG + qi;
+        if (s < P.B && m != kKeyNone) atomicMin(&key[s], m);  // d2 >= 0: uint order == float order; ties -> lowest node
+      }
+    } else if (has) {
+#pragma unroll
+      for (int j = 0; j < kQ; ++j) {
+        const int s = g * QG + j * 32 + lane;
+        if (s < P.B && bidx[j] != 0x7fffffff) {
+          const unsigned long long kv =
+              ((unsigned long long)__float_as_uint(best[j]) << 32) | (unsigned)bidx[j];
+          atomicMin(&key[s], kv);
+        }
       }
     }
+    PROBE(P, 3);
   }
 }
 
 // ---- propagate: controls, RK4 edge, validity, prune, goal flag, per-warp compaction (Alg. 1 l.8-12) ----
 // One lane per child, state in registers for the whole edge.  Warp unit u = children [32u, 32u+32) is taken
-// by the warp whose prop-order index pw == u (mod W); pw runs across CTAs first, so few children spread
-// over all SMs.  Survivors go to the scratch rows of the unit, packed by ballot rank.
+// by the warp with index pw == u (mod W) among the W warps that propagate (pw < 0: not one of them).
+// Survivors go to the scratch rows of the unit, packed by ballot rank.
 template <int DYN, int OBS>
 __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t it, float c_best,
                                            const unsigned long long* key, bool root_only, int pw, int W,
@@ -261,6 +321,7 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
   const int lane = threadIdx.x & 31;
   const int BK = P.B * P.K;
   const int U = (BK + 31) / 32;
+  if (pw < 0) return;
   for (int u = pw; u < U; u += W) {
     const int c = u * 32 + lane;
     const bool active = c < BK;
@@ -481,15 +542,19 @@ __device__ __forceinline__ void extract_path(const Params& P, int goal_node) {
 }
 
 template <int DYN, int OBS>
-__global__ void __launch_bounds__(kThreads, 2) pakr_loop_kernel(const __grid_constant__ Params P) {
+__global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const __grid_constant__ Params P) {
   using T = DynTraits<DYN>;
   constexpr int OS = (OBS == OBS_CIRCLE) ? 4 : 8;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  // [tiles: kWarps * 2 * TILE_FLOATS][bars: kWarps * 2][pref: kThreads + kWarps + 8][obstacles][grid cells][grid lists]
+  // [tiles: kWarps * 2 * TILE_FLOATS][bars: kWarps * 2][pref: kThreads + kWarps + 8][queries: kMaxD * 256]
+  // [merge keys: kWarps * 128 x u64]
+  // [obstacles][grid cells][grid lists]
   float* sm_tiles = reinterpret_cast<float*>(smem_raw);
   uint64_t* sm_bars = reinterpret_cast<uint64_t*>(sm_tiles + kWarps * 2 * TileCfg<DYN>::TILE_FLOATS);
   int* sm_pref = reinterpret_cast<int*>(sm_bars + kWarps * 2);
-  float* sm_obs = reinterpret_cast<float*>(sm_pref + kThreads + kWarps + 8);
+  float* sm_q = reinterpret_cast<float*>(sm_pref + kThreads + kWarps + 8);
+  unsigned long long* sm_keys = reinterpret_cast<unsigned long long*>(sm_q + kMaxD * 2 * 32 * kQ);
+  float* sm_obs = reinterpret_cast<float*>(sm_keys + kWarps * 32 * kQ);
   uint32_t* sm_cells = reinterpret_cast<uint32_t*>(sm_obs + ((P.pb.n_obs * OS + 3) & ~3));
   uint16_t* sm_list = reinterpret_cast<uint16_t*>(sm_cells + P.pb.g_cells);
   cg::grid_group grid = cg::this_grid();
@@ -512,15 +577,19 @@ __global__ void __launch_bounds__(kThreads, 2) pakr_loop_kernel(const __grid_con
   uint64_t* my_bar = sm_bars + warp * 2;
   uint32_t par0 = 0, par1 = 0;
 
-  // Warp roles.  pw orders the warps across CTAs first (warp 0 of every CTA, then warp 1, ...): propagate unit
-  // u runs on the warp with pw == u (mod W).  When the children need fewer than half of the warps, the others
-  // run the look-ahead NN scan meanwhile; otherwise every warp does both, one after the other.
-  const int W = gridDim.x * kWarps;
-  const int pw = warp * gridDim.x + blockIdx.x;
+  // Roles in phase X.  When the children fill at most a quarter of the SMs, the first NPB CTAs only
+  // propagate (latency-bound dependent chains, kept away from the issue-bound scan warps) and the other
+  // CTAs run the look-ahead NN scan meanwhile; otherwise every warp does both, one after the other.
+  const int NB = gridDim.x;
+  const int W = NB * kWarps;
+  const int gw = blockIdx.x * kWarps + warp;
   const int U_prop = (P.B * P.K + 31) / 32;
-  const bool split = U_prop * 2 <= W;
-  const int x_vw = split ? pw - U_prop : pw;  // < 0: propagate-only warp
-  const int x_cnt = split ? W - U_prop : W;
+  const int NPB = (U_prop + kWarps - 1) / kWarps;
+  const bool split = NPB * 4 <= NB;
+  const int x_pw = split ? (blockIdx.x < NPB ? gw : -1) : gw;  // propagate warp index, count
+  const int x_pcnt = split ? NPB * kWarps : W;
+  const int x_vb = split ? (int)blockIdx.x - NPB : (int)blockIdx.x;  // scan CTA index (< 0: none), count
+  const int x_vbcnt = split ? NB - NPB : NB;
   unsigned long long* const key0 = P.nn_key;
   unsigned long long* const key1 = P.nn_key + P.B;
 
@@ -549,24 +618,29 @@ __global__ void __launch_bounds__(kThreads, 2) pakr_loop_kernel(const __grid_con
       const bool root_only = (n == 1) && !P.n_nodes_io;
       // phase A': rows appended since the look-ahead scan
       if (!root_only && n_scanned < n) {
-        if (P.pb.unit_weights) nn_phase<DYN, true>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, pw, W, my_tile, my_bar, par0, par1 PROBE_PASS);
-        else nn_phase<DYN, false>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, pw, W, my_tile, my_bar, par0, par1 PROBE_PASS);
-        PROBE(P, 3);
+        if (P.pb.unit_weights) nn_phase<DYN, true>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
+        else nn_phase<DYN, false>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
         grid.sync();
       }
       PROBE(P, 4);
       if (leader) { const unsigned long long t = globaltimer_ns(); ph0 += t - tp; tp = t; }
+#ifdef PAKR_PROBE
+      const long long g_xstart = clock64();
+#endif
       // phase X: propagate(it) and, meanwhile, NN(it+1) over the frozen snapshot [0, n)
 #ifdef PAKR_EXP_NOAHEAD
       const bool ahead = false;
 #else
       const bool ahead = (iters + 1 < P.max_iters);
 #endif
-      prop_phase<DYN, OBS>(P, (uint32_t)r, (uint32_t)it, c_best, kcur, root_only, pw, W, sm_obs, sm_cells, sm_list PROBE_PASS);
+      prop_phase<DYN, OBS>(P, (uint32_t)r, (uint32_t)it, c_best, kcur, root_only, x_pw, x_pcnt, sm_obs, sm_cells, sm_list PROBE_PASS);
       if (ahead) {
-        if (P.pb.unit_weights) nn_phase<DYN, true>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vw, x_cnt, my_tile, my_bar, par0, par1 PROBE_PASS);
-        else nn_phase<DYN, false>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vw, x_cnt, my_tile, my_bar, par0, par1 PROBE_PASS);
+        if (P.pb.unit_weights) nn_phase<DYN, true>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
+        else nn_phase<DYN, false>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
       }
+#ifdef PAKR_PROBE
+      if (threadIdx.x == 0 && blockIdx.x < 160) atomicAdd(&P.ctrl->probe[32 + blockIdx.x], (unsigned long long)(clock64() - g_xstart));
+#endif
       // goal-key slots alternate over the whole launch (not per replan): the other slot was last
       // read before the previous grid sync and is next written after the following one
       const int slot = (int)(iterations & 1);
