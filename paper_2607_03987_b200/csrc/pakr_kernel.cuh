@@ -41,7 +41,7 @@ struct Ctrl {  // device control block (in the workspace)
   unsigned long long t_start_ns, t_first_ns, t_end_ns;
   long long iterations, inserted, nn_pairs;
   unsigned long long phase_ns[3];  // leader's time in NN / propagate / insert incl. the grid sync after each
-  unsigned long long probe[192];    // -DPAKR_PROBE: SM cycles of thread 0 of CTA 0 between probe points
+  unsigned long long probe[352];    // -DPAKR_PROBE: SM cycles of thread 0 of CTA 0 between probe points
   int n_nodes, stop;
   int path_len, solved;
   float best_cost;
@@ -164,6 +164,55 @@ __device__ __forceinline__ float dist2(const DevProblem& pb, const float (&q)[Dy
   return acc;
 }
 
+// Packed pairs of fp32 (Blackwell f32x2 instructions, SASS FADD2 / FFMA2): one issue slot does the arithmetic
+// of two queries; every component is rounded exactly like the scalar instruction, so results are bit-identical.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+  f32x2 r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) {
+  f32x2 r;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+  f32x2 r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+  f32x2 r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+
+// squared weighted distances of two queries (packed) to one node; same operations per component as dist2()
+template <int DYN, bool UNIT_W>
+__device__ __forceinline__ void dist2x2(const DevProblem& pb, const f32x2 (&q2)[DynTraits<DYN>::D],
+                                        const float (&p)[DynTraits<DYN>::DP], float& d_lo, float& d_hi) {
+  constexpr int D = DynTraits<DYN>::D;
+  f32x2 acc = pack2(0.0f, 0.0f);
+#pragma unroll
+  for (int d = 0; d < D; ++d) {
+    f32x2 delta;
+    if (d == DynTraits<DYN>::ANGLE) {
+      float qa, qb;
+      unpack2(q2[d], qa, qb);
+      delta = pack2(angle_absdiff(qa, p[d]), angle_absdiff(qb, p[d]));
+    } else {
+      delta = sub2(q2[d], pack2(p[d], p[d]));
+    }
+    if (UNIT_W) acc = fma2(delta, delta, acc);
+    else acc = fma2(mul2(delta, pack2(pb.w[d], pb.w[d])), delta, acc);
+  }
+  unpack2(acc, d_lo, d_hi);
+}
+
 // ---- NN scan of tree rows [nbeg, nend) for the queries of iteration `it` (Alg. 1 l.6-7) ----
 // CTAs vb = 0..vbcount-1 take part (vb < 0: this CTA sits out; the call is CTA-uniform).  Work units are
 // (query group of 128, node range); a CTA takes kWarps consecutive units per round, one per warp.  The
@@ -197,7 +246,7 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
     const int end = min(nend, beg + len);
     const int g_lo = ub / Reff, g_hi = min(U - 1, ub + kWarps - 1) / Reff;
     const bool shared_q = (g_hi - g_lo) <= 1;  // CTA-uniform
-    float q[kQ][D];
+    f32x2 q2[kQ / 2][D];  // queries 2h and 2h+1 of this lane, packed per dimension
     float best[kQ];
     int bidx[kQ];
     if (shared_q) {
@@ -212,23 +261,35 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
       __syncthreads();
     }
 #pragma unroll
-    for (int j = 0; j < kQ; ++j) {
-      const int s = g * QG + j * 32 + lane;
+    for (int h = 0; h < kQ / 2; ++h) {
+      float qa[D], qb[D];
+      const int sa = g * QG + (2 * h) * 32 + lane, sb = sa + 32;
       if (shared_q) {
 #pragma unroll
-        for (int d = 0; d < D; ++d) q[j][d] = sm_q[d * (2 * QG) + (g - g_lo) * QG + j * 32 + lane];
+        for (int d = 0; d < D; ++d) {
+          qa[d] = sm_q[d * (2 * QG) + (g - g_lo) * QG + (2 * h) * 32 + lane];
+          qb[d] = sm_q[d * (2 * QG) + (g - g_lo) * QG + (2 * h + 1) * 32 + lane];
+        }
       } else {
-        sample_state<D>(P.pb, P.seed, r, it, (uint32_t)s, q[j]);
+        sample_state<D>(P.pb, P.seed, r, it, (uint32_t)sa, qa);
+        sample_state<D>(P.pb, P.seed, r, it, (uint32_t)sb, qb);
       }
-      best[j] = __int_as_float(0x7f800000);
-      bidx[j] = 0x7fffffff;
-      if (P.dbg_x_rand && has && rr == 0 && nbeg == 0 && s < P.B) {
 #pragma unroll
-        for (int d = 0; d < DP; ++d) P.dbg_x_rand[(size_t)s * DP + d] = d < D ? q[j][d] : 0.0f;
+      for (int d = 0; d < D; ++d) q2[h][d] = pack2(qa[d], qb[d]);
+      if (P.dbg_x_rand && has && rr == 0 && nbeg == 0) {
+#pragma unroll
+        for (int d = 0; d < DP; ++d) {
+          if (sa < P.B) P.dbg_x_rand[(size_t)sa * DP + d] = d < D ? qa[d] : 0.0f;
+          if (sb < P.B) P.dbg_x_rand[(size_t)sb * DP + d] = d < D ? qb[d] : 0.0f;
+        }
       }
     }
+#pragma unroll
+    for (int j = 0; j < kQ; ++j) {
+      best[j] = __int_as_float(0x7f800000);
+      bidx[j] = 0x7fffffff;
+    }
     if (has) {
-    PROBE_DEP(q[0][0]);
     PROBE(P, 0);
     const int ntiles = (end - beg + TILE - 1) / TILE;
     const float* src = P.states + (size_t)beg * DP;
@@ -264,9 +325,11 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
 #pragma unroll
         for (int v = 0; v < DP / 4; ++v) nx[v] = tp[in * (DP / 4) + v];  // warp-uniform address: broadcast
 #pragma unroll
-        for (int j = 0; j < kQ; ++j) {
-          const float d2 = dist2<DYN, UNIT_W>(P.pb, q[j], p);
-          if (d2 < best[j]) { best[j] = d2; bidx[j] = base + i; }  // strict <: lowest index wins
+        for (int h = 0; h < kQ / 2; ++h) {
+          float da, db;
+          dist2x2<DYN, UNIT_W>(P.pb, q2[h], p, da, db);
+          if (da < best[2 * h]) { best[2 * h] = da; bidx[2 * h] = base + i; }  // strict <: lowest index wins
+          if (db < best[2 * h + 1]) { best[2 * h + 1] = db; bidx[2 * h + 1] = base + i; }
         }
       }
       __syncwarp();  // every lane is done with this buffer before lane 0 refills it
@@ -639,7 +702,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
         else nn_phase<DYN, false>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
       }
 #ifdef PAKR_PROBE
-      if (threadIdx.x == 0 && blockIdx.x < 160) atomicAdd(&P.ctrl->probe[32 + blockIdx.x], (unsigned long long)(clock64() - g_xstart));
+      if (threadIdx.x == 0 && blockIdx.x < 320) atomicAdd(&P.ctrl->probe[32 + blockIdx.x], (unsigned long long)(clock64() - g_xstart));
 #endif
       // goal-key slots alternate over the whole launch (not per replan): the other slot was last
       // read before the previous grid sync and is next written after the following one
