@@ -187,6 +187,13 @@ typedef struct {
 pakr_status pakr_expand_step(pakr_planner* planner, const pakr_step_args* args, void* d_workspace,
                              size_t workspace_bytes, void* cuda_stream);
 
+/* Statistics of the last pakr_plan / pakr_expand_step launch that used this workspace with the same
+ * (B, K, tree_capacity): synchronises `cuda_stream`, then copies the device control block into *out (HOST).
+ * After pakr_expand_step: iterations = 1, phase_ms[0] = the NN scan of the whole tree, [1] = propagate,
+ * [2] = insert, each including its grid barrier. */
+pakr_status pakr_read_stats(pakr_planner* planner, int32_t B, int32_t K, int64_t tree_capacity,
+                            void* d_workspace, size_t workspace_bytes, void* cuda_stream, pakr_stats* out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -37,7 +37,7 @@ size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
   size_t states, actions, parents, costs, nn_key, unit_count, scr_state, scr_ctrl, scr_cost, scr_parent,
-      scr_flags, ctrl, path_rev, path_nodes, path_states, path_controls, total;
+      scr_flags, xq, ctrl, path_rev, path_nodes, path_states, path_controls, total;
 };
 
 Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap) {
@@ -50,7 +50,8 @@ Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap) {
   L.parents = take((size_t)cap * 4);
   L.costs = take((size_t)cap * 4);
   L.nn_key = take((size_t)B * 16);  // two iterations in flight
-  L.unit_count = take(U * 4);
+  L.unit_count = take(std::max<size_t>(U, kFuseUnits + 8) * 4);
+  L.xq = take((size_t)B * pl->DP * 4);
   L.scr_state = take(slots * pl->DP * 4);
   L.scr_ctrl = take(slots * 16);
   L.scr_cost = take(slots * 4);
@@ -363,6 +364,7 @@ void fill_common(const pakr_planner* pl, Params& P, const Layout& L, char* ws, i
   P.pb = pl->pb;
   P.nn_key = reinterpret_cast<unsigned long long*>(ws + L.nn_key);
   P.unit_count = reinterpret_cast<unsigned*>(ws + L.unit_count);
+  P.xq = reinterpret_cast<float*>(ws + L.xq);
   P.scr_state = reinterpret_cast<float*>(ws + L.scr_state);
   P.scr_ctrl = reinterpret_cast<float*>(ws + L.scr_ctrl);
   P.scr_cost = reinterpret_cast<float*>(ws + L.scr_cost);
@@ -374,6 +376,28 @@ void fill_common(const pakr_planner* pl, Params& P, const Layout& L, char* ws, i
   P.path_states = reinterpret_cast<float*>(ws + L.path_states);
   P.path_controls = reinterpret_cast<float*>(ws + L.path_controls);
   P.B = B; P.K = K; P.cap = (int)cap;
+}
+
+void fill_stats(const Ctrl* hc, int64_t BK, pakr_stats* out) {
+  pakr_stats& s = *out;
+  std::memset(&s, 0, sizeof(s));
+  s.iterations = hc->iterations;
+  s.children = hc->iterations * BK;
+  s.inserted = hc->inserted;
+  s.nn_pairs = hc->nn_pairs;
+  for (int i = 0; i < 3; ++i) s.phase_ms[i] = (double)hc->phase_ns[i] * 1e-6;
+  for (int i = 0; i < 352; ++i) s.probe_cycles[i] = (int64_t)hc->probe[i];
+  s.replans_run = hc->replans_run;
+  s.replans_solved = hc->replans_solved;
+  s.termination = hc->termination;
+  s.first_solution_ms = hc->replans_solved > 0 ? (double)(hc->t_first_ns - hc->t_start_ns) * 1e-6 : -1.0;
+  s.device_ms = (double)(hc->t_end_ns - hc->t_start_ns) * 1e-6;
+  for (int i = 0; i < kStatsMax && i < hc->replans_run; ++i) {
+    s.replan_cost[i] = hc->replan_cost[i];
+    s.replan_nodes[i] = hc->replan_nodes[i];
+    s.replan_iters[i] = hc->replan_iters[i];
+    s.replan_end_ms[i] = (double)(hc->replan_end_ns[i] - hc->t_start_ns) * 1e-6;
+  }
 }
 
 // memset of the control words + one cooperative launch; everything on `stream`
@@ -432,25 +456,7 @@ extern "C" pakr_status pakr_plan(pakr_planner* pl, const pakr_plan_opts* o, void
   CUDA_TRY(pl, cudaMemcpyAsync(hc, P.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, stream));
   CUDA_TRY(pl, cudaStreamSynchronize(stream));
   // results
-  pakr_stats& s = out->stats;
-  std::memset(&s, 0, sizeof(s));
-  s.iterations = hc->iterations;
-  s.children = hc->iterations * BK;
-  s.inserted = hc->inserted;
-  s.nn_pairs = hc->nn_pairs;
-  for (int i = 0; i < 3; ++i) s.phase_ms[i] = (double)hc->phase_ns[i] * 1e-6;
-  for (int i = 0; i < 352; ++i) s.probe_cycles[i] = (int64_t)hc->probe[i];
-  s.replans_run = hc->replans_run;
-  s.replans_solved = hc->replans_solved;
-  s.termination = hc->termination;
-  s.first_solution_ms = hc->replans_solved > 0 ? (double)(hc->t_first_ns - hc->t_start_ns) * 1e-6 : -1.0;
-  s.device_ms = (double)(hc->t_end_ns - hc->t_start_ns) * 1e-6;
-  for (int i = 0; i < kStatsMax && i < hc->replans_run; ++i) {
-    s.replan_cost[i] = hc->replan_cost[i];
-    s.replan_nodes[i] = hc->replan_nodes[i];
-    s.replan_iters[i] = hc->replan_iters[i];
-    s.replan_end_ms[i] = (double)(hc->replan_end_ns[i] - hc->t_start_ns) * 1e-6;
-  }
+  fill_stats(hc, BK, &out->stats);
   out->final_tree_nodes = hc->n_nodes;
   out->outcome = hc->solved ? PAKR_SOLVED : PAKR_NO_SOLUTION;
   out->cost = hc->solved ? (double)hc->best_cost : (double)INFINITY;
@@ -504,4 +510,19 @@ extern "C" pakr_status pakr_expand_step(pakr_planner* pl, const pakr_step_args* 
   P.dbg_child_flags = a->child_flags; P.dbg_n_inserted = a->n_inserted; P.dbg_goal_node = a->goal_node;
   P.dbg_new_c_best = a->new_c_best;
   return launch(pl, P, reinterpret_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" pakr_status pakr_read_stats(pakr_planner* pl, int32_t B, int32_t K, int64_t cap, void* d_ws,
+                                       size_t ws_bytes, void* cuda_stream, pakr_stats* out) {
+  if (!pl) return PAKR_ERR_INVALID_ARG;
+  if (!d_ws || !out || !sizes_ok(B, K, cap)) return fail(pl, PAKR_ERR_INVALID_ARG, "null pointer or sizes out of range");
+  const Layout L = make_layout(pl, B, K, cap);
+  if (ws_bytes < L.total) return fail(pl, PAKR_ERR_WORKSPACE_TOO_SMALL, "workspace smaller than pakr_workspace_bytes()");
+  cudaStream_t stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+  Ctrl* hc = static_cast<Ctrl*>(pl->h_pinned);
+  CUDA_TRY(pl, cudaSetDevice(pl->device));
+  CUDA_TRY(pl, cudaMemcpyAsync(hc, static_cast<char*>(d_ws) + L.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, stream));
+  CUDA_TRY(pl, cudaStreamSynchronize(stream));
+  fill_stats(hc, (int64_t)B * K, out);
+  return PAKR_OK;
 }

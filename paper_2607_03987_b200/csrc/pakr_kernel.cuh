@@ -58,6 +58,7 @@ struct Params {
   float* states; float* actions; int* parents; float* costs;
   // per-iteration work buffers
   unsigned long long* nn_key;  // [2][B] (d2 bits << 32) | node, combined with atomicMin; two iterations in flight
+  float* xq;                   // [B][Dp] sampled states of the iteration whose NN is being prepared
   unsigned* unit_count;        // [ceil(B*K/32)] survivors per warp unit
   float* scr_state; float* scr_ctrl; float* scr_cost; int* scr_parent; int* scr_flags;
   Ctrl* ctrl;
@@ -213,6 +214,35 @@ __device__ __forceinline__ void dist2x2(const DevProblem& pb, const f32x2 (&q2)[
   unpack2(acc, d_lo, d_hi);
 }
 
+// Scores `cnt` rows of a shared-memory tile (node ids base, base+1, ...) against the lane's kQ queries.
+template <int DYN, bool UNIT_W>
+__device__ __forceinline__ void scan_rows(const DevProblem& pb, const float4* __restrict__ tp, int cnt, int base,
+                                          const f32x2 (&q2)[kQ / 2][DynTraits<DYN>::D], float (&best)[kQ],
+                                          int (&bidx)[kQ]) {
+  constexpr int DP = DynTraits<DYN>::DP;
+  float4 nx[DP / 4];  // row i+1 is fetched while row i is scored (hides the shared-memory latency)
+#pragma unroll
+  for (int v = 0; v < DP / 4; ++v) nx[v] = tp[v];
+#pragma unroll 2
+  for (int i = 0; i < cnt; ++i) {
+    float p[DP];
+#pragma unroll
+    for (int v = 0; v < DP / 4; ++v) {
+      p[4 * v] = nx[v].x; p[4 * v + 1] = nx[v].y; p[4 * v + 2] = nx[v].z; p[4 * v + 3] = nx[v].w;
+    }
+    const int in = min(i + 1, cnt - 1);
+#pragma unroll
+    for (int v = 0; v < DP / 4; ++v) nx[v] = tp[in * (DP / 4) + v];  // warp-uniform address: broadcast
+#pragma unroll
+    for (int h = 0; h < kQ / 2; ++h) {
+      float da, db;
+      dist2x2<DYN, UNIT_W>(pb, q2[h], p, da, db);
+      if (da < best[2 * h]) { best[2 * h] = da; bidx[2 * h] = base + i; }  // strict <: lowest index wins
+      if (db < best[2 * h + 1]) { best[2 * h + 1] = db; bidx[2 * h + 1] = base + i; }
+    }
+  }
+}
+
 // ---- NN scan of tree rows [nbeg, nend) for the queries of iteration `it` (Alg. 1 l.6-7) ----
 // CTAs vb = 0..vbcount-1 take part (vb < 0: this CTA sits out; the call is CTA-uniform).  Work units are
 // (query group of 128, node range); a CTA takes kWarps consecutive units per round, one per warp.  The
@@ -221,7 +251,7 @@ __device__ __forceinline__ void dist2x2(const DevProblem& pb, const f32x2 (&q2)[
 // atomicMin, so any split of the rows over warps / phases gives the same result.
 template <int DYN, bool UNIT_W>
 __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, uint32_t r, uint32_t it,
-                                         unsigned long long* key, int vb, int vbcount, float* sm_tile,
+                                         unsigned long long* key, int vb, int vbcount, bool write_q, float* sm_tile,
                                          uint64_t* sm_bar, float* sm_q, unsigned long long* sm_keys, uint32_t& par0,
                                          uint32_t& par1 PROBE_ARG) {
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
@@ -283,6 +313,13 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
           if (sb < P.B) P.dbg_x_rand[(size_t)sb * DP + d] = d < D ? qb[d] : 0.0f;
         }
       }
+      if (write_q && has && rr == 0) {  // keep the sampled states for the tail scan of the insert phase
+#pragma unroll
+        for (int d = 0; d < D; ++d) {
+          if (sa < P.B) P.xq[(size_t)sa * DP + d] = qa[d];
+          if (sb < P.B) P.xq[(size_t)sb * DP + d] = qb[d];
+        }
+      }
     }
 #pragma unroll
     for (int j = 0; j < kQ; ++j) {
@@ -311,27 +348,7 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
       if (t == 0) PROBE(P, 1);
       const float4* tp = reinterpret_cast<const float4*>(sm_tile + (t & 1) * TF);
       const int base = beg + t * TILE;
-      float4 nx[DP / 4];  // row i+1 is fetched while row i is scored (hides the shared-memory latency)
-#pragma unroll
-      for (int v = 0; v < DP / 4; ++v) nx[v] = tp[v];
-#pragma unroll 2
-      for (int i = 0; i < cnt; ++i) {
-        float p[DP];
-#pragma unroll
-        for (int v = 0; v < DP / 4; ++v) {
-          p[4 * v] = nx[v].x; p[4 * v + 1] = nx[v].y; p[4 * v + 2] = nx[v].z; p[4 * v + 3] = nx[v].w;
-        }
-        const int in = min(i + 1, cnt - 1);
-#pragma unroll
-        for (int v = 0; v < DP / 4; ++v) nx[v] = tp[in * (DP / 4) + v];  // warp-uniform address: broadcast
-#pragma unroll
-        for (int h = 0; h < kQ / 2; ++h) {
-          float da, db;
-          dist2x2<DYN, UNIT_W>(P.pb, q2[h], p, da, db);
-          if (da < best[2 * h]) { best[2 * h] = da; bidx[2 * h] = base + i; }  // strict <: lowest index wins
-          if (db < best[2 * h + 1]) { best[2 * h + 1] = db; bidx[2 * h + 1] = base + i; }
-        }
-      }
+      scan_rows<DYN, UNIT_W>(P.pb, tp, cnt, base, q2, best, bidx);
       __syncwarp();  // every lane is done with this buffer before lane 0 refills it
     }
     PROBE_DEP(best[0]);
@@ -512,9 +529,67 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
 
 // ---- phase C: ordered insert at the tree tail, goal winner (Alg. 1 l.13-15; P19, P20) ----
 // Returns the number of survivors of this iteration (identical in every thread of the grid).
+//
+// Fused tail scan: when the survivors are few, the NN of the NEXT iteration is completed here as well, straight
+// from the scratch rows (their node ids n + rank are known from the prefix), so that no separate scan phase and
+// barrier is needed before the next propagate.  `fused` tells the caller (grid-uniform).
+constexpr int kFuseUnits = 2048;  // per-unit prefix kept in shared memory up to this many warp units
+
+template <int DYN, bool UNIT_W>
+__device__ __forceinline__ void tail_scan_items(const Params& P, int n, int U, const int* sm_upre,
+                                                unsigned long long* key_next, float* sm_tile, uint64_t* sm_bar,
+                                                uint32_t& par0) {
+  using T = DynTraits<DYN>;
+  constexpr int D = T::D, DP = T::DP, QG = 32 * kQ;
+  constexpr int RU = TileCfg<DYN>::TILE / 32;  // units per item: their survivors always fit one tile buffer
+  const int lane = threadIdx.x & 31;
+  const int W = gridDim.x * kWarps;
+  const int gw = blockIdx.x * kWarps + (threadIdx.x >> 5);
+  const int G = (P.B + QG - 1) / QG;
+  const int NR = (U + RU - 1) / RU;
+  for (int i = W - 1 - gw; i < G * NR; i += W) {  // from the far end: the copy units start at warp 0
+    const int g = i / NR, rg = i - g * NR;
+    const int ua = rg * RU, ub = min(U, ua + RU);
+    const int rows = sm_upre[ub] - sm_upre[ua];
+    if (rows == 0) continue;
+    if (lane == 0) mbar_expect_tx(&sm_bar[0], (uint32_t)rows * DP * 4);
+    __syncwarp();
+    if (lane < ub - ua) {
+      const int u = ua + lane;
+      const int cnt = sm_upre[u + 1] - sm_upre[u];
+      if (cnt > 0)
+        tma_load_1d(sm_tile + (size_t)(sm_upre[u] - sm_upre[ua]) * DP, P.scr_state + (size_t)u * 32 * DP,
+                    (uint32_t)cnt * DP * 4, &sm_bar[0]);
+    }
+    f32x2 q2[kQ / 2][D];
+    float best[kQ];
+    int bidx[kQ];
+#pragma unroll
+    for (int h = 0; h < kQ / 2; ++h) {
+      const int sa = min(g * QG + (2 * h) * 32 + lane, P.B - 1), sb = min(g * QG + (2 * h + 1) * 32 + lane, P.B - 1);
+#pragma unroll
+      for (int d = 0; d < D; ++d) q2[h][d] = pack2(__ldcg(&P.xq[(size_t)sa * DP + d]), __ldcg(&P.xq[(size_t)sb * DP + d]));
+    }
+#pragma unroll
+    for (int j = 0; j < kQ; ++j) { best[j] = __int_as_float(0x7f800000); bidx[j] = 0x7fffffff; }
+    mbar_wait(&sm_bar[0], par0);
+    par0 ^= 1;
+    scan_rows<DYN, UNIT_W>(P.pb, reinterpret_cast<const float4*>(sm_tile), rows, n + sm_upre[ua], q2, best, bidx);
+#pragma unroll
+    for (int j = 0; j < kQ; ++j) {
+      const int s = g * QG + j * 32 + lane;
+      if (s < P.B && bidx[j] != 0x7fffffff)
+        atomicMin(&key_next[s], ((unsigned long long)__float_as_uint(best[j]) << 32) | (unsigned)bidx[j]);
+    }
+    __syncwarp();  // every lane is done with the tile before it is refilled
+  }
+}
+
 template <int DYN>
 __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, unsigned long long* key_done,
-                                            int* sm_pref PROBE_ARG) {
+                                            bool want_tail, unsigned long long* key_next, int* sm_pref,
+                                            int* sm_upre, float* sm_tile, uint64_t* sm_bar, uint32_t& par0,
+                                            bool& fused PROBE_ARG) {
   using T = DynTraits<DYN>;
   constexpr int DP = T::DP;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -523,17 +598,29 @@ __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, u
   const int BK = P.B * P.K;
   constexpr int cpw = 32;
   const int U = (BK + cpw - 1) / cpw;  // warp units of the propagate phase (32 children each)
-  // exclusive prefix of the per-unit counts at chunk granularity, redundantly in every CTA
-  const int cpt = (U + kThreads - 1) / kThreads;  // units per thread-chunk
+  const bool small = U <= kFuseUnits;  // per-unit prefix in shared memory, else per thread-chunk
+  constexpr int UPT = kFuseUnits / kThreads;
+  const int cpt = small ? UPT : (U + kThreads - 1) / kThreads;  // units per thread-chunk
   int mine = 0;
-  for (int v = threadIdx.x * cpt; v < min(U, (threadIdx.x + 1) * cpt); ++v) mine += (int)__ldcg(&P.unit_count[v]);
+  int c[UPT];
+  if (small) {
+#pragma unroll
+    for (int k = 0; k < UPT; ++k) {
+      const int v = threadIdx.x * UPT + k;
+      c[k] = v < U ? (int)__ldcg(&P.unit_count[v]) : 0;
+    }
+#pragma unroll
+    for (int k = 0; k < UPT; ++k) mine += c[k];
+  } else {
+    for (int v = threadIdx.x * cpt; v < min(U, (threadIdx.x + 1) * cpt); ++v) mine += (int)__ldcg(&P.unit_count[v]);
+  }
   int incl = mine;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) {
     const int t = __shfl_up_sync(0xffffffffu, incl, o);
     if (lane >= o) incl += t;
   }
-  __syncthreads();  // sm_pref reuse across iterations
+  __syncthreads();  // shared-memory reuse across iterations
   if (lane == 31) sm_pref[kThreads + warp] = incl;
   __syncthreads();
   int wbase = 0, total = 0;
@@ -544,17 +631,32 @@ __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, u
     total += t;
   }
   sm_pref[threadIdx.x] = wbase + incl - mine;
+  if (small) {
+    int run = wbase + incl - mine;
+#pragma unroll
+    for (int k = 0; k < UPT; ++k) {
+      sm_upre[threadIdx.x * UPT + k] = run;
+      run += c[k];
+    }
+    if (threadIdx.x == kThreads - 1) sm_upre[kFuseUnits] = run;  // == total
+  }
   __syncthreads();
   PROBE(P, 10);
   const int room = P.cap - n;
   for (int u = gw; u < U; u += W) {
-    const int ch = u / cpt;
-    int part = 0;
-    for (int v = ch * cpt + lane; v < u; v += 32) part += (int)__ldcg(&P.unit_count[v]);
+    int off, cnt;
+    if (small) {
+      off = sm_upre[u];
+      cnt = sm_upre[u + 1] - off;
+    } else {
+      const int ch = u / cpt;
+      int part = 0;
+      for (int v = ch * cpt + lane; v < u; v += 32) part += (int)__ldcg(&P.unit_count[v]);
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
-    const int off = sm_pref[ch] + part;
-    const int cnt = (int)__ldcg(&P.unit_count[u]);
+      for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+      off = sm_pref[ch] + part;
+      cnt = (int)__ldcg(&P.unit_count[u]);
+    }
     const int pos = off + lane;
     if (lane < cnt && pos < room) {
       const size_t slot = (size_t)u * cpw + lane;
@@ -574,6 +676,16 @@ __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, u
     }
   }
   PROBE(P, 11);
+  // fused tail scan of the next iteration's NN (one item per warp at most, every survivor inserted)
+  {
+    constexpr int RU = TileCfg<DYN>::TILE / 32;
+    const int G = (P.B + 32 * kQ - 1) / (32 * kQ);
+    fused = want_tail && small && total <= room && G * ((U + RU - 1) / RU) <= W;
+    if (fused && total > 0) {
+      if (P.pb.unit_weights) tail_scan_items<DYN, true>(P, n, U, sm_upre, key_next, sm_tile, sm_bar, par0);
+      else tail_scan_items<DYN, false>(P, n, U, sm_upre, key_next, sm_tile, sm_bar, par0);
+    }
+  }
   // the NN keys this iteration consumed are free again: reset them for iteration i+2
   for (int s = blockIdx.x * kThreads + threadIdx.x; s < P.B; s += gridDim.x * kThreads) key_done[s] = kKeyNone;
   return total;
@@ -681,8 +793,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       const bool root_only = (n == 1) && !P.n_nodes_io;
       // phase A': rows appended since the look-ahead scan
       if (!root_only && n_scanned < n) {
-        if (P.pb.unit_weights) nn_phase<DYN, true>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
-        else nn_phase<DYN, false>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
+        if (P.pb.unit_weights) nn_phase<DYN, true>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
+        else nn_phase<DYN, false>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
         grid.sync();
       }
       PROBE(P, 4);
@@ -698,8 +810,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
 #endif
       prop_phase<DYN, OBS>(P, (uint32_t)r, (uint32_t)it, c_best, kcur, root_only, x_pw, x_pcnt, sm_obs, sm_cells, sm_list PROBE_PASS);
       if (ahead) {
-        if (P.pb.unit_weights) nn_phase<DYN, true>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
-        else nn_phase<DYN, false>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
+        if (P.pb.unit_weights) nn_phase<DYN, true>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
+        else nn_phase<DYN, false>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
       }
 #ifdef PAKR_PROBE
       if (threadIdx.x == 0 && blockIdx.x < 320) atomicAdd(&P.ctrl->probe[32 + blockIdx.x], (unsigned long long)(clock64() - g_xstart));
@@ -708,11 +820,15 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       // read before the previous grid sync and is next written after the following one
       const int slot = (int)(iterations & 1);
       if (leader) P.ctrl->goal_key[slot ^ 1] = kKeyNone;
+      fence_proxy_async();  // scratch rows written with st.global may be read by TMA in the insert phase
       grid.sync();
+      fence_proxy_async();
       PROBE(P, 9);
       if (leader) { const unsigned long long t = globaltimer_ns(); ph1 += t - tp; tp = t; }
       // phase C
-      const int total = insert_phase<DYN>(P, n, slot, kcur, sm_pref PROBE_PASS);
+      bool fused = false;
+      const int total = insert_phase<DYN>(P, n, slot, kcur, ahead, knext, sm_pref, reinterpret_cast<int*>(sm_q), my_tile,
+                                          my_bar, par0, fused PROBE_PASS);
       const int added = min(total, P.cap - n);
       if (leader && P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) P.ctrl->stop = 1;
       __threadfence();
@@ -723,7 +839,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       if (leader) { const unsigned long long t = globaltimer_ns(); ph2 += t - tp; tp = t; }
       fence_proxy_async();
       nn_pairs += (long long)P.B * n;  // (query, node) pairs of this iteration's NN
-      n_scanned = ahead ? n : 0;
+      n_scanned = ahead ? (fused ? n + added : n) : 0;  // fused: NN(it+1) already covers the new rows
       n += added;
       inserted += added;
       ++iterations;

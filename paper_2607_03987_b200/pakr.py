@@ -102,7 +102,7 @@ class _StepArgs(C.Structure):
 
 
 EXPORTS = ["pakr_create", "pakr_destroy", "pakr_last_error", "pakr_workspace_bytes", "pakr_get_tree_layout",
-           "pakr_plan", "pakr_expand_step"]
+           "pakr_plan", "pakr_expand_step", "pakr_read_stats"]
 
 _lib = None
 
@@ -127,6 +127,9 @@ def lib():
                                 C.POINTER(_Result)]
         L.pakr_expand_step.restype = C.c_int
         L.pakr_expand_step.argtypes = [C.c_void_p, C.POINTER(_StepArgs), C.c_void_p, C.c_size_t, C.c_void_p]
+        L.pakr_read_stats.restype = C.c_int
+        L.pakr_read_stats.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.c_size_t, C.c_void_p,
+                                      C.POINTER(_Stats)]
         _lib = L
     return _lib
 
@@ -242,6 +245,16 @@ class Planner:
                     actions=view(lay.actions_off, n * 4, torch.float32).reshape(n, 4)[:, :self.m].copy(),
                     parents=view(lay.parents_off, n, torch.int32).copy(),
                     costs=view(lay.costs_off, n, torch.float32).copy())
+
+    def read_stats(self, B: int, K: int, tree_capacity: int, workspace=None) -> dict:
+        """pakr_read_stats: statistics of the last launch on this workspace (synchronises the stream)."""
+        ws = workspace if workspace is not None else self.workspace(B, K, tree_capacity)
+        st = _Stats()
+        self._check(lib().pakr_read_stats(self._h, B, K, tree_capacity, C.c_void_p(ws.data_ptr()), ws.numel(),
+                                          C.c_void_p(self._stream()), C.byref(st)))
+        return dict(iterations=int(st.iterations), children=int(st.children), inserted=int(st.inserted),
+                    nn_pairs=int(st.nn_pairs), device_ms=float(st.device_ms), phase_ms=[float(v) for v in st.phase_ms],
+                    probe_cycles=[int(v) for v in st.probe_cycles])
 
     # ---- pakr_expand_step ----
     def new_tree(self, capacity: int, host: Optional[dict] = None) -> dict:

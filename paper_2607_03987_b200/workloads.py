@@ -235,12 +235,13 @@ def config5(B: int = 1024, K: int = 16, env_seed: int = 505,
 CONFIGS = {"C1": config1, "C2": config2, "C3": config3, "C4": config4, "C5": config5}
 
 
-def random_tree(problem: Problem, n: int, seed: int) -> dict[str, np.ndarray]:
+def random_tree(problem: Problem, n: int, seed: int, flat: bool = False) -> dict[str, np.ndarray]:
     """Teacher-forcing / NN-microbench input: n nodes uniform in the state box.
 
     Node 0 is the start.  Parents point to a uniformly random earlier node, costs grow by one
     edge duration along parents, so the tree invariants hold by construction.  Positions are NOT
-    filtered against obstacles (the NN scan and the propagation do not care).
+    filtered against obstacles (the NN scan and the propagation do not care).  flat=True makes every node a
+    child of the root (vectorised; for multi-million-node microbenchmark trees).
     """
     rng = np.random.Generator(np.random.PCG64(seed))
     D, m = problem.state_dim, problem.control_dim
@@ -251,10 +252,15 @@ def random_tree(problem: Problem, n: int, seed: int) -> dict[str, np.ndarray]:
     actions = rng.uniform(problem.control_lo, problem.control_hi, size=(n, m)).astype(np.float32)
     actions[0] = 0
     parents = np.full(n, -1, np.int32)
-    if n > 1:
+    if n > 1 and not flat:
         parents[1:] = (rng.random(n - 1) * np.arange(1, n)).astype(np.int32)
+    elif n > 1:
+        parents[1:] = 0
     edge = np.float32(problem.steps_per_edge) * np.float32(problem.dt)
     costs = np.zeros(n, np.float32)
-    for i in range(1, n):
-        costs[i] = costs[parents[i]] + edge
+    if flat:
+        costs[1:] = edge
+    else:
+        for i in range(1, n):
+            costs[i] = costs[parents[i]] + edge
     return {"states": states, "actions": actions, "parents": parents, "costs": costs}

@@ -159,3 +159,32 @@ def test_abi_errors(pakr):
             pakr.Planner(bad)
         assert e.value.status in (1, 2)
     pl.close()
+
+
+@pytest.mark.parametrize("name,iters", [("C1", 12), ("C2", 9), ("C3", 6)])
+def test_plan_loop_equals_chain_of_single_steps(pakr, name, iters):
+    """The device-resident loop (NN look-ahead scan, fused tail scan, two key buffers) must build exactly
+    the tree that `iters` separate pakr_expand_step calls build (no look-ahead there): bit-exact."""
+    p, cfg = wl.CONFIGS[name]()
+    pl = pakr.Planner(p)
+    cap = 1 + iters * cfg.B * cfg.K
+    res = pl.plan(7, cfg.B, cfg.K, cap, 1, max_iters_per_replan=iters)
+    n_loop = res["final_tree_nodes"]
+    loop_tree = pl.read_tree(cfg.B, cfg.K, cap, n_loop)
+    tree = pl.new_tree(cap)
+    c_best = float("inf")
+    done = 0
+    for it in range(iters):
+        out = pl.expand_step(tree, 7, 0, it, cfg.B, cfg.K, c_best=c_best)
+        done += 1
+        if out["goal_node"] >= 0:
+            break
+    assert done == res["iterations"]
+    n_chain = int(tree["n_nodes"][0].item())
+    assert n_chain == n_loop and n_loop > cfg.B
+    D, m = p.state_dim, p.control_dim
+    np.testing.assert_array_equal(tree["states"][:n_chain, :D].cpu().numpy(), loop_tree["states"])
+    np.testing.assert_array_equal(tree["actions"][:n_chain, :m].cpu().numpy(), loop_tree["actions"])
+    np.testing.assert_array_equal(tree["parents"][:n_chain].cpu().numpy(), loop_tree["parents"])
+    np.testing.assert_array_equal(tree["costs"][:n_chain].cpu().numpy(), loop_tree["costs"])
+    pl.close()
