@@ -24,7 +24,7 @@ sys.path.insert(0, ROOT)
 
 import numpy as np  # noqa: E402
 
-from paper_2607_03987_b200 import workloads as wl  # noqa: E402
+from paper_2607_03987_b200 import replicas, workloads as wl  # noqa: E402
 
 WORKLOAD = "C2"
 METRIC = "expanded nodes/s"
@@ -35,10 +35,11 @@ NCU_TRAFFIC_BYTES_PER_LAUNCH = None
 
 
 def algorithmic_ops(problem, nn_pairs: int, children: int) -> dict:
-    """Algorithmic fp32 lane-operations of one launch (DESIGN.md "Roofline"): the NN scan evaluates
+    """Algorithmic fp32 lane-operations of one launch (DESIGN.md "Measurement"): the NN scan evaluates
     nn_pairs (query, node) pairs at D sub + D fma + compare + select each (+ D mul if weighted, +2 on an
-    angle dim); a child costs S steps of (8 D integrator ops + F dynamics ops + 2 per bounded dim + c_obs
-    per obstacle)."""
+    angle dim); a child costs S steps of (8 D integrator ops + F dynamics ops + 2 per bounded dim + the
+    obstacle broad phase: cell index and header, 10 ops, plus ONE obstacle test -- not one per obstacle,
+    because the grid culls the rest exactly)."""
     D = problem.state_dim
     weighted = not np.all(problem.nn_weight == 1.0)
     n_angle = int((problem.dim_kind == 1).sum())
@@ -48,7 +49,7 @@ def algorithmic_ops(problem, nn_pairs: int, children: int) -> dict:
     integ = 8 * D if problem.integrator == wl.INT_RK4 else 2 * D
     n_bounded = int((np.isfinite(problem.state_lo) & (problem.dim_kind == 0)).sum())
     c_obs = 2 * problem.pos_dim if problem.obstacle_type == wl.OBS_AABB else 5
-    per_child = problem.steps_per_edge * (stages * f_dyn + integ + 2 * n_bounded + c_obs * problem.n_obstacles)
+    per_child = problem.steps_per_edge * (stages * f_dyn + integ + 2 * n_bounded + 10 + c_obs)
     return dict(nn=nn_pairs * nn_per_pair, prop=children * per_child, nn_per_pair=nn_per_pair, per_child=per_child)
 
 
@@ -158,7 +159,7 @@ def main():
         torch.cuda.synchronize()
 
     # replicas only: rank r plans seeds r, r + world, ...
-    seeds = [rank + world * i for i in range(args.warmup + args.steps)]
+    seeds = replicas.replica_seeds(rank, world, args.warmup + args.steps)
     for s in seeds[:max(args.warmup, 3)]:
         pl.plan(s, cfg.B, cfg.K, cfg.tree_capacity, cfg.n_replans)
     sampler = ClockSampler(local)
@@ -181,15 +182,10 @@ def main():
     clocks = sampler.finish()
     dev_ms = [a.elapsed_time(b) for a, b in ev]
     kern_ms = [r["device_ms"] for r in results]
-    t = torch.tensor([sum(dev_ms), sum(wall) * 1e3, float(sum(r["children"] for r in results))], dtype=torch.float64,
-                     device=f"cuda:{local}")
-    tmax, tsum = t.clone(), t.clone()
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-    total_children = float(tsum[2].item())
-    value = total_children / (tmax[0].item() * 1e-3)
-    e2e = total_children / (tmax[1].item() * 1e-3)
+    agg = replicas.aggregate(sum(dev_ms), sum(wall) * 1e3, float(sum(r["children"] for r in results)),
+                             dist=dist if world > 1 else None, device=f"cuda:{local}")
+    value, e2e = agg["value"], agg["e2e"]
+    ms_per_step = agg["device_ms"] / args.steps
 
     if rank == 0:
         # roofline of the one kernel (ALU-bound: DESIGN.md "Roofline")
@@ -204,7 +200,7 @@ def main():
         best100 = [pl.plan(s, cfg.B, cfg.K, cfg.tree_capacity, 4096, time_budget_ms=100.0)["cost"] for s in range(5)]
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": tmax[0].item() / args.steps, "higher_is_better": True,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": WORKLOAD, "dynamics": problem.name, "B": cfg.B, "K": cfg.K,
                        "tree_capacity": cfg.tree_capacity, "n_replans": cfg.n_replans,
@@ -219,7 +215,8 @@ def main():
                          "kernel": "pakr_loop_kernel<DI3,BOX>", "avg_launch_ms": 1e3 * launch_s / args.steps,
                          "algorithmic_ops_per_launch": alg / args.steps,
                          "nn_share_of_ops": sum(o["nn"] for o in ops) / alg,
-                         "peak_basis": f"148 SM x 128 fp32 lanes x {sm_max:.0f} MHz (nominal max clock)",
+                         "nn_fma_pipe_frac": sum(r["nn_pairs"] for r in results) * 2 * problem.state_dim / launch_s / 1e12 / peak,
+                         "peak_basis": f"148 SM x 4 schedulers x 32 lanes x {sm_max:.0f} MHz issue slots (= FMA-pipe lane-ops/s)",
                          "frac_at_measured_clock": (achieved / (148 * 128 * clocks['sm_mhz'] * 1e6 / 1e12))
                          if clocks["sm_mhz"] else None},
             "first_solution_ms_median": statistics.median(first) if first else None,
@@ -227,7 +224,7 @@ def main():
             "final_cost_median": statistics.median(r["cost"] for r in results),
             "iterations_per_step": float(np.mean([r["iterations"] for r in results])),
             "phase_share": {k: sum(r["phase_ms"][i] for r in results) / sum(kern_ms)
-                            for i, k in enumerate(("nn", "propagate", "insert"))},
+                            for i, k in enumerate(("nn_tail_scan", "propagate_and_nn_lookahead", "insert_and_fused_tail"))},
             "inserted_nodes_per_s": sum(r["inserted"] for r in results) / (sum(dev_ms) * 1e-3),
             "solved": sum(r["outcome"] for r in results),
         }
