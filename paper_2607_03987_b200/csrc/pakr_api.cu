@@ -23,12 +23,17 @@ struct pakr_planner {
   uint16_t* d_grid_list = nullptr;
   int num_sms = 0, blocks_per_sm = 0;
   size_t smem_bytes = 0;
-  const void* kernel = nullptr;
+  const void* kernel = nullptr;         // tiled NN scan
+  const void* kernel_stream = nullptr;  // streaming NN tier (B <= kStreamB)
   void* h_pinned = nullptr;  // Ctrl + path staging
   std::string err;
 };
 
 static thread_local std::string g_create_err;
+
+// defined in pakr_kernel_inst.cu (one translation unit per NN tier)
+extern "C" const void* pakr_select_kernel_tiled(int dyn, int obs);
+extern "C" const void* pakr_select_kernel_stream(int dyn, int obs);
 
 namespace {
 
@@ -68,22 +73,6 @@ Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap) {
 
 bool sizes_ok(int64_t B, int64_t K, int64_t cap) {
   return B >= 1 && K >= 1 && K <= 4096 && B * K <= (1ll << 24) && cap >= 2 && cap <= (1ll << 30);
-}
-
-template <int DYN, int OBS> const void* kernel_ptr() { return (const void*)&pakr_loop_kernel<DYN, OBS>; }
-
-const void* select_kernel(int dyn, int obs) {
-  switch (dyn * 2 + obs) {
-    case DYN_DI2 * 2 + OBS_CIRCLE: return kernel_ptr<DYN_DI2, OBS_CIRCLE>();
-    case DYN_DI2 * 2 + OBS_BOX: return kernel_ptr<DYN_DI2, OBS_BOX>();
-    case DYN_DI3 * 2 + OBS_CIRCLE: return kernel_ptr<DYN_DI3, OBS_CIRCLE>();
-    case DYN_DI3 * 2 + OBS_BOX: return kernel_ptr<DYN_DI3, OBS_BOX>();
-    case DYN_UNI2 * 2 + OBS_CIRCLE: return kernel_ptr<DYN_UNI2, OBS_CIRCLE>();
-    case DYN_UNI2 * 2 + OBS_BOX: return kernel_ptr<DYN_UNI2, OBS_BOX>();
-    case DYN_QUAD * 2 + OBS_CIRCLE: return kernel_ptr<DYN_QUAD, OBS_CIRCLE>();
-    case DYN_QUAD * 2 + OBS_BOX: return kernel_ptr<DYN_QUAD, OBS_BOX>();
-  }
-  return nullptr;
 }
 
 size_t tile_floats(int DP) { return (size_t)(DP == 4 ? 256 : DP == 8 ? 128 : 64) * DP; }
@@ -319,11 +308,17 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
       pb.grid_list = pl->d_grid_list;
     }
   }
-  pl->kernel = select_kernel(dyn, obs);
+  pl->kernel = pakr_select_kernel_tiled(dyn, obs);
+  pl->kernel_stream = pakr_select_kernel_stream(dyn, obs);
   pl->smem_bytes = smem_for(pl);
   e = cudaFuncSetAttribute(pl->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(pl->kernel_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes);
   if (e != cudaSuccess) return bail(PAKR_ERR_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&pl->blocks_per_sm, pl->kernel, kThreads, pl->smem_bytes);
+  int occ_stream = 0;
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_stream, pl->kernel_stream, kThreads, pl->smem_bytes);
+  pl->blocks_per_sm = std::min(pl->blocks_per_sm, occ_stream);  // one grid size for both tiers
   if (e != cudaSuccess || pl->blocks_per_sm < 1)
     return bail(PAKR_ERR_CUDA, "kernel does not fit on an SM (occupancy 0)");
   e = cudaMallocHost(&pl->h_pinned, sizeof(Ctrl) + (size_t)kPathMax * (4 + kMaxD * 4 + kMaxM * 4));
@@ -408,7 +403,8 @@ pakr_status launch(pakr_planner* pl, Params& P, cudaStream_t stream) {
   CUDA_TRY(pl, cudaMemsetAsync(P.ctrl, 0xFF, 16, stream));  // goal_key[2] = none
   void* args[] = {&P};
   const dim3 grid(pl->num_sms * std::min(pl->blocks_per_sm, kCtasPerSm)), block(kThreads);
-  CUDA_TRY(pl, cudaLaunchCooperativeKernel(pl->kernel, grid, block, args, pl->smem_bytes, stream));
+  const void* kernel = P.B <= kStreamB ? pl->kernel_stream : pl->kernel;
+  CUDA_TRY(pl, cudaLaunchCooperativeKernel(kernel, grid, block, args, pl->smem_bytes, stream));
   return PAKR_OK;
 }
 

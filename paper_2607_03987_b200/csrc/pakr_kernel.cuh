@@ -243,13 +243,87 @@ __device__ __forceinline__ void scan_rows(const DevProblem& pb, const float4* __
   }
 }
 
+// ---- streaming tier of the NN scan: few queries (B <= kStreamB) -------------------------------------
+// With only a handful of queries sharing one pass over the tree the scan is HBM-bound, not ALU-bound
+// (DESIGN.md "Kernels"): here every LANE owns tree rows (coalesced 16-byte loads straight from global
+// memory, several rows in flight per lane) and the queries sit in registers; a warp-level min per query
+// and one atomicMin per (warp, query) finish it.  Same per-pair arithmetic (dist2x2) and the same
+// (d2, index) ordering as the tiled tier, so both tiers return identical results.
+constexpr int kStreamB = 16;
+
+template <int DYN, bool UNIT_W>
+__device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, uint32_t r, uint32_t it,
+                                       unsigned long long* key, int vb, int vbcount, bool write_q, float* sm_q) {
+  constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
+  constexpr int QS = (D <= 8) ? 8 : 4;  // queries held in registers per pass over the rows
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  __syncthreads();  // earlier readers of sm_q are done
+  for (int t = threadIdx.x; t < P.B; t += kThreads) {
+    float x[D];
+    sample_state<D>(P.pb, P.seed, r, it, (uint32_t)t, x);
+#pragma unroll
+    for (int d = 0; d < D; ++d) sm_q[t * D + d] = x[d];
+    if (vb == 0) {
+#pragma unroll
+      for (int d = 0; d < DP; ++d) {
+        if (write_q && d < D) P.xq[(size_t)t * DP + d] = x[d];
+        if (P.dbg_x_rand && nbeg == 0) P.dbg_x_rand[(size_t)t * DP + d] = d < D ? x[d] : 0.0f;
+      }
+    }
+  }
+  __syncthreads();
+  const int W = vbcount * kWarps, gw = vb * kWarps + warp;
+  for (int q0 = 0; q0 < P.B; q0 += QS) {
+    f32x2 q2[QS / 2][D];
+    float best[QS];
+    int bidx[QS];
+#pragma unroll
+    for (int h = 0; h < QS / 2; ++h) {
+      const int sa = min(q0 + 2 * h, P.B - 1), sb = min(q0 + 2 * h + 1, P.B - 1);
+#pragma unroll
+      for (int d = 0; d < D; ++d) q2[h][d] = pack2(sm_q[sa * D + d], sm_q[sb * D + d]);
+    }
+#pragma unroll
+    for (int j = 0; j < QS; ++j) { best[j] = __int_as_float(0x7f800000); bidx[j] = 0x7fffffff; }
+    const int span = nend - nbeg;
+    const int trips = (span + W * 32 - 1) / (W * 32);  // warp-uniform
+#pragma unroll 8
+    for (int k = 0; k < trips; ++k) {
+      const int row = nbeg + (k * W + gw) * 32 + lane;
+      const bool ok = row < nend;
+      const float4* src = reinterpret_cast<const float4*>(P.states + (size_t)(ok ? row : nbeg) * DP);
+      float p[DP];
+#pragma unroll
+      for (int v = 0; v < DP / 4; ++v) {
+        const float4 a = __ldcg(src + v);
+        p[4 * v] = a.x; p[4 * v + 1] = a.y; p[4 * v + 2] = a.z; p[4 * v + 3] = a.w;
+      }
+#pragma unroll
+      for (int h = 0; h < QS / 2; ++h) {
+        float da, db;
+        dist2x2<DYN, UNIT_W>(P.pb, q2[h], p, da, db);
+        if (ok && da < best[2 * h]) { best[2 * h] = da; bidx[2 * h] = row; }  // ascending rows per lane, strict <
+        if (ok && db < best[2 * h + 1]) { best[2 * h + 1] = db; bidx[2 * h + 1] = row; }
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < QS; ++j) {
+      unsigned long long kv = ((unsigned long long)__float_as_uint(best[j]) << 32) | (unsigned)bidx[j];
+      if (bidx[j] == 0x7fffffff) kv = kKeyNone;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) kv = min(kv, __shfl_xor_sync(0xffffffffu, kv, o));
+      if (lane == 0 && q0 + j < P.B && kv != kKeyNone) atomicMin(&key[q0 + j], kv);
+    }
+  }
+}
+
 // ---- NN scan of tree rows [nbeg, nend) for the queries of iteration `it` (Alg. 1 l.6-7) ----
 // CTAs vb = 0..vbcount-1 take part (vb < 0: this CTA sits out; the call is CTA-uniform).  Work units are
 // (query group of 128, node range); a CTA takes kWarps consecutive units per round, one per warp.  The
 // sampled states of the (at most two) query groups a CTA touches in a round are drawn once by the CTA into
 // shared memory (Alg. 1 l.6) instead of once per warp.  Partial minima are merged into key[s] with a 64-bit
 // atomicMin, so any split of the rows over warps / phases gives the same result.
-template <int DYN, bool UNIT_W>
+template <int DYN, bool UNIT_W, bool STREAM>
 __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, uint32_t r, uint32_t it,
                                          unsigned long long* key, int vb, int vbcount, bool write_q, float* sm_tile,
                                          uint64_t* sm_bar, float* sm_q, unsigned long long* sm_keys, uint32_t& par0,
@@ -260,6 +334,10 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int n = nend - nbeg;
   if (vb < 0 || n <= 0) return;
+  if constexpr (STREAM) {  // few queries (B <= kStreamB, chosen by the host): HBM-bound streaming tier
+    nn_stream<DYN, UNIT_W>(P, nbeg, nend, r, it, key, vb, vbcount, write_q, sm_q);
+    return;
+  }
   const int W = vbcount * kWarps;
   const int G = (P.B + QG - 1) / QG;  // query groups
   int R = W / G;                      // node ranges per group
@@ -716,7 +794,7 @@ __device__ __forceinline__ void extract_path(const Params& P, int goal_node) {
   }
 }
 
-template <int DYN, int OBS>
+template <int DYN, int OBS, bool STREAM>
 __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const __grid_constant__ Params P) {
   using T = DynTraits<DYN>;
   constexpr int OS = (OBS == OBS_CIRCLE) ? 4 : 8;
@@ -793,8 +871,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       const bool root_only = (n == 1) && !P.n_nodes_io;
       // phase A': rows appended since the look-ahead scan
       if (!root_only && n_scanned < n) {
-        if (P.pb.unit_weights) nn_phase<DYN, true>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
-        else nn_phase<DYN, false>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
+        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
+        else nn_phase<DYN, false, STREAM>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
         grid.sync();
       }
       PROBE(P, 4);
@@ -810,8 +888,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
 #endif
       prop_phase<DYN, OBS>(P, (uint32_t)r, (uint32_t)it, c_best, kcur, root_only, x_pw, x_pcnt, sm_obs, sm_cells, sm_list PROBE_PASS);
       if (ahead) {
-        if (P.pb.unit_weights) nn_phase<DYN, true>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
-        else nn_phase<DYN, false>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
+        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
+        else nn_phase<DYN, false, STREAM>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
       }
 #ifdef PAKR_PROBE
       if (threadIdx.x == 0 && blockIdx.x < 320) atomicAdd(&P.ctrl->probe[32 + blockIdx.x], (unsigned long long)(clock64() - g_xstart));

@@ -16,7 +16,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "libpakr.so")
 _CSRC = os.path.join(_HERE, "csrc")
-_SOURCES = ["pakr_api.cu", "pakr_kernel.cuh", "pakr_device.cuh"]
+_SOURCES = ["pakr_api.cu", "pakr_kernel_inst.cu", "pakr_kernel.cuh", "pakr_device.cuh"]
 
 F_VALID, F_INBOUNDS, F_COLLFREE, F_NOTPRUNED, F_GOAL, F_INSERTED = 1, 2, 4, 8, 16, 32
 MAX_REPLAN_STATS = 64
@@ -31,18 +31,36 @@ class PakrError(RuntimeError):
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """nvcc -gencode arch=compute_100a,code=sm_100a -> paper_2607_03987_b200/libpakr.so (in-tree)."""
+    """nvcc -gencode arch=compute_100a,code=sm_100a -> paper_2607_03987_b200/libpakr.so (in-tree).
+    Three translation units (host API, tiled-tier kernels, streaming-tier kernels) compile in parallel."""
     srcs = [os.path.join(_CSRC, s) for s in _SOURCES] + [os.path.join(_HERE, "..", "include", "pakr.h")]
     stale = (not os.path.exists(_SO)) or any(os.path.getmtime(s) > os.path.getmtime(_SO) for s in srcs)
     if force or stale:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        tmp = _SO + f".{os.getpid()}.tmp"
-        cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-               "-shared", "-Xcompiler", "-fPIC", "-o", tmp, srcs[0]]
-        if verbose:
-            cmd.insert(1, "-Xptxas=-v")
-        subprocess.check_call(cmd)
-        os.replace(tmp, _SO)
+        tag = f".{os.getpid()}.tmp"
+        flags = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+                 "-Xcompiler", "-fPIC"] + (["-Xptxas=-v"] if verbose else [])
+        units = [("pakr_api.cu", [], "api"), ("pakr_kernel_inst.cu", ["-DPAKR_STREAM_TIER=0"], "tiled"),
+                 ("pakr_kernel_inst.cu", ["-DPAKR_STREAM_TIER=1"], "stream")]
+        objs, procs = [], []
+        for src, defs, name in units:
+            obj = os.path.join(_HERE, f"_{name}{tag}.o")
+            objs.append(obj)
+            procs.append(subprocess.Popen(flags + defs + ["-c", "-o", obj, os.path.join(_CSRC, src)]))
+        try:
+            for pr in procs:
+                if pr.wait() != 0:
+                    raise subprocess.CalledProcessError(pr.returncode, pr.args)
+            tmp = _SO + tag
+            subprocess.check_call([nvcc, "-shared", "-o", tmp] + objs)
+            os.replace(tmp, _SO)
+        finally:
+            for pr in procs:
+                if pr.poll() is None:
+                    pr.kill()
+            for o in objs:
+                if os.path.exists(o):
+                    os.remove(o)
     return _SO
 
 

@@ -188,3 +188,38 @@ def test_full_size_c2_sampled(pakr, orc):
     keep = (out["child_flags"] & 9) == 9
     assert out["n_inserted"] == int(keep.sum()) == int(tree["n_nodes"][0].item()) - n0
     pl.close()
+
+
+@pytest.mark.parametrize("name,n0,B,K", [("C2", 5000, 8, 4), ("C2", 70001, 16, 2), ("C3", 33, 5, 3),
+                                         ("C4", 9000, 8, 16), ("C1", 1, 3, 2), ("C4", 40000, 13, 1)])
+def test_step_streaming_tier_matches_oracle(pakr, orc, name, n0, B, K):
+    """B <= 16 takes the HBM-bound streaming NN tier (one row per lane): same parity bar."""
+    from parity_util import check_iteration, run_both
+    p, _ = wl.CONFIGS[name]()
+    pl = pakr.Planner(p)
+    op = orc.OracleProblem(p)
+    host = wl.random_tree(p, n0, seed=n0 + B, flat=n0 > 20000)
+    cap = n0 + B * K
+    out, after, ref, _ = run_both(pl, orc, op, p, host, seed=4, r=1, it=2, B=B, K=K, cap=cap)
+    check_iteration(orc, op, p, host, out, after, ref, B, K, cap)
+    pl.close()
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4"])
+def test_nn_tiers_agree_bit_for_bit(pakr, name):
+    """The tiers have no observable semantics (P26): query s is the same Philox draw whatever B is,
+    so the streaming tier (B = 16) and the tiled tier (B = 48) must return identical NN indices and d2."""
+    p, _ = wl.CONFIGS[name]()
+    pl = pakr.Planner(p)
+    n0 = 50000
+    host = wl.random_tree(p, n0, seed=12, flat=True)
+    host["states"][25000:] = host["states"][:25000]  # every node twice: lowest index must win in both tiers
+    outs = []
+    for B in (16, 48):
+        tree = pl.new_tree(n0 + B, host)
+        outs.append(pl.expand_step(tree, 9, 0, 3, B, 1))
+    np.testing.assert_array_equal(outs[0]["x_rand"], outs[1]["x_rand"][:16])
+    np.testing.assert_array_equal(outs[0]["nn_idx"], outs[1]["nn_idx"][:16])
+    np.testing.assert_array_equal(outs[0]["nn_d2"], outs[1]["nn_d2"][:16])
+    assert outs[0]["nn_idx"].max() < 25000
+    pl.close()
