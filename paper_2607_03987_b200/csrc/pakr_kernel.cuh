@@ -245,15 +245,16 @@ __device__ __forceinline__ void scan_rows(const DevProblem& pb, const float4* __
 
 // ---- streaming tier of the NN scan: few queries (B <= kStreamB) -------------------------------------
 // With only a handful of queries sharing one pass over the tree the scan is HBM-bound, not ALU-bound
-// (DESIGN.md "Kernels"): here every LANE owns tree rows (coalesced 16-byte loads straight from global
-// memory, several rows in flight per lane) and the queries sit in registers; a warp-level min per query
+// (DESIGN.md "Kernels"): here every LANE owns tree rows (each warp streams one contiguous chunk of the
+// tree through its double-buffered TMA tiles) and the queries sit in registers; a warp-level min per query
 // and one atomicMin per (warp, query) finish it.  Same per-pair arithmetic (dist2x2) and the same
 // (d2, index) ordering as the tiled tier, so both tiers return identical results.
 constexpr int kStreamB = 16;
 
 template <int DYN, bool UNIT_W>
 __device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, uint32_t r, uint32_t it,
-                                       unsigned long long* key, int vb, int vbcount, bool write_q, float* sm_q) {
+                                       unsigned long long* key, int vb, int vbcount, bool write_q, float* sm_q,
+                                          float* sm_tile, uint64_t* sm_bar, uint32_t& par0, uint32_t& par1) {
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
   constexpr int QS = (D <= 8) ? 8 : 4;  // queries held in registers per pass over the rows
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -272,7 +273,15 @@ __device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, u
     }
   }
   __syncthreads();
+  constexpr int TILE = TileCfg<DYN>::TILE, TF = TileCfg<DYN>::TILE_FLOATS;
   const int W = vbcount * kWarps, gw = vb * kWarps + warp;
+  // every warp streams ONE contiguous chunk of rows through its double-buffered TMA tiles; inside a tile
+  // lane l scores rows l, l+32, ... (ascending per lane)
+  const int span = nend - nbeg;
+  const int chunk = ((span + W - 1) / W + 31) & ~31;
+  const int cb = nbeg + min(span, gw * chunk), ce = nbeg + min(span, (gw + 1) * chunk);
+  const int ntiles = (ce - cb + TILE - 1) / TILE;
+  const float* src = P.states + (size_t)cb * DP;
   for (int q0 = 0; q0 < P.B; q0 += QS) {
     f32x2 q2[QS / 2][D];
     float best[QS];
@@ -285,26 +294,40 @@ __device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, u
     }
 #pragma unroll
     for (int j = 0; j < QS; ++j) { best[j] = __int_as_float(0x7f800000); bidx[j] = 0x7fffffff; }
-    const int span = nend - nbeg;
-    const int trips = (span + W * 32 - 1) / (W * 32);  // warp-uniform
-#pragma unroll 8
-    for (int k = 0; k < trips; ++k) {
-      const int row = nbeg + (k * W + gw) * 32 + lane;
-      const bool ok = row < nend;
-      const float4* src = reinterpret_cast<const float4*>(P.states + (size_t)(ok ? row : nbeg) * DP);
-      float p[DP];
-#pragma unroll
-      for (int v = 0; v < DP / 4; ++v) {
-        const float4 a = __ldcg(src + v);
-        p[4 * v] = a.x; p[4 * v + 1] = a.y; p[4 * v + 2] = a.z; p[4 * v + 3] = a.w;
+    if (ntiles > 0 && lane == 0) {
+      const uint32_t bytes = (uint32_t)min(TILE, ce - cb) * DP * 4;
+      mbar_expect_tx(&sm_bar[0], bytes);
+      tma_load_1d(sm_tile, src, bytes, &sm_bar[0]);
+    }
+    for (int t = 0; t < ntiles; ++t) {
+      const int cnt = min(TILE, ce - cb - t * TILE);
+      if (t + 1 < ntiles && lane == 0) {  // prefetch the next tile into the other buffer
+        const int nb = (t + 1) & 1;
+        const uint32_t bytes = (uint32_t)min(TILE, ce - cb - (t + 1) * TILE) * DP * 4;
+        mbar_expect_tx(&sm_bar[nb], bytes);
+        tma_load_1d(sm_tile + nb * TF, src + (size_t)(t + 1) * TF, bytes, &sm_bar[nb]);
       }
+      if (t & 1) { mbar_wait(&sm_bar[1], par1); par1 ^= 1; }
+      else { mbar_wait(&sm_bar[0], par0); par0 ^= 1; }
+      const float4* tp = reinterpret_cast<const float4*>(sm_tile + (t & 1) * TF);
+#pragma unroll 2
+      for (int i = lane; i < cnt; i += 32) {
+        float p[DP];
 #pragma unroll
-      for (int h = 0; h < QS / 2; ++h) {
-        float da, db;
-        dist2x2<DYN, UNIT_W>(P.pb, q2[h], p, da, db);
-        if (ok && da < best[2 * h]) { best[2 * h] = da; bidx[2 * h] = row; }  // ascending rows per lane, strict <
-        if (ok && db < best[2 * h + 1]) { best[2 * h + 1] = db; bidx[2 * h + 1] = row; }
+        for (int v = 0; v < DP / 4; ++v) {
+          const float4 a = tp[i * (DP / 4) + v];
+          p[4 * v] = a.x; p[4 * v + 1] = a.y; p[4 * v + 2] = a.z; p[4 * v + 3] = a.w;
+        }
+        const int row = cb + t * TILE + i;
+#pragma unroll
+        for (int h = 0; h < QS / 2; ++h) {
+          float da, db;
+          dist2x2<DYN, UNIT_W>(P.pb, q2[h], p, da, db);
+          if (da < best[2 * h]) { best[2 * h] = da; bidx[2 * h] = row; }  // ascending rows per lane, strict <
+          if (db < best[2 * h + 1]) { best[2 * h + 1] = db; bidx[2 * h + 1] = row; }
+        }
       }
+      __syncwarp();  // every lane is done with this buffer before lane 0 refills it
     }
 #pragma unroll
     for (int j = 0; j < QS; ++j) {
@@ -335,7 +358,7 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
   const int n = nend - nbeg;
   if (vb < 0 || n <= 0) return;
   if constexpr (STREAM) {  // few queries (B <= kStreamB, chosen by the host): HBM-bound streaming tier
-    nn_stream<DYN, UNIT_W>(P, nbeg, nend, r, it, key, vb, vbcount, write_q, sm_q);
+    nn_stream<DYN, UNIT_W>(P, nbeg, nend, r, it, key, vb, vbcount, write_q, sm_q, sm_tile, sm_bar, par0, par1);
     return;
   }
   const int W = vbcount * kWarps;
