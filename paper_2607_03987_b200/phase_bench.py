@@ -42,7 +42,8 @@ def prop_ops_per_child(problem) -> int:
     integ = 8 * D if problem.integrator == wl.INT_RK4 else 2 * D
     n_bounded = int((np.isfinite(problem.state_lo) & (problem.dim_kind == 0)).sum())
     c_obs = 2 * problem.pos_dim if problem.obstacle_type == wl.OBS_AABB else 5
-    return problem.steps_per_edge * (stages * f_dyn + integ + 2 * n_bounded + c_obs * problem.n_obstacles)
+    # obstacle term: broad-phase cell lookup (10 ops) + one obstacle test; the grid culls the rest exactly
+    return problem.steps_per_edge * (stages * f_dyn + integ + 2 * n_bounded + 10 + c_obs)
 
 
 def measure(pl, problem, n, B, K, reps, flush):
@@ -86,6 +87,7 @@ def main():
         print(json.dumps({"phase": "nn", "workload": name, "D": p.state_dim, "n": n, "B": B, "ms": ph[0],
                           "pairs_per_s": B * n / t, "alg_lane_ops_per_pair": ops,
                           "alu_frac": B * n * ops / t / PEAK_LANE_OPS,
+                          "fma_pipe_frac": B * n * 2 * p.state_dim / t / PEAK_LANE_OPS,
                           "tree_GBps": 4 * p.state_stride * n / t / 1e9}), flush=True)
         pl.close()
     for name, B in (("C2", 8), ("C4", 8), ("C4", 4)):  # HBM-bound regime: few queries share one pass over a tree > L2
