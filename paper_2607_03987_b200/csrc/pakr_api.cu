@@ -75,7 +75,7 @@ bool sizes_ok(int64_t B, int64_t K, int64_t cap) {
   return B >= 1 && K >= 1 && K <= 4096 && B * K <= (1ll << 24) && cap >= 2 && cap <= (1ll << 30);
 }
 
-size_t tile_floats(int DP) { return (size_t)(DP == 4 ? 256 : DP == 8 ? 128 : 64) * DP; }
+size_t tile_floats(int DP) { return (size_t)TileCfg<DYN_DI2>::TILE * 4; }  // every tile buffer is the same size
 
 size_t smem_for(const pakr_planner* pl) {
   const int os = pl->obs == OBS_CIRCLE ? 4 : 8;

@@ -29,7 +29,13 @@ namespace cg = cooperative_groups;
 #define PAKR_THREADS 256
 #endif
 constexpr int kThreads = PAKR_THREADS;  // 256 x 2 CTAs per SM measured 1.4x faster in the NN scan than 512 x 1
-constexpr int kCtasPerSm = 1024 / (2 * PAKR_THREADS);
+#ifndef PAKR_CTAS
+#define PAKR_CTAS (1024 / (2 * PAKR_THREADS))
+#endif
+constexpr int kCtasPerSm = PAKR_CTAS;
+#ifndef PAKR_TILE_DIV
+#define PAKR_TILE_DIV 1
+#endif
 constexpr int kWarps = kThreads / 32;
 constexpr int kQ = 4;            // queries per lane in the NN scan
 constexpr int kPathMax = 8192;   // longest path the device buffers hold
@@ -146,7 +152,7 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 
 template <int DYN> struct TileCfg {  // nodes per TMA tile: <= 4 KB per buffer
   static constexpr int DP = DynTraits<DYN>::DP;
-  static constexpr int TILE = (DP == 4) ? 256 : (DP == 8) ? 128 : 64;
+  static constexpr int TILE = ((DP == 4) ? 256 : (DP == 8) ? 128 : 64) / PAKR_TILE_DIV;
   static constexpr int TILE_FLOATS = TILE * DP;
 };
 
