@@ -31,7 +31,7 @@ METRIC = "expanded nodes/s"
 UNIT = "nodes/s"
 # dram__bytes_read.sum + dram__bytes_write.sum of one pakr_loop_kernel launch on this workload, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists for the current kernel).
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 1092352  # profiles/r01_s2_ncu_full.md
 
 
 def algorithmic_ops(problem, nn_pairs: int, children: int) -> dict:
@@ -117,7 +117,9 @@ def run_reference(args, problem, cfg):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_total / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": WORKLOAD, "B": cfg.B, "K": cfg.K, "tree_capacity": cfg.tree_capacity, "n_replans": 1},
+            "config": {"workload": WORKLOAD, "dynamics": problem.name, "B": cfg.B, "K": cfg.K,
+                       "tree_capacity": cfg.tree_capacity, "n_replans": cfg.n_replans,
+                       "sampled": "replan 0 only (the oracle needs ~3 s per replan-0, minutes for all 20)"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "first_solution_ms_median": statistics.median(firsts)}

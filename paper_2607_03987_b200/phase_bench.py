@@ -11,7 +11,7 @@ about 1.2 us).  Prints one JSON line per point:
   stream the regime where HBM binds: B = 8 queries, n = 2^23 (tree 268-403 MB > 126 MB L2)
   prop   B*K children: children/s and algorithmic lane-ops/s of propagate + validity + prune
 
-  python -m paper_2607_03987_b200.phase_bench [--quick]
+  python -m paper_2607_03987_b200.phase_bench [--quick] [--only nn|stream|prop]
 """
 from __future__ import annotations
 
@@ -70,6 +70,7 @@ def main():
     from paper_2607_03987_b200 import pakr
     ap = argparse.ArgumentParser()
     ap.add_argument("--quick", action="store_true")
+    ap.add_argument("--only", default="", help="nn | stream | prop: run that phase's points only (ncu captures)")
     args = ap.parse_args()
     pakr.lib()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
@@ -78,7 +79,7 @@ def main():
                  ("C4", 1 << 18, 4096), ("C4", 1 << 22, 4096)]
     if args.quick:
         nn_points = nn_points[1:3] + nn_points[5:]
-    for name, n, B in nn_points:
+    for name, n, B in (nn_points if args.only in ("", "nn") else []):
         p, _ = wl.CONFIGS[name]()
         pl = pakr.Planner(p)
         ph = measure(pl, p, n, B, 1, reps, None)
@@ -90,7 +91,7 @@ def main():
                           "fma_pipe_frac": B * n * 2 * p.state_dim / t / PEAK_LANE_OPS,
                           "tree_GBps": 4 * p.state_stride * n / t / 1e9}), flush=True)
         pl.close()
-    for name, B in (("C2", 8), ("C4", 8), ("C4", 4)):  # HBM-bound regime: few queries share one pass over a tree > L2
+    for name, B in ((("C2", 8), ("C4", 8), ("C4", 4)) if args.only in ("", "stream") else ()):  # HBM-bound regime: few queries share one pass over a tree > L2
         p, _ = wl.CONFIGS[name]()
         pl = pakr.Planner(p)
         n = 1 << 23
@@ -101,7 +102,7 @@ def main():
                           "l2": "flushed before every call"}),
               flush=True)
         pl.close()
-    for name, B, K in (("C2", 1024, 8), ("C3", 2048, 8), ("C4", 4096, 16), ("C5", 16384, 64)):
+    for name, B, K in ((("C2", 1024, 8), ("C3", 2048, 8), ("C4", 4096, 16), ("C5", 16384, 64)) if args.only in ("", "prop") else ()):
         if args.quick and name in ("C3",):
             continue
         p, _ = wl.CONFIGS[name]()
