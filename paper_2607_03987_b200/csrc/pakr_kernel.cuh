@@ -37,7 +37,10 @@ constexpr int kCtasPerSm = PAKR_CTAS;
 #define PAKR_TILE_DIV 1
 #endif
 constexpr int kWarps = kThreads / 32;
-constexpr int kQ = 4;            // queries per lane in the NN scan
+#ifndef PAKR_KQ
+#define PAKR_KQ 4
+#endif
+constexpr int kQ = PAKR_KQ;      // queries per lane in the NN scan
 constexpr int kPathMax = 8192;   // longest path the device buffers hold
 constexpr int kStatsMax = 64;
 constexpr unsigned long long kKeyNone = ~0ull;
