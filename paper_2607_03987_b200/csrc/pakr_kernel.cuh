@@ -52,6 +52,8 @@ struct Ctrl {  // device control block (in the workspace)
   unsigned long long phase_ns[3];  // leader's time in NN / propagate / insert incl. the grid sync after each
   unsigned long long probe[352];    // -DPAKR_PROBE: SM cycles of thread 0 of CTA 0 between probe points
   int n_nodes, stop;
+  unsigned pbar;      // arrival counter of the barrier among the propagate CTAs (insert inside phase X)
+  int iter_total[2];  // survivors of the iteration, published by CTA 0 when the insert ran inside phase X
   int path_len, solved;
   float best_cost;
   int replans_run, replans_solved, termination;
@@ -152,6 +154,19 @@ __device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t
       : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
+// Barrier among a subset of the (co-resident, cooperative-launch) CTAs: monotonic counter, `target` = number
+// of participants x generation.  Same release / acquire pattern as the cooperative-groups grid barrier.
+__device__ __forceinline__ void cta_group_barrier(unsigned* ctr, unsigned target) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    atomicAdd(ctr, 1u);
+    while (*reinterpret_cast<volatile unsigned*>(ctr) < target) {}
+    __threadfence();
+  }
+  __syncthreads();
+}
 
 template <int DYN> struct TileCfg {  // nodes per TMA tile: <= 4 KB per buffer
   static constexpr int DP = DynTraits<DYN>::DP;
@@ -644,14 +659,57 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
 // from the scratch rows (their node ids n + rank are known from the prefix), so that no separate scan phase and
 // barrier is needed before the next propagate.  `fused` tells the caller (grid-uniform).
 constexpr int kFuseUnits = 2048;  // per-unit prefix kept in shared memory up to this many warp units
+#ifndef PAKR_XTAIL
+#define PAKR_XTAIL 1024
+#endif
+constexpr int kXTailRows = PAKR_XTAIL;  // larger batches of new rows get a scan phase of their own on all CTAs
 
+// One tail-scan item: the survivors of warp units [rg*RU, rg*RU+RU) (gathered by TMA into one tile buffer, in
+// node order) against the 128 queries of group g held in q2.
+template <int DYN, bool UNIT_W>
+__device__ __forceinline__ void tail_item(const Params& P, int n, int g, int rg, int U, const int* sm_upre,
+                                          unsigned long long* key_next,
+                                          const f32x2 (&q2)[kQ / 2][DynTraits<DYN>::D], float* sm_tile,
+                                          uint64_t* sm_bar, uint32_t& par0) {
+  constexpr int DP = DynTraits<DYN>::DP, QG = 32 * kQ;
+  constexpr int RU = TileCfg<DYN>::TILE / 32;  // units per item: their survivors always fit one tile buffer
+  const int lane = threadIdx.x & 31;
+  const int ua = rg * RU, ub = min(U, ua + RU);
+  const int rows = sm_upre[ub] - sm_upre[ua];
+  if (rows == 0) return;
+  if (lane == 0) mbar_expect_tx(&sm_bar[0], (uint32_t)rows * DP * 4);
+  __syncwarp();
+  if (lane < ub - ua) {
+    const int u = ua + lane;
+    const int cnt = sm_upre[u + 1] - sm_upre[u];
+    if (cnt > 0)
+      tma_load_1d(sm_tile + (size_t)(sm_upre[u] - sm_upre[ua]) * DP, P.scr_state + (size_t)u * 32 * DP,
+                  (uint32_t)cnt * DP * 4, &sm_bar[0]);
+  }
+  float best[kQ];
+  int bidx[kQ];
+#pragma unroll
+  for (int j = 0; j < kQ; ++j) { best[j] = __int_as_float(0x7f800000); bidx[j] = 0x7fffffff; }
+  mbar_wait(&sm_bar[0], par0);
+  par0 ^= 1;
+  scan_rows<DYN, UNIT_W>(P.pb, reinterpret_cast<const float4*>(sm_tile), rows, n + sm_upre[ua], q2, best, bidx);
+#pragma unroll
+  for (int j = 0; j < kQ; ++j) {
+    const int s = g * QG + j * 32 + lane;
+    if (s < P.B && bidx[j] != 0x7fffffff)
+      atomicMin(&key_next[s], ((unsigned long long)__float_as_uint(best[j]) << 32) | (unsigned)bidx[j]);
+  }
+  __syncwarp();  // every lane is done with the tile before it is refilled
+}
+
+// All CTAs take part (insert phase of its own): items from the far end of the warp list, queries from P.xq.
 template <int DYN, bool UNIT_W>
 __device__ __forceinline__ void tail_scan_items(const Params& P, int n, int U, const int* sm_upre,
                                                 unsigned long long* key_next, float* sm_tile, uint64_t* sm_bar,
                                                 uint32_t& par0) {
   using T = DynTraits<DYN>;
   constexpr int D = T::D, DP = T::DP, QG = 32 * kQ;
-  constexpr int RU = TileCfg<DYN>::TILE / 32;  // units per item: their survivors always fit one tile buffer
+  constexpr int RU = TileCfg<DYN>::TILE / 32;
   const int lane = threadIdx.x & 31;
   const int W = gridDim.x * kWarps;
   const int gw = blockIdx.x * kWarps + (threadIdx.x >> 5);
@@ -659,51 +717,68 @@ __device__ __forceinline__ void tail_scan_items(const Params& P, int n, int U, c
   const int NR = (U + RU - 1) / RU;
   for (int i = W - 1 - gw; i < G * NR; i += W) {  // from the far end: the copy units start at warp 0
     const int g = i / NR, rg = i - g * NR;
-    const int ua = rg * RU, ub = min(U, ua + RU);
-    const int rows = sm_upre[ub] - sm_upre[ua];
-    if (rows == 0) continue;
-    if (lane == 0) mbar_expect_tx(&sm_bar[0], (uint32_t)rows * DP * 4);
-    __syncwarp();
-    if (lane < ub - ua) {
-      const int u = ua + lane;
-      const int cnt = sm_upre[u + 1] - sm_upre[u];
-      if (cnt > 0)
-        tma_load_1d(sm_tile + (size_t)(sm_upre[u] - sm_upre[ua]) * DP, P.scr_state + (size_t)u * 32 * DP,
-                    (uint32_t)cnt * DP * 4, &sm_bar[0]);
-    }
+    if (sm_upre[min(U, rg * RU + RU)] == sm_upre[rg * RU]) continue;
     f32x2 q2[kQ / 2][D];
-    float best[kQ];
-    int bidx[kQ];
 #pragma unroll
     for (int h = 0; h < kQ / 2; ++h) {
       const int sa = min(g * QG + (2 * h) * 32 + lane, P.B - 1), sb = min(g * QG + (2 * h + 1) * 32 + lane, P.B - 1);
 #pragma unroll
       for (int d = 0; d < D; ++d) q2[h][d] = pack2(__ldcg(&P.xq[(size_t)sa * DP + d]), __ldcg(&P.xq[(size_t)sb * DP + d]));
     }
-#pragma unroll
-    for (int j = 0; j < kQ; ++j) { best[j] = __int_as_float(0x7f800000); bidx[j] = 0x7fffffff; }
-    mbar_wait(&sm_bar[0], par0);
-    par0 ^= 1;
-    scan_rows<DYN, UNIT_W>(P.pb, reinterpret_cast<const float4*>(sm_tile), rows, n + sm_upre[ua], q2, best, bidx);
-#pragma unroll
-    for (int j = 0; j < kQ; ++j) {
-      const int s = g * QG + j * 32 + lane;
-      if (s < P.B && bidx[j] != 0x7fffffff)
-        atomicMin(&key_next[s], ((unsigned long long)__float_as_uint(best[j]) << 32) | (unsigned)bidx[j]);
-    }
-    __syncwarp();  // every lane is done with the tile before it is refilled
+    tail_item<DYN, UNIT_W>(P, n, g, rg, U, sm_upre, key_next, q2, sm_tile, sm_bar, par0);
   }
 }
 
+// Only the propagate CTAs take part (insert inside phase X): CTA-sized chunks of items that share one query
+// group; the CTA draws that group's 128 sampled states of iteration it_next itself (Alg. 1 l.6) into sm_qt.
+template <int DYN, bool UNIT_W>
+__device__ __forceinline__ void tail_scan_rounds(const Params& P, int n, int U, const int* sm_upre,
+                                                 unsigned long long* key_next, uint32_t r, uint32_t it_next, int pcta,
+                                                 int npcta, float* sm_qt, float* sm_tile, uint64_t* sm_bar,
+                                                 uint32_t& par0) {
+  using T = DynTraits<DYN>;
+  constexpr int D = T::D, QG = 32 * kQ;
+  constexpr int RU = TileCfg<DYN>::TILE / 32;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int G = (P.B + QG - 1) / QG;
+  const int NR = (U + RU - 1) / RU;
+  const int NRp = (NR + kWarps - 1) / kWarps * kWarps;  // items per group, padded to whole CTA chunks
+  const int chunks = G * (NRp / kWarps);
+  for (int ch = pcta; ch < chunks; ch += npcta) {  // CTA-uniform trip count
+    const int g = ch / (NRp / kWarps);
+    const int rg = (ch - g * (NRp / kWarps)) * kWarps + warp;
+    __syncthreads();  // the previous chunk's readers are done with sm_qt
+    for (int t = threadIdx.x; t < QG; t += kThreads) {
+      float x[D];
+      sample_state<D>(P.pb, P.seed, r, it_next, (uint32_t)min(g * QG + t, P.B - 1), x);
+#pragma unroll
+      for (int d = 0; d < D; ++d) sm_qt[d * QG + t] = x[d];
+    }
+    __syncthreads();
+    if (rg < NR) {
+      f32x2 q2[kQ / 2][D];
+#pragma unroll
+      for (int h = 0; h < kQ / 2; ++h) {
+#pragma unroll
+        for (int d = 0; d < D; ++d)
+          q2[h][d] = pack2(sm_qt[d * QG + (2 * h) * 32 + lane], sm_qt[d * QG + (2 * h + 1) * 32 + lane]);
+      }
+      tail_item<DYN, UNIT_W>(P, n, g, rg, U, sm_upre, key_next, q2, sm_tile, sm_bar, par0);
+    }
+  }
+}
+
+// The first `npcta` CTAs take part (all of them when the insert is a phase of its own; only the propagate CTAs
+// when it runs inside phase X).  tail_mode: 0 none, 1 items with queries from P.xq, 2 CTA rounds (r, it_next).
 template <int DYN>
 __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, unsigned long long* key_done,
-                                            bool want_tail, unsigned long long* key_next, int* sm_pref,
-                                            int* sm_upre, float* sm_tile, uint64_t* sm_bar, uint32_t& par0,
-                                            bool& fused PROBE_ARG) {
+                                            int tail_mode, unsigned long long* key_next, uint32_t r, uint32_t it_next,
+                                            int npcta, int* sm_pref, int* sm_upre, float* sm_qt, float* sm_tile,
+                                            uint64_t* sm_bar, uint32_t& par0, bool& fused PROBE_ARG) {
   using T = DynTraits<DYN>;
   constexpr int DP = T::DP;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int W = gridDim.x * kWarps;
+  const int W = npcta * kWarps;
   const int gw = blockIdx.x * kWarps + warp;
   const int BK = P.B * P.K;
   constexpr int cpw = 32;
@@ -786,18 +861,24 @@ __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, u
     }
   }
   PROBE(P, 11);
-  // fused tail scan of the next iteration's NN (one item per warp at most, every survivor inserted)
+  // fused tail scan of the next iteration's NN (every survivor inserted)
   {
     constexpr int RU = TileCfg<DYN>::TILE / 32;
     const int G = (P.B + 32 * kQ - 1) / (32 * kQ);
-    fused = want_tail && small && total <= room && G * ((U + RU - 1) / RU) <= W;
+    if (tail_mode == 1) fused = small && total <= room && G * ((U + RU - 1) / RU) <= W;
+    else fused = tail_mode == 2 && small && total <= room && total <= kXTailRows;
     if (fused && total > 0) {
-      if (P.pb.unit_weights) tail_scan_items<DYN, true>(P, n, U, sm_upre, key_next, sm_tile, sm_bar, par0);
-      else tail_scan_items<DYN, false>(P, n, U, sm_upre, key_next, sm_tile, sm_bar, par0);
+      if (tail_mode == 1) {
+        if (P.pb.unit_weights) tail_scan_items<DYN, true>(P, n, U, sm_upre, key_next, sm_tile, sm_bar, par0);
+        else tail_scan_items<DYN, false>(P, n, U, sm_upre, key_next, sm_tile, sm_bar, par0);
+      } else {
+        if (P.pb.unit_weights) tail_scan_rounds<DYN, true>(P, n, U, sm_upre, key_next, r, it_next, (int)blockIdx.x, npcta, sm_qt, sm_tile, sm_bar, par0);
+        else tail_scan_rounds<DYN, false>(P, n, U, sm_upre, key_next, r, it_next, (int)blockIdx.x, npcta, sm_qt, sm_tile, sm_bar, par0);
+      }
     }
   }
   // the NN keys this iteration consumed are free again: reset them for iteration i+2
-  for (int s = blockIdx.x * kThreads + threadIdx.x; s < P.B; s += gridDim.x * kThreads) key_done[s] = kKeyNone;
+  for (int s = blockIdx.x * kThreads + threadIdx.x; s < P.B; s += npcta * kThreads) key_done[s] = kKeyNone;
   return total;
 }
 
@@ -875,6 +956,9 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
   const int x_pcnt = split ? NPB * kWarps : W;
   const int x_vb = split ? (int)blockIdx.x - NPB : (int)blockIdx.x;  // scan CTA index (< 0: none), count
   const int x_vbcnt = split ? NB - NPB : NB;
+  // insert inside phase X by the propagate CTAs (one grid barrier per iteration) when the children are few
+  const bool xins = split && U_prop <= kFuseUnits;
+  unsigned pgen = 0;
   unsigned long long* const key0 = P.nn_key;
   unsigned long long* const key1 = P.nn_key + P.B;
 
@@ -919,6 +1003,28 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       const bool ahead = (iters + 1 < P.max_iters);
 #endif
       prop_phase<DYN, OBS>(P, (uint32_t)r, (uint32_t)it, c_best, kcur, root_only, x_pw, x_pcnt, sm_obs, sm_cells, sm_list PROBE_PASS);
+      // goal-key slots alternate over the whole launch (not per replan): the other slot was last
+      // read before the previous grid sync and is next written after the following one
+      const int slot = (int)(iterations & 1);
+      bool fused = false;
+      int total = 0;
+      if (xins) {
+        // The propagate CTAs finish the iteration among themselves while the scan CTAs are still busy:
+        // barrier of their own, ordered insert, tail of NN(it+1) over the new rows.
+        if ((int)blockIdx.x < NPB) {
+          fence_proxy_async();  // scratch rows written with st.global are gathered by TMA below
+          ++pgen;
+          cta_group_barrier(&P.ctrl->pbar, (unsigned)NPB * pgen);
+          fence_proxy_async();
+          PROBE(P, 10);
+          total = insert_phase<DYN>(P, n, slot, kcur, ahead ? 2 : 0, knext, (uint32_t)r, (uint32_t)(it + 1), NPB, sm_pref,
+                                    reinterpret_cast<int*>(sm_q), reinterpret_cast<float*>(sm_keys), my_tile, my_bar, par0,
+                                    fused PROBE_PASS);
+          if (leader) P.ctrl->iter_total[slot] = total;
+          __threadfence();
+          fence_proxy_async();  // tree rows written with st.global are read next by TMA (async proxy)
+        }
+      }
       if (ahead) {
         if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
         else nn_phase<DYN, false, STREAM>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
@@ -926,28 +1032,31 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
 #ifdef PAKR_PROBE
       if (threadIdx.x == 0 && blockIdx.x < 320) atomicAdd(&P.ctrl->probe[32 + blockIdx.x], (unsigned long long)(clock64() - g_xstart));
 #endif
-      // goal-key slots alternate over the whole launch (not per replan): the other slot was last
-      // read before the previous grid sync and is next written after the following one
-      const int slot = (int)(iterations & 1);
       if (leader) P.ctrl->goal_key[slot ^ 1] = kKeyNone;
+      if (leader && xins && P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) P.ctrl->stop = 1;
       fence_proxy_async();  // scratch rows written with st.global may be read by TMA in the insert phase
       grid.sync();
       fence_proxy_async();
       PROBE(P, 9);
       if (leader) { const unsigned long long t = globaltimer_ns(); ph1 += t - tp; tp = t; }
-      // phase C
-      bool fused = false;
-      const int total = insert_phase<DYN>(P, n, slot, kcur, ahead, knext, sm_pref, reinterpret_cast<int*>(sm_q), my_tile,
-                                          my_bar, par0, fused PROBE_PASS);
+      if (xins) {
+        total = __ldcg(&P.ctrl->iter_total[slot]);
+        fused = ahead && total <= P.cap - n && total <= kXTailRows;
+      } else {
+        // phase C: insert as a phase of its own (every CTA takes part)
+        total = insert_phase<DYN>(P, n, slot, kcur, ahead ? 1 : 0, knext, (uint32_t)r, (uint32_t)(it + 1), NB, sm_pref,
+                                  reinterpret_cast<int*>(sm_q), reinterpret_cast<float*>(sm_keys), my_tile, my_bar, par0,
+                                  fused PROBE_PASS);
+        if (leader && P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) P.ctrl->stop = 1;
+        __threadfence();
+        fence_proxy_async();  // tree rows written with st.global are read next by TMA (async proxy)
+        PROBE(P, 12);
+        grid.sync();
+        PROBE(P, 13);
+        if (leader) { const unsigned long long t = globaltimer_ns(); ph2 += t - tp; tp = t; }
+        fence_proxy_async();
+      }
       const int added = min(total, P.cap - n);
-      if (leader && P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) P.ctrl->stop = 1;
-      __threadfence();
-      fence_proxy_async();  // tree rows written with st.global are read next by TMA (async proxy)
-      PROBE(P, 12);
-      grid.sync();
-      PROBE(P, 13);
-      if (leader) { const unsigned long long t = globaltimer_ns(); ph2 += t - tp; tp = t; }
-      fence_proxy_async();
       nn_pairs += (long long)P.B * n;  // (query, node) pairs of this iteration's NN
       n_scanned = ahead ? (fused ? n + added : n) : 0;  // fused: NN(it+1) already covers the new rows
       n += added;
