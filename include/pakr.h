@@ -132,8 +132,9 @@ typedef struct {
   int32_t termination;     /* 0 all replans run, 1 time budget */
   double first_solution_ms;/* device time from kernel start to the end of the first solved replan; -1 if none */
   double device_ms;        /* device time of the whole loop (%globaltimer) */
-  double phase_ms[3];      /* CTA 0's time in: NN scan of the newly appended rows / propagate (with the next
-                              iteration's NN look-ahead scan beside it) / insert; each incl. its grid barrier */
+  double phase_ms[3];      /* CTA 0's time in: separate NN (tail) scan phases / the propagate phase (with the next
+                              iteration's NN look-ahead scan beside it and, when children are few, the insert
+                              inside it) / insert phases of their own; each incl. its grid barrier */
   /* first PAKR_MAX_REPLAN_STATS replans: */
   float replan_cost[PAKR_MAX_REPLAN_STATS];   /* c_best after the replan (+INF before any solution) */
   int32_t replan_nodes[PAKR_MAX_REPLAN_STATS];/* tree size at its end */
@@ -189,8 +190,8 @@ pakr_status pakr_expand_step(pakr_planner* planner, const pakr_step_args* args, 
 
 /* Statistics of the last pakr_plan / pakr_expand_step launch that used this workspace with the same
  * (B, K, tree_capacity): synchronises `cuda_stream`, then copies the device control block into *out (HOST).
- * After pakr_expand_step: iterations = 1, phase_ms[0] = the NN scan of the whole tree, [1] = propagate,
- * [2] = insert, each including its grid barrier. */
+ * After pakr_expand_step: iterations = 1, phase_ms[0] = the NN scan of the whole tree, [1] = propagate (+ insert
+ * when the children are few), [2] = insert as a phase of its own, each including its grid barrier. */
 pakr_status pakr_read_stats(pakr_planner* planner, int32_t B, int32_t K, int64_t tree_capacity,
                             void* d_workspace, size_t workspace_bytes, void* cuda_stream, pakr_stats* out);
 

@@ -1,20 +1,20 @@
 // pakr_kernel.cuh -- the persistent cooperative kernel that runs Alg. 1 on device.
 //
-// One launch = the whole AO-x loop (or one iteration for pakr_expand_step).  Per iteration i:
-//   phase A' NN tail scan   (Alg. 1 l.6-7)   finishes NN(i) over the nodes appended by iteration i-1;
-//                                             warps own 32*Q queries in registers, tree tiles are
-//                                             streamed into shared memory by TMA bulk copies
-//   -- grid sync --
-//   phase X  propagate(i)   (Alg. 1 l.8-12)  one lane per child, state in registers, obstacles and
-//                                             their broad-phase grid in shared memory, ballot compaction
-//          + NN(i+1) over the frozen snapshot [0, n_i) on the warps that have no child unit
-//            (speculative: dropped when iteration i ends the replan)
-//   -- grid sync --
-//   phase C  insert + goal  (Alg. 1 l.13-15) ordered prefix over the per-warp counts, coalesced
-//                                             append at the tree tail, goal winner by atomicMin
-//   -- grid sync --
-// NN(i+1) = min(scan of [0, n_i) done in X(i), scan of [n_i, n_{i+1}) done in A'(i+1)): the snapshot a
-// batch sees is exactly the tree after the previous batch's inserts.
+// One launch = the whole AO-x loop (or one iteration for pakr_expand_step).  Per iteration i, when the children
+// are few (the usual case):
+//   phase X, one grid barrier at its end
+//     propagate CTAs: propagate(i)  (Alg. 1 l.8-12)  one lane per child, state in registers, obstacles and
+//                                     their broad-phase grid in shared memory, ballot compaction to scratch
+//                     barrier among themselves, then
+//                     insert(i)     (Alg. 1 l.13-15) ordered prefix of survivor counts, append at the tree
+//                                     tail, goal winner by atomicMin
+//                     tail of NN(i+1) over the rows just appended (TMA gather from the scratch rows)
+//     scan CTAs:      NN(i+1) over the frozen snapshot [0, n_i)  (Alg. 1 l.6-7): warps own 32*Q queries in
+//                                     registers, tree tiles stream into shared memory by TMA bulk copies
+//                                     (speculative: dropped when iteration i ends the replan)
+// NN(i+1) = min(scan of [0, n_i), scan of [n_i, n_{i+1})): the snapshot a batch sees is exactly the tree after
+// the previous batch's inserts.  Large batches of new rows get a tail-scan phase of their own
+// ("A'"), and with many children every warp propagates, then scans, and the insert is a phase of its own.
 // Loop state (n, c_best, replan, iteration) is replicated in registers of every thread and
 // recomputed from the same global values, so no broadcast step is needed.
 #pragma once

@@ -3,8 +3,8 @@
 
 One `pakr_expand_step` on a synthetic tree of n uniform-in-bounds nodes (workloads.random_tree, flat) is
 one iteration whose three phases are timed on the device by the kernel itself (`pakr_read_stats`:
-phase_ms[0] = NN scan of the whole tree, [1] = propagate, [2] = insert; each includes its grid barrier,
-about 1.2 us).  Prints one JSON line per point:
+phase_ms[0] = NN scan of the whole tree, [1] = propagate (+ insert when B*K is small), [2] = insert as a phase
+of its own; each includes its grid barrier, about 1.2 us).  Prints one JSON line per point:
 
   nn     B x n (query, node) pairs: pairs/s, algorithmic fp32 lane-ops/s against the issue-slot peak,
          and the DRAM-side GB/s the scan would need if the tree were streamed once (4*Dp*n bytes)
