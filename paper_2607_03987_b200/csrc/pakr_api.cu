@@ -257,7 +257,9 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
   for (int a = 0; a < PD; ++a) pb.goal[a] = p->goal_center[a];
   pb.goal_r = p->goal_radius; pb.goal_angle = p->goal_angle; pb.goal_angle_tol = p->goal_angle_tol;
   pb.goal_angle_dim = p->goal_angle_dim;
-  for (int i = 0; i < 8 && i < p->n_dyn_params; ++i) pb.dyn[i] = p->dyn_params[i];
+  for (int i = 0; i < 5 && i < p->n_dyn_params; ++i) pb.dyn[i] = p->dyn_params[i];
+  if (dyn == DYN_QUAD)
+    for (int i = 0; i < 4; ++i) pb.dyn[5 + i] = 1.0f / p->dyn_params[i];
   pb.dt = p->dt; pb.S = p->steps_per_edge; pb.integrator = p->integrator; pb.cost_mode = p->cost_mode;
   pb.inv_hspeed = std::isinf(p->heuristic_speed) ? 0.0f : 1.0f / p->heuristic_speed;
   pb.unit_weights = unit ? 1 : 0;

@@ -35,7 +35,7 @@ struct DevProblem {
   float goal[3];
   float goal_r, goal_angle, goal_angle_tol;
   int goal_angle_dim;
-  float dyn[8];                        // quadrotor: m, Ixx, Iyy, Izz, g
+  float dyn[12];                       // quadrotor: m, Ixx, Iyy, Izz, g, then 1/m, 1/Ixx, 1/Iyy, 1/Izz
   float dt;
   int S;
   int integrator;                      // 0 Euler, 1 RK4
@@ -138,15 +138,24 @@ __device__ __forceinline__ void dyn_f(const DevProblem& pb, const float (&x)[Dyn
     xd[3] = u[0];
     xd[4] = u[1];
   } else {
-    const float m = pb.dyn[0], Ixx = pb.dyn[1], Iyy = pb.dyn[2], Izz = pb.dyn[3], g = pb.dyn[4];
+    const float Ixx = pb.dyn[1], Iyy = pb.dyn[2], Izz = pb.dyn[3], g = pb.dyn[4];
     float sphi, cphi, sth, cth, spsi, cpsi;
+#ifndef PAKR_ACCURATE_SINCOS
+    // MUFU-based sin/cos (abs error <= 2^-21.4 on [-pi, pi]; roll and pitch are bounded by the state box, yaw is
+    // folded into [-pi, pi] first): 2.2x faster quadrotor edges than sincosf, whose inlined slow path also evicts
+    // the edge loop from the instruction cache.  State error vs the fp64 oracle stays ~1e-5 (tolerance 1e-4).
+    __sincosf(x[6], &sphi, &cphi);
+    __sincosf(x[7], &sth, &cth);
+    __sincosf(x[8] - kTwoPiF * rintf(x[8] * (1.0f / kTwoPiF)), &spsi, &cpsi);
+#else
     sincosf(x[6], &sphi, &cphi);
     sincosf(x[7], &sth, &cth);
     sincosf(x[8], &spsi, &cpsi);
+#endif
     const float p = x[9], q = x[10], r = x[11];
-    const float icth = 1.0f / cth;
+    const float icth = __frcp_rn(cth);
     const float tth = sth * icth;
-    const float a = u[0] / m;
+    const float a = u[0] * pb.dyn[5];  // 1/m
     xd[0] = x[3];
     xd[1] = x[4];
     xd[2] = x[5];
@@ -157,36 +166,58 @@ __device__ __forceinline__ void dyn_f(const DevProblem& pb, const float (&x)[Dyn
     xd[6] = p + tth * sq_cr;
     xd[7] = cphi * q - sphi * r;
     xd[8] = sq_cr * icth;
-    xd[9] = (u[1] - (Izz - Iyy) * q * r) / Ixx;
-    xd[10] = (u[2] - (Ixx - Izz) * p * r) / Iyy;
-    xd[11] = (u[3] - (Iyy - Ixx) * p * q) / Izz;
+    xd[9] = (u[1] - (Izz - Iyy) * q * r) * pb.dyn[6];   // 1/Ixx, 1/Iyy, 1/Izz (set by the host)
+    xd[10] = (u[2] - (Ixx - Izz) * p * r) * pb.dyn[7];
+    xd[11] = (u[3] - (Iyy - Ixx) * p * q) * pb.dyn[8];
   }
 }
 
 // One fixed step of dt: forward Euler or classical RK4 (P9).
+// RK4 is a rolled loop over the four stages (t = x + a_s h k, acc += b_s k with a = 0, 1/2, 1/2, 1 and
+// b = 1, 2, 2, 1): ONE inlined copy of f instead of four keeps the quadrotor edge inside the instruction cache.
+// Every operation rounds exactly like the unrolled textbook form (a_0 = 0 and b = 1 cases are exact).
 template <int DYN>
 __device__ __forceinline__ void dyn_step(const DevProblem& pb, float (&x)[DynTraits<DYN>::D],
                                          const float (&u)[DynTraits<DYN>::M]) {
   constexpr int D = DynTraits<DYN>::D;
   const float h = pb.dt;
   float k[D], t[D], acc[D];
-  dyn_f<DYN>(pb, x, u, k);
   if (pb.integrator == 0) {
+    dyn_f<DYN>(pb, x, u, k);
 #pragma unroll
     for (int d = 0; d < D; ++d) x[d] = fmaf(h, k[d], x[d]);
     return;
   }
 #pragma unroll
-  for (int d = 0; d < D; ++d) { acc[d] = k[d]; t[d] = fmaf(0.5f * h, k[d], x[d]); }
-  dyn_f<DYN>(pb, t, u, k);
+  for (int d = 0; d < D; ++d) { k[d] = 0.0f; acc[d] = 0.0f; }
+  constexpr bool kRoll = (DYN == DYN_QUAD);  // measured: rolling slows the unicycle (less ILP), f of the others is tiny
+#pragma unroll 1
+  for (int s = 0; s < (kRoll ? 4 : 1); ++s) {
+    if constexpr (kRoll) {
+      const float a = (s == 0) ? 0.0f : (s == 3) ? h : 0.5f * h;
+      const float b = (s == 1 || s == 2) ? 2.0f : 1.0f;
 #pragma unroll
-  for (int d = 0; d < D; ++d) { acc[d] = fmaf(2.0f, k[d], acc[d]); t[d] = fmaf(0.5f * h, k[d], x[d]); }
-  dyn_f<DYN>(pb, t, u, k);
+      for (int d = 0; d < D; ++d) t[d] = fmaf(a, k[d], x[d]);
+      dyn_f<DYN>(pb, t, u, k);
 #pragma unroll
-  for (int d = 0; d < D; ++d) { acc[d] = fmaf(2.0f, k[d], acc[d]); t[d] = fmaf(h, k[d], x[d]); }
-  dyn_f<DYN>(pb, t, u, k);
+      for (int d = 0; d < D; ++d) acc[d] = fmaf(b, k[d], acc[d]);
+    } else {
+      dyn_f<DYN>(pb, x, u, k);
 #pragma unroll
-  for (int d = 0; d < D; ++d) x[d] = fmaf(h * (1.0f / 6.0f), acc[d] + k[d], x[d]);
+      for (int d = 0; d < D; ++d) { acc[d] = k[d]; t[d] = fmaf(0.5f * h, k[d], x[d]); }
+      dyn_f<DYN>(pb, t, u, k);
+#pragma unroll
+      for (int d = 0; d < D; ++d) { acc[d] = fmaf(2.0f, k[d], acc[d]); t[d] = fmaf(0.5f * h, k[d], x[d]); }
+      dyn_f<DYN>(pb, t, u, k);
+#pragma unroll
+      for (int d = 0; d < D; ++d) { acc[d] = fmaf(2.0f, k[d], acc[d]); t[d] = fmaf(h, k[d], x[d]); }
+      dyn_f<DYN>(pb, t, u, k);
+#pragma unroll
+      for (int d = 0; d < D; ++d) acc[d] = acc[d] + k[d];
+    }
+  }
+#pragma unroll
+  for (int d = 0; d < D; ++d) x[d] = fmaf(h * (1.0f / 6.0f), acc[d], x[d]);
 }
 
 // ---- validity ("validity checked at each step"; P10-P13) ----------------

@@ -162,7 +162,7 @@ __device__ __forceinline__ void cta_group_barrier(unsigned* ctr, unsigned target
   if (threadIdx.x == 0) {
     __threadfence();
     atomicAdd(ctr, 1u);
-    while (*reinterpret_cast<volatile unsigned*>(ctr) < target) {}
+    while ((int)(*reinterpret_cast<volatile unsigned*>(ctr) - target) < 0) {}  // wrap-safe
     __threadfence();
   }
   __syncthreads();

@@ -37,6 +37,7 @@ _CASES = [
     ("C3", 9000, 512, 8),
     ("C4", 2500, 384, 16),
     ("C4", 12345, 200, 9),
+    ("C4", 30000, 1024, 16),
     ("C5", 7777, 256, 16),
 ]
 
