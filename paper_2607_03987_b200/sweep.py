@@ -34,6 +34,7 @@ def run_configs(pakr, seeds):
         pl = pakr.Planner(p)
         pl.plan(1000, cfg.B, cfg.K, cfg.tree_capacity, 1)  # warm-up
         first, nodes1, cost1, costf, ms_all, iters, solved, rate = [], [], [], [], [], [], 0, []
+        curve_c, curve_t = [], []
         for s in range(seeds):
             r = pl.plan(s, cfg.B, cfg.K, cfg.tree_capacity, cfg.n_replans)
             solved += r["outcome"]
@@ -43,6 +44,8 @@ def run_configs(pakr, seeds):
                 nodes1.append(int(r["replan_nodes"][k]))
                 cost1.append(float(r["replan_cost"][k]))
             costf.append(r["cost"])
+            curve_c.append([float(v) if v < float("inf") else None for v in r["replan_cost"]])
+            curve_t.append([float(v) for v in r["replan_end_ms"]])
             ms_all.append(r["device_ms"])
             iters.append(r["iterations"])
             rate.append(r["children"] / (r["device_ms"] * 1e-3))
@@ -53,7 +56,11 @@ def run_configs(pakr, seeds):
                           "first_solution_nodes_median": med(nodes1), "first_cost_median": med(cost1),
                           "final_cost_median": med(costf), "all_replans_ms_median": med(ms_all),
                           "iterations_median": med(iters), "expanded_nodes_per_s_median": med(rate),
-                          "best_cost_at_100ms_median": med(best100)}), flush=True)
+                          "best_cost_at_100ms_median": med(best100),
+                          # cost-vs-time curve of AO-x (Table II, Fig. 2): median over seeds of c_best
+                          # and of the device time at the end of each replan
+                          "cost_after_replan_median": [med(c) for c in zip(*curve_c)],
+                          "ms_at_end_of_replan_median": [med(t) for t in zip(*curve_t)]}), flush=True)
         pl.close()
 
 
