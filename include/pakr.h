@@ -45,7 +45,8 @@ typedef enum {
   PAKR_ERR_CUDA = 5
 } pakr_status;
 
-enum { PAKR_DYN_DOUBLE_INTEGRATOR = 0, PAKR_DYN_UNICYCLE2 = 1, PAKR_DYN_QUADROTOR = 2 };
+enum { PAKR_DYN_DOUBLE_INTEGRATOR = 0, PAKR_DYN_UNICYCLE2 = 1, PAKR_DYN_QUADROTOR = 2,
+       PAKR_DYN_DUBINS_AIRPLANE = 3, PAKR_DYN_UNICYCLE1 = 4 };
 enum { PAKR_INT_EULER = 0, PAKR_INT_RK4 = 1 };
 enum { PAKR_OBS_CIRCLE2D = 0, PAKR_OBS_AABB = 1, PAKR_OBS_ZCYLINDER = 2 };
 enum { PAKR_COST_DURATION = 0, PAKR_COST_PATH_LENGTH = 1 };
@@ -67,13 +68,15 @@ enum {
 typedef struct {
   int32_t dynamics_id; /* PAKR_DYN_*: double integrator [p, pdot], second-order
                           unicycle [x,y,theta,v,omega], quadrotor [p, v, (phi,theta,
-                          psi) ZYX, (p,q,r)] with control (T, tau) (BASELINE.json config 4) */
+                          psi) ZYX, (p,q,r)] with control (T, tau) (BASELINE.json config 4), Dubins airplane
+                          [x,y,z,yaw,pitch,v] with control (yaw rate, pitch rate, acceleration),
+                          first-order unicycle [x,y,theta] with control (v, omega) */
   int32_t integrator;  /* PAKR_INT_*: forward Euler or classical RK4 */
   int32_t state_dim, control_dim, pos_dim; /* must match dynamics_id: DI (2*pos_dim, pos_dim,
-                          2|3), unicycle (5,2,2), quadrotor (12,4,3) */
+                          2|3), unicycle2 (5,2,2), quadrotor (12,4,3), Dubins airplane (6,3,3), unicycle1 (3,2,2) */
   const float* dyn_params; int32_t n_dyn_params; /* quadrotor: m, Ixx, Iyy, Izz, g; else 0 */
   const float* state_lo; const float* state_hi;  /* [D]; +-INF = unbounded; box-tested every step */
-  const uint8_t* dim_kind; /* [D] PAKR_DIM_*; angle dims (unicycle theta, quadrotor psi) are wrapped
+  const uint8_t* dim_kind; /* [D] PAKR_DIM_*; angle dims (unicycle theta, quadrotor psi, airplane yaw) are wrapped
                           to [-pi,pi) and never bounds-tested; must match the dynamics */
   const float* nn_weight;  /* [D] >= 0, d^2 = sum_d w_d delta_d^2; 0 drops a dim */
   const float* control_lo; const float* control_hi; /* [m] */

@@ -175,6 +175,25 @@ extern "C" void orc_f(const orc_problem* P, const double* x, const double* u, do
       xd[11] = (u[3] - (Iyy - Ixx) * p * q) / Izz;
       break;
     }
+    case ORC_DYN_DUBINS_AIRPLANE: {
+      // state [x, y, z, phi (yaw), theta (pitch), v], control [phi_dot, theta_dot, v_dot].
+      // The paper gives no equations; reading (P33): the velocity vector has magnitude v along
+      // the heading given by yaw and pitch.
+      const double yaw = x[3], pitch = x[4], v = x[5];
+      xd[0] = v * std::cos(pitch) * std::cos(yaw);
+      xd[1] = v * std::cos(pitch) * std::sin(yaw);
+      xd[2] = v * std::sin(pitch);
+      xd[3] = u[0];
+      xd[4] = u[1];
+      xd[5] = u[2];
+      break;
+    }
+    case ORC_DYN_UNICYCLE1: {  // [x, y, theta], control [v, omega]
+      xd[0] = u[0] * std::cos(x[2]);
+      xd[1] = u[0] * std::sin(x[2]);
+      xd[2] = u[1];
+      break;
+    }
     default:
       for (int d = 0; d < P->state_dim; ++d) xd[d] = 0.0;
   }

@@ -195,6 +195,14 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
     for (int i = 0; i < 4; ++i)
       if (!(p->dyn_params[i] > 0.0f)) return fail(nullptr, PAKR_ERR_INVALID_ARG, "mass/inertia must be > 0");
     dyn = DYN_QUAD;
+  } else if (p->dynamics_id == PAKR_DYN_DUBINS_AIRPLANE) {
+    if (p->pos_dim != 3 || p->state_dim != 6 || p->control_dim != 3)
+      return fail(nullptr, PAKR_ERR_INVALID_ARG, "dubins airplane needs (D,m,pos)=(6,3,3)");
+    dyn = DYN_DA;
+  } else if (p->dynamics_id == PAKR_DYN_UNICYCLE1) {
+    if (p->pos_dim != 2 || p->state_dim != 3 || p->control_dim != 2)
+      return fail(nullptr, PAKR_ERR_INVALID_ARG, "unicycle1 needs (D,m,pos)=(3,2,2)");
+    dyn = DYN_UNI1;
   } else {
     return fail(nullptr, PAKR_ERR_UNSUPPORTED, "unknown dynamics_id");
   }
@@ -214,7 +222,7 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
     for (int i = 0; i < p->n_obstacles * per; ++i)
       if (!std::isfinite(p->obstacles[i])) return fail(nullptr, PAKR_ERR_INVALID_ARG, "obstacle coordinates must be finite");
   }
-  const int angle = dyn == DYN_UNI2 ? 2 : dyn == DYN_QUAD ? 8 : -1;
+  const int angle = dyn == DYN_UNI2 ? 2 : dyn == DYN_QUAD ? 8 : dyn == DYN_DA ? 3 : dyn == DYN_UNI1 ? 2 : -1;
   for (int d = 0; d < D; ++d) {
     const bool is_angle = p->dim_kind[d] == PAKR_DIM_ANGLE;
     if (p->dim_kind[d] > 1 || is_angle != (d == angle))

@@ -16,7 +16,7 @@ constexpr float kPiF = 3.14159274101257324f;   // (float)pi
 constexpr float kTwoPiF = 6.28318548202514648f;
 
 // ---- compile-time description of a dynamics model -------------------------------------------
-enum DynKind { DYN_DI2 = 0, DYN_DI3 = 1, DYN_UNI2 = 2, DYN_QUAD = 3 };
+enum DynKind { DYN_DI2 = 0, DYN_DI3 = 1, DYN_UNI2 = 2, DYN_QUAD = 3, DYN_DA = 4, DYN_UNI1 = 5 };
 enum ObsKind { OBS_CIRCLE = 0, OBS_BOX = 1 };
 
 template <int DYN> struct DynTraits;
@@ -24,6 +24,8 @@ template <> struct DynTraits<DYN_DI2> { static constexpr int D = 4, M = 2, PD = 
 template <> struct DynTraits<DYN_DI3> { static constexpr int D = 6, M = 3, PD = 3, DP = 8, ANGLE = -1; };
 template <> struct DynTraits<DYN_UNI2> { static constexpr int D = 5, M = 2, PD = 2, DP = 8, ANGLE = 2; };
 template <> struct DynTraits<DYN_QUAD> { static constexpr int D = 12, M = 4, PD = 3, DP = 12, ANGLE = 8; };
+template <> struct DynTraits<DYN_DA> { static constexpr int D = 6, M = 3, PD = 3, DP = 8, ANGLE = 3; };
+template <> struct DynTraits<DYN_UNI1> { static constexpr int D = 3, M = 2, PD = 2, DP = 4, ANGLE = 2; };
 
 // Problem constants, passed by value in the kernel parameter block.
 struct DevProblem {
@@ -137,6 +139,22 @@ __device__ __forceinline__ void dyn_f(const DevProblem& pb, const float (&x)[Dyn
     xd[2] = x[4];
     xd[3] = u[0];
     xd[4] = u[1];
+  } else if constexpr (DYN == DYN_DA) {  // Dubins airplane [x,y,z,yaw,pitch,v], u = (yaw rate, pitch rate, accel)
+    float sy, cy, sp, cp;
+    sincosf(x[3], &sy, &cy);
+    sincosf(x[4], &sp, &cp);
+    xd[0] = x[5] * cp * cy;
+    xd[1] = x[5] * cp * sy;
+    xd[2] = x[5] * sp;
+    xd[3] = u[0];
+    xd[4] = u[1];
+    xd[5] = u[2];
+  } else if constexpr (DYN == DYN_UNI1) {  // first-order unicycle [x,y,theta], u = (v, omega)
+    float s, c;
+    sincosf(x[2], &s, &c);
+    xd[0] = u[0] * c;
+    xd[1] = u[0] * s;
+    xd[2] = u[1];
   } else {
     const float Ixx = pb.dyn[1], Iyy = pb.dyn[2], Izz = pb.dyn[3], g = pb.dyn[4];
     float sphi, cphi, sth, cth, spsi, cpsi;

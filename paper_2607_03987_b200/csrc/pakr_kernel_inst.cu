@@ -28,6 +28,10 @@ extern "C" const void* pakr_select_kernel_tiled(int dyn, int obs) {
     case DYN_UNI2 * 2 + OBS_BOX: return kernel_ptr<DYN_UNI2, OBS_BOX>();
     case DYN_QUAD * 2 + OBS_CIRCLE: return kernel_ptr<DYN_QUAD, OBS_CIRCLE>();
     case DYN_QUAD * 2 + OBS_BOX: return kernel_ptr<DYN_QUAD, OBS_BOX>();
+    case DYN_DA * 2 + OBS_CIRCLE: return kernel_ptr<DYN_DA, OBS_CIRCLE>();
+    case DYN_DA * 2 + OBS_BOX: return kernel_ptr<DYN_DA, OBS_BOX>();
+    case DYN_UNI1 * 2 + OBS_CIRCLE: return kernel_ptr<DYN_UNI1, OBS_CIRCLE>();
+    case DYN_UNI1 * 2 + OBS_BOX: return kernel_ptr<DYN_UNI1, OBS_BOX>();
   }
   return nullptr;
 }

@@ -21,7 +21,7 @@ import numpy as np
 
 # ABI constants (numeric values documented in DESIGN.md; restated in include/pakr.h and
 # oracle/pakr_oracle.h independently).
-DYN_DOUBLE_INTEGRATOR, DYN_UNICYCLE2, DYN_QUADROTOR = 0, 1, 2
+DYN_DOUBLE_INTEGRATOR, DYN_UNICYCLE2, DYN_QUADROTOR, DYN_DUBINS_AIRPLANE, DYN_UNICYCLE1 = 0, 1, 2, 3, 4
 INT_EULER, INT_RK4 = 0, 1
 OBS_CIRCLE2D, OBS_AABB, OBS_ZCYLINDER = 0, 1, 2
 COST_DURATION, COST_PATH_LENGTH = 0, 1
@@ -232,7 +232,44 @@ def config5(B: int = 1024, K: int = 16, env_seed: int = 505,
     return _di3d("C5-di3d-128", 128, env_seed), PlanConfig(B=B, K=K, tree_capacity=cap, n_replans=1)
 
 
-CONFIGS = {"C1": config1, "C2": config2, "C3": config3, "C4": config4, "C5": config5}
+def config6(env_seed: int = 606) -> tuple[Problem, PlanConfig]:
+    """N1 (not a BASELINE config): 6D Dubins airplane [x,y,z,yaw,pitch,v]
+    among 32 boxes in [0,10]^3; level start and goal, speed in [0.5, 1.5], pitch within +-0.6 rad."""
+    rng = np.random.Generator(np.random.PCG64(env_seed))
+    start = np.array([0.5, 0.5, 5.0, 0.0, 0.0, 1.0])
+    goal = np.array([9.5, 9.5, 5.0])
+    obs = _boxes(rng, 32, [0, 0, 0], [10, 10, 10], 0.5, 2.0, start[:3], goal, 0.7)
+    pi = math.pi
+    p = Problem(
+        name="N1-dubins-airplane", dynamics_id=DYN_DUBINS_AIRPLANE, integrator=INT_RK4, state_dim=6,
+        control_dim=3, pos_dim=3, dyn_params=_f32([]), state_lo=_f32([0, 0, 0, -pi, -0.6, 0.5]),
+        state_hi=_f32([10, 10, 10, pi, 0.6, 1.5]), dim_kind=np.array([0, 0, 0, 1, 0, 0], np.uint8),
+        nn_weight=_f32([1, 1, 1, 0.5, 0.5, 0.5]), control_lo=_f32([-1.0, -0.5, -0.5]),
+        control_hi=_f32([1.0, 0.5, 0.5]), obstacle_type=OBS_AABB, obstacles=obs, start=_f32(start),
+        goal_center=_f32(goal), goal_radius=0.7, goal_angle_dim=-1, goal_angle=0.0, goal_angle_tol=0.0,
+        dt=0.05, steps_per_edge=20, cost_mode=COST_DURATION, heuristic_speed=1.5)
+    return p, PlanConfig(B=1024, K=8, tree_capacity=1 << 20, n_replans=10)
+
+
+def config7(env_seed: int = 707) -> tuple[Problem, PlanConfig]:
+    """N2 (NEXT-2, not a BASELINE config): first-order unicycle [x,y,theta], control (v, omega)
+    among 40 circles in [0,20]^2 (the paper's custom problem has 40 obstacles)."""
+    rng = np.random.Generator(np.random.PCG64(env_seed))
+    start = np.array([1.0, 1.0, 0.0])
+    goal = np.array([19.0, 19.0])
+    obs = _circles(rng, 40, [0, 0], [20, 20], 0.3, 1.2, start[:2], goal, 0.5)
+    pi = math.pi
+    p = Problem(
+        name="N2-unicycle1", dynamics_id=DYN_UNICYCLE1, integrator=INT_RK4, state_dim=3, control_dim=2,
+        pos_dim=2, dyn_params=_f32([]), state_lo=_f32([0, 0, -pi]), state_hi=_f32([20, 20, pi]),
+        dim_kind=np.array([0, 0, 1], np.uint8), nn_weight=_f32([1, 1, 0.5]), control_lo=_f32([-0.5, -1.5]),
+        control_hi=_f32([1.0, 1.5]), obstacle_type=OBS_CIRCLE2D, obstacles=obs, start=_f32(start),
+        goal_center=_f32(goal), goal_radius=0.5, goal_angle_dim=-1, goal_angle=0.0, goal_angle_tol=0.0,
+        dt=0.05, steps_per_edge=20, cost_mode=COST_DURATION, heuristic_speed=1.0)
+    return p, PlanConfig(B=1024, K=8, tree_capacity=1 << 20, n_replans=10)
+
+
+CONFIGS = {"C1": config1, "C2": config2, "C3": config3, "C4": config4, "C5": config5, "N1": config6, "N2": config7}
 
 
 def random_tree(problem: Problem, n: int, seed: int, flat: bool = False) -> dict[str, np.ndarray]:

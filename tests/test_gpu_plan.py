@@ -61,7 +61,7 @@ def _check_tree(orc, op, p, tree, cap, n_samples=300):
         assert d.max() < 1e-4
 
 
-@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4"])
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "N1", "N2"])
 def test_plan_configs(pakr, orc, name):
     p, cfg = wl.CONFIGS[name]()
     pl = pakr.Planner(p)
@@ -161,7 +161,7 @@ def test_abi_errors(pakr):
     pl.close()
 
 
-@pytest.mark.parametrize("name,iters", [("C1", 12), ("C2", 9), ("C3", 6)])
+@pytest.mark.parametrize("name,iters", [("C1", 12), ("C2", 9), ("C3", 6), ("N1", 7), ("N2", 8)])
 def test_plan_loop_equals_chain_of_single_steps(pakr, name, iters):
     """The device-resident loop (NN look-ahead scan, fused tail scan, two key buffers) must build exactly
     the tree that `iters` separate pakr_expand_step calls build (no look-ahead there): bit-exact."""

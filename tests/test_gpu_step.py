@@ -39,6 +39,10 @@ _CASES = [
     ("C4", 12345, 200, 9),
     ("C4", 30000, 1024, 16),
     ("C5", 7777, 256, 16),
+    ("N1", 6000, 512, 8),   # Dubins airplane (NEXT-2)
+    ("N1", 31, 100, 3),
+    ("N2", 4097, 300, 5),   # first-order unicycle (NEXT-2)
+    ("N2", 20000, 1024, 8),
 ]
 
 

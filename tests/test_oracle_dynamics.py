@@ -197,3 +197,58 @@ def test_angle_wrap(orc):
     T = p.steps_per_edge * float(np.float32(p.dt))
     x, *_ = op.propagate([2, 3, 3.0, 0.0, 1.0], [0.0, 0.0])  # theta -> 3 + T ~ 4.0 -> 4 - 2pi
     assert x[2] == pytest.approx(3.0 + T - 2 * math.pi, abs=1e-12)
+
+
+def test_rk4_unicycle1_closed_forms(orc):
+    """NEXT-2 model: straight line exact; constant (v, omega) is a circular arc
+    x = x0 + (v/w)(sin(th0 + wT) - sin th0), y = y0 - (v/w)(cos(th0 + wT) - cos th0); heading th0 + wT (wrapped)."""
+    p, _ = wl.config7()
+    op = orc.OracleProblem(_free(p))
+    T = p.steps_per_edge * float(np.float32(p.dt))
+    x, *_ = op.propagate([2, 3, 0.6], [0.8, 0.0])
+    np.testing.assert_allclose(x, [2 + 0.8 * T * math.cos(0.6), 3 + 0.8 * T * math.sin(0.6), 0.6], atol=1e-13)
+    v, w, th0 = 0.9, -1.3, 2.9
+    x, *_ = op.propagate([5, 6, th0], [v, w])
+    np.testing.assert_allclose(x[0], 5 + (v / w) * (math.sin(th0 + w * T) - math.sin(th0)), atol=2e-8)
+    np.testing.assert_allclose(x[1], 6 - (v / w) * (math.cos(th0 + w * T) - math.cos(th0)), atol=2e-8)
+    assert x[2] == pytest.approx(orc.wrap_pi(th0 + w * T), abs=1e-13)
+    # reversing (v < 0) moves against the heading: catches a dropped sign / swapped sin-cos
+    x, *_ = op.propagate([5, 6, math.pi / 2], [-0.5, 0.0])
+    np.testing.assert_allclose(x[:2], [5, 6 - 0.5 * T], atol=1e-13)
+
+
+def test_rk4_dubins_airplane_closed_forms(orc):
+    """NEXT-2 model (reading P33): velocity of magnitude v along (yaw, pitch).
+    Zero rates + constant acceleration: straight line of length v0 T + a T^2/2 (RK4 exact for a quadratic);
+    yaw rate only at level flight: horizontal circular arc; pitch rate only at yaw 0: vertical arc."""
+    p, _ = wl.config6()
+    op = orc.OracleProblem(_free(p))
+    T = p.steps_per_edge * float(np.float32(p.dt))
+    yaw, pitch, v0, a = 0.7, -0.3, 1.1, 0.4
+    x, *_ = op.propagate([1, 2, 3, yaw, pitch, v0], [0.0, 0.0, a])
+    s = v0 * T + 0.5 * a * T * T
+    d = np.array([math.cos(pitch) * math.cos(yaw), math.cos(pitch) * math.sin(yaw), math.sin(pitch)])
+    np.testing.assert_allclose(x[:3], np.array([1, 2, 3]) + s * d, atol=1e-13)
+    np.testing.assert_allclose(x[3:], [yaw, pitch, v0 + a * T], atol=1e-13)
+    w = 0.8  # level turn
+    x, *_ = op.propagate([1, 2, 3, yaw, 0.0, v0], [w, 0.0, 0.0])
+    np.testing.assert_allclose(x[0], 1 + (v0 / w) * (math.sin(yaw + w * T) - math.sin(yaw)), atol=2e-8)
+    np.testing.assert_allclose(x[1], 2 - (v0 / w) * (math.cos(yaw + w * T) - math.cos(yaw)), atol=2e-8)
+    assert x[2] == pytest.approx(3.0, abs=1e-13) and x[3] == pytest.approx(yaw + w * T, abs=1e-13)
+    q = -0.45  # pull-down in the x-z plane
+    x, *_ = op.propagate([1, 2, 3, 0.0, 0.2, v0], [0.0, q, 0.0])
+    np.testing.assert_allclose(x[0], 1 + (v0 / q) * (math.sin(0.2 + q * T) - math.sin(0.2)), atol=2e-8)
+    np.testing.assert_allclose(x[2], 3 - (v0 / q) * (math.cos(0.2 + q * T) - math.cos(0.2)), atol=2e-8)
+    assert x[1] == pytest.approx(2.0, abs=1e-13) and x[4] == pytest.approx(0.2 + q * T, abs=1e-13)
+
+
+def test_rk4_convergence_new_models(orc):
+    """General motion of both NEXT-2 models against the same RK4 at dt/16: 4th-order (error ratio ~16 per halving)."""
+    for cfgf, x0, u in ((wl.config6, [1, 2, 3, 0.4, 0.1, 1.0], [0.9, -0.4, 0.3]), (wl.config7, [1, 2, 0.4], [0.9, 1.2])):
+        p, _ = cfgf()
+        errs = []
+        fine = orc.OracleProblem(_free(p, dt=p.dt / 16, steps_per_edge=p.steps_per_edge * 16)).propagate(x0, u)[0]
+        for k in (1, 2):
+            x = orc.OracleProblem(_free(p, dt=p.dt / k, steps_per_edge=p.steps_per_edge * k)).propagate(x0, u)[0]
+            errs.append(np.abs(x - fine).max())
+        assert errs[0] < 1e-6 and 10 < errs[0] / errs[1] < 24, errs
