@@ -123,6 +123,9 @@ typedef struct {
   double time_budget_ms;  /* > 0: stop at the first iteration boundary past the budget (device
                              %globaltimer; non-deterministic); <= 0: none (deterministic) */
   int64_t max_iters_per_replan; /* 0 = default max(32, capacity / (B*K)) */
+  double initial_cost_bound;    /* c_best before the first replan (Alg. 1 l.1); <= 0 or +INF = none.  A finite bound
+                                   (e.g. the best cost another replica found) prunes from the start;
+                                   the result reports only what THIS call found (NO_SOLUTION if nothing cheaper) */
 } pakr_plan_opts;
 
 #define PAKR_MAX_REPLAN_STATS 64

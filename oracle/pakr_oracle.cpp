@@ -430,6 +430,7 @@ extern "C" int32_t orc_plan(const orc_problem* P, const orc_plan_opts* O, orc_tr
   int64_t max_iters = O->max_iters_per_replan;
   if (max_iters <= 0) max_iters = std::max<int64_t>(32, O->tree_capacity / BK);  // P21
   double c_best = kInf;  // l.1
+  if (O->initial_cost_bound > 0.0 && std::isfinite(O->initial_cost_bound)) c_best = O->initial_cost_bound;
   R->path_len = 0;       // l.2
   R->outcome = 0;
   R->cost = kInf;

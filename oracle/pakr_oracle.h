@@ -124,6 +124,7 @@ typedef struct {
   uint64_t seed; int32_t B, K; int64_t tree_capacity; int32_t n_replans;
   double time_budget_ms;          /* <=0: none */
   int64_t max_iters_per_replan;   /* 0: default max(32, cap/(B*K)) (P21) */
+  double initial_cost_bound;      /* c_best of Alg. 1 l.1; <= 0 or inf: +inf (the paper's value) */
 } orc_plan_opts;
 
 typedef struct {

@@ -63,7 +63,8 @@ class _IterDebug(C.Structure):
 class _PlanOpts(C.Structure):
     _fields_ = [("seed", C.c_uint64), ("B", C.c_int32), ("K", C.c_int32),
                 ("tree_capacity", C.c_int64), ("n_replans", C.c_int32),
-                ("time_budget_ms", C.c_double), ("max_iters_per_replan", C.c_int64)]
+                ("time_budget_ms", C.c_double), ("max_iters_per_replan", C.c_int64),
+                ("initial_cost_bound", C.c_double)]
 
 
 class _PlanResult(C.Structure):
@@ -260,7 +261,7 @@ def expand_iteration(op: OracleProblem, tree: OracleTree, seed: int, r: int, it:
 
 def plan(op: OracleProblem, seed: int, B: int, K: int, tree_capacity: int, n_replans: int,
          time_budget_ms: float = 0.0, max_iters_per_replan: int = 0, path_capacity: int = 4096,
-         tree: Optional[OracleTree] = None) -> dict:
+         tree: Optional[OracleTree] = None, initial_cost_bound: float = 0.0) -> dict:
     """Alg. 1 l.1-18.  Returns the path (nodes, states, controls), cost, stats and the final tree."""
     tree = tree or OracleTree(op, tree_capacity)
     nodes = np.zeros(path_capacity, np.int32)
@@ -269,7 +270,7 @@ def plan(op: OracleProblem, seed: int, B: int, K: int, tree_capacity: int, n_rep
     rc = np.full(n_replans, np.inf)
     rn = np.zeros(n_replans, np.int64)
     ri = np.zeros(n_replans, np.int64)
-    opts = _PlanOpts(seed, B, K, tree_capacity, n_replans, time_budget_ms, max_iters_per_replan)
+    opts = _PlanOpts(seed, B, K, tree_capacity, n_replans, time_budget_ms, max_iters_per_replan, initial_cost_bound)
     res = _PlanResult(_ptr(nodes, _ip), _ptr(states), _ptr(ctrls), path_capacity, 0, 0.0, 0, 0, 0, 0, 0, 0,
                       0.0, 0.0, _ptr(rc), _ptr(rn, _lp), _ptr(ri, _lp))
     status = lib().orc_plan(op.ref, C.byref(opts), tree.ref, C.byref(res))

@@ -425,7 +425,8 @@ extern "C" pakr_status pakr_plan(pakr_planner* pl, const pakr_plan_opts* o, void
   if (!pl) return PAKR_ERR_INVALID_ARG;
   if (!o || !out || !d_ws) return fail(pl, PAKR_ERR_INVALID_ARG, "null opts, result or workspace");
   if (!sizes_ok(o->B, o->K, o->tree_capacity) || o->n_replans < 1 || o->n_replans > 4096 ||
-      o->max_iters_per_replan < 0 || o->max_iters_per_replan > (1ll << 30) || out->path_capacity < 0)
+      o->max_iters_per_replan < 0 || o->max_iters_per_replan > (1ll << 30) || out->path_capacity < 0 ||
+      std::isnan(o->initial_cost_bound))
     return fail(pl, PAKR_ERR_INVALID_ARG, "B, K, tree_capacity, n_replans or max_iters out of range");
   if (reinterpret_cast<uintptr_t>(d_ws) % kAlign) return fail(pl, PAKR_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
   const Layout L = make_layout(pl, o->B, o->K, o->tree_capacity);
@@ -445,7 +446,7 @@ extern "C" pakr_status pakr_plan(pakr_planner* pl, const pakr_plan_opts* o, void
   P.max_iters = (int)mi;
   P.budget_ns = o->time_budget_ms > 0 ? (unsigned long long)(o->time_budget_ms * 1e6) : 0ull;
   P.r0 = 0; P.it0 = 0;
-  P.c_best0 = INFINITY;
+  P.c_best0 = (o->initial_cost_bound > 0.0 && std::isfinite(o->initial_cost_bound)) ? (float)o->initial_cost_bound : INFINITY;
   P.early_exit = 1;
   // Alg. 1 l.4: root node (x_init, no action, parent -1, cost 0); rewritten never, read by every replan
   float root[kMaxD + kMaxM + 2] = {0};

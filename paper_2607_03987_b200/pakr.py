@@ -91,7 +91,8 @@ class _TreeLayout(C.Structure):
 
 class _PlanOpts(C.Structure):
     _fields_ = [("seed", C.c_uint64), ("B", C.c_int32), ("K", C.c_int32), ("tree_capacity", C.c_int64),
-                ("n_replans", C.c_int32), ("time_budget_ms", C.c_double), ("max_iters_per_replan", C.c_int64)]
+                ("n_replans", C.c_int32), ("time_budget_ms", C.c_double), ("max_iters_per_replan", C.c_int64),
+                ("initial_cost_bound", C.c_double)]
 
 
 class _Stats(C.Structure):
@@ -225,12 +226,13 @@ class Planner:
 
     # ---- pakr_plan ----
     def plan(self, seed: int, B: int, K: int, tree_capacity: int, n_replans: int, time_budget_ms: float = 0.0,
-             max_iters_per_replan: int = 0, path_capacity: int = 8192, workspace=None) -> dict:
+             max_iters_per_replan: int = 0, path_capacity: int = 8192, workspace=None,
+             initial_cost_bound: float = 0.0) -> dict:
         ws = workspace if workspace is not None else self.workspace(B, K, tree_capacity)
         nodes = np.zeros(path_capacity, np.int32)
         states = np.zeros((path_capacity, self.D), np.float32)
         ctrls = np.zeros((max(path_capacity - 1, 1), self.m), np.float32)
-        opts = _PlanOpts(seed, B, K, tree_capacity, n_replans, time_budget_ms, max_iters_per_replan)
+        opts = _PlanOpts(seed, B, K, tree_capacity, n_replans, time_budget_ms, max_iters_per_replan, initial_cost_bound)
         res = _Result(_ptr(nodes, _ip), _ptr(states), _ptr(ctrls), path_capacity, 0, 0.0, 0, 0, _Stats())
         st = lib().pakr_plan(self._h, C.byref(opts), C.c_void_p(ws.data_ptr()), ws.numel(), C.c_void_p(self._stream()),
                              C.byref(res))

@@ -42,3 +42,25 @@ def best_of_replicas(costs: Sequence[float], dist=None, device=None) -> float:
     if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MIN)
     return float(t[0])
+
+
+def shared_bound_rounds(plan_fn, rounds: int, dist=None, device=None) -> dict:
+    """Replicas that share the cost bound between rounds (C-FOREST-style).
+
+    plan_fn(bound, round) -> (cost, payload) runs this rank's planner for one round under `bound` (+inf = none;
+    with the CUDA library: pakr_plan(..., initial_cost_bound=bound), a different seed per rank and round) and
+    returns the cost it found (+inf if nothing cheaper) with anything describing the plan.  After every round
+    one scalar MIN all-reduce makes the best cost of ANY replica the bound of ALL replicas for the next round:
+    4-8 bytes per round over NCCL / NVLink, latency-bound, never on the per-iteration path.
+    Returns {"cost": global best, "payload": this rank's plan for its own best cost, "owner": whether this rank
+    holds a plan achieving the global best, "history": global best after each round}."""
+    bound = float("inf")
+    my_cost, my_payload, history = float("inf"), None, []
+    for rnd in range(rounds):
+        cost, payload = plan_fn(bound, rnd)
+        if cost < my_cost:
+            my_cost, my_payload = cost, payload
+        bound = min(bound, best_of_replicas([my_cost], dist=dist, device=device))
+        history.append(bound)
+    return {"cost": bound, "payload": my_payload, "owner": my_cost == bound and my_payload is not None,
+            "history": history}

@@ -188,3 +188,43 @@ def test_plan_loop_equals_chain_of_single_steps(pakr, name, iters):
     np.testing.assert_array_equal(tree["parents"][:n_chain].cpu().numpy(), loop_tree["parents"])
     np.testing.assert_array_equal(tree["costs"][:n_chain].cpu().numpy(), loop_tree["costs"])
     pl.close()
+
+
+@pytest.mark.parametrize("name,seeds", [("C1", 12), ("C2", 8), ("N2", 6)])
+def test_plan_many_seeds_validated(pakr, orc, name, seeds):
+    """Every returned plan of a spread of planner seeds is re-propagated by the oracle (north_star end-to-end bar)."""
+    p, cfg = wl.CONFIGS[name]()
+    pl = pakr.Planner(p)
+    costs = []
+    for seed in range(100, 100 + seeds):
+        res = pl.plan(seed, cfg.B, cfg.K, cfg.tree_capacity, 3)
+        _check_plan(orc, p, res)
+        costs.append(res["cost"])
+    assert len(set(costs)) >= 1
+    pl.close()
+
+
+def test_plan_initial_cost_bound(pakr, orc):
+    """pakr_plan under a bound handed in from outside (NEXT-4): prunes from the first replan; reports only
+    what this call found; the oracle's loop with the same bound agrees on C1."""
+    p, cfg = wl.config1()
+    pl = pakr.Planner(p)
+    free = pl.plan(3, cfg.B, cfg.K, cfg.tree_capacity, 1)
+    assert free["outcome"] == 1
+    c0 = free["cost"]
+    res = pl.plan(4, cfg.B, cfg.K, cfg.tree_capacity, 4, initial_cost_bound=c0)
+    if res["outcome"]:
+        assert res["cost"] < c0
+        _check_plan(orc, p, res)
+    else:
+        assert res["path_len"] == 0 and np.isinf(res["cost"])
+    assert np.all(res["replan_cost"] <= np.float32(c0))
+    # a bound nothing can beat: every child is pruned, no solution, and that is not an error
+    res = pl.plan(4, cfg.B, cfg.K, cfg.tree_capacity, 2, initial_cost_bound=1e-3, max_iters_per_replan=5)
+    assert res["outcome"] == 0 and res["inserted"] == 0
+    op = orc.OracleProblem(p)
+    ref = orc.plan(op, 4, cfg.B, cfg.K, cfg.tree_capacity, 1, initial_cost_bound=c0)
+    one = pl.plan(4, cfg.B, cfg.K, cfg.tree_capacity, 1, initial_cost_bound=c0)
+    assert one["outcome"] == ref["outcome"]
+    assert abs(int(one["replan_iters"][0]) - int(ref["replan_iters"][0])) <= 2
+    pl.close()

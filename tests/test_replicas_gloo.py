@@ -31,8 +31,18 @@ def _worker(rank, world, port, q):
     # rank r "takes" (r+1)*10 ms on the device and (r+1)*12 ms wall for 100*(r+1) units
     out = replicas.aggregate(10.0 * (rank + 1), 12.0 * (rank + 1), 100.0 * (rank + 1), dist=dist)
     best = replicas.best_of_replicas([5.0 - rank, 9.0], dist=dist)
+    # NEXT-4: the bound found by one replica prunes the others from the next round on
+    table = {0: [9.0, 7.0, 7.5], 1: [8.0, 8.5, 6.0]}[rank]
+    seen = []
+
+    def plan_fn(bound, rnd):
+        seen.append(bound)
+        c = table[rnd]
+        return (c, (rank, rnd)) if c < bound else (float("inf"), None)
+
+    shared = replicas.shared_bound_rounds(plan_fn, 3, dist=dist)
     dist.barrier()
-    q.put((rank, seeds, out, best))
+    q.put((rank, seeds, out, best, shared, seen))
     dist.destroy_process_group()
 
 
@@ -52,7 +62,11 @@ def test_two_rank_gloo_aggregation():
         p.join(timeout=60)
         assert p.exitcode == 0
     assert res[0][1] == [0, 2, 4] and res[1][1] == [1, 3, 5]
-    for _, _, out, best in res:  # identical on every rank: max time, summed units, min cost
+    for rank, _, _, _, shared, seen in res:
+        assert seen == [float("inf"), 8.0, 7.0]          # bounds handed to the planner: global best so far
+        assert shared["history"] == [8.0, 7.0, 6.0] and shared["cost"] == 6.0
+        assert shared["owner"] == (rank == 1) and shared["payload"] == ((0, 1) if rank == 0 else (1, 2))
+    for _, _, out, best, _, _ in res:  # identical on every rank: max time, summed units, min cost
         assert out["device_ms"] == 20.0 and out["wall_ms"] == 24.0 and out["units"] == 300.0
         assert out["value"] == pytest.approx(300.0 / 0.020)
         assert best == 4.0
