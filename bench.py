@@ -45,7 +45,7 @@ def algorithmic_ops(problem, nn_pairs: int, children: int) -> dict:
     n_angle = int((problem.dim_kind == 1).sum())
     nn_per_pair = 2 * D + 2 + (D if weighted else 0) + 2 * n_angle
     f_dyn = {wl.DYN_DOUBLE_INTEGRATOR: 0, wl.DYN_UNICYCLE2: 25, wl.DYN_QUADROTOR: 140, wl.DYN_DUBINS_AIRPLANE: 50,
-             wl.DYN_UNICYCLE1: 24}[problem.dynamics_id]
+             wl.DYN_UNICYCLE1: 24, wl.DYN_QUADROTOR_BODY: 170}[problem.dynamics_id]
     stages = 4 if problem.integrator == wl.INT_RK4 else 1
     integ = 8 * D if problem.integrator == wl.INT_RK4 else 2 * D
     n_bounded = int((np.isfinite(problem.state_lo) & (problem.dim_kind == 0)).sum())

@@ -46,7 +46,7 @@ typedef enum {
 } pakr_status;
 
 enum { PAKR_DYN_DOUBLE_INTEGRATOR = 0, PAKR_DYN_UNICYCLE2 = 1, PAKR_DYN_QUADROTOR = 2,
-       PAKR_DYN_DUBINS_AIRPLANE = 3, PAKR_DYN_UNICYCLE1 = 4 };
+       PAKR_DYN_DUBINS_AIRPLANE = 3, PAKR_DYN_UNICYCLE1 = 4, PAKR_DYN_QUADROTOR_BODY = 5 };
 enum { PAKR_INT_EULER = 0, PAKR_INT_RK4 = 1 };
 enum { PAKR_OBS_CIRCLE2D = 0, PAKR_OBS_AABB = 1, PAKR_OBS_ZCYLINDER = 2 };
 enum { PAKR_COST_DURATION = 0, PAKR_COST_PATH_LENGTH = 1 };
@@ -70,11 +70,12 @@ typedef struct {
                           unicycle [x,y,theta,v,omega], quadrotor [p, v, (phi,theta,
                           psi) ZYX, (p,q,r)] with control (T, tau) (BASELINE.json config 4), Dubins airplane
                           [x,y,z,yaw,pitch,v] with control (yaw rate, pitch rate, acceleration),
-                          first-order unicycle [x,y,theta] with control (v, omega) */
+                          first-order unicycle [x,y,theta] with control (v, omega), quadcopter with
+                          body-frame velocities [p, (phi,theta,psi), (u,v,w) body, (p,q,r)] exactly as PAPER.md:174 */
   int32_t integrator;  /* PAKR_INT_*: forward Euler or classical RK4 */
   int32_t state_dim, control_dim, pos_dim; /* must match dynamics_id: DI (2*pos_dim, pos_dim,
-                          2|3), unicycle2 (5,2,2), quadrotor (12,4,3), Dubins airplane (6,3,3), unicycle1 (3,2,2) */
-  const float* dyn_params; int32_t n_dyn_params; /* quadrotor: m, Ixx, Iyy, Izz, g; else 0 */
+                          2|3), unicycle2 (5,2,2), both quadrotors (12,4,3), Dubins airplane (6,3,3), unicycle1 (3,2,2) */
+  const float* dyn_params; int32_t n_dyn_params; /* quadrotors: m, Ixx, Iyy, Izz, g; else 0 */
   const float* state_lo; const float* state_hi;  /* [D]; +-INF = unbounded; box-tested every step */
   const uint8_t* dim_kind; /* [D] PAKR_DIM_*; angle dims (unicycle theta, quadrotor psi, airplane yaw) are wrapped
                           to [-pi,pi) and never bounds-tested; must match the dynamics */

@@ -194,6 +194,33 @@ extern "C" void orc_f(const orc_problem* P, const double* x, const double* u, do
       xd[2] = u[1];
       break;
     }
+    case ORC_DYN_QUADROTOR_BODY: {
+      // state [x,y,z, phi,theta,psi, u,v,w, p,q,r] with linear and angular velocities in the body
+      // frame, control [T, tau_x, tau_y, tau_z].  Rigid body in body axes (reading P34: phi roll, theta pitch,
+      // psi yaw, ZYX; thrust along body z):  p_dot = R v_b;  v_b_dot = -w x v_b + R^T (0,0,-g) + (0,0,T/m).
+      const double m = P->dyn_params[0], Ixx = P->dyn_params[1], Iyy = P->dyn_params[2],
+                   Izz = P->dyn_params[3], g = P->dyn_params[4];
+      const double phi = x[3], th = x[4], psi = x[5];
+      const double ub = x[6], vb = x[7], wb = x[8], p = x[9], q = x[10], r = x[11];
+      const double sphi = std::sin(phi), cphi = std::cos(phi), sth = std::sin(th), cth = std::cos(th),
+                   spsi = std::sin(psi), cpsi = std::cos(psi);
+      const double R[3][3] = {
+          {cpsi * cth, cpsi * sth * sphi - spsi * cphi, cpsi * sth * cphi + spsi * sphi},
+          {spsi * cth, spsi * sth * sphi + cpsi * cphi, spsi * sth * cphi - cpsi * sphi},
+          {-sth, cth * sphi, cth * cphi}};
+      for (int i = 0; i < 3; ++i) xd[i] = R[i][0] * ub + R[i][1] * vb + R[i][2] * wb;
+      xd[3] = p + sphi * (sth / cth) * q + cphi * (sth / cth) * r;
+      xd[4] = cphi * q - sphi * r;
+      xd[5] = (sphi * q + cphi * r) / cth;
+      // -w x v_b = (r v - q w, p w - r u, q u - p v);  R^T (0,0,-g) = -g * third row of R
+      xd[6] = r * vb - q * wb - g * R[2][0];
+      xd[7] = p * wb - r * ub - g * R[2][1];
+      xd[8] = q * ub - p * vb - g * R[2][2] + u[0] / m;
+      xd[9] = (u[1] - (Izz - Iyy) * q * r) / Ixx;
+      xd[10] = (u[2] - (Ixx - Izz) * p * r) / Iyy;
+      xd[11] = (u[3] - (Iyy - Ixx) * p * q) / Izz;
+      break;
+    }
     default:
       for (int d = 0; d < P->state_dim; ++d) xd[d] = 0.0;
   }

@@ -24,7 +24,7 @@ extern "C" {
 #endif
 
 enum { ORC_DYN_DOUBLE_INTEGRATOR = 0, ORC_DYN_UNICYCLE2 = 1, ORC_DYN_QUADROTOR = 2,
-       ORC_DYN_DUBINS_AIRPLANE = 3, ORC_DYN_UNICYCLE1 = 4 };
+       ORC_DYN_DUBINS_AIRPLANE = 3, ORC_DYN_UNICYCLE1 = 4, ORC_DYN_QUADROTOR_BODY = 5 };
 enum { ORC_INT_EULER = 0, ORC_INT_RK4 = 1 };
 enum { ORC_OBS_CIRCLE2D = 0, ORC_OBS_AABB = 1, ORC_OBS_ZCYLINDER = 2 };
 enum { ORC_COST_DURATION = 0, ORC_COST_PATH_LENGTH = 1 };

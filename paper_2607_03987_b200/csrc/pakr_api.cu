@@ -187,14 +187,14 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
     if (p->pos_dim != 2 || p->state_dim != 5 || p->control_dim != 2)
       return fail(nullptr, PAKR_ERR_INVALID_ARG, "unicycle2 needs (D,m,pos)=(5,2,2)");
     dyn = DYN_UNI2;
-  } else if (p->dynamics_id == PAKR_DYN_QUADROTOR) {
+  } else if (p->dynamics_id == PAKR_DYN_QUADROTOR || p->dynamics_id == PAKR_DYN_QUADROTOR_BODY) {
     if (p->pos_dim != 3 || p->state_dim != 12 || p->control_dim != 4)
       return fail(nullptr, PAKR_ERR_INVALID_ARG, "quadrotor needs (D,m,pos)=(12,4,3)");
     if (p->n_dyn_params < 5 || !p->dyn_params)
       return fail(nullptr, PAKR_ERR_INVALID_ARG, "quadrotor needs dyn_params m,Ixx,Iyy,Izz,g");
     for (int i = 0; i < 4; ++i)
       if (!(p->dyn_params[i] > 0.0f)) return fail(nullptr, PAKR_ERR_INVALID_ARG, "mass/inertia must be > 0");
-    dyn = DYN_QUAD;
+    dyn = p->dynamics_id == PAKR_DYN_QUADROTOR ? DYN_QUAD : DYN_QUADB;
   } else if (p->dynamics_id == PAKR_DYN_DUBINS_AIRPLANE) {
     if (p->pos_dim != 3 || p->state_dim != 6 || p->control_dim != 3)
       return fail(nullptr, PAKR_ERR_INVALID_ARG, "dubins airplane needs (D,m,pos)=(6,3,3)");
@@ -222,7 +222,7 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
     for (int i = 0; i < p->n_obstacles * per; ++i)
       if (!std::isfinite(p->obstacles[i])) return fail(nullptr, PAKR_ERR_INVALID_ARG, "obstacle coordinates must be finite");
   }
-  const int angle = dyn == DYN_UNI2 ? 2 : dyn == DYN_QUAD ? 8 : dyn == DYN_DA ? 3 : dyn == DYN_UNI1 ? 2 : -1;
+  const int angle = dyn == DYN_UNI2 ? 2 : dyn == DYN_QUAD ? 8 : dyn == DYN_DA ? 3 : dyn == DYN_UNI1 ? 2 : dyn == DYN_QUADB ? 5 : -1;
   for (int d = 0; d < D; ++d) {
     const bool is_angle = p->dim_kind[d] == PAKR_DIM_ANGLE;
     if (p->dim_kind[d] > 1 || is_angle != (d == angle))
@@ -266,7 +266,7 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
   pb.goal_r = p->goal_radius; pb.goal_angle = p->goal_angle; pb.goal_angle_tol = p->goal_angle_tol;
   pb.goal_angle_dim = p->goal_angle_dim;
   for (int i = 0; i < 5 && i < p->n_dyn_params; ++i) pb.dyn[i] = p->dyn_params[i];
-  if (dyn == DYN_QUAD)
+  if (dyn == DYN_QUAD || dyn == DYN_QUADB)
     for (int i = 0; i < 4; ++i) pb.dyn[5 + i] = 1.0f / p->dyn_params[i];
   pb.dt = p->dt; pb.S = p->steps_per_edge; pb.integrator = p->integrator; pb.cost_mode = p->cost_mode;
   pb.inv_hspeed = std::isinf(p->heuristic_speed) ? 0.0f : 1.0f / p->heuristic_speed;

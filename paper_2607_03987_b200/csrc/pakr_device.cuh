@@ -16,7 +16,7 @@ constexpr float kPiF = 3.14159274101257324f;   // (float)pi
 constexpr float kTwoPiF = 6.28318548202514648f;
 
 // ---- compile-time description of a dynamics model -------------------------------------------
-enum DynKind { DYN_DI2 = 0, DYN_DI3 = 1, DYN_UNI2 = 2, DYN_QUAD = 3, DYN_DA = 4, DYN_UNI1 = 5 };
+enum DynKind { DYN_DI2 = 0, DYN_DI3 = 1, DYN_UNI2 = 2, DYN_QUAD = 3, DYN_DA = 4, DYN_UNI1 = 5, DYN_QUADB = 6 };
 enum ObsKind { OBS_CIRCLE = 0, OBS_BOX = 1 };
 
 template <int DYN> struct DynTraits;
@@ -26,6 +26,7 @@ template <> struct DynTraits<DYN_UNI2> { static constexpr int D = 5, M = 2, PD =
 template <> struct DynTraits<DYN_QUAD> { static constexpr int D = 12, M = 4, PD = 3, DP = 12, ANGLE = 8; };
 template <> struct DynTraits<DYN_DA> { static constexpr int D = 6, M = 3, PD = 3, DP = 8, ANGLE = 3; };
 template <> struct DynTraits<DYN_UNI1> { static constexpr int D = 3, M = 2, PD = 2, DP = 4, ANGLE = 2; };
+template <> struct DynTraits<DYN_QUADB> { static constexpr int D = 12, M = 4, PD = 3, DP = 12, ANGLE = 5; };
 
 // Problem constants, passed by value in the kernel parameter block.
 struct DevProblem {
@@ -155,6 +156,32 @@ __device__ __forceinline__ void dyn_f(const DevProblem& pb, const float (&x)[Dyn
     xd[0] = u[0] * c;
     xd[1] = u[0] * s;
     xd[2] = u[1];
+  } else if constexpr (DYN == DYN_QUADB) {
+    // [x,y,z, phi,theta,psi, u,v,w (body), p,q,r (body)], control (T, tau).  Same rigid body as
+    // DYN_QUAD written in body axes: pdot = R v_b, v_b dot = -w x v_b + R^T (0,0,-g) + (0,0,T/m).
+    const float Ixx = pb.dyn[1], Iyy = pb.dyn[2], Izz = pb.dyn[3], g = pb.dyn[4];
+    float sphi, cphi, sth, cth, spsi, cpsi;
+    __sincosf(x[3], &sphi, &cphi);
+    __sincosf(x[4], &sth, &cth);
+    __sincosf(x[5] - kTwoPiF * rintf(x[5] * (1.0f / kTwoPiF)), &spsi, &cpsi);
+    const float ub = x[6], vb = x[7], wb = x[8];
+    const float p = x[9], q = x[10], r = x[11];
+    const float icth = __frcp_rn(cth);
+    const float tth = sth * icth;
+    // rows of R = Rz(psi) Ry(theta) Rx(phi)
+    xd[0] = cpsi * cth * ub + (cpsi * sth * sphi - spsi * cphi) * vb + (cpsi * sth * cphi + spsi * sphi) * wb;
+    xd[1] = spsi * cth * ub + (spsi * sth * sphi + cpsi * cphi) * vb + (spsi * sth * cphi - cpsi * sphi) * wb;
+    xd[2] = -sth * ub + cth * sphi * vb + cth * cphi * wb;
+    const float sq_cr = sphi * q + cphi * r;
+    xd[3] = p + tth * sq_cr;
+    xd[4] = cphi * q - sphi * r;
+    xd[5] = sq_cr * icth;
+    xd[6] = r * vb - q * wb + g * sth;
+    xd[7] = p * wb - r * ub - g * sphi * cth;
+    xd[8] = q * ub - p * vb - g * cphi * cth + u[0] * pb.dyn[5];
+    xd[9] = (u[1] - (Izz - Iyy) * q * r) * pb.dyn[6];
+    xd[10] = (u[2] - (Ixx - Izz) * p * r) * pb.dyn[7];
+    xd[11] = (u[3] - (Iyy - Ixx) * p * q) * pb.dyn[8];
   } else {
     const float Ixx = pb.dyn[1], Iyy = pb.dyn[2], Izz = pb.dyn[3], g = pb.dyn[4];
     float sphi, cphi, sth, cth, spsi, cpsi;
@@ -208,7 +235,7 @@ __device__ __forceinline__ void dyn_step(const DevProblem& pb, float (&x)[DynTra
   }
 #pragma unroll
   for (int d = 0; d < D; ++d) { k[d] = 0.0f; acc[d] = 0.0f; }
-  constexpr bool kRoll = (DYN == DYN_QUAD);  // measured: rolling slows the unicycle (less ILP), f of the others is tiny
+  constexpr bool kRoll = (DYN == DYN_QUAD) || (DYN == DYN_QUADB);  // measured: rolling slows the unicycle (less ILP), f of the others is tiny
 #pragma unroll 1
   for (int s = 0; s < (kRoll ? 4 : 1); ++s) {
     if constexpr (kRoll) {

@@ -32,6 +32,8 @@ extern "C" const void* pakr_select_kernel_tiled(int dyn, int obs) {
     case DYN_DA * 2 + OBS_BOX: return kernel_ptr<DYN_DA, OBS_BOX>();
     case DYN_UNI1 * 2 + OBS_CIRCLE: return kernel_ptr<DYN_UNI1, OBS_CIRCLE>();
     case DYN_UNI1 * 2 + OBS_BOX: return kernel_ptr<DYN_UNI1, OBS_BOX>();
+    case DYN_QUADB * 2 + OBS_CIRCLE: return kernel_ptr<DYN_QUADB, OBS_CIRCLE>();
+    case DYN_QUADB * 2 + OBS_BOX: return kernel_ptr<DYN_QUADB, OBS_BOX>();
   }
   return nullptr;
 }

@@ -38,7 +38,7 @@ def nn_ops_per_pair(problem) -> int:
 def prop_ops_per_child(problem) -> int:
     D = problem.state_dim
     f_dyn = {wl.DYN_DOUBLE_INTEGRATOR: 0, wl.DYN_UNICYCLE2: 25, wl.DYN_QUADROTOR: 140, wl.DYN_DUBINS_AIRPLANE: 50,
-             wl.DYN_UNICYCLE1: 24}[problem.dynamics_id]
+             wl.DYN_UNICYCLE1: 24, wl.DYN_QUADROTOR_BODY: 170}[problem.dynamics_id]
     stages = 4 if problem.integrator == wl.INT_RK4 else 1
     integ = 8 * D if problem.integrator == wl.INT_RK4 else 2 * D
     n_bounded = int((np.isfinite(problem.state_lo) & (problem.dim_kind == 0)).sum())

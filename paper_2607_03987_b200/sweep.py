@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """BASELINE.json metrics over seeds: expanded nodes/s, median ms to first solution, best cost at 100 ms.
 
-  configs  C1-C4 at their BASELINE sizes (and the NEXT-2 workloads N1, N2): first-solution time (replan 0, device clock), cost after all
+  configs  C1-C4 at their BASELINE sizes (and the NEXT-2 workloads N1-N3): first-solution time (replan 0, device clock), cost after all
            replans, best cost under a 100 ms device budget; medians over planner seeds 0..N-1
   c5       BASELINE config 5: the B x K scaling sweep on the 6D double integrator with 128 boxes
            (first solution only, like the paper's Table IV)
@@ -29,7 +29,7 @@ def med(v):
 
 
 def run_configs(pakr, seeds):
-    for name in ("C1", "C2", "C3", "C4", "N1", "N2"):
+    for name in ("C1", "C2", "C3", "C4", "N1", "N2", "N3"):
         p, cfg = wl.CONFIGS[name]()
         pl = pakr.Planner(p)
         pl.plan(1000, cfg.B, cfg.K, cfg.tree_capacity, 1)  # warm-up

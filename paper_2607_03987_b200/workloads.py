@@ -22,6 +22,7 @@ import numpy as np
 # ABI constants (numeric values documented in DESIGN.md; restated in include/pakr.h and
 # oracle/pakr_oracle.h independently).
 DYN_DOUBLE_INTEGRATOR, DYN_UNICYCLE2, DYN_QUADROTOR, DYN_DUBINS_AIRPLANE, DYN_UNICYCLE1 = 0, 1, 2, 3, 4
+DYN_QUADROTOR_BODY = 5
 INT_EULER, INT_RK4 = 0, 1
 OBS_CIRCLE2D, OBS_AABB, OBS_ZCYLINDER = 0, 1, 2
 COST_DURATION, COST_PATH_LENGTH = 0, 1
@@ -269,7 +270,25 @@ def config7(env_seed: int = 707) -> tuple[Problem, PlanConfig]:
     return p, PlanConfig(B=1024, K=8, tree_capacity=1 << 20, n_replans=10)
 
 
-CONFIGS = {"C1": config1, "C2": config2, "C3": config3, "C4": config4, "C5": config5, "N1": config6, "N2": config7}
+def config8(env_seed: int = 404) -> tuple[Problem, PlanConfig]:
+    """N3 (NEXT-2, not a BASELINE config): the quadcopter exactly as the paper states it: state
+    [x,y,z, phi,theta,psi, u,v,w, p,q,r] with body-frame linear velocities; C4's cylinder forest, limits and sizes."""
+    c4, cfg = config4(env_seed)
+    start = np.zeros(12)
+    start[:3] = c4.start[:3]
+    vmax, amax, wmax = 5.0, 1.2, 6.0
+    inf = np.inf
+    lo = [0, 0, 0, -amax, -amax, -inf, -vmax, -vmax, -vmax, -wmax, -wmax, -wmax]
+    hi = [20, 20, 5, amax, amax, inf, vmax, vmax, vmax, wmax, wmax, wmax]
+    kind = np.zeros(12, np.uint8)
+    kind[5] = DIM_ANGLE
+    w = [1, 1, 1, 0.2, 0.2, 0.02, 0.1, 0.1, 0.1, 0.02, 0.02, 0.02]
+    p = dataclasses.replace(c4, name="N3-quadcopter-body", dynamics_id=DYN_QUADROTOR_BODY, state_lo=_f32(lo),
+                            state_hi=_f32(hi), dim_kind=kind, nn_weight=_f32(w), start=_f32(start))
+    return p, cfg
+
+
+CONFIGS = {"C1": config1, "C2": config2, "C3": config3, "C4": config4, "C5": config5, "N1": config6, "N2": config7, "N3": config8}
 
 
 def random_tree(problem: Problem, n: int, seed: int, flat: bool = False) -> dict[str, np.ndarray]:

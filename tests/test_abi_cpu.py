@@ -63,7 +63,7 @@ def test_create_without_gpu_fails_loudly():
         pakr.Planner(p)
 
 
-@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C5", "N1", "N2"])
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C5", "N1", "N2", "N3"])
 def test_workloads_deterministic_and_clear(name):
     a, cfg = wl.CONFIGS[name]()
     b, _ = wl.CONFIGS[name]()
@@ -80,7 +80,7 @@ def test_workloads_deterministic_and_clear(name):
         for q, clear in ((ps[:2], 0.5), (g[:2], 0.5 + a.goal_radius)):
             d = np.linalg.norm(a.obstacles[:, :2] - q, axis=1) - a.obstacles[:, 2]
             assert d.min() > clear - 1e-6
-    expected = {"C1": 8, "C2": 32, "C3": 64, "C4": 128, "C5": 128, "N1": 32, "N2": 40}[name]
+    expected = {"C1": 8, "C2": 32, "C3": 64, "C4": 128, "C5": 128, "N1": 32, "N2": 40, "N3": 128}[name]
     assert a.n_obstacles == expected
     assert cfg.B >= 1 and cfg.K >= 1
 

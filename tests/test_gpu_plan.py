@@ -61,7 +61,7 @@ def _check_tree(orc, op, p, tree, cap, n_samples=300):
         assert d.max() < 1e-4
 
 
-@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "N1", "N2"])
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "N1", "N2", "N3"])
 def test_plan_configs(pakr, orc, name):
     p, cfg = wl.CONFIGS[name]()
     pl = pakr.Planner(p)

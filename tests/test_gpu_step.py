@@ -43,6 +43,8 @@ _CASES = [
     ("N1", 31, 100, 3),
     ("N2", 4097, 300, 5),   # first-order unicycle (NEXT-2)
     ("N2", 20000, 1024, 8),
+    ("N3", 2500, 384, 16),  # quadcopter with body-frame velocities, PAPER.md:174 (NEXT-2)
+    ("N3", 15000, 1024, 8),
 ]
 
 

@@ -252,3 +252,53 @@ def test_rk4_convergence_new_models(orc):
             x = orc.OracleProblem(_free(p, dt=p.dt / k, steps_per_edge=p.steps_per_edge * k)).propagate(x0, u)[0]
             errs.append(np.abs(x - fine).max())
         assert errs[0] < 1e-6 and 10 < errs[0] / errs[1] < 24, errs
+
+
+def _rot_zyx(phi, th, psi):
+    cz, sz, cy, sy, cx, sx = math.cos(psi), math.sin(psi), math.cos(th), math.sin(th), math.cos(phi), math.sin(phi)
+    Rz = np.array([[cz, -sz, 0], [sz, cz, 0], [0, 0, 1]])
+    Ry = np.array([[cy, 0, sy], [0, 1, 0], [-sy, 0, cy]])
+    Rx = np.array([[1, 0, 0], [0, cx, -sx], [0, sx, cx]])
+    return Rz @ Ry @ Rx
+
+
+def test_quadcopter_body_frame_model(orc):
+    """NEXT-2 model exactly as PAPER.md:174 (body-frame velocities, reading P34).
+    (i) hover is a fixed point; (ii) free fall from level rest: w_b = -g t, z = z0 - g t^2/2 (RK4 exact);
+    (iii) forward body speed at yaw psi moves along the heading; (iv) the SAME physical motion as the
+    world-frame model of config 4 (pinned separately): equivalent initial states (v_world = R v_b) and equal
+    controls give equal position, angles, rates and world velocity after an edge."""
+    pb, _ = wl.config8()
+    pw, _ = wl.config4()
+    ob, ow = orc.OracleProblem(_free(pb)), orc.OracleProblem(_free(pw))
+    m, g = 1.0, float(np.float32(9.81))
+    T = pb.steps_per_edge * float(np.float32(pb.dt))
+    x0 = np.zeros(12)
+    x0[:3] = [3, 4, 2]
+    x, *_ = ob.propagate(x0, [m * g, 0, 0, 0])
+    np.testing.assert_allclose(x, x0, atol=1e-12)
+    x, *_ = ob.propagate(x0, [0, 0, 0, 0])
+    assert x[8] == pytest.approx(-g * T, abs=1e-12) and x[2] == pytest.approx(2 - 0.5 * g * T * T, abs=1e-12)
+    x1 = x0.copy()
+    x1[5], x1[6] = 0.9, 1.5  # yaw, forward body speed
+    x, *_ = ob.propagate(x1, [m * g, 0, 0, 0])
+    np.testing.assert_allclose(x[:3], [3 + 1.5 * T * math.cos(0.9), 4 + 1.5 * T * math.sin(0.9), 2], atol=1e-12)
+    # both are 4th-order discretisations of the same ODE: compare at dt/4, where their truncation errors (a few
+    # 1e-6 at the config's dt) are ~256 times smaller
+    fine = dict(dt=pb.dt / 4, steps_per_edge=pb.steps_per_edge * 4)
+    ob, ow = orc.OracleProblem(_free(pb, **fine)), orc.OracleProblem(_free(pw, **fine))
+    rng = np.random.default_rng(5)
+    for _ in range(4):
+        ang = rng.uniform([-0.5, -0.5, -3], [0.5, 0.5, 3])
+        vb = rng.uniform(-2, 2, 3)
+        rates = rng.uniform(-1, 1, 3)
+        u = [rng.uniform(5, 15), *rng.uniform(-0.1, 0.1, 3)]
+        R0 = _rot_zyx(*ang)
+        xb = np.concatenate([[3, 4, 2], ang, vb, rates])
+        xw = np.concatenate([[3, 4, 2], R0 @ vb, ang, rates])
+        yb, *_ = ob.propagate(xb, u)
+        yw, *_ = ow.propagate(xw, u)
+        np.testing.assert_allclose(yb[:3], yw[:3], atol=1e-7)           # position
+        np.testing.assert_allclose(yb[3:6], yw[6:9], atol=1e-7)         # Euler angles
+        np.testing.assert_allclose(yb[9:], yw[9:], atol=1e-7)           # body rates
+        np.testing.assert_allclose(_rot_zyx(*yb[3:6]) @ yb[6:9], yw[3:6], atol=1e-7)  # world velocity
