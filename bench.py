@@ -210,8 +210,8 @@ def main():
                        "seeds": f"rank + {world} * step", "l2": "flushed between timed steps (256 MiB fill)",
                        "parallelism": f"replicas x{world}"},
             "clocks": clocks,
-            "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 4 * pl.Dp + 4 + 8 * cfg.B,
-                    "d2h_bytes_per_step": int(np.mean([1624 + 4 * r["path_len"] * (1 + pl.D + pl.m) for r in results]))},
+            "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 4 * pl.Dp + 4,
+                    "d2h_bytes_per_step": int(np.mean([1700 + 4 * r["path_len"] * (1 + pl.D + pl.m) for r in results]))},
             "gpu_launches": args.steps,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tlaneop/s (fp32 lane-instructions)",
                          "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,

@@ -147,7 +147,7 @@ typedef struct {
   int32_t replan_nodes[PAKR_MAX_REPLAN_STATS];/* tree size at its end */
   int32_t replan_iters[PAKR_MAX_REPLAN_STATS];
   double replan_end_ms[PAKR_MAX_REPLAN_STATS];/* device time at its end */
-  int64_t probe_cycles[352]; /* diagnostic: all 0 unless the library was built with -DPAKR_PROBE (SM cycles of
+  int64_t probe_cycles[32]; /* diagnostic: all 0 unless the library was built with -DPAKR_PROBE (SM cycles of
                                thread 0 of CTA 0 between probe points, summed over the launch) */
 } pakr_stats;
 

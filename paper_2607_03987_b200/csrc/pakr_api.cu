@@ -391,7 +391,7 @@ void fill_stats(const Ctrl* hc, int64_t BK, pakr_stats* out) {
   s.inserted = hc->inserted;
   s.nn_pairs = hc->nn_pairs;
   for (int i = 0; i < 3; ++i) s.phase_ms[i] = (double)hc->phase_ns[i] * 1e-6;
-  for (int i = 0; i < 352; ++i) s.probe_cycles[i] = (int64_t)hc->probe[i];
+  for (int i = 0; i < 32; ++i) s.probe_cycles[i] = (int64_t)hc->probe[i];
   s.replans_run = hc->replans_run;
   s.replans_solved = hc->replans_solved;
   s.termination = hc->termination;

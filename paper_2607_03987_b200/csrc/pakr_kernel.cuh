@@ -50,7 +50,7 @@ struct Ctrl {  // device control block (in the workspace)
   unsigned long long t_start_ns, t_first_ns, t_end_ns;
   long long iterations, inserted, nn_pairs;
   unsigned long long phase_ns[3];  // leader's time in NN / propagate / insert incl. the grid sync after each
-  unsigned long long probe[352];    // -DPAKR_PROBE: SM cycles of thread 0 of CTA 0 between probe points
+  unsigned long long probe[32];    // -DPAKR_PROBE: SM cycles of thread 0 of CTA 0 between probe points
   int n_nodes, stop;
   unsigned pbar;      // arrival counter of the barrier among the propagate CTAs (insert inside phase X)
   int iter_total[2];  // survivors of the iteration, published by CTA 0 when the insert ran inside phase X
@@ -993,15 +993,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       }
       PROBE(P, 4);
       if (leader) { const unsigned long long t = globaltimer_ns(); ph0 += t - tp; tp = t; }
-#ifdef PAKR_PROBE
-      const long long g_xstart = clock64();
-#endif
       // phase X: propagate(it) and, meanwhile, NN(it+1) over the frozen snapshot [0, n)
-#ifdef PAKR_EXP_NOAHEAD
-      const bool ahead = false;
-#else
       const bool ahead = (iters + 1 < P.max_iters);
-#endif
       prop_phase<DYN, OBS>(P, (uint32_t)r, (uint32_t)it, c_best, kcur, root_only, x_pw, x_pcnt, sm_obs, sm_cells, sm_list PROBE_PASS);
       // goal-key slots alternate over the whole launch (not per replan): the other slot was last
       // read before the previous grid sync and is next written after the following one
@@ -1029,9 +1022,6 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
         if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
         else nn_phase<DYN, false, STREAM>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
       }
-#ifdef PAKR_PROBE
-      if (threadIdx.x == 0 && blockIdx.x < 320) atomicAdd(&P.ctrl->probe[32 + blockIdx.x], (unsigned long long)(clock64() - g_xstart));
-#endif
       if (leader) P.ctrl->goal_key[slot ^ 1] = kKeyNone;
       if (leader && xins && P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) P.ctrl->stop = 1;
       fence_proxy_async();  // scratch rows written with st.global may be read by TMA in the insert phase

@@ -101,7 +101,7 @@ class _Stats(C.Structure):
                 ("first_solution_ms", C.c_double), ("device_ms", C.c_double), ("phase_ms", C.c_double * 3),
                 ("replan_cost", C.c_float * MAX_REPLAN_STATS), ("replan_nodes", C.c_int32 * MAX_REPLAN_STATS),
                 ("replan_iters", C.c_int32 * MAX_REPLAN_STATS), ("replan_end_ms", C.c_double * MAX_REPLAN_STATS),
-                ("probe_cycles", C.c_int64 * 352)]
+                ("probe_cycles", C.c_int64 * 32)]
 
 
 class _Result(C.Structure):
