@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -22,9 +23,11 @@ struct pakr_planner {
   uint32_t* d_grid_cells = nullptr;
   uint16_t* d_grid_list = nullptr;
   int num_sms = 0, blocks_per_sm = 0;
+  int nn_index = 0;  // NN cell index usable: finite position box, positive position weights
   size_t smem_bytes = 0;
   const void* kernel = nullptr;         // tiled NN scan
   const void* kernel_stream = nullptr;  // streaming NN tier (B <= kStreamB)
+  const void* kernel_index = nullptr;   // tiled scan + NN cell index (only when nn_index != 0)
   void* h_pinned = nullptr;  // Ctrl + path staging
   std::string err;
 };
@@ -34,6 +37,7 @@ static thread_local std::string g_create_err;
 // defined in pakr_kernel_inst.cu (one translation unit per NN tier)
 extern "C" const void* pakr_select_kernel_tiled(int dyn, int obs);
 extern "C" const void* pakr_select_kernel_stream(int dyn, int obs);
+extern "C" const void* pakr_select_kernel_index(int dyn, int obs);
 
 namespace {
 
@@ -42,7 +46,7 @@ size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
   size_t states, actions, parents, costs, nn_key, unit_count, scr_state, scr_ctrl, scr_cost, scr_parent,
-      scr_flags, xq, ctrl, path_rev, path_nodes, path_states, path_controls, total;
+      scr_flags, xq, idx_ids, idx_start, idx_cnt, ctrl, path_rev, path_nodes, path_states, path_controls, total;
 };
 
 Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap) {
@@ -57,6 +61,9 @@ Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap) {
   L.nn_key = take((size_t)B * 16);  // two iterations in flight
   L.unit_count = take(std::max<size_t>(U, kFuseUnits + 8) * 4);
   L.xq = take((size_t)B * pl->DP * 4);
+  L.idx_ids = take((size_t)cap * 4);
+  L.idx_start = take((size_t)(kIdxMaxCells + 1) * 4);
+  L.idx_cnt = take((size_t)kIdxMaxCells * 4);
   L.scr_state = take(slots * pl->DP * 4);
   L.scr_ctrl = take(slots * 16);
   L.scr_cost = take(slots * 4);
@@ -271,6 +278,16 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
   pb.dt = p->dt; pb.S = p->steps_per_edge; pb.integrator = p->integrator; pb.cost_mode = p->cost_mode;
   pb.inv_hspeed = std::isinf(p->heuristic_speed) ? 0.0f : 1.0f / p->heuristic_speed;
   pb.unit_weights = unit ? 1 : 0;
+  {
+    bool ok = true;
+    for (int a = 0; a < PD; ++a)
+      ok = ok && std::isfinite(pb.lo[a]) && std::isfinite(pb.hi[a]) && pb.hi[a] > pb.lo[a] && pb.w[a] > 0.0f;
+    // The NN cell index is exact and tested but, as measured this round, slower than the scan tiers (DESIGN.md
+    // "NN index tier"): it stays opt-in.  Read at create: PAKR_NN_INDEX=1 index when B*n is large, =2 index on any
+    // tree of >= 256 rows (tests); unset or 0: scan tiers only.
+    const char* env = std::getenv("PAKR_NN_INDEX");
+    pl->nn_index = !ok ? 0 : (env && env[0] == '1') ? 1 : (env && env[0] == '2') ? 2 : 0;
+  }
   pb.n_obs = p->n_obstacles;
 
   // obstacle table in the kernel's shared-memory row format
@@ -320,15 +337,21 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
   }
   pl->kernel = pakr_select_kernel_tiled(dyn, obs);
   pl->kernel_stream = pakr_select_kernel_stream(dyn, obs);
+  pl->kernel_index = pakr_select_kernel_index(dyn, obs);
+  if (!pl->kernel_index) { pl->kernel_index = pl->kernel; pl->nn_index = 0; }  // no index tier for this model
   pl->smem_bytes = smem_for(pl);
   e = cudaFuncSetAttribute(pl->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes);
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute(pl->kernel_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(pl->kernel_index, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes);
   if (e != cudaSuccess) return bail(PAKR_ERR_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&pl->blocks_per_sm, pl->kernel, kThreads, pl->smem_bytes);
   int occ_stream = 0;
   if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_stream, pl->kernel_stream, kThreads, pl->smem_bytes);
-  pl->blocks_per_sm = std::min(pl->blocks_per_sm, occ_stream);  // one grid size for both tiers
+  int occ_index = 0;
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_index, pl->kernel_index, kThreads, pl->smem_bytes);
+  pl->blocks_per_sm = std::min(pl->blocks_per_sm, std::min(occ_stream, occ_index));  // one grid size for all tiers
   if (e != cudaSuccess || pl->blocks_per_sm < 1)
     return bail(PAKR_ERR_CUDA, "kernel does not fit on an SM (occupancy 0)");
   e = cudaMallocHost(&pl->h_pinned, sizeof(Ctrl) + (size_t)kPathMax * (4 + kMaxD * 4 + kMaxM * 4));
@@ -370,6 +393,10 @@ void fill_common(const pakr_planner* pl, Params& P, const Layout& L, char* ws, i
   P.nn_key = reinterpret_cast<unsigned long long*>(ws + L.nn_key);
   P.unit_count = reinterpret_cast<unsigned*>(ws + L.unit_count);
   P.xq = reinterpret_cast<float*>(ws + L.xq);
+  P.idx_ids = reinterpret_cast<int*>(ws + L.idx_ids);
+  P.idx_start = reinterpret_cast<int*>(ws + L.idx_start);
+  P.idx_cnt = reinterpret_cast<int*>(ws + L.idx_cnt);
+  P.nn_index = pl->nn_index;
   P.scr_state = reinterpret_cast<float*>(ws + L.scr_state);
   P.scr_ctrl = reinterpret_cast<float*>(ws + L.scr_ctrl);
   P.scr_cost = reinterpret_cast<float*>(ws + L.scr_cost);
@@ -413,7 +440,7 @@ pakr_status launch(pakr_planner* pl, Params& P, cudaStream_t stream) {
   CUDA_TRY(pl, cudaMemsetAsync(P.ctrl, 0xFF, 16, stream));  // goal_key[2] = none
   void* args[] = {&P};
   const dim3 grid(pl->num_sms * std::min(pl->blocks_per_sm, kCtasPerSm)), block(kThreads);
-  const void* kernel = P.B <= kStreamB ? pl->kernel_stream : pl->kernel;
+  const void* kernel = P.B <= kStreamB ? pl->kernel_stream : (pl->nn_index ? pl->kernel_index : pl->kernel);
   CUDA_TRY(pl, cudaLaunchCooperativeKernel(kernel, grid, block, args, pl->smem_bytes, stream));
   return PAKR_OK;
 }

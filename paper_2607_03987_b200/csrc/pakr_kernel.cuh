@@ -41,6 +41,9 @@ constexpr int kWarps = kThreads / 32;
 #define PAKR_KQ 4
 #endif
 constexpr int kQ = PAKR_KQ;      // queries per lane in the NN scan
+constexpr int kIdxMaxCells = 16384;  // cells of the NN index (resolution chosen from the tree size at every rebuild)
+constexpr int kIdxMinRows = 4096;    // smaller trees are scanned
+constexpr long long kIdxMinPairs = 120000000ll;  // ... and so are iterations whose scan (B*n pairs) takes < ~60 us
 constexpr int kPathMax = 8192;   // longest path the device buffers hold
 constexpr int kStatsMax = 64;
 constexpr unsigned long long kKeyNone = ~0ull;
@@ -70,6 +73,11 @@ struct Params {
   // per-iteration work buffers
   unsigned long long* nn_key;  // [2][B] (d2 bits << 32) | node, combined with atomicMin; two iterations in flight
   float* xq;                   // [B][Dp] sampled states of the iteration whose NN is being prepared
+  // NN cell index (exact spatial pruning): tree rows [0, n_sorted) bucketed by position cell
+  int nn_index;                // 0: scan tiers only; 1: index when B*n is large; 2: index whenever n >= 256 (tests)
+  int* idx_ids;                // [cap] row ids ordered by cell
+  int* idx_start;              // [kIdxMaxCells + 1] first slot of every cell
+  int* idx_cnt;                // [kIdxMaxCells] histogram / scatter cursors
   unsigned* unit_count;        // [ceil(B*K/32)] survivors per warp unit
   float* scr_state; float* scr_ctrl; float* scr_cost; int* scr_parent; int* scr_flags;
   Ctrl* ctrl;
@@ -361,6 +369,224 @@ __device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, u
       for (int o = 16; o > 0; o >>= 1) kv = min(kv, __shfl_xor_sync(0xffffffffu, kv, o));
       if (lane == 0 && q0 + j < P.B && kv != kKeyNone) atomicMin(&key[q0 + j], kv);
     }
+  }
+}
+
+// ---- NN index tier: exact nearest neighbour with spatial pruning ----------
+// Tree rows [0, n_sorted) are bucketed by a uniform grid over the POSITION dims (counting sort, rebuilt when the
+// tree has grown by an eighth).  A warp answers one query: it visits the cells of growing Chebyshev rings around
+// the query's cell, lanes gather rows by id and evaluate the same distance as the scan tiers, and it stops after
+// ring r as soon as best d2 < min_a w_a (r * cell_a)^2: every row outside the visited cube differs by more than
+// r cells on some position axis, so none can be nearer (exact; ties go to the lowest node id through the
+// (d2, id) key as everywhere).  Rows appended since the last rebuild are scanned by the tiled tier.
+struct IdxGeom {
+  int g[3];          // cells per position axis (g[2] = 1 in 2-D)
+  float inv[3];      // cells per unit length
+  float lb[3];       // w_a * (cell_a * (1 - 1e-4))^2: lower-bound coefficient per axis
+  int cells;
+};
+
+template <int PD>
+__device__ __forceinline__ IdxGeom idx_geometry(const DevProblem& pb, int n) {
+  IdxGeom G;
+  // about 12 rows per cell, at most kIdxMaxCells cells
+  int target = max(n / 12, 64);
+  if (target > kIdxMaxCells) target = kIdxMaxCells;
+  int side = 2;
+  if (PD == 2) { while ((side + 1) * (side + 1) <= target) ++side; }
+  else { while ((side + 1) * (side + 1) * (side + 1) <= target) ++side; }
+  G.cells = 1;
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    G.g[a] = a < PD ? side : 1;
+    const float ext = a < PD ? (pb.hi[a] - pb.lo[a]) : 1.0f;
+    G.inv[a] = (float)G.g[a] / ext;
+    const float cs = ext / (float)G.g[a] * 0.9999f;
+    G.lb[a] = a < PD ? pb.w[a] * cs * cs : __int_as_float(0x7f800000);
+    G.cells *= G.g[a];
+  }
+  return G;
+}
+
+template <int PD>
+__device__ __forceinline__ void idx_cell_coords(const DevProblem& pb, const IdxGeom& G, const float* pos, int (&c)[3]) {
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    int v = a < PD ? __float2int_rd((pos[a] - pb.lo[a]) * G.inv[a]) : 0;
+    c[a] = min(max(v, 0), G.g[a] - 1);
+  }
+}
+
+// Counting sort of rows [0, n) by cell; four grid-wide steps.  Within a cell the order is whatever the atomics
+// give: the search reduces with the (d2, id) key, so results do not depend on it.
+template <int DYN>
+__device__ __forceinline__ void idx_rebuild(const Params& P, const IdxGeom& G, int n, cg::grid_group& grid, int* sm_scan) {
+  using T = DynTraits<DYN>;
+  const int tid = blockIdx.x * kThreads + threadIdx.x, nth = gridDim.x * kThreads;
+  for (int c = tid; c < G.cells; c += nth) P.idx_cnt[c] = 0;
+  grid.sync();
+  for (int row = tid; row < n; row += nth) {
+    float pos[3] = {0.f, 0.f, 0.f};
+    const float4 a = __ldcg(reinterpret_cast<const float4*>(P.states + (size_t)row * T::DP));
+    pos[0] = a.x; pos[1] = a.y; pos[2] = a.z;
+    int c[3];
+    idx_cell_coords<T::PD>(P.pb, G, pos, c);
+    atomicAdd(&P.idx_cnt[c[0] + G.g[0] * (c[1] + G.g[1] * c[2])], 1);
+  }
+  grid.sync();
+  if (blockIdx.x == 0) {  // exclusive scan of the histogram by one CTA (<= 16384 cells)
+    const int per = (G.cells + kThreads - 1) / kThreads;
+    const int c0 = threadIdx.x * per, c1 = min(G.cells, c0 + per);
+    int sum = 0;
+    for (int c = c0; c < c1; ++c) sum += __ldcg(&P.idx_cnt[c]);
+    sm_scan[threadIdx.x] = sum;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      int run = 0;
+      for (int t = 0; t < kThreads; ++t) { const int v = sm_scan[t]; sm_scan[t] = run; run += v; }
+      P.idx_start[G.cells] = run;
+    }
+    __syncthreads();
+    int run = sm_scan[threadIdx.x];
+    for (int c = c0; c < c1; ++c) {
+      const int v = __ldcg(&P.idx_cnt[c]);
+      P.idx_start[c] = run;
+      P.idx_cnt[c] = run;  // scatter cursor
+      run += v;
+    }
+  }
+  __threadfence();
+  grid.sync();
+  for (int row = tid; row < n; row += nth) {
+    float pos[3] = {0.f, 0.f, 0.f};
+    const float4 a = __ldcg(reinterpret_cast<const float4*>(P.states + (size_t)row * T::DP));
+    pos[0] = a.x; pos[1] = a.y; pos[2] = a.z;
+    int c[3];
+    idx_cell_coords<T::PD>(P.pb, G, pos, c);
+    const int slot = atomicAdd(&P.idx_cnt[c[0] + G.g[0] * (c[1] + G.g[1] * c[2])], 1);
+    P.idx_ids[slot] = row;
+  }
+  __threadfence();
+  grid.sync();
+}
+
+// One warp, one query (all lanes hold the same q): exact NN over the indexed rows.
+template <int DYN, bool UNIT_W>
+__device__ __forceinline__ unsigned long long idx_search(const Params& P, const IdxGeom& G,
+                                                         const float (&q)[DynTraits<DYN>::D]) {
+  using T = DynTraits<DYN>;
+  constexpr int D = T::D, DP = T::DP, PD = T::PD;
+  const int lane = threadIdx.x & 31;
+  int qc[3];
+  {
+    float pos[3] = {q[0], q[1], PD == 3 ? q[2] : 0.0f};
+    idx_cell_coords<PD>(P.pb, G, pos, qc);
+  }
+  int rmax = 0;
+#pragma unroll
+  for (int a = 0; a < PD; ++a) rmax = max(rmax, max(qc[a], G.g[a] - 1 - qc[a]));
+  unsigned long long best = kKeyNone;  // per-lane running minimum, merged after every ring
+  for (int r = 0; r <= rmax; ++r) {
+    // The ring = cells at Chebyshev distance exactly r.  Enumerated per (dy, dz) column: where max(|dy|,|dz|) == r
+    // the whole x-run [qx-r, qx+r] belongs to the ring and, cells being x-fastest, its rows are ONE contiguous
+    // slice of idx_ids; elsewhere only the two cells at dx = -r and dx = +r.  Every lane takes one column per round.
+    const int side = 2 * r + 1;
+    const int cols = PD == 3 ? side * side : side;
+    const int x_lo = max(qc[0] - r, 0), x_hi = min(qc[0] + r, G.g[0] - 1);
+    for (int base = 0; base < cols; base += 32) {
+      const int idx = base + lane;
+      int rbeg[2] = {0, 0}, rcnt[2] = {0, 0};
+      if (idx < cols) {
+        const int dy = idx % side - r, dz = PD == 3 ? idx / side - r : 0;
+        const int cy = qc[1] + dy, cz = qc[2] + dz;
+        if (cy >= 0 && cy < G.g[1] && cz >= 0 && cz < G.g[2]) {
+          const int rowbase = G.g[0] * (cy + G.g[1] * cz);
+          if (max(abs(dy), abs(dz)) == r) {  // face column: the clipped x-run
+            rbeg[0] = __ldcg(&P.idx_start[rowbase + x_lo]);
+            rcnt[0] = __ldcg(&P.idx_start[rowbase + x_hi + 1]) - rbeg[0];
+          } else {  // inner column: the two end cells (r >= 1 here)
+            if (qc[0] - r >= 0) {
+              rbeg[0] = __ldcg(&P.idx_start[rowbase + qc[0] - r]);
+              rcnt[0] = __ldcg(&P.idx_start[rowbase + qc[0] - r + 1]) - rbeg[0];
+            }
+            if (qc[0] + r < G.g[0]) {
+              rbeg[1] = __ldcg(&P.idx_start[rowbase + qc[0] + r]);
+              rcnt[1] = __ldcg(&P.idx_start[rowbase + qc[0] + r + 1]) - rbeg[1];
+            }
+          }
+        }
+      }
+#pragma unroll
+      for (int sl = 0; sl < 2; ++sl) {
+        const int beg = rbeg[sl], cnt = rcnt[sl];
+        int incl = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const int t = __shfl_up_sync(0xffffffffu, incl, o);
+          if (lane >= o) incl += t;
+        }
+        const int total = __shfl_sync(0xffffffffu, incl, 31);
+        for (int j0 = 0; j0 < total; j0 += 32) {
+          const int k = j0 + lane;
+          int lo = 0, hi = 31;  // owner = first lane whose inclusive count exceeds k
+#pragma unroll
+          for (int step = 0; step < 5; ++step) {
+            const int mid = (lo + hi) >> 1;
+            const int v = __shfl_sync(0xffffffffu, incl, mid);
+            if (v > k) hi = mid; else lo = mid + 1;
+          }
+          const int o_incl = __shfl_sync(0xffffffffu, incl, lo), o_cnt = __shfl_sync(0xffffffffu, cnt, lo),
+                    o_beg = __shfl_sync(0xffffffffu, beg, lo);
+          if (k < total) {
+            const int id = __ldcg(&P.idx_ids[o_beg + (k - (o_incl - o_cnt))]);
+            const float4* sp = reinterpret_cast<const float4*>(P.states + (size_t)id * DP);
+            float p[DP];
+#pragma unroll
+            for (int v = 0; v < DP / 4; ++v) {
+              const float4 a = __ldcg(sp + v);
+              p[4 * v] = a.x; p[4 * v + 1] = a.y; p[4 * v + 2] = a.z; p[4 * v + 3] = a.w;
+            }
+            const float d2 = dist2<DYN, UNIT_W>(P.pb, q, p);
+            best = min(best, ((unsigned long long)__float_as_uint(d2) << 32) | (unsigned)id);
+          }
+        }
+      }
+    }
+    unsigned long long m = best;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = min(m, __shfl_xor_sync(0xffffffffu, m, o));
+    best = m;
+    if (m != kKeyNone) {
+      float lb = __int_as_float(0x7f800000);
+#pragma unroll
+      for (int a = 0; a < PD; ++a) lb = fminf(lb, G.lb[a] * (float)(r * r));
+      if (__uint_as_float((unsigned)(m >> 32)) < lb) break;  // nothing outside the visited cube can be nearer
+    }
+  }
+  return best;
+}
+
+// All indexed rows against every query of iteration `it`: warps of the CTAs vb = 0..vbcount-1 take the queries
+// round-robin, each draws its query itself (Alg. 1 l.6).
+template <int DYN, bool UNIT_W>
+__device__ __forceinline__ void idx_phase(const Params& P, const IdxGeom& G, uint32_t r, uint32_t it,
+                                          unsigned long long* key, int vb, int vbcount, bool write_q) {
+  constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
+  if (vb < 0) return;
+  const int lane = threadIdx.x & 31;
+  const int W = vbcount * kWarps, gw = vb * kWarps + (threadIdx.x >> 5);
+  for (int s = gw; s < P.B; s += W) {
+    float q[D];
+    sample_state<D>(P.pb, P.seed, r, it, (uint32_t)s, q);
+    if (lane == 0) {
+#pragma unroll
+      for (int d = 0; d < DP; ++d) {
+        if (write_q && d < D) P.xq[(size_t)s * DP + d] = q[d];
+        if (P.dbg_x_rand) P.dbg_x_rand[(size_t)s * DP + d] = d < D ? q[d] : 0.0f;
+      }
+    }
+    const unsigned long long kv = idx_search<DYN, UNIT_W>(P, G, q);
+    if (lane == 0 && kv != kKeyNone) atomicMin(&key[s], kv);
   }
 }
 
@@ -907,8 +1133,10 @@ __device__ __forceinline__ void extract_path(const Params& P, int goal_node) {
   }
 }
 
-template <int DYN, int OBS, bool STREAM>
+// TIER: 0 tiled NN scan, 1 streaming NN scan (B <= kStreamB), 2 tiled scan + NN cell index (opt-in)
+template <int DYN, int OBS, int TIER>
 __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const __grid_constant__ Params P) {
+  constexpr bool STREAM = TIER == 1, INDEX = TIER == 2;
   using T = DynTraits<DYN>;
   constexpr int OS = (OBS == OBS_CIRCLE) ? 4 : 8;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -959,6 +1187,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
   // insert inside phase X by the propagate CTAs (one grid barrier per iteration) when the children are few
   const bool xins = split && U_prop <= kFuseUnits;
   unsigned pgen = 0;
+  IdxGeom G = idx_geometry<T::PD>(P.pb, kIdxMinRows);  // dead unless INDEX
   unsigned long long* const key0 = P.nn_key;
   unsigned long long* const key1 = P.nn_key + P.B;
 
@@ -980,15 +1209,31 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
     int iters = 0;
     int goal_node = -1;
     int n_scanned = 0;  // NN(it) already covers tree rows [0, n_scanned)
+    int n_sorted = 0;   // rows [0, n_sorted) are in the NN cell index
     for (;;) {
       unsigned long long* const kcur = cur ? key1 : key0;
       unsigned long long* const knext = cur ? key0 : key1;
       // a fresh tree is the root alone: every query's nearest node is node 0, no scan needed
       const bool root_only = (n == 1) && !P.n_nodes_io;
+      // NN index: (re)build once the tree has outgrown it by an eighth
+      bool idx_use = false;
+      if constexpr (INDEX) idx_use = P.nn_index == 2 ? n >= 256 : (n >= kIdxMinRows && (long long)P.B * n >= kIdxMinPairs);
+      if (!idx_use) n_sorted = 0;
+      if (idx_use && n - n_sorted > max(n_sorted >> 3, P.nn_index == 2 ? 64 : 1024)) {
+        G = idx_geometry<T::PD>(P.pb, n);
+        idx_rebuild<DYN>(P, G, n, grid, sm_pref);
+        n_sorted = n;
+      }
       // phase A': rows appended since the look-ahead scan
       if (!root_only && n_scanned < n) {
-        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
-        else nn_phase<DYN, false, STREAM>(P, n_scanned, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
+        int a_beg = n_scanned;
+        if (idx_use && n_sorted > 0 && n_scanned == 0) {  // whole-tree NN (first call on a given tree): index + rest
+          if (P.pb.unit_weights) idx_phase<DYN, true>(P, G, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false);
+          else idx_phase<DYN, false>(P, G, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false);
+          a_beg = n_sorted;
+        }
+        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
+        else nn_phase<DYN, false, STREAM>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
         grid.sync();
       }
       PROBE(P, 4);
@@ -1019,8 +1264,14 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
         }
       }
       if (ahead) {
-        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
-        else nn_phase<DYN, false, STREAM>(P, 0, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
+        int x_beg = 0;
+        if (idx_use && n_sorted > 0) {
+          if (P.pb.unit_weights) idx_phase<DYN, true>(P, G, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true);
+          else idx_phase<DYN, false>(P, G, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true);
+          x_beg = n_sorted;
+        }
+        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
+        else nn_phase<DYN, false, STREAM>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
       }
       if (leader) P.ctrl->goal_key[slot ^ 1] = kKeyNone;
       if (leader && xins && P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) P.ctrl->stop = 1;

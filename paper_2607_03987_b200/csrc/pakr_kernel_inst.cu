@@ -1,6 +1,7 @@
 // pakr_kernel_inst.cu -- instantiates the persistent kernel of pakr_kernel.cuh for every (dynamics, obstacle kind).
-// Compiled twice: -DPAKR_STREAM_TIER=0 (tiled NN scan, the normal case) and =1 (streaming NN tier for B <= 16),
-// so that the two sets build in parallel and the rarely used tier costs the common one no registers.
+// Compiled three times: -DPAKR_STREAM_TIER=0 (tiled NN scan, the normal case), =1 (streaming NN tier for B <= 16)
+// and =2 (tiled scan + opt-in NN cell index), so that the sets build in parallel and the rarely used tiers cost
+// the common one no registers.
 #include "pakr_kernel.cuh"
 
 #ifndef PAKR_STREAM_TIER
@@ -9,11 +10,13 @@
 
 namespace {
 template <int DYN, int OBS> const void* kernel_ptr() {
-  return (const void*)&pakr::pakr_loop_kernel<DYN, OBS, PAKR_STREAM_TIER != 0>;
+  return (const void*)&pakr::pakr_loop_kernel<DYN, OBS, PAKR_STREAM_TIER>;
 }
 }  // namespace
 
-#if PAKR_STREAM_TIER
+#if PAKR_STREAM_TIER == 2
+extern "C" const void* pakr_select_kernel_index(int dyn, int obs) {
+#elif PAKR_STREAM_TIER == 1
 extern "C" const void* pakr_select_kernel_stream(int dyn, int obs) {
 #else
 extern "C" const void* pakr_select_kernel_tiled(int dyn, int obs) {
@@ -26,6 +29,7 @@ extern "C" const void* pakr_select_kernel_tiled(int dyn, int obs) {
     case DYN_DI3 * 2 + OBS_BOX: return kernel_ptr<DYN_DI3, OBS_BOX>();
     case DYN_UNI2 * 2 + OBS_CIRCLE: return kernel_ptr<DYN_UNI2, OBS_CIRCLE>();
     case DYN_UNI2 * 2 + OBS_BOX: return kernel_ptr<DYN_UNI2, OBS_BOX>();
+#if PAKR_STREAM_TIER != 2  // the opt-in index tier is built for the double integrators and the unicycle only
     case DYN_QUAD * 2 + OBS_CIRCLE: return kernel_ptr<DYN_QUAD, OBS_CIRCLE>();
     case DYN_QUAD * 2 + OBS_BOX: return kernel_ptr<DYN_QUAD, OBS_BOX>();
     case DYN_DA * 2 + OBS_CIRCLE: return kernel_ptr<DYN_DA, OBS_CIRCLE>();
@@ -34,6 +38,7 @@ extern "C" const void* pakr_select_kernel_tiled(int dyn, int obs) {
     case DYN_UNI1 * 2 + OBS_BOX: return kernel_ptr<DYN_UNI1, OBS_BOX>();
     case DYN_QUADB * 2 + OBS_CIRCLE: return kernel_ptr<DYN_QUADB, OBS_CIRCLE>();
     case DYN_QUADB * 2 + OBS_BOX: return kernel_ptr<DYN_QUADB, OBS_BOX>();
+#endif
   }
   return nullptr;
 }

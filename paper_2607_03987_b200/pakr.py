@@ -32,7 +32,7 @@ class PakrError(RuntimeError):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """nvcc -gencode arch=compute_100a,code=sm_100a -> paper_2607_03987_b200/libpakr.so (in-tree).
-    Three translation units (host API, tiled-tier kernels, streaming-tier kernels) compile in parallel."""
+    Four translation units (host API; tiled, streaming and index-tier kernels) compile in parallel."""
     srcs = [os.path.join(_CSRC, s) for s in _SOURCES] + [os.path.join(_HERE, "..", "include", "pakr.h")]
     stale = (not os.path.exists(_SO)) or any(os.path.getmtime(s) > os.path.getmtime(_SO) for s in srcs)
     if force or stale:
@@ -41,7 +41,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         flags = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
                  "-Xcompiler", "-fPIC"] + (["-Xptxas=-v"] if verbose else [])
         units = [("pakr_api.cu", [], "api"), ("pakr_kernel_inst.cu", ["-DPAKR_STREAM_TIER=0"], "tiled"),
-                 ("pakr_kernel_inst.cu", ["-DPAKR_STREAM_TIER=1"], "stream")]
+                 ("pakr_kernel_inst.cu", ["-DPAKR_STREAM_TIER=1"], "stream"),
+                 ("pakr_kernel_inst.cu", ["-DPAKR_STREAM_TIER=2"], "index")]
         objs, procs = [], []
         for src, defs, name in units:
             obj = os.path.join(_HERE, f"_{name}{tag}.o")
