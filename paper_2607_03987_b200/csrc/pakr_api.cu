@@ -35,9 +35,21 @@ struct pakr_planner {
 static thread_local std::string g_create_err;
 
 // defined in pakr_kernel_inst.cu (one translation unit per NN tier)
-extern "C" const void* pakr_select_kernel_tiled(int dyn, int obs);
-extern "C" const void* pakr_select_kernel_stream(int dyn, int obs);
-extern "C" const void* pakr_select_kernel_index(int dyn, int obs);
+extern "C" const void* pakr_select_kernel_t0_0(int dyn, int obs);
+extern "C" const void* pakr_select_kernel_t0_1(int dyn, int obs);
+extern "C" const void* pakr_select_kernel_t1_0(int dyn, int obs);
+extern "C" const void* pakr_select_kernel_t1_1(int dyn, int obs);
+extern "C" const void* pakr_select_kernel_t2_0(int dyn, int obs);
+
+static const void* pakr_select_kernel_tiled(int dyn, int obs) {
+  const void* k = pakr_select_kernel_t0_0(dyn, obs);
+  return k ? k : pakr_select_kernel_t0_1(dyn, obs);
+}
+static const void* pakr_select_kernel_stream(int dyn, int obs) {
+  const void* k = pakr_select_kernel_t1_0(dyn, obs);
+  return k ? k : pakr_select_kernel_t1_1(dyn, obs);
+}
+static const void* pakr_select_kernel_index(int dyn, int obs) { return pakr_select_kernel_t2_0(dyn, obs); }
 
 namespace {
 

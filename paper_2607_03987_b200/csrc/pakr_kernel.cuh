@@ -475,7 +475,7 @@ template <int DYN, bool UNIT_W>
 __device__ __forceinline__ unsigned long long idx_search(const Params& P, const IdxGeom& G,
                                                          const float (&q)[DynTraits<DYN>::D]) {
   using T = DynTraits<DYN>;
-  constexpr int D = T::D, DP = T::DP, PD = T::PD;
+  constexpr int DP = T::DP, PD = T::PD;
   const int lane = threadIdx.x & 31;
   int qc[3];
   {

@@ -32,7 +32,7 @@ class PakrError(RuntimeError):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """nvcc -gencode arch=compute_100a,code=sm_100a -> paper_2607_03987_b200/libpakr.so (in-tree).
-    Four translation units (host API; tiled, streaming and index-tier kernels) compile in parallel."""
+    Six translation units (host API; kernels per NN tier and model group) compile in parallel."""
     srcs = [os.path.join(_CSRC, s) for s in _SOURCES] + [os.path.join(_HERE, "..", "include", "pakr.h")]
     stale = (not os.path.exists(_SO)) or any(os.path.getmtime(s) > os.path.getmtime(_SO) for s in srcs)
     if force or stale:
@@ -40,9 +40,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
         tag = f".{os.getpid()}.tmp"
         flags = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
                  "-Xcompiler", "-fPIC"] + (["-Xptxas=-v"] if verbose else [])
-        units = [("pakr_api.cu", [], "api"), ("pakr_kernel_inst.cu", ["-DPAKR_STREAM_TIER=0"], "tiled"),
-                 ("pakr_kernel_inst.cu", ["-DPAKR_STREAM_TIER=1"], "stream"),
-                 ("pakr_kernel_inst.cu", ["-DPAKR_STREAM_TIER=2"], "index")]
+        units = [("pakr_api.cu", [], "api")]
+        for tier, part in ((0, 0), (0, 1), (1, 0), (1, 1), (2, 0)):
+            units.append(("pakr_kernel_inst.cu", [f"-DPAKR_STREAM_TIER={tier}", f"-DPAKR_PART={part}"], f"t{tier}p{part}"))
         objs, procs = [], []
         for src, defs, name in units:
             obj = os.path.join(_HERE, f"_{name}{tag}.o")
