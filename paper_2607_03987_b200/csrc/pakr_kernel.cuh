@@ -470,9 +470,74 @@ __device__ __forceinline__ void idx_rebuild(const Params& P, const IdxGeom& G, i
   grid.sync();
 }
 
-// One warp, one query (all lanes hold the same q): exact NN over the indexed rows.
+// Scores the rows of up to 32 contiguous slices of idx_ids (one slice per lane: beg, cnt) against q.  Four 32-row
+// batches are in flight at a time (ids first, then rows), so the dependent L2 round trips overlap.
 template <int DYN, bool UNIT_W>
-__device__ __forceinline__ unsigned long long idx_search(const Params& P, const IdxGeom& G,
+__device__ __forceinline__ void idx_score_slices(const Params& P, const float (&q)[DynTraits<DYN>::D], int beg, int cnt,
+                                                 unsigned long long& best) {
+  constexpr int DP = DynTraits<DYN>::DP;
+  const int lane = threadIdx.x & 31;
+  int incl = cnt;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int t = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += t;
+  }
+  const int total = __shfl_sync(0xffffffffu, incl, 31);
+  for (int j0 = 0; j0 < total; j0 += 128) {
+    int slot[4];
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+      const int k = j0 + b * 32 + lane;
+      int lo = 0, hi = 31;  // owner = first lane whose inclusive count exceeds k
+#pragma unroll
+      for (int step = 0; step < 5; ++step) {
+        const int mid = (lo + hi) >> 1;
+        const int v = __shfl_sync(0xffffffffu, incl, mid);
+        if (v > k) hi = mid; else lo = mid + 1;
+      }
+      const int o_incl = __shfl_sync(0xffffffffu, incl, lo), o_cnt = __shfl_sync(0xffffffffu, cnt, lo),
+                o_beg = __shfl_sync(0xffffffffu, beg, lo);
+      slot[b] = k < total ? o_beg + (k - (o_incl - o_cnt)) : -1;
+    }
+    int id[4];
+#pragma unroll
+    for (int b = 0; b < 4; ++b) id[b] = slot[b] >= 0 ? __ldcg(&P.idx_ids[slot[b]]) : -1;
+    float4 rowv[4][DP / 4];
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+      const float4* sp = reinterpret_cast<const float4*>(P.states + (size_t)max(id[b], 0) * DP);
+#pragma unroll
+      for (int v = 0; v < DP / 4; ++v) rowv[b][v] = __ldcg(sp + v);
+    }
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+      float p[DP];
+#pragma unroll
+      for (int v = 0; v < DP / 4; ++v) {
+        p[4 * v] = rowv[b][v].x; p[4 * v + 1] = rowv[b][v].y; p[4 * v + 2] = rowv[b][v].z; p[4 * v + 3] = rowv[b][v].w;
+      }
+      const float d2 = dist2<DYN, UNIT_W>(P.pb, q, p);
+      if (id[b] >= 0) best = min(best, ((unsigned long long)__float_as_uint(d2) << 32) | (unsigned)id[b]);
+    }
+  }
+}
+
+__device__ __forceinline__ unsigned long long warp_min_key(unsigned long long m) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = min(m, __shfl_xor_sync(0xffffffffu, m, o));
+  return m;
+}
+
+// One warp, one query (all lanes hold the same q): exact NN over the indexed rows.
+//   stage 1: the query's cell and its neighbours (Chebyshev radius 1); if nothing is there, 64 rows spread evenly
+//            over the cell-ordered id list stand in.  Either way `best` is now the exact distance of a real row:
+//            an upper bound.
+//   stage 2: only rows with |p_a - q_a| <= sqrt(best / w_a) on every position axis can beat it, i.e. rows in the
+//            box of cells within ceil(sqrt(best / w_a) / cell_a) of the query's cell.  That box is visited in one
+//            pass, (y, z) column by column; cells being x-fastest, a column is ONE contiguous slice of idx_ids.
+template <int DYN, bool UNIT_W>
+__device__ __forceinline__ unsigned long long idx_search(const Params& P, const IdxGeom& G, int n_sorted,
                                                          const float (&q)[DynTraits<DYN>::D]) {
   using T = DynTraits<DYN>;
   constexpr int DP = T::DP, PD = T::PD;
@@ -482,94 +547,53 @@ __device__ __forceinline__ unsigned long long idx_search(const Params& P, const 
     float pos[3] = {q[0], q[1], PD == 3 ? q[2] : 0.0f};
     idx_cell_coords<PD>(P.pb, G, pos, qc);
   }
-  int rmax = 0;
-#pragma unroll
-  for (int a = 0; a < PD; ++a) rmax = max(rmax, max(qc[a], G.g[a] - 1 - qc[a]));
-  unsigned long long best = kKeyNone;  // per-lane running minimum, merged after every ring
-  for (int r = 0; r <= rmax; ++r) {
-    // The ring = cells at Chebyshev distance exactly r.  Enumerated per (dy, dz) column: where max(|dy|,|dz|) == r
-    // the whole x-run [qx-r, qx+r] belongs to the ring and, cells being x-fastest, its rows are ONE contiguous
-    // slice of idx_ids; elsewhere only the two cells at dx = -r and dx = +r.  Every lane takes one column per round.
-    const int side = 2 * r + 1;
-    const int cols = PD == 3 ? side * side : side;
-    const int x_lo = max(qc[0] - r, 0), x_hi = min(qc[0] + r, G.g[0] - 1);
+  unsigned long long best = kKeyNone;
+  int rad[3] = {1, 1, PD == 3 ? 1 : 0};  // half-widths of the box of cells, per axis
+  for (int stage = 0; stage < 2; ++stage) {
+    const int y0 = max(qc[1] - rad[1], 0), y1 = min(qc[1] + rad[1], G.g[1] - 1);
+    const int z0 = max(qc[2] - rad[2], 0), z1 = min(qc[2] + rad[2], G.g[2] - 1);
+    const int x0 = max(qc[0] - rad[0], 0), x1 = min(qc[0] + rad[0], G.g[0] - 1);
+    const int ny = y1 - y0 + 1, cols = ny * (z1 - z0 + 1);
     for (int base = 0; base < cols; base += 32) {
       const int idx = base + lane;
-      int rbeg[2] = {0, 0}, rcnt[2] = {0, 0};
+      int beg = 0, cnt = 0;
       if (idx < cols) {
-        const int dy = idx % side - r, dz = PD == 3 ? idx / side - r : 0;
-        const int cy = qc[1] + dy, cz = qc[2] + dz;
-        if (cy >= 0 && cy < G.g[1] && cz >= 0 && cz < G.g[2]) {
-          const int rowbase = G.g[0] * (cy + G.g[1] * cz);
-          if (max(abs(dy), abs(dz)) == r) {  // face column: the clipped x-run
-            rbeg[0] = __ldcg(&P.idx_start[rowbase + x_lo]);
-            rcnt[0] = __ldcg(&P.idx_start[rowbase + x_hi + 1]) - rbeg[0];
-          } else {  // inner column: the two end cells (r >= 1 here)
-            if (qc[0] - r >= 0) {
-              rbeg[0] = __ldcg(&P.idx_start[rowbase + qc[0] - r]);
-              rcnt[0] = __ldcg(&P.idx_start[rowbase + qc[0] - r + 1]) - rbeg[0];
-            }
-            if (qc[0] + r < G.g[0]) {
-              rbeg[1] = __ldcg(&P.idx_start[rowbase + qc[0] + r]);
-              rcnt[1] = __ldcg(&P.idx_start[rowbase + qc[0] + r + 1]) - rbeg[1];
-            }
-          }
-        }
+        const int cy = y0 + idx % ny, cz = z0 + idx / ny;
+        const int rowbase = G.g[0] * (cy + G.g[1] * cz);
+        beg = __ldcg(&P.idx_start[rowbase + x0]);
+        cnt = __ldcg(&P.idx_start[rowbase + x1 + 1]) - beg;
       }
-#pragma unroll
-      for (int sl = 0; sl < 2; ++sl) {
-        const int beg = rbeg[sl], cnt = rcnt[sl];
-        int incl = cnt;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-          const int t = __shfl_up_sync(0xffffffffu, incl, o);
-          if (lane >= o) incl += t;
-        }
-        const int total = __shfl_sync(0xffffffffu, incl, 31);
-        for (int j0 = 0; j0 < total; j0 += 32) {
-          const int k = j0 + lane;
-          int lo = 0, hi = 31;  // owner = first lane whose inclusive count exceeds k
-#pragma unroll
-          for (int step = 0; step < 5; ++step) {
-            const int mid = (lo + hi) >> 1;
-            const int v = __shfl_sync(0xffffffffu, incl, mid);
-            if (v > k) hi = mid; else lo = mid + 1;
-          }
-          const int o_incl = __shfl_sync(0xffffffffu, incl, lo), o_cnt = __shfl_sync(0xffffffffu, cnt, lo),
-                    o_beg = __shfl_sync(0xffffffffu, beg, lo);
-          if (k < total) {
-            const int id = __ldcg(&P.idx_ids[o_beg + (k - (o_incl - o_cnt))]);
-            const float4* sp = reinterpret_cast<const float4*>(P.states + (size_t)id * DP);
-            float p[DP];
-#pragma unroll
-            for (int v = 0; v < DP / 4; ++v) {
-              const float4 a = __ldcg(sp + v);
-              p[4 * v] = a.x; p[4 * v + 1] = a.y; p[4 * v + 2] = a.z; p[4 * v + 3] = a.w;
-            }
-            const float d2 = dist2<DYN, UNIT_W>(P.pb, q, p);
-            best = min(best, ((unsigned long long)__float_as_uint(d2) << 32) | (unsigned)id);
-          }
-        }
-      }
+      idx_score_slices<DYN, UNIT_W>(P, q, beg, cnt, best);
     }
-    unsigned long long m = best;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) m = min(m, __shfl_xor_sync(0xffffffffu, m, o));
-    best = m;
-    if (m != kKeyNone) {
-      float lb = __int_as_float(0x7f800000);
-#pragma unroll
-      for (int a = 0; a < PD; ++a) lb = fminf(lb, G.lb[a] * (float)(r * r));
-      if (__uint_as_float((unsigned)(m >> 32)) < lb) break;  // nothing outside the visited cube can be nearer
+    best = warp_min_key(best);
+    if (stage == 1) break;
+    if (best == kKeyNone) {  // empty neighbourhood: take the bound from 64 rows spread over the whole index
+      const int k0 = (int)(((long long)n_sorted * (2 * lane)) >> 6), k1 = (int)(((long long)n_sorted * (2 * lane + 1)) >> 6);
+      idx_score_slices<DYN, UNIT_W>(P, q, k0, 1, best);
+      idx_score_slices<DYN, UNIT_W>(P, q, k1, 1, best);
+      best = warp_min_key(best);
     }
+    // box that can still hold a nearer row; done if it is inside what stage 1 covered
+    const float ub = __uint_as_float((unsigned)(best >> 32));
+    bool inside = true;
+#pragma unroll
+    for (int a = 0; a < PD; ++a) {
+      // rows beyond r cells differ by more than r * cell_a * 0.9999 on axis a; need w_a * that^2 > ub to exclude them
+      const float cells_f = sqrtf(ub / G.lb[a]);  // G.lb[a] = w_a * (0.9999 cell_a)^2
+      const int r = min((int)cells_f + 1, G.g[a]);
+      inside = inside && (r <= 1);
+      rad[a] = r;
+    }
+    if (inside) break;
   }
   return best;
 }
 
+
 // All indexed rows against every query of iteration `it`: warps of the CTAs vb = 0..vbcount-1 take the queries
 // round-robin, each draws its query itself (Alg. 1 l.6).
 template <int DYN, bool UNIT_W>
-__device__ __forceinline__ void idx_phase(const Params& P, const IdxGeom& G, uint32_t r, uint32_t it,
+__device__ __forceinline__ void idx_phase(const Params& P, const IdxGeom& G, int n_sorted, uint32_t r, uint32_t it,
                                           unsigned long long* key, int vb, int vbcount, bool write_q) {
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
   if (vb < 0) return;
@@ -585,7 +609,7 @@ __device__ __forceinline__ void idx_phase(const Params& P, const IdxGeom& G, uin
         if (P.dbg_x_rand) P.dbg_x_rand[(size_t)s * DP + d] = d < D ? q[d] : 0.0f;
       }
     }
-    const unsigned long long kv = idx_search<DYN, UNIT_W>(P, G, q);
+    const unsigned long long kv = idx_search<DYN, UNIT_W>(P, G, n_sorted, q);
     if (lane == 0 && kv != kKeyNone) atomicMin(&key[s], kv);
   }
 }
@@ -1228,8 +1252,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       if (!root_only && n_scanned < n) {
         int a_beg = n_scanned;
         if (idx_use && n_sorted > 0 && n_scanned == 0) {  // whole-tree NN (first call on a given tree): index + rest
-          if (P.pb.unit_weights) idx_phase<DYN, true>(P, G, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false);
-          else idx_phase<DYN, false>(P, G, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false);
+          if (P.pb.unit_weights) idx_phase<DYN, true>(P, G, n_sorted, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false);
+          else idx_phase<DYN, false>(P, G, n_sorted, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false);
           a_beg = n_sorted;
         }
         if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
@@ -1266,8 +1290,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       if (ahead) {
         int x_beg = 0;
         if (idx_use && n_sorted > 0) {
-          if (P.pb.unit_weights) idx_phase<DYN, true>(P, G, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true);
-          else idx_phase<DYN, false>(P, G, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true);
+          if (P.pb.unit_weights) idx_phase<DYN, true>(P, G, n_sorted, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true);
+          else idx_phase<DYN, false>(P, G, n_sorted, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true);
           x_beg = n_sorted;
         }
         if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
