@@ -31,7 +31,7 @@ METRIC = "expanded nodes/s"
 UNIT = "nodes/s"
 # dram__bytes_read.sum + dram__bytes_write.sum of one pakr_loop_kernel launch on this workload, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists for the current kernel).
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 932096  # profiles/r01_s3_ncu_bench.md
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 1222656  # profiles/r01_s3_ncu_bench.md
 
 
 def algorithmic_ops(problem, nn_pairs: int, children: int) -> dict:
