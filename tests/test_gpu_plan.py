@@ -246,3 +246,28 @@ def test_plan_loop_with_nn_index_equals_scan(pakr, name, iters, monkeypatch):
     assert trees["0"][0] == trees["2"][0] > cfg.B
     for k in ("states", "actions", "parents", "costs"):
         np.testing.assert_array_equal(trees["0"][1][k], trees["2"][1][k])
+
+
+def test_plan_small_b_stream_tier_and_no_obstacles(pakr, orc):
+    """B <= 16 runs the streaming-tier kernel through the whole device loop (look-ahead, in-phase insert, tail
+    rounds): same tree as the chain of single steps; and a problem without obstacles plans fine."""
+    import dataclasses
+    p, _ = wl.config2()
+    pl = pakr.Planner(p)
+    B, K, iters = 8, 16, 10
+    cap = 1 + iters * B * K
+    res = pl.plan(5, B, K, cap, 1, max_iters_per_replan=iters)
+    loop_tree = pl.read_tree(B, K, cap, res["final_tree_nodes"])
+    tree = pl.new_tree(cap)
+    for it in range(res["iterations"]):
+        pl.expand_step(tree, 5, 0, it, B, K)
+    n = int(tree["n_nodes"][0].item())
+    assert n == res["final_tree_nodes"] > 200
+    np.testing.assert_array_equal(tree["states"][:n, :p.state_dim].cpu().numpy(), loop_tree["states"])
+    np.testing.assert_array_equal(tree["parents"][:n].cpu().numpy(), loop_tree["parents"])
+    pl.close()
+    p0 = dataclasses.replace(p, obstacles=p.obstacles[:0])
+    pl = pakr.Planner(p0)
+    res = pl.plan(0, 512, 8, 1 << 18, 2)
+    _check_plan(orc, p0, res)
+    pl.close()
