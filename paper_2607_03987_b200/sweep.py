@@ -8,7 +8,9 @@
 
 One JSON line per row.  Every plan comes back through pakr_plan (C ABI); nothing here computes.
 
-  python -m paper_2607_03987_b200.sweep [--seeds N] [--what configs|c5|all]
+  pathlen  C1, C2 with cost = path length (the paper's Table II metric): AO-x cost-vs-time curve
+
+  python -m paper_2607_03987_b200.sweep [--seeds N] [--what configs|c5|all|pathlen]
 """
 from __future__ import annotations
 
@@ -28,9 +30,12 @@ def med(v):
     return statistics.median(v) if v else None
 
 
-def run_configs(pakr, seeds):
-    for name in ("C1", "C2", "C3", "C4", "N1", "N2", "N3"):
+def run_configs(pakr, seeds, path_length=False):
+    import dataclasses
+    for name in (("C1", "C2") if path_length else ("C1", "C2", "C3", "C4", "N1", "N2", "N3")):
         p, cfg = wl.CONFIGS[name]()
+        if path_length:  # the paper's convergence metric (Table II, Fig. 2: cost = distance travelled)
+            p = dataclasses.replace(p, cost_mode=wl.COST_PATH_LENGTH, heuristic_speed=1.0, name=p.name + "-pathlen")
         pl = pakr.Planner(p)
         pl.plan(1000, cfg.B, cfg.K, cfg.tree_capacity, 1)  # warm-up
         first, nodes1, cost1, costf, ms_all, iters, solved, rate = [], [], [], [], [], [], 0, []
@@ -51,7 +56,7 @@ def run_configs(pakr, seeds):
             rate.append(r["children"] / (r["device_ms"] * 1e-3))
         best100 = [pl.plan(s, cfg.B, cfg.K, cfg.tree_capacity, 4096, time_budget_ms=100.0)["cost"]
                    for s in range(min(seeds, 10))]
-        print(json.dumps({"row": "config", "workload": name, "B": cfg.B, "K": cfg.K, "replans": cfg.n_replans,
+        print(json.dumps({"row": "config", "workload": p.name if path_length else name, "B": cfg.B, "K": cfg.K, "replans": cfg.n_replans,
                           "seeds": seeds, "solved": solved, "first_solution_ms_median": med(first),
                           "first_solution_nodes_median": med(nodes1), "first_cost_median": med(cost1),
                           "final_cost_median": med(costf), "all_replans_ms_median": med(ms_all),
@@ -93,11 +98,13 @@ def main():
     from paper_2607_03987_b200 import pakr
     ap = argparse.ArgumentParser()
     ap.add_argument("--seeds", type=int, default=10)
-    ap.add_argument("--what", default="all", choices=["configs", "c5", "all"])
+    ap.add_argument("--what", default="all", choices=["configs", "c5", "all", "pathlen"])
     args = ap.parse_args()
     pakr.lib()
     if args.what in ("configs", "all"):
         run_configs(pakr, args.seeds)
+    if args.what == "pathlen":
+        run_configs(pakr, args.seeds, path_length=True)
     if args.what in ("c5", "all"):
         run_c5(pakr, args.seeds)
 
