@@ -58,7 +58,7 @@ size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
   size_t states, actions, parents, costs, nn_key, unit_count, scr_state, scr_ctrl, scr_cost, scr_parent,
-      scr_flags, xq, idx_ids, idx_start, idx_cnt, ctrl, path_rev, path_nodes, path_states, path_controls, total;
+      scr_flags, idx_ids, idx_start, idx_cnt, ctrl, path_rev, path_nodes, path_states, path_controls, total;
 };
 
 Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap) {
@@ -72,7 +72,6 @@ Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap) {
   L.costs = take((size_t)cap * 4);
   L.nn_key = take((size_t)B * 16);  // two iterations in flight
   L.unit_count = take(std::max<size_t>(U, kFuseUnits + 8) * 4);
-  L.xq = take((size_t)B * pl->DP * 4);
   L.idx_ids = take((size_t)cap * 4);
   L.idx_start = take((size_t)(kIdxMaxCells + 1) * 4);
   L.idx_cnt = take((size_t)kIdxMaxCells * 4);
@@ -404,7 +403,6 @@ void fill_common(const pakr_planner* pl, Params& P, const Layout& L, char* ws, i
   P.pb = pl->pb;
   P.nn_key = reinterpret_cast<unsigned long long*>(ws + L.nn_key);
   P.unit_count = reinterpret_cast<unsigned*>(ws + L.unit_count);
-  P.xq = reinterpret_cast<float*>(ws + L.xq);
   P.idx_ids = reinterpret_cast<int*>(ws + L.idx_ids);
   P.idx_start = reinterpret_cast<int*>(ws + L.idx_start);
   P.idx_cnt = reinterpret_cast<int*>(ws + L.idx_cnt);

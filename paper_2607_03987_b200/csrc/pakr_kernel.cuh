@@ -72,7 +72,6 @@ struct Params {
   float* states; float* actions; int* parents; float* costs;
   // per-iteration work buffers
   unsigned long long* nn_key;  // [2][B] (d2 bits << 32) | node, combined with atomicMin; two iterations in flight
-  float* xq;                   // [B][Dp] sampled states of the iteration whose NN is being prepared
   // NN cell index (exact spatial pruning): tree rows [0, n_sorted) bucketed by position cell
   int nn_index;                // 0: scan tiers only; 1: index when B*n is large; 2: index whenever n >= 256 (tests)
   int* idx_ids;                // [cap] row ids ordered by cell
@@ -285,7 +284,7 @@ constexpr int kStreamB = 16;
 
 template <int DYN, bool UNIT_W>
 __device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, uint32_t r, uint32_t it,
-                                       unsigned long long* key, int vb, int vbcount, bool write_q, float* sm_q,
+                                       unsigned long long* key, int vb, int vbcount, float* sm_q,
                                           float* sm_tile, uint64_t* sm_bar, uint32_t& par0, uint32_t& par1) {
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
   constexpr int QS = (D <= 8) ? 8 : 4;  // queries held in registers per pass over the rows
@@ -299,7 +298,6 @@ __device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, u
     if (vb == 0) {
 #pragma unroll
       for (int d = 0; d < DP; ++d) {
-        if (write_q && d < D) P.xq[(size_t)t * DP + d] = x[d];
         if (P.dbg_x_rand && nbeg == 0) P.dbg_x_rand[(size_t)t * DP + d] = d < D ? x[d] : 0.0f;
       }
     }
@@ -594,7 +592,7 @@ __device__ __forceinline__ unsigned long long idx_search(const Params& P, const 
 // round-robin, each draws its query itself (Alg. 1 l.6).
 template <int DYN, bool UNIT_W>
 __device__ __forceinline__ void idx_phase(const Params& P, const IdxGeom& G, int n_sorted, uint32_t r, uint32_t it,
-                                          unsigned long long* key, int vb, int vbcount, bool write_q) {
+                                          unsigned long long* key, int vb, int vbcount) {
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
   if (vb < 0) return;
   const int lane = threadIdx.x & 31;
@@ -605,7 +603,6 @@ __device__ __forceinline__ void idx_phase(const Params& P, const IdxGeom& G, int
     if (lane == 0) {
 #pragma unroll
       for (int d = 0; d < DP; ++d) {
-        if (write_q && d < D) P.xq[(size_t)s * DP + d] = q[d];
         if (P.dbg_x_rand) P.dbg_x_rand[(size_t)s * DP + d] = d < D ? q[d] : 0.0f;
       }
     }
@@ -622,7 +619,7 @@ __device__ __forceinline__ void idx_phase(const Params& P, const IdxGeom& G, int
 // atomicMin, so any split of the rows over warps / phases gives the same result.
 template <int DYN, bool UNIT_W, bool STREAM>
 __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, uint32_t r, uint32_t it,
-                                         unsigned long long* key, int vb, int vbcount, bool write_q, float* sm_tile,
+                                         unsigned long long* key, int vb, int vbcount, float* sm_tile,
                                          uint64_t* sm_bar, float* sm_q, unsigned long long* sm_keys, uint32_t& par0,
                                          uint32_t& par1 PROBE_ARG) {
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
@@ -632,7 +629,7 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
   const int n = nend - nbeg;
   if (vb < 0 || n <= 0) return;
   if constexpr (STREAM) {  // few queries (B <= kStreamB, chosen by the host): HBM-bound streaming tier
-    nn_stream<DYN, UNIT_W>(P, nbeg, nend, r, it, key, vb, vbcount, write_q, sm_q, sm_tile, sm_bar, par0, par1);
+    nn_stream<DYN, UNIT_W>(P, nbeg, nend, r, it, key, vb, vbcount, sm_q, sm_tile, sm_bar, par0, par1);
     return;
   }
   const int W = vbcount * kWarps;
@@ -686,13 +683,6 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
         for (int d = 0; d < DP; ++d) {
           if (sa < P.B) P.dbg_x_rand[(size_t)sa * DP + d] = d < D ? qa[d] : 0.0f;
           if (sb < P.B) P.dbg_x_rand[(size_t)sb * DP + d] = d < D ? qb[d] : 0.0f;
-        }
-      }
-      if (write_q && has && rr == 0) {  // keep the sampled states for the tail scan of the insert phase
-#pragma unroll
-        for (int d = 0; d < D; ++d) {
-          if (sa < P.B) P.xq[(size_t)sa * DP + d] = qa[d];
-          if (sb < P.B) P.xq[(size_t)sb * DP + d] = qb[d];
         }
       }
     }
@@ -952,33 +942,6 @@ __device__ __forceinline__ void tail_item(const Params& P, int n, int g, int rg,
   __syncwarp();  // every lane is done with the tile before it is refilled
 }
 
-// All CTAs take part (insert phase of its own): items from the far end of the warp list, queries from P.xq.
-template <int DYN, bool UNIT_W>
-__device__ __forceinline__ void tail_scan_items(const Params& P, int n, int U, const int* sm_upre,
-                                                unsigned long long* key_next, float* sm_tile, uint64_t* sm_bar,
-                                                uint32_t& par0) {
-  using T = DynTraits<DYN>;
-  constexpr int D = T::D, DP = T::DP, QG = 32 * kQ;
-  constexpr int RU = TileCfg<DYN>::TILE / 32;
-  const int lane = threadIdx.x & 31;
-  const int W = gridDim.x * kWarps;
-  const int gw = blockIdx.x * kWarps + (threadIdx.x >> 5);
-  const int G = (P.B + QG - 1) / QG;
-  const int NR = (U + RU - 1) / RU;
-  for (int i = W - 1 - gw; i < G * NR; i += W) {  // from the far end: the copy units start at warp 0
-    const int g = i / NR, rg = i - g * NR;
-    if (sm_upre[min(U, rg * RU + RU)] == sm_upre[rg * RU]) continue;
-    f32x2 q2[kQ / 2][D];
-#pragma unroll
-    for (int h = 0; h < kQ / 2; ++h) {
-      const int sa = min(g * QG + (2 * h) * 32 + lane, P.B - 1), sb = min(g * QG + (2 * h + 1) * 32 + lane, P.B - 1);
-#pragma unroll
-      for (int d = 0; d < D; ++d) q2[h][d] = pack2(__ldcg(&P.xq[(size_t)sa * DP + d]), __ldcg(&P.xq[(size_t)sb * DP + d]));
-    }
-    tail_item<DYN, UNIT_W>(P, n, g, rg, U, sm_upre, key_next, q2, sm_tile, sm_bar, par0);
-  }
-}
-
 // Only the propagate CTAs take part (insert inside phase X): CTA-sized chunks of items that share one query
 // group; the CTA draws that group's 128 sampled states of iteration it_next itself (Alg. 1 l.6) into sm_qt.
 template <int DYN, bool UNIT_W>
@@ -1019,7 +982,7 @@ __device__ __forceinline__ void tail_scan_rounds(const Params& P, int n, int U, 
 }
 
 // The first `npcta` CTAs take part (all of them when the insert is a phase of its own; only the propagate CTAs
-// when it runs inside phase X).  tail_mode: 0 none, 1 items with queries from P.xq, 2 CTA rounds (r, it_next).
+// when it runs inside phase X).  tail_mode: 0 none, 2 CTA rounds (r, it_next) when the insert runs inside phase X.
 template <int DYN>
 __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, unsigned long long* key_done,
                                             int tail_mode, unsigned long long* key_next, uint32_t r, uint32_t it_next,
@@ -1113,18 +1076,10 @@ __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, u
   PROBE(P, 11);
   // fused tail scan of the next iteration's NN (every survivor inserted)
   {
-    constexpr int RU = TileCfg<DYN>::TILE / 32;
-    const int G = (P.B + 32 * kQ - 1) / (32 * kQ);
-    if (tail_mode == 1) fused = small && total <= room && G * ((U + RU - 1) / RU) <= W;
-    else fused = tail_mode == 2 && small && total <= room && total <= kXTailRows;
+    fused = tail_mode == 2 && small && total <= room && total <= kXTailRows;
     if (fused && total > 0) {
-      if (tail_mode == 1) {
-        if (P.pb.unit_weights) tail_scan_items<DYN, true>(P, n, U, sm_upre, key_next, sm_tile, sm_bar, par0);
-        else tail_scan_items<DYN, false>(P, n, U, sm_upre, key_next, sm_tile, sm_bar, par0);
-      } else {
-        if (P.pb.unit_weights) tail_scan_rounds<DYN, true>(P, n, U, sm_upre, key_next, r, it_next, (int)blockIdx.x, npcta, sm_qt, sm_tile, sm_bar, par0);
-        else tail_scan_rounds<DYN, false>(P, n, U, sm_upre, key_next, r, it_next, (int)blockIdx.x, npcta, sm_qt, sm_tile, sm_bar, par0);
-      }
+      if (P.pb.unit_weights) tail_scan_rounds<DYN, true>(P, n, U, sm_upre, key_next, r, it_next, (int)blockIdx.x, npcta, sm_qt, sm_tile, sm_bar, par0);
+      else tail_scan_rounds<DYN, false>(P, n, U, sm_upre, key_next, r, it_next, (int)blockIdx.x, npcta, sm_qt, sm_tile, sm_bar, par0);
     }
   }
   // the NN keys this iteration consumed are free again: reset them for iteration i+2
@@ -1252,12 +1207,12 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       if (!root_only && n_scanned < n) {
         int a_beg = n_scanned;
         if (idx_use && n_sorted > 0 && n_scanned == 0) {  // whole-tree NN (first call on a given tree): index + rest
-          if (P.pb.unit_weights) idx_phase<DYN, true>(P, G, n_sorted, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false);
-          else idx_phase<DYN, false>(P, G, n_sorted, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false);
+          if (P.pb.unit_weights) idx_phase<DYN, true>(P, G, n_sorted, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB);
+          else idx_phase<DYN, false>(P, G, n_sorted, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB);
           a_beg = n_sorted;
         }
-        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
-        else nn_phase<DYN, false, STREAM>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, false, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
+        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
+        else nn_phase<DYN, false, STREAM>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
         grid.sync();
       }
       PROBE(P, 4);
@@ -1290,12 +1245,12 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       if (ahead) {
         int x_beg = 0;
         if (idx_use && n_sorted > 0) {
-          if (P.pb.unit_weights) idx_phase<DYN, true>(P, G, n_sorted, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true);
-          else idx_phase<DYN, false>(P, G, n_sorted, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true);
+          if (P.pb.unit_weights) idx_phase<DYN, true>(P, G, n_sorted, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt);
+          else idx_phase<DYN, false>(P, G, n_sorted, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt);
           x_beg = n_sorted;
         }
-        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
-        else nn_phase<DYN, false, STREAM>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, true, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
+        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
+        else nn_phase<DYN, false, STREAM>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
       }
       if (leader) P.ctrl->goal_key[slot ^ 1] = kKeyNone;
       if (leader && xins && P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) P.ctrl->stop = 1;
@@ -1309,7 +1264,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
         fused = ahead && total <= P.cap - n && total <= kXTailRows;
       } else {
         // phase C: insert as a phase of its own (every CTA takes part)
-        total = insert_phase<DYN>(P, n, slot, kcur, ahead ? 1 : 0, knext, (uint32_t)r, (uint32_t)(it + 1), NB, sm_pref,
+        total = insert_phase<DYN>(P, n, slot, kcur, 0, knext, (uint32_t)r, (uint32_t)(it + 1), NB, sm_pref,
                                   reinterpret_cast<int*>(sm_q), reinterpret_cast<float*>(sm_keys), my_tile, my_bar, par0,
                                   fused PROBE_PASS);
         if (leader && P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) P.ctrl->stop = 1;
