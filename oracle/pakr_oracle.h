@@ -11,10 +11,14 @@
  * restated there (they are ABI constants documented in DESIGN.md, not shared code).
  *
  * Parity pins (tests/test_oracle_*.py): Philox against the Random123 known-answer vectors and
- * cuRAND's host generator; NN against hand cases; integrators against closed forms; collision
- * against analytic cases; insert order against a Python copy_if; tree invariants; plan
- * re-propagation.  Whole-method trajectory of the randomised planner: "parity unpinned" by the
- * paper (it prints no worked example) -- see DESIGN.md.
+ * cuRAND's host generator; NN against hand cases; integrators against closed forms (incl. the
+ * sign of w x Iw: axisymmetric precession); PATH_LENGTH edge cost against chord-sum closed forms;
+ * collision and state-box closedness against analytic rim cases through orc_propagate's flags;
+ * prune strictness at c_new + h == c_best and the GOAL flag of a pruned child; insert order
+ * against a Python copy_if; tree invariants; how orc_plan ends a replan (goal, tree full,
+ * default iteration cap) and the initial cost bound against hand counts; plan re-propagation.
+ * Every pin was mutation-checked.  Whole-method trajectory of the randomised
+ * planner: "parity unpinned" by the paper (it prints no worked example) -- see DESIGN.md.
  */
 #ifndef PAKR_ORACLE_H
 #define PAKR_ORACLE_H
