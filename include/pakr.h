@@ -52,6 +52,11 @@ enum { PAKR_OBS_CIRCLE2D = 0, PAKR_OBS_AABB = 1, PAKR_OBS_ZCYLINDER = 2 };
 enum { PAKR_COST_DURATION = 0, PAKR_COST_PATH_LENGTH = 1 };
 enum { PAKR_DIM_REAL = 0, PAKR_DIM_ANGLE = 1 };
 enum { PAKR_NO_SOLUTION = 0, PAKR_SOLVED = 1 }; /* "no solution" is not an error */
+/* nearest-neighbour tier (pakr_plan_opts.nn_mode, pakr_step_args.nn_mode) */
+enum { PAKR_NN_AUTO = 0,  /* the library picks: brute-force scan tiers while the tree is small, the spatial index
+                             once B*n is large enough to pay for building it */
+       PAKR_NN_SCAN = 1,  /* brute-force scan tiers only (tiled; streaming when B <= 16) */
+       PAKR_NN_INDEX = 2  /* spatial index on every tree of >= 256 nodes (tests) */ };
 
 /* child flag bits written by pakr_expand_step (Alg. 1 l.10-14) */
 enum {
@@ -93,7 +98,8 @@ typedef struct {
   float heuristic_speed;  /* h(x) = max(0, |p - goal| - r) / heuristic_speed; +INF => h = 0 */
 } pakr_problem;
 
-/* Validates and copies the problem; selects the compiled kernel variant; binds `cuda_device`.
+/* Validates and copies the problem; selects the compiled kernel variant; binds `cuda_device` (the caller's current
+ * device is restored before returning, here and in every other call).
  * INVALID_ARG: NULL, dims that do not match the dynamics, lo > hi, NaN, weight < 0, a sampled
  * real dim (weight > 0) with an infinite bound, dt <= 0, steps < 1.  UNSUPPORTED: unknown ids,
  * dim_kind not the dynamics' own.  CUDA: device not usable (no sm_100 device). */
@@ -127,9 +133,12 @@ typedef struct {
   double initial_cost_bound;    /* c_best before the first replan (Alg. 1 l.1); <= 0 or +INF = none.  A finite bound
                                    (e.g. the best cost another replica found) prunes from the start;
                                    the result reports only what THIS call found (NO_SOLUTION if nothing cheaper) */
+  int32_t nn_mode;              /* PAKR_NN_*: which nearest-neighbour tier answers Alg. 1 l.7.  Every tier returns the
+                                   same (d^2, lowest index) result bit for bit (PAPER.md:142 tiers have no semantics) */
 } pakr_plan_opts;
 
 #define PAKR_MAX_REPLAN_STATS 64
+#define PAKR_MAX_PATH_NODES 8192 /* longest path (nodes) the device-side extraction holds */
 typedef struct {
   int64_t iterations;      /* inner-loop trips over all replans */
   int64_t children;        /* = iterations * B * K propagated and checked ("expanded nodes") */
@@ -137,6 +146,9 @@ typedef struct {
   int64_t nn_pairs;        /* sum over iterations of B * n: (query, node) distance evaluations */
   int32_t replans_run, replans_solved;
   int32_t termination;     /* 0 all replans run, 1 time budget */
+  int32_t replan_stats_truncated; /* 1 if replans_run > PAKR_MAX_REPLAN_STATS: the per-replan arrays hold the first 64 */
+  int32_t path_truncated;  /* 1 if a solved replan's path had more than PAKR_MAX_PATH_NODES nodes: it tightened c_best
+                              but could not be extracted; pakr_result then holds the last path that fit and ITS cost */
   double first_solution_ms;/* device time from kernel start to the end of the first solved replan; -1 if none */
   double device_ms;        /* device time of the whole loop (%globaltimer) */
   double phase_ms[3];      /* CTA 0's time in: separate NN (tail) scan phases / the propagate phase (with the next
@@ -147,8 +159,6 @@ typedef struct {
   int32_t replan_nodes[PAKR_MAX_REPLAN_STATS];/* tree size at its end */
   int32_t replan_iters[PAKR_MAX_REPLAN_STATS];
   double replan_end_ms[PAKR_MAX_REPLAN_STATS];/* device time at its end */
-  int64_t probe_cycles[32]; /* diagnostic: all 0 unless the library was built with -DPAKR_PROBE (SM cycles of
-                               thread 0 of CTA 0 between probe points, summed over the launch) */
 } pakr_stats;
 
 typedef struct {
@@ -158,7 +168,7 @@ typedef struct {
   float* path_controls;   /* [path_capacity-1][control_dim]; control i is held for steps_per_edge*dt */
   int32_t path_capacity;  /* in  */
   int32_t path_len;       /* out: nodes on the best path (L+1), 0 if none */
-  double cost;            /* out: c_best, +INF if none */
+  double cost;            /* out: cost of the returned path = c_best (see stats.path_truncated), +INF if none */
   int32_t outcome;        /* out: PAKR_SOLVED / PAKR_NO_SOLUTION */
   int32_t final_tree_nodes; /* out: size of the tree left in the workspace (the last replan's) */
   pakr_stats stats;       /* out */
@@ -167,7 +177,8 @@ typedef struct {
 /* Alg. 1 whole: AO-x loop around the batched expansion, one persistent cooperative kernel, no
  * host round trip per iteration.  Returns the best path found (sigma*, Alg. 1 l.18).
  * BUFFER_TOO_SMALL: path longer than path_capacity (path_len = needed length, cost/outcome
- * still set).  WORKSPACE_TOO_SMALL / INVALID_ARG: nothing launched. */
+ * still set), or no solved replan's path fit PAKR_MAX_PATH_NODES.  WORKSPACE_TOO_SMALL / INVALID_ARG: nothing
+ * launched.  The caller's current CUDA device is left as it was. */
 pakr_status pakr_plan(pakr_planner* planner, const pakr_plan_opts* opts, void* d_workspace,
                       size_t workspace_bytes, void* cuda_stream, pakr_result* out);
 
@@ -176,6 +187,7 @@ typedef struct {
   uint64_t seed; uint32_t replan, iteration;
   int32_t B, K; int64_t tree_capacity;
   float c_best;                 /* +INF = no bound yet */
+  int32_t nn_mode;              /* PAKR_NN_* */
   /* tree, DEVICE, layouts as in the header comment; in/out */
   float* states; float* actions; int32_t* parents; float* costs;
   int32_t* n_nodes;             /* DEVICE scalar, in/out */

@@ -3,6 +3,7 @@
 // kernel of pakr_kernel.cuh and copies the small result block back.  No compute happens here.
 #include <algorithm>
 #include <cmath>
+#include <cstddef>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -23,7 +24,7 @@ struct pakr_planner {
   uint32_t* d_grid_cells = nullptr;
   uint16_t* d_grid_list = nullptr;
   int num_sms = 0, blocks_per_sm = 0;
-  int nn_index = 0;  // NN cell index usable: finite position box, positive position weights
+  bool index_ok = false;  // NN spatial index usable: finite position box, positive position weights, kernel built
   size_t smem_bytes = 0;
   const void* kernel = nullptr;         // tiled NN scan
   const void* kernel_stream = nullptr;  // streaming NN tier (B <= kStreamB)
@@ -181,6 +182,20 @@ pakr_status fail(pakr_planner* pl, pakr_status st, const std::string& msg) {
   return st;
 }
 
+// Binds the planner's device for the duration of one ABI call and puts the caller's device back afterwards
+// (a host process with several GPUs, e.g. PyTorch, must not find its current device changed).
+struct DeviceGuard {
+  int prev = -1;
+  cudaError_t err;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+    err = cudaSetDevice(dev);
+  }
+  ~DeviceGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+
 #define CUDA_TRY(pl, expr)                                                                       \
   do {                                                                                           \
     cudaError_t e_ = (expr);                                                                     \
@@ -263,6 +278,10 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
     return fail(nullptr, PAKR_ERR_INVALID_ARG, "goal_radius >= 0 and heuristic_speed > 0 required");
   if (p->goal_angle_dim != -1 && p->goal_angle_dim != angle)
     return fail(nullptr, PAKR_ERR_INVALID_ARG, "goal_angle_dim must be -1 or the dynamics' angle dim");
+  if (p->goal_angle_dim != -1 && (!std::isfinite(p->goal_angle) || !std::isfinite(p->goal_angle_tol) || p->goal_angle_tol < 0.0f))
+    return fail(nullptr, PAKR_ERR_INVALID_ARG, "goal_angle must be finite and goal_angle_tol finite and >= 0");
+  for (int a = 0; a < p->pos_dim; ++a)
+    if (!std::isfinite(p->goal_center[a])) return fail(nullptr, PAKR_ERR_INVALID_ARG, "goal_center must be finite");
 
   auto* pl = new pakr_planner();
   pl->device = cuda_device;
@@ -293,11 +312,7 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
     bool ok = true;
     for (int a = 0; a < PD; ++a)
       ok = ok && std::isfinite(pb.lo[a]) && std::isfinite(pb.hi[a]) && pb.hi[a] > pb.lo[a] && pb.w[a] > 0.0f;
-    // The NN cell index is exact and tested but, as measured this round, slower than the scan tiers (DESIGN.md
-    // "NN index tier"): it stays opt-in.  Read at create: PAKR_NN_INDEX=1 index when B*n is large, =2 index on any
-    // tree of >= 256 rows (tests); unset or 0: scan tiers only.
-    const char* env = std::getenv("PAKR_NN_INDEX");
-    pl->nn_index = !ok ? 0 : (env && env[0] == '1') ? 1 : (env && env[0] == '2') ? 2 : 0;
+    pl->index_ok = ok;  // the tier itself is chosen per call (pakr_plan_opts.nn_mode / pakr_step_args.nn_mode)
   }
   pb.n_obs = p->n_obstacles;
 
@@ -317,7 +332,8 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
     }
   }
   auto bail = [&](pakr_status st, const std::string& m) { g_create_err = m; pakr_destroy(pl); return st; };
-  cudaError_t e = cudaSetDevice(cuda_device);
+  DeviceGuard guard(cuda_device);
+  cudaError_t e = guard.err;
   if (e != cudaSuccess) return bail(PAKR_ERR_CUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(e));
   cudaDeviceProp prop;
   e = cudaGetDeviceProperties(&prop, cuda_device);
@@ -349,7 +365,7 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
   pl->kernel = pakr_select_kernel_tiled(dyn, obs);
   pl->kernel_stream = pakr_select_kernel_stream(dyn, obs);
   pl->kernel_index = pakr_select_kernel_index(dyn, obs);
-  if (!pl->kernel_index) { pl->kernel_index = pl->kernel; pl->nn_index = 0; }  // no index tier for this model
+  if (!pl->kernel_index) { pl->kernel_index = pl->kernel; pl->index_ok = false; }  // no index tier for this model
   pl->smem_bytes = smem_for(pl);
   e = cudaFuncSetAttribute(pl->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes);
   if (e == cudaSuccess)
@@ -373,6 +389,7 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
 
 extern "C" void pakr_destroy(pakr_planner* pl) {
   if (!pl) return;
+  DeviceGuard guard(pl->device);
   if (pl->d_obstacles) cudaFree(pl->d_obstacles);
   if (pl->d_grid_cells) cudaFree(pl->d_grid_cells);
   if (pl->d_grid_list) cudaFree(pl->d_grid_list);
@@ -406,7 +423,6 @@ void fill_common(const pakr_planner* pl, Params& P, const Layout& L, char* ws, i
   P.idx_ids = reinterpret_cast<int*>(ws + L.idx_ids);
   P.idx_start = reinterpret_cast<int*>(ws + L.idx_start);
   P.idx_cnt = reinterpret_cast<int*>(ws + L.idx_cnt);
-  P.nn_index = pl->nn_index;
   P.scr_state = reinterpret_cast<float*>(ws + L.scr_state);
   P.scr_ctrl = reinterpret_cast<float*>(ws + L.scr_ctrl);
   P.scr_cost = reinterpret_cast<float*>(ws + L.scr_cost);
@@ -428,10 +444,11 @@ void fill_stats(const Ctrl* hc, int64_t BK, pakr_stats* out) {
   s.inserted = hc->inserted;
   s.nn_pairs = hc->nn_pairs;
   for (int i = 0; i < 3; ++i) s.phase_ms[i] = (double)hc->phase_ns[i] * 1e-6;
-  for (int i = 0; i < 32; ++i) s.probe_cycles[i] = (int64_t)hc->probe[i];
   s.replans_run = hc->replans_run;
   s.replans_solved = hc->replans_solved;
   s.termination = hc->termination;
+  s.replan_stats_truncated = hc->replans_run > kStatsMax ? 1 : 0;
+  s.path_truncated = hc->path_overflow > 0 ? 1 : 0;
   s.first_solution_ms = hc->replans_solved > 0 ? (double)(hc->t_first_ns - hc->t_start_ns) * 1e-6 : -1.0;
   s.device_ms = (double)(hc->t_end_ns - hc->t_start_ns) * 1e-6;
   for (int i = 0; i < kStatsMax && i < hc->replans_run; ++i) {
@@ -443,14 +460,22 @@ void fill_stats(const Ctrl* hc, int64_t BK, pakr_stats* out) {
 }
 
 // memset of the control words + one cooperative launch; everything on `stream`
+// nn_mode (PAKR_NN_*) -> Params::nn_index
+bool set_nn_mode(pakr_planner* pl, Params& P, int nn_mode) {
+  if (nn_mode != PAKR_NN_AUTO && nn_mode != PAKR_NN_SCAN && nn_mode != PAKR_NN_INDEX) return false;
+  constexpr int kAutoIndex = 0;  // what PAKR_NN_AUTO means for the index: 0 never, 1 when B*n is large
+  P.nn_index = !pl->index_ok ? 0 : nn_mode == PAKR_NN_INDEX ? 2 : nn_mode == PAKR_NN_AUTO ? kAutoIndex : 0;
+  return true;
+}
+
 pakr_status launch(pakr_planner* pl, Params& P, cudaStream_t stream) {
-  CUDA_TRY(pl, cudaSetDevice(pl->device));
   CUDA_TRY(pl, cudaMemsetAsync(P.nn_key, 0xFF, (size_t)P.B * 16, stream));
   CUDA_TRY(pl, cudaMemsetAsync(P.ctrl, 0, sizeof(Ctrl), stream));
-  CUDA_TRY(pl, cudaMemsetAsync(P.ctrl, 0xFF, 16, stream));  // goal_key[2] = none
+  static_assert(offsetof(Ctrl, goal_key) == 0, "goal keys first");
+  CUDA_TRY(pl, cudaMemsetAsync(P.ctrl, 0xFF, sizeof(unsigned long long) * kSlots, stream));  // goal_key[] = none
   void* args[] = {&P};
   const dim3 grid(pl->num_sms * std::min(pl->blocks_per_sm, kCtasPerSm)), block(kThreads);
-  const void* kernel = P.B <= kStreamB ? pl->kernel_stream : (pl->nn_index ? pl->kernel_index : pl->kernel);
+  const void* kernel = P.B <= kStreamB ? pl->kernel_stream : (P.nn_index ? pl->kernel_index : pl->kernel);
   CUDA_TRY(pl, cudaLaunchCooperativeKernel(kernel, grid, block, args, pl->smem_bytes, stream));
   return PAKR_OK;
 }
@@ -472,6 +497,10 @@ extern "C" pakr_status pakr_plan(pakr_planner* pl, const pakr_plan_opts* o, void
   char* ws = static_cast<char*>(d_ws);
   Params P;
   fill_common(pl, P, L, ws, o->B, o->K, o->tree_capacity);
+  if (!set_nn_mode(pl, P, o->nn_mode)) return fail(pl, PAKR_ERR_INVALID_ARG, "nn_mode must be a PAKR_NN_* value");
+  pl->err.clear();
+  DeviceGuard guard(pl->device);
+  CUDA_TRY(pl, guard.err);
   P.states = reinterpret_cast<float*>(ws + L.states);
   P.actions = reinterpret_cast<float*>(ws + L.actions);
   P.parents = reinterpret_cast<int*>(ws + L.parents);
@@ -489,7 +518,6 @@ extern "C" pakr_status pakr_plan(pakr_planner* pl, const pakr_plan_opts* o, void
   float root[kMaxD + kMaxM + 2] = {0};
   for (int d = 0; d < pl->D; ++d) root[d] = pl->pb.start[d];
   const int minus1 = -1;
-  CUDA_TRY(pl, cudaSetDevice(pl->device));
   CUDA_TRY(pl, cudaMemcpyAsync(P.states, root, (size_t)pl->DP * 4, cudaMemcpyHostToDevice, stream));
   CUDA_TRY(pl, cudaMemsetAsync(P.actions, 0, 16, stream));
   CUDA_TRY(pl, cudaMemcpyAsync(P.parents, &minus1, 4, cudaMemcpyHostToDevice, stream));
@@ -506,8 +534,18 @@ extern "C" pakr_status pakr_plan(pakr_planner* pl, const pakr_plan_opts* o, void
   out->cost = hc->solved ? (double)hc->best_cost : (double)INFINITY;
   out->path_len = hc->solved ? hc->path_len : 0;
   if (!hc->solved) return PAKR_OK;
-  if (hc->path_len > kPathMax || hc->path_len > out->path_capacity) {
-    if (out->path_nodes || out->path_states || out->path_controls || hc->path_len > kPathMax)
+  if (hc->path_overflow > 0) {
+    // a path of more than PAKR_MAX_PATH_NODES nodes tightened c_best but was not extracted: hand back the last
+    // path that fit, with ITS cost; if none did, say how long the buffers would have had to be
+    if (hc->path_len == 0) {
+      out->path_len = hc->path_overflow;
+      return fail(pl, PAKR_ERR_BUFFER_TOO_SMALL, "best path exceeds PAKR_MAX_PATH_NODES nodes");
+    }
+    out->cost = (double)hc->path_cost;
+    pl->err = "a cheaper path exceeded PAKR_MAX_PATH_NODES nodes; the last path that fit is returned (stats.path_truncated)";
+  }
+  if (hc->path_len > out->path_capacity) {
+    if (out->path_nodes || out->path_states || out->path_controls)
       return fail(pl, PAKR_ERR_BUFFER_TOO_SMALL, "path longer than path_capacity");
     return PAKR_OK;
   }
@@ -542,6 +580,9 @@ extern "C" pakr_status pakr_expand_step(pakr_planner* pl, const pakr_step_args* 
   if (ws_bytes < L.total) return fail(pl, PAKR_ERR_WORKSPACE_TOO_SMALL, "workspace smaller than pakr_workspace_bytes()");
   Params P;
   fill_common(pl, P, L, static_cast<char*>(d_ws), a->B, a->K, a->tree_capacity);
+  if (!set_nn_mode(pl, P, a->nn_mode)) return fail(pl, PAKR_ERR_INVALID_ARG, "nn_mode must be a PAKR_NN_* value");
+  DeviceGuard guard(pl->device);
+  CUDA_TRY(pl, guard.err);
   P.states = a->states; P.actions = a->actions; P.parents = a->parents; P.costs = a->costs;
   P.seed = a->seed;
   P.n_replans = 1; P.max_iters = 1; P.budget_ns = 0;
@@ -564,7 +605,8 @@ extern "C" pakr_status pakr_read_stats(pakr_planner* pl, int32_t B, int32_t K, i
   if (ws_bytes < L.total) return fail(pl, PAKR_ERR_WORKSPACE_TOO_SMALL, "workspace smaller than pakr_workspace_bytes()");
   cudaStream_t stream = reinterpret_cast<cudaStream_t>(cuda_stream);
   Ctrl* hc = static_cast<Ctrl*>(pl->h_pinned);
-  CUDA_TRY(pl, cudaSetDevice(pl->device));
+  DeviceGuard guard(pl->device);
+  CUDA_TRY(pl, guard.err);
   CUDA_TRY(pl, cudaMemcpyAsync(hc, static_cast<char*>(d_ws) + L.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, stream));
   CUDA_TRY(pl, cudaStreamSynchronize(stream));
   fill_stats(hc, (int64_t)B * K, out);

@@ -25,22 +25,10 @@
 namespace pakr {
 namespace cg = cooperative_groups;
 
-#ifndef PAKR_THREADS
-#define PAKR_THREADS 256
-#endif
-constexpr int kThreads = PAKR_THREADS;  // 256 x 2 CTAs per SM measured 1.4x faster in the NN scan than 512 x 1
-#ifndef PAKR_CTAS
-#define PAKR_CTAS (1024 / (2 * PAKR_THREADS))
-#endif
-constexpr int kCtasPerSm = PAKR_CTAS;
-#ifndef PAKR_TILE_DIV
-#define PAKR_TILE_DIV 1
-#endif
+constexpr int kThreads = 256;    // 256 x 2 CTAs per SM measured 1.4x faster in the NN scan than 512 x 1
+constexpr int kCtasPerSm = 2;
 constexpr int kWarps = kThreads / 32;
-#ifndef PAKR_KQ
-#define PAKR_KQ 4
-#endif
-constexpr int kQ = PAKR_KQ;      // queries per lane in the NN scan
+constexpr int kQ = 4;            // queries per lane in the NN scan
 constexpr int kIdxMaxCells = 16384;  // cells of the NN index (resolution chosen from the tree size at every rebuild)
 constexpr int kIdxMinRows = 4096;    // smaller trees are scanned
 constexpr long long kIdxMinPairs = 120000000ll;  // ... and so are iterations whose scan (B*n pairs) takes < ~60 us
@@ -48,16 +36,23 @@ constexpr int kPathMax = 8192;   // longest path the device buffers hold
 constexpr int kStatsMax = 64;
 constexpr unsigned long long kKeyNone = ~0ull;
 
+// Per-iteration words the whole grid reads right after the barrier that ends iteration i live in slot i % 3:
+// slot (i+1) % 3 is re-armed during iteration i, and its last readers (iteration i-2's) all passed the barrier of
+// iteration i-1 before that, so no read can ever see a later iteration's value.
+constexpr int kSlots = 3;
+
 struct Ctrl {  // device control block (in the workspace)
-  unsigned long long goal_key[2];
+  unsigned long long goal_key[kSlots];  // min (cost bits, node) over the goal children inserted in the iteration
   unsigned long long t_start_ns, t_first_ns, t_end_ns;
   long long iterations, inserted, nn_pairs;
   unsigned long long phase_ns[3];  // leader's time in NN / propagate / insert incl. the grid sync after each
-  unsigned long long probe[32];    // -DPAKR_PROBE: SM cycles of thread 0 of CTA 0 between probe points
-  int n_nodes, stop;
-  unsigned pbar;      // arrival counter of the barrier among the propagate CTAs (insert inside phase X)
-  int iter_total[2];  // survivors of the iteration, published by CTA 0 when the insert ran inside phase X
+  int n_nodes;
+  int stop[kSlots];        // 1: the time budget ran out during the iteration (written by the leader every iteration)
+  unsigned pbar;           // arrival counter of the barrier among the propagate CTAs (insert inside phase X)
+  int iter_total[kSlots];  // survivors of the iteration, published by CTA 0 when the insert ran inside phase X
   int path_len, solved;
+  int path_overflow;       // a solved replan's path was longer than kPathMax and was not extracted
+  float path_cost;         // cost of the path held in the path buffers
   float best_cost;
   int replans_run, replans_solved, termination;
   float replan_cost[kStatsMax];
@@ -103,35 +98,6 @@ __device__ __forceinline__ unsigned long long globaltimer_ns() {
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
   return t;
 }
-#ifdef PAKR_PROBE
-#ifndef PAKR_PROBE_BLOCK
-#define PAKR_PROBE_BLOCK 0
-#endif
-#define PROBE(P, i)                                                                   \
-  do {                                                                                \
-    if (blockIdx.x == PAKR_PROBE_BLOCK && threadIdx.x == 0) {                         \
-      const long long t_ = clock64();                                                 \
-      atomicAdd(&(P).ctrl->probe[(i) + g_pb], (unsigned long long)(t_ - g_probe_prev)); \
-      g_probe_prev = t_;                                                              \
-    }                                                                                 \
-  } while (0)
-#define PROBE_DEP(v)                                                                                 \
-  do {                                                                                               \
-    float d_;                                                                                        \
-    asm volatile("shfl.sync.idx.b32 %0, %1, 0, 31, 0xffffffff;" : "=f"(d_) : "f"((float)(v)));       \
-  } while (0)
-#define PROBE_DECL long long g_probe_prev = clock64(); const int g_pb = 0
-#define PROBE_ARG , long long& g_probe_prev, int g_pb
-#define PROBE_PASS , g_probe_prev, 0
-#define PROBE_PASSX , g_probe_prev, 16
-#else
-#define PROBE(P, i) do {} while (0)
-#define PROBE_DEP(v) do {} while (0)
-#define PROBE_DECL
-#define PROBE_ARG
-#define PROBE_PASS
-#define PROBE_PASSX
-#endif
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return (uint32_t)__cvta_generic_to_shared(p);
 }
@@ -177,7 +143,7 @@ __device__ __forceinline__ void cta_group_barrier(unsigned* ctr, unsigned target
 
 template <int DYN> struct TileCfg {  // nodes per TMA tile: <= 4 KB per buffer
   static constexpr int DP = DynTraits<DYN>::DP;
-  static constexpr int TILE = ((DP == 4) ? 256 : (DP == 8) ? 128 : 64) / PAKR_TILE_DIV;
+  static constexpr int TILE = ((DP == 4) ? 256 : (DP == 8) ? 128 : 64) ; 
   static constexpr int TILE_FLOATS = TILE * DP;
 };
 
@@ -621,7 +587,7 @@ template <int DYN, bool UNIT_W, bool STREAM>
 __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, uint32_t r, uint32_t it,
                                          unsigned long long* key, int vb, int vbcount, float* sm_tile,
                                          uint64_t* sm_bar, float* sm_q, unsigned long long* sm_keys, uint32_t& par0,
-                                         uint32_t& par1 PROBE_ARG) {
+                                         uint32_t& par1) {
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
   constexpr int TILE = TileCfg<DYN>::TILE, TF = TileCfg<DYN>::TILE_FLOATS;
   constexpr int QG = 32 * kQ;  // queries per group
@@ -692,7 +658,6 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
       bidx[j] = 0x7fffffff;
     }
     if (has) {
-    PROBE(P, 0);
     const int ntiles = (end - beg + TILE - 1) / TILE;
     const float* src = P.states + (size_t)beg * DP;
     if (lane == 0) {
@@ -710,14 +675,11 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
       }
       if (t & 1) { mbar_wait(&sm_bar[1], par1); par1 ^= 1; }
       else { mbar_wait(&sm_bar[0], par0); par0 ^= 1; }
-      if (t == 0) PROBE(P, 1);
       const float4* tp = reinterpret_cast<const float4*>(sm_tile + (t & 1) * TF);
       const int base = beg + t * TILE;
       scan_rows<DYN, UNIT_W>(P.pb, tp, cnt, base, q2, best, bidx);
       __syncwarp();  // every lane is done with this buffer before lane 0 refills it
     }
-    PROBE_DEP(best[0]);
-    PROBE(P, 2);
     }  // has
     if (shared_q) {
       // CTA-level merge: one global atomicMin per (CTA, query) instead of one per (warp, query)
@@ -747,7 +709,6 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
         }
       }
     }
-    PROBE(P, 3);
   }
 }
 
@@ -759,7 +720,7 @@ template <int DYN, int OBS>
 __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t it, float c_best,
                                            const unsigned long long* key, bool root_only, int pw, int W,
                                            const float* sm_obs, const uint32_t* sm_cells,
-                                           const uint16_t* sm_list PROBE_ARG) {
+                                           const uint16_t* sm_list) {
   using T = DynTraits<DYN>;
   constexpr int D = T::D, M = T::M, DP = T::DP, PD = T::PD;
   const DevProblem& pb = P.pb;
@@ -795,10 +756,6 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
     }
     const float parent_cost = __ldcg(&P.costs[parent]);
     sample_control<M>(pb, P.seed, r, it, (uint32_t)s, (uint32_t)k, ctl);
-    PROBE_DEP(ctl[0]);
-    PROBE(P, 5);
-    PROBE_DEP(x[0] + parent_cost);
-    PROBE(P, 6);
     // margins: bm >= 0 / om > 0 mean still valid.  Inactive lanes start dead.
     float bm = active ? __int_as_float(0x7f800000) : -1.0f;
     float om = bm;
@@ -838,8 +795,6 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
       }
       if (P.early_exit && __all_sync(0xffffffffu, !(bm >= 0.0f) || !(om > 0.0f))) break;  // whole warp dead
     }
-    PROBE_DEP(bm + om);
-    PROBE(P, 7);
     bool finite = true;
 #pragma unroll
     for (int d = 0; d < D; ++d) finite = finite & (fabsf(x[d]) <= 3.4e38f);
@@ -879,7 +834,6 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
       __stcg(&P.scr_parent[slot], parent);
       __stcg(&P.scr_flags[slot], flags | (lane << 8));
     }
-    PROBE(P, 8);
     if (active && P.dbg_child_flags) {
       P.dbg_child_flags[c] = flags;
       if (P.dbg_child_cost) P.dbg_child_cost[c] = c_new;
@@ -899,10 +853,7 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
 // from the scratch rows (their node ids n + rank are known from the prefix), so that no separate scan phase and
 // barrier is needed before the next propagate.  `fused` tells the caller (grid-uniform).
 constexpr int kFuseUnits = 2048;  // per-unit prefix kept in shared memory up to this many warp units
-#ifndef PAKR_XTAIL
-#define PAKR_XTAIL 1024
-#endif
-constexpr int kXTailRows = PAKR_XTAIL;  // larger batches of new rows get a scan phase of their own on all CTAs
+constexpr int kXTailRows = 1024;  // larger batches of new rows get a scan phase of their own on all CTAs
 
 // One tail-scan item: the survivors of warp units [rg*RU, rg*RU+RU) (gathered by TMA into one tile buffer, in
 // node order) against the 128 queries of group g held in q2.
@@ -987,7 +938,7 @@ template <int DYN>
 __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, unsigned long long* key_done,
                                             int tail_mode, unsigned long long* key_next, uint32_t r, uint32_t it_next,
                                             int npcta, int* sm_pref, int* sm_upre, float* sm_qt, float* sm_tile,
-                                            uint64_t* sm_bar, uint32_t& par0, bool& fused PROBE_ARG) {
+                                            uint64_t* sm_bar, uint32_t& par0, bool& fused) {
   using T = DynTraits<DYN>;
   constexpr int DP = T::DP;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -1039,7 +990,6 @@ __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, u
     if (threadIdx.x == kThreads - 1) sm_upre[kFuseUnits] = run;  // == total
   }
   __syncthreads();
-  PROBE(P, 10);
   const int room = P.cap - n;
   for (int u = gw; u < U; u += W) {
     int off, cnt;
@@ -1073,7 +1023,6 @@ __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, u
       if (P.dbg_child_flags) P.dbg_child_flags[u * cpw + (fl >> 8)] |= 32;
     }
   }
-  PROBE(P, 11);
   // fused tail scan of the next iteration's NN (every survivor inserted)
   {
     fused = tail_mode == 2 && small && total <= room && total <= kXTailRows;
@@ -1088,17 +1037,22 @@ __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, u
 }
 
 // Alg. 1 l.16 ExtractPath: warp 0 of block 0 walks parents, then copies in parallel.
+// A path of more than kPathMax nodes is not extracted: the buffers keep the last path that fit (with its cost).
 template <int DYN>
-__device__ __forceinline__ void extract_path(const Params& P, int goal_node) {
+__device__ __forceinline__ void extract_path(const Params& P, int goal_node, float cost) {
   using T = DynTraits<DYN>;
   const int lane = threadIdx.x & 31;
   int len = 0;
   if (lane == 0) {
-    for (int i = goal_node; i >= 0; i = __ldcg(&P.parents[i])) {
-      if (len < kPathMax) P.path_nodes_rev[kPathMax - 1 - len] = i;
-      ++len;
+    for (int i = goal_node; i >= 0; i = __ldcg(&P.parents[i])) ++len;
+    if (len <= kPathMax) {
+      int at = kPathMax;
+      for (int i = goal_node; i >= 0; i = __ldcg(&P.parents[i])) P.path_nodes_rev[--at] = i;
+      P.ctrl->path_len = len;
+      P.ctrl->path_cost = cost;
+    } else {
+      P.ctrl->path_overflow = len;
     }
-    P.ctrl->path_len = len;
   }
   len = __shfl_sync(0xffffffffu, len, 0);
   if (len > kPathMax) return;
@@ -1170,7 +1124,6 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
   unsigned long long* const key0 = P.nn_key;
   unsigned long long* const key1 = P.nn_key + P.B;
 
-  PROBE_DECL;
   unsigned long long t_start = 0;
   if (leader) { t_start = globaltimer_ns(); P.ctrl->t_start_ns = t_start; }
 
@@ -1211,18 +1164,17 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
           else idx_phase<DYN, false>(P, G, n_sorted, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB);
           a_beg = n_sorted;
         }
-        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
-        else nn_phase<DYN, false, STREAM>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASS);
+        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1);
+        else nn_phase<DYN, false, STREAM>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1);
         grid.sync();
       }
-      PROBE(P, 4);
       if (leader) { const unsigned long long t = globaltimer_ns(); ph0 += t - tp; tp = t; }
       // phase X: propagate(it) and, meanwhile, NN(it+1) over the frozen snapshot [0, n)
       const bool ahead = (iters + 1 < P.max_iters);
-      prop_phase<DYN, OBS>(P, (uint32_t)r, (uint32_t)it, c_best, kcur, root_only, x_pw, x_pcnt, sm_obs, sm_cells, sm_list PROBE_PASS);
-      // goal-key slots alternate over the whole launch (not per replan): the other slot was last
-      // read before the previous grid sync and is next written after the following one
-      const int slot = (int)(iterations & 1);
+      prop_phase<DYN, OBS>(P, (uint32_t)r, (uint32_t)it, c_best, kcur, root_only, x_pw, x_pcnt, sm_obs, sm_cells, sm_list);
+      // slots rotate over the whole launch (not per replan); see kSlots
+      const int slot = (int)(iterations % kSlots);
+      const int slot_next = (slot + 1) % kSlots;
       bool fused = false;
       int total = 0;
       if (xins) {
@@ -1233,10 +1185,9 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
           ++pgen;
           cta_group_barrier(&P.ctrl->pbar, (unsigned)NPB * pgen);
           fence_proxy_async();
-          PROBE(P, 10);
           total = insert_phase<DYN>(P, n, slot, kcur, ahead ? 2 : 0, knext, (uint32_t)r, (uint32_t)(it + 1), NPB, sm_pref,
                                     reinterpret_cast<int*>(sm_q), reinterpret_cast<float*>(sm_keys), my_tile, my_bar, par0,
-                                    fused PROBE_PASS);
+                                    fused);
           if (leader) P.ctrl->iter_total[slot] = total;
           __threadfence();
           fence_proxy_async();  // tree rows written with st.global are read next by TMA (async proxy)
@@ -1249,15 +1200,16 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
           else idx_phase<DYN, false>(P, G, n_sorted, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt);
           x_beg = n_sorted;
         }
-        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
-        else nn_phase<DYN, false, STREAM>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1 PROBE_PASSX);
+        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1);
+        else nn_phase<DYN, false, STREAM>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1);
       }
-      if (leader) P.ctrl->goal_key[slot ^ 1] = kKeyNone;
-      if (leader && xins && P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) P.ctrl->stop = 1;
+      if (leader) {
+        P.ctrl->goal_key[slot_next] = kKeyNone;
+        if (xins) P.ctrl->stop[slot] = (P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) ? 1 : 0;
+      }
       fence_proxy_async();  // scratch rows written with st.global may be read by TMA in the insert phase
       grid.sync();
       fence_proxy_async();
-      PROBE(P, 9);
       if (leader) { const unsigned long long t = globaltimer_ns(); ph1 += t - tp; tp = t; }
       if (xins) {
         total = __ldcg(&P.ctrl->iter_total[slot]);
@@ -1266,13 +1218,11 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
         // phase C: insert as a phase of its own (every CTA takes part)
         total = insert_phase<DYN>(P, n, slot, kcur, 0, knext, (uint32_t)r, (uint32_t)(it + 1), NB, sm_pref,
                                   reinterpret_cast<int*>(sm_q), reinterpret_cast<float*>(sm_keys), my_tile, my_bar, par0,
-                                  fused PROBE_PASS);
-        if (leader && P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) P.ctrl->stop = 1;
+                                  fused);
+        if (leader) P.ctrl->stop[slot] = (P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) ? 1 : 0;
         __threadfence();
         fence_proxy_async();  // tree rows written with st.global are read next by TMA (async proxy)
-        PROBE(P, 12);
         grid.sync();
-        PROBE(P, 13);
         if (leader) { const unsigned long long t = globaltimer_ns(); ph2 += t - tp; tp = t; }
         fence_proxy_async();
       }
@@ -1285,7 +1235,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       ++iters;
       cur ^= 1;
       const unsigned long long gk = __ldcg(&P.ctrl->goal_key[slot]);
-      stop = __ldcg(&P.ctrl->stop) != 0;
+      stop = __ldcg(&P.ctrl->stop[slot]) != 0;
       ++it;
       if (gk != kKeyNone) {  // Alg. 1 l.14-17
         c_best = __uint_as_float((unsigned)(gk >> 32));
@@ -1298,7 +1248,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
     if (goal_node >= 0) {
       ++replans_solved;
       solved_any = 1;
-      if (blockIdx.x == 0 && warp == 0) extract_path<DYN>(P, goal_node);
+      if (blockIdx.x == 0 && warp == 0) extract_path<DYN>(P, goal_node, c_best);
     }
     if (leader) {
       const unsigned long long now = globaltimer_ns();

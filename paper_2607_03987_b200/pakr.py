@@ -19,7 +19,9 @@ _CSRC = os.path.join(_HERE, "csrc")
 _SOURCES = ["pakr_api.cu", "pakr_kernel_inst.cu", "pakr_kernel.cuh", "pakr_device.cuh"]
 
 F_VALID, F_INBOUNDS, F_COLLFREE, F_NOTPRUNED, F_GOAL, F_INSERTED = 1, 2, 4, 8, 16, 32
+NN_AUTO, NN_SCAN, NN_INDEX = 0, 1, 2
 MAX_REPLAN_STATS = 64
+MAX_PATH_NODES = 8192
 _STATUS = {0: "PAKR_OK", 1: "PAKR_ERR_INVALID_ARG", 2: "PAKR_ERR_UNSUPPORTED", 3: "PAKR_ERR_WORKSPACE_TOO_SMALL",
            4: "PAKR_ERR_BUFFER_TOO_SMALL", 5: "PAKR_ERR_CUDA"}
 
@@ -34,12 +36,20 @@ def build(force: bool = False, verbose: bool = False) -> str:
     """nvcc -gencode arch=compute_100a,code=sm_100a -> paper_2607_03987_b200/libpakr.so (in-tree).
     Six translation units (host API; kernels per NN tier and model group) compile in parallel."""
     srcs = [os.path.join(_CSRC, s) for s in _SOURCES] + [os.path.join(_HERE, "..", "include", "pakr.h")]
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    flags = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+             "-Xcompiler", "-fPIC"] + (["-Xptxas=-v"] if verbose else [])
+    # the stamp records the flags the library was built with: a build with other flags is never silently reused
+    stamp = " ".join(f for f in flags if f != "-Xptxas=-v")
+    stamp_file = _SO + ".stamp"
     stale = (not os.path.exists(_SO)) or any(os.path.getmtime(s) > os.path.getmtime(_SO) for s in srcs)
+    if not stale:
+        try:
+            stale = open(stamp_file).read() != stamp
+        except OSError:
+            stale = True
     if force or stale:
-        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         tag = f".{os.getpid()}.tmp"
-        flags = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-                 "-Xcompiler", "-fPIC"] + (["-Xptxas=-v"] if verbose else [])
         units = [("pakr_api.cu", [], "api")]
         for tier, part in ((0, 0), (0, 1), (1, 0), (1, 1), (2, 0)):
             units.append(("pakr_kernel_inst.cu", [f"-DPAKR_STREAM_TIER={tier}", f"-DPAKR_PART={part}"], f"t{tier}p{part}"))
@@ -55,6 +65,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
             tmp = _SO + tag
             subprocess.check_call([nvcc, "-shared", "-o", tmp] + objs)
             os.replace(tmp, _SO)
+            with open(stamp_file, "w") as f:
+                f.write(stamp)
         finally:
             for pr in procs:
                 if pr.poll() is None:
@@ -93,16 +105,16 @@ class _TreeLayout(C.Structure):
 class _PlanOpts(C.Structure):
     _fields_ = [("seed", C.c_uint64), ("B", C.c_int32), ("K", C.c_int32), ("tree_capacity", C.c_int64),
                 ("n_replans", C.c_int32), ("time_budget_ms", C.c_double), ("max_iters_per_replan", C.c_int64),
-                ("initial_cost_bound", C.c_double)]
+                ("initial_cost_bound", C.c_double), ("nn_mode", C.c_int32)]
 
 
 class _Stats(C.Structure):
     _fields_ = [("iterations", C.c_int64), ("children", C.c_int64), ("inserted", C.c_int64), ("nn_pairs", C.c_int64),
                 ("replans_run", C.c_int32), ("replans_solved", C.c_int32), ("termination", C.c_int32),
+                ("replan_stats_truncated", C.c_int32), ("path_truncated", C.c_int32),
                 ("first_solution_ms", C.c_double), ("device_ms", C.c_double), ("phase_ms", C.c_double * 3),
                 ("replan_cost", C.c_float * MAX_REPLAN_STATS), ("replan_nodes", C.c_int32 * MAX_REPLAN_STATS),
-                ("replan_iters", C.c_int32 * MAX_REPLAN_STATS), ("replan_end_ms", C.c_double * MAX_REPLAN_STATS),
-                ("probe_cycles", C.c_int64 * 32)]
+                ("replan_iters", C.c_int32 * MAX_REPLAN_STATS), ("replan_end_ms", C.c_double * MAX_REPLAN_STATS)]
 
 
 class _Result(C.Structure):
@@ -114,6 +126,7 @@ class _Result(C.Structure):
 class _StepArgs(C.Structure):
     _fields_ = [("seed", C.c_uint64), ("replan", C.c_uint32), ("iteration", C.c_uint32),
                 ("B", C.c_int32), ("K", C.c_int32), ("tree_capacity", C.c_int64), ("c_best", C.c_float),
+                ("nn_mode", C.c_int32),
                 ("states", C.c_void_p), ("actions", C.c_void_p), ("parents", C.c_void_p), ("costs", C.c_void_p),
                 ("n_nodes", C.c_void_p),
                 ("x_rand", C.c_void_p), ("nn_idx", C.c_void_p), ("nn_d2", C.c_void_p), ("child_state", C.c_void_p),
@@ -193,6 +206,7 @@ class Planner:
             raise PakrError(st, (lib().pakr_last_error(None) or b"").decode())
         self._h = h
         self._ws = None
+        self._last_ws = None  # the workspace the last plan() ran in (read_tree's default)
 
     def close(self):
         if getattr(self, "_h", None):
@@ -228,12 +242,14 @@ class Planner:
     # ---- pakr_plan ----
     def plan(self, seed: int, B: int, K: int, tree_capacity: int, n_replans: int, time_budget_ms: float = 0.0,
              max_iters_per_replan: int = 0, path_capacity: int = 8192, workspace=None,
-             initial_cost_bound: float = 0.0) -> dict:
+             initial_cost_bound: float = 0.0, nn_mode: int = NN_AUTO) -> dict:
         ws = workspace if workspace is not None else self.workspace(B, K, tree_capacity)
+        self._last_ws = ws
         nodes = np.zeros(path_capacity, np.int32)
         states = np.zeros((path_capacity, self.D), np.float32)
         ctrls = np.zeros((max(path_capacity - 1, 1), self.m), np.float32)
-        opts = _PlanOpts(seed, B, K, tree_capacity, n_replans, time_budget_ms, max_iters_per_replan, initial_cost_bound)
+        opts = _PlanOpts(seed, B, K, tree_capacity, n_replans, time_budget_ms, max_iters_per_replan, initial_cost_bound,
+                         nn_mode)
         res = _Result(_ptr(nodes, _ip), _ptr(states), _ptr(ctrls), path_capacity, 0, 0.0, 0, 0, _Stats())
         st = lib().pakr_plan(self._h, C.byref(opts), C.c_void_p(ws.data_ptr()), ws.numel(), C.c_void_p(self._stream()),
                              C.byref(res))
@@ -249,14 +265,17 @@ class Planner:
                     device_ms=float(s.device_ms), phase_ms=[float(v) for v in s.phase_ms], replan_cost=np.array(s.replan_cost[:R], np.float32),
                     replan_nodes=np.array(s.replan_nodes[:R], np.int64), replan_iters=np.array(s.replan_iters[:R], np.int64),
                     replan_end_ms=np.array(s.replan_end_ms[:R], np.float64),
-                    probe_cycles=[int(v) for v in s.probe_cycles])
+                    replan_stats_truncated=int(s.replan_stats_truncated), path_truncated=int(s.path_truncated))
 
-    def read_tree(self, B: int, K: int, tree_capacity: int, n: int) -> dict:
-        """Copies the first n nodes of the tree pakr_plan left in the workspace to numpy."""
+    def read_tree(self, B: int, K: int, tree_capacity: int, n: int, workspace=None) -> dict:
+        """Copies the first n nodes of the tree pakr_plan left in `workspace` (default: the workspace of the last
+        plan() call) to numpy."""
         torch = self._torch
         lay = _TreeLayout()
         self._check(lib().pakr_get_tree_layout(self._h, B, K, tree_capacity, C.byref(lay)))
-        ws = self._ws
+        ws = workspace if workspace is not None else self._last_ws
+        if ws is None:
+            raise PakrError(1, "read_tree: no workspace given and plan() has not run")
 
         def view(off, count, dtype):
             nbytes = count * 4
@@ -274,8 +293,7 @@ class Planner:
         self._check(lib().pakr_read_stats(self._h, B, K, tree_capacity, C.c_void_p(ws.data_ptr()), ws.numel(),
                                           C.c_void_p(self._stream()), C.byref(st)))
         return dict(iterations=int(st.iterations), children=int(st.children), inserted=int(st.inserted),
-                    nn_pairs=int(st.nn_pairs), device_ms=float(st.device_ms), phase_ms=[float(v) for v in st.phase_ms],
-                    probe_cycles=[int(v) for v in st.probe_cycles])
+                    nn_pairs=int(st.nn_pairs), device_ms=float(st.device_ms), phase_ms=[float(v) for v in st.phase_ms])
 
     # ---- pakr_expand_step ----
     def new_tree(self, capacity: int, host: Optional[dict] = None) -> dict:
@@ -299,7 +317,8 @@ class Planner:
         return t
 
     def expand_step(self, tree: dict, seed: int, replan: int, iteration: int, B: int, K: int,
-                    c_best: float = float("inf"), debug: bool = True, workspace=None) -> Optional[dict]:
+                    c_best: float = float("inf"), debug: bool = True, workspace=None,
+                    nn_mode: int = NN_AUTO) -> Optional[dict]:
         torch = self._torch
         dev = f"cuda:{self.device}"
         cap = tree["capacity"]
@@ -320,7 +339,7 @@ class Planner:
                        goal_node=torch.zeros(1, dtype=torch.int32, device=dev),
                        new_c_best=torch.zeros(1, dtype=torch.float32, device=dev))
         g = (lambda k: ptr(dbg[k])) if debug else (lambda k: null)
-        a = _StepArgs(seed, replan, iteration, B, K, cap, c_best, ptr(tree["states"]), ptr(tree["actions"]),
+        a = _StepArgs(seed, replan, iteration, B, K, cap, c_best, nn_mode, ptr(tree["states"]), ptr(tree["actions"]),
                       ptr(tree["parents"]), ptr(tree["costs"]), ptr(tree["n_nodes"]), g("x_rand"), g("nn_idx"),
                       g("nn_d2"), g("child_state"), g("child_ctrl"), g("child_cost"), g("child_flags"),
                       g("n_inserted"), g("goal_node"), g("new_c_best"))

@@ -12,13 +12,13 @@ STATE_ABS_TOL = 1e-4
 MARGIN_TOL = 1e-5
 
 
-def run_both(pl, orc, op, problem, host_tree, seed, r, it, B, K, c_best=float("inf"), cap=None):
+def run_both(pl, orc, op, problem, host_tree, seed, r, it, B, K, c_best=float("inf"), cap=None, nn_mode=0):
     """-> (gpu_out, gpu_tree_after (numpy), oracle_out, oracle_tree)"""
     import torch
     n0 = len(host_tree["parents"])
     cap = cap or n0 + B * K
     tree = pl.new_tree(cap, host_tree)
-    out = pl.expand_step(tree, seed, r, it, B, K, c_best=c_best)
+    out = pl.expand_step(tree, seed, r, it, B, K, c_best=c_best, nn_mode=nn_mode)
     n1 = int(tree["n_nodes"][0].item())
     D, m = problem.state_dim, problem.control_dim
     after = dict(states=tree["states"][:n1, :D].cpu().numpy(), actions=tree["actions"][:n1, :m].cpu().numpy(),

@@ -38,10 +38,13 @@ def test_sass_is_sm100a_with_tma():
     assert "UBLKCP" in out
 
 
-def test_struct_field_order_matches_header():
-    from paper_2607_03987_b200 import pakr
+_STRUCTS = {"pakr_problem": "_Problem", "pakr_tree_layout": "_TreeLayout", "pakr_plan_opts": "_PlanOpts",
+            "pakr_stats": "_Stats", "pakr_result": "_Result", "pakr_step_args": "_StepArgs"}
+
+
+def _header_fields(name):
     text = open(os.path.join(ROOT, "include", "pakr.h")).read()
-    body = re.search(r"typedef struct \{(.*?)\} pakr_problem;", text, flags=re.S).group(1)
+    body = re.search(r"typedef struct \{((?:(?!typedef struct).)*?)\} %s;" % name, text, flags=re.S).group(1)
     body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
     fields = []
     for decl in body.split(";"):
@@ -49,8 +52,36 @@ def test_struct_field_order_matches_header():
         if not decl:
             continue
         names = re.sub(r"^(const\s+)?\w+\s*\*?", "", decl, count=1)
-        fields += [n.strip(" *") for n in names.split(",")]
-    assert fields == [f[0] for f in pakr._Problem._fields_]
+        fields += [re.sub(r"\[.*", "", n).strip(" *") for n in names.split(",")]
+    return fields
+
+
+@pytest.mark.parametrize("cname", sorted(_STRUCTS))
+def test_struct_field_order_matches_header(cname):
+    from paper_2607_03987_b200 import pakr
+    assert _header_fields(cname) == [f[0] for f in getattr(pakr, _STRUCTS[cname])._fields_]
+
+
+def test_struct_layout_matches_a_c_compiler(tmp_path):
+    """include/pakr.h is plain C; sizeof / offsetof of every struct as gcc lays it out equal the ctypes mirrors."""
+    import subprocess
+    from paper_2607_03987_b200 import pakr
+    lines = ['#include <stdio.h>', '#include <stddef.h>', '#include "pakr.h"', 'int main(void) {']
+    for cname in sorted(_STRUCTS):
+        lines.append('printf("%s %%zu\\n", sizeof(%s));' % (cname, cname))
+        for f in _header_fields(cname):
+            lines.append('printf("%s.%s %%zu\\n", offsetof(%s, %s));' % (cname, f, cname, f))
+    lines += ['return 0; }']
+    src = tmp_path / "abi.c"
+    src.write_text("\n".join(lines))
+    exe = tmp_path / "abi"
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), "-o", str(exe), str(src)])
+    got = dict(l.split() for l in subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.splitlines())
+    for cname, pyname in _STRUCTS.items():
+        st = getattr(pakr, pyname)
+        assert int(got[cname]) == ctypes.sizeof(st), cname
+        for f, _ in st._fields_:
+            assert int(got[f"{cname}.{f}"]) == getattr(st, f).offset, (cname, f)
 
 
 def test_create_without_gpu_fails_loudly():

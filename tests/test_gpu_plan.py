@@ -231,21 +231,20 @@ def test_plan_initial_cost_bound(pakr, orc):
 
 
 @pytest.mark.parametrize("name,iters", [("C2", 9), ("C3", 6), ("C1", 12)])
-def test_plan_loop_with_nn_index_equals_scan(pakr, name, iters, monkeypatch):
+def test_plan_loop_with_nn_index_equals_scan(pakr, name, iters):
     """Inside the device loop the index is rebuilt as the tree grows and the rows added since are scanned:
     the tree must be bit-identical to the one the scan tiers build."""
     p, cfg = wl.CONFIGS[name]()
     cap = 1 + iters * cfg.B * cfg.K
     trees = {}
-    for mode in ("0", "2"):
-        monkeypatch.setenv("PAKR_NN_INDEX", mode)
-        pl = pakr.Planner(p)
-        res = pl.plan(7, cfg.B, cfg.K, cap, 1, max_iters_per_replan=iters)
+    pl = pakr.Planner(p)
+    for mode in (pakr.NN_SCAN, pakr.NN_INDEX):
+        res = pl.plan(7, cfg.B, cfg.K, cap, 1, max_iters_per_replan=iters, nn_mode=mode)
         trees[mode] = (res["final_tree_nodes"], pl.read_tree(cfg.B, cfg.K, cap, res["final_tree_nodes"]))
-        pl.close()
-    assert trees["0"][0] == trees["2"][0] > cfg.B
+    pl.close()
+    assert trees[pakr.NN_SCAN][0] == trees[pakr.NN_INDEX][0] > cfg.B
     for k in ("states", "actions", "parents", "costs"):
-        np.testing.assert_array_equal(trees["0"][1][k], trees["2"][1][k])
+        np.testing.assert_array_equal(trees[pakr.NN_SCAN][1][k], trees[pakr.NN_INDEX][1][k])
 
 
 def test_plan_small_b_stream_tier_and_no_obstacles(pakr, orc):

@@ -237,10 +237,10 @@ def test_nn_tiers_agree_bit_for_bit(pakr, name):
 
 @pytest.mark.parametrize("name,n0,B,K", [("C2", 20000, 512, 2), ("C3", 9000, 300, 3), ("C3", 40000, 257, 2),
                                          ("C1", 700, 64, 4), ("C5", 60000, 1024, 1)])
-def test_nn_index_tier_equals_scan_tier(pakr, orc, name, n0, B, K, monkeypatch):
-    """The NN cell index (exact spatial pruning) must return bit-identical NN indices
-    and distances to the brute-force scan, on clustered trees too (queries far from every node walk many rings),
-    and meets the oracle bar.  PAKR_NN_INDEX is read at pakr_create: 0 = scan only, 2 = index on any tree."""
+def test_nn_index_tier_equals_scan_tier(pakr, orc, name, n0, B, K):
+    """The NN index (exact spatial pruning) must return bit-identical NN indices
+    and distances to the brute-force scan, on clustered trees too (queries far from every node search wide),
+    and meets the oracle bar.  nn_mode: PAKR_NN_SCAN = scan tiers only, PAKR_NN_INDEX = index on any tree."""
     from parity_util import check_iteration, run_both
     p, _ = wl.CONFIGS[name]()
     host = wl.random_tree(p, n0, seed=n0, flat=n0 > 30000)
@@ -249,17 +249,15 @@ def test_nn_index_tier_equals_scan_tier(pakr, orc, name, n0, B, K, monkeypatch):
     host["states"][n0 // 3:, :pd] = (p.state_lo[:pd] + 0.15 * (host["states"][n0 // 3:, :pd] - p.state_lo[:pd]))
     host["states"][n0 - 50:] = host["states"][100:150]
     outs = {}
-    for mode in ("0", "2"):
-        monkeypatch.setenv("PAKR_NN_INDEX", mode)
-        pl = pakr.Planner(p)
+    pl = pakr.Planner(p)
+    for mode in (pakr.NN_SCAN, pakr.NN_INDEX):
         tree = pl.new_tree(n0 + B * K, host)
-        outs[mode] = pl.expand_step(tree, 5, 1, 4, B, K)
-        if mode == "2":
+        outs[mode] = pl.expand_step(tree, 5, 1, 4, B, K, nn_mode=mode)
+        if mode == pakr.NN_INDEX:
             op = orc.OracleProblem(p)
-            out, after, ref, _ = run_both(pl, orc, op, p, host, seed=5, r=1, it=4, B=B, K=K, cap=n0 + B * K)
+            out, after, ref, _ = run_both(pl, orc, op, p, host, seed=5, r=1, it=4, B=B, K=K, cap=n0 + B * K,
+                                          nn_mode=mode)
             check_iteration(orc, op, p, host, out, after, ref, B, K, n0 + B * K)
-        pl.close()
-    np.testing.assert_array_equal(outs["0"]["x_rand"], outs["2"]["x_rand"])
-    np.testing.assert_array_equal(outs["0"]["nn_idx"], outs["2"]["nn_idx"])
-    np.testing.assert_array_equal(outs["0"]["nn_d2"], outs["2"]["nn_d2"])
-    np.testing.assert_array_equal(outs["0"]["child_state"], outs["2"]["child_state"])
+    pl.close()
+    for k in ("x_rand", "nn_idx", "nn_d2", "child_state"):
+        np.testing.assert_array_equal(outs[pakr.NN_SCAN][k], outs[pakr.NN_INDEX][k])
