@@ -1,18 +1,28 @@
 #!/usr/bin/env python
-"""bench.py -- headline measurement of the PAKR hot path on B200 (contract: see DESIGN.md "Measurement").
+"""bench.py -- measurements of the PAKR hot path on B200 (contract: DESIGN.md "Measurement").
 
-A "step" is one pass of the whole hot path: one pakr_plan call (AO-x replanning around the batched
-expansion iteration, every row of SURVEY.md 8(a)) on BASELINE.json configs[1] (C2: 3D double
-integrator, 32 boxes, B=1024, K=8, cap 2^20, 20 replans) with planner seed = step index.
-metric = expanded nodes/s = children propagated and checked per second (B*K*iterations / time).
+Default mode (`--what bench`): a "step" is one pass of the whole hot path, i.e. one pakr_plan call (AO-x
+replanning around the batched expansion iteration, every row of SURVEY.md 8(a)) on the LARGEST single-GPU
+config of BASELINE.json, configs[3] = C4 (12-D quadrotor, 128 cylinders, B=4096, K=16, cap 2^22, 30 replans),
+planner seed = step index.  metric = expanded nodes/s = children propagated and checked per second
+(B*K*iterations / time).  The other configs (C1-C3 and one C5 point) are reported as extra keys of the same line.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+  python bench.py --what peak                 measured FFMA / FFMA2 rates (the ALU roofline's denominators)
+  python bench.py --what phases [--only nn|stream|prop] [--quick]      single phases through pakr_expand_step
+  python bench.py --what sweep|c5|pathlen [--seeds N]                  BASELINE metrics over seeds, config 5 sweep
+
+With --gpus N > 1 and no RANK in the environment it starts the N ranks itself (torch.distributed.run, one
+planner replica per GPU, NCCL only for the timing harness' scalar reductions).
 """
 from __future__ import annotations
 
 import argparse
+import dataclasses
 import json
+import multiprocessing as mp
 import os
+import socket
 import statistics
 import subprocess
 import sys
@@ -26,32 +36,45 @@ import numpy as np  # noqa: E402
 
 from paper_2607_03987_b200 import replicas, workloads as wl  # noqa: E402
 
-WORKLOAD = "C2"
+WORKLOAD = "C4"
 METRIC = "expanded nodes/s"
 UNIT = "nodes/s"
-# dram__bytes_read.sum + dram__bytes_write.sum of one pakr_loop_kernel launch on this workload, from the
+C5_POINT = (4096, 16)  # the fixed config-5 point reported beside the headline
+# dram__bytes_read.sum + dram__bytes_write.sum of one pakr_loop_kernel launch on WORKLOAD, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists for the current kernel).
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 1222656  # profiles/r01_s3_ncu_bench.md
+NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+NOMINAL_LANES = 148 * 4 * 32  # SMs x schedulers x lanes: issue slots per clock = fp32 FMA lanes per clock
+
+# Arithmetic of one evaluation of f(x, u), counted on the formulas of DESIGN.md "Readings" Q / P33 / P34 with every
+# multiply-add fused (one lane-op each), a sine/cosine pair as 2, a reciprocal as 1 (DESIGN.md "Measurement" has
+# the count line by line).
+F_DYN = {wl.DYN_DOUBLE_INTEGRATOR: 0, wl.DYN_UNICYCLE2: 4, wl.DYN_QUADROTOR: 37, wl.DYN_DUBINS_AIRPLANE: 8,
+         wl.DYN_UNICYCLE1: 4, wl.DYN_QUADROTOR_BODY: 59}
+
+
+def nn_ops_per_pair(problem) -> int:
+    """D sub + D fma + compare + select per (query, node) pair (+ D mul if weighted, +2 per angle
+    dim for the wrap)."""
+    D = problem.state_dim
+    weighted = not np.all(problem.nn_weight == 1.0)
+    return 2 * D + 2 + (D if weighted else 0) + 2 * int((problem.dim_kind == 1).sum())
+
+
+def prop_ops_per_child(problem) -> int:
+    """S steps of: stages * f + integrator combination (RK4: 7 fused ops per dim; Euler: 1) + closed-box test
+    (2 compares + 1 combine per bounded dim) + obstacle broad phase (cell index and header: 10) + ONE obstacle
+    test (the exact grid culls the rest)."""
+    D = problem.state_dim
+    rk4 = problem.integrator == wl.INT_RK4
+    n_bounded = int((np.isfinite(problem.state_lo) & (problem.dim_kind == 0)).sum())
+    c_obs = 2 * problem.pos_dim if problem.obstacle_type == wl.OBS_AABB else 5
+    per_step = (4 if rk4 else 1) * F_DYN[problem.dynamics_id] + (7 if rk4 else 1) * D + 3 * n_bounded + 10 + c_obs
+    return problem.steps_per_edge * per_step
 
 
 def algorithmic_ops(problem, nn_pairs: int, children: int) -> dict:
-    """Algorithmic fp32 lane-operations of one launch: the NN scan evaluates
-    nn_pairs (query, node) pairs at D sub + D fma + compare + select each (+ D mul if weighted, +2 on an
-    angle dim); a child costs S steps of (8 D integrator ops + F dynamics ops + 2 per bounded dim + the
-    obstacle broad phase: cell index and header, 10 ops, plus ONE obstacle test -- not one per obstacle,
-    because the grid culls the rest exactly)."""
-    D = problem.state_dim
-    weighted = not np.all(problem.nn_weight == 1.0)
-    n_angle = int((problem.dim_kind == 1).sum())
-    nn_per_pair = 2 * D + 2 + (D if weighted else 0) + 2 * n_angle
-    f_dyn = {wl.DYN_DOUBLE_INTEGRATOR: 0, wl.DYN_UNICYCLE2: 25, wl.DYN_QUADROTOR: 140, wl.DYN_DUBINS_AIRPLANE: 50,
-             wl.DYN_UNICYCLE1: 24, wl.DYN_QUADROTOR_BODY: 170}[problem.dynamics_id]
-    stages = 4 if problem.integrator == wl.INT_RK4 else 1
-    integ = 8 * D if problem.integrator == wl.INT_RK4 else 2 * D
-    n_bounded = int((np.isfinite(problem.state_lo) & (problem.dim_kind == 0)).sum())
-    c_obs = 2 * problem.pos_dim if problem.obstacle_type == wl.OBS_AABB else 5
-    per_child = problem.steps_per_edge * (stages * f_dyn + integ + 2 * n_bounded + 10 + c_obs)
-    return dict(nn=nn_pairs * nn_per_pair, prop=children * per_child, nn_per_pair=nn_per_pair, per_child=per_child)
+    a, b = nn_ops_per_pair(problem), prop_ops_per_child(problem)
+    return dict(nn=nn_pairs * a, prop=children * b, nn_per_pair=a, per_child=b)
 
 
 class ClockSampler(threading.Thread):
@@ -89,58 +112,158 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(reasons), "samples": len(self.rows)}
 
 
-def oracle_sample(problem, cfg, seed: int) -> dict:
-    """The CPU oracle as it stands on a bounded sample of the workload: replan 0 (first solution) of the
-    same config and seed, one thread."""
+# ---------------------------------------------------------------------------------------------------------
+# CPU oracle, timed as it stands (BASELINE.md "CPU-baseline plan"): single-threaded fp64
+# C++, one process PINNED to one core for latency, expansions/s and per-phase shares, plus a seed fan-out over
+# every core the process may run on (count read at run time) for the aggregate rate.  Child processes are
+# spawned (never forked: the parent may hold a CUDA context) and import only numpy + the oracle.
+# ---------------------------------------------------------------------------------------------------------
+def _workload(name: str):
+    if name == "C5":
+        return wl.config5(B=C5_POINT[0], K=C5_POINT[1])
+    return wl.CONFIGS[name]()
+
+
+def _oracle_worker(job):
+    name, seed, budget_ms, core = job
+    if core is not None:
+        try:
+            os.sched_setaffinity(0, {core})
+        except OSError:
+            core = None
     from oracle import pakr_oracle as orc
+    problem, cfg = _workload(name)
     op = orc.OracleProblem(problem)
     t0 = time.perf_counter()
-    res = orc.plan(op, seed, cfg.B, cfg.K, cfg.tree_capacity, 1)
+    # replan 0 (first solution) under a wall-clock cap: the oracle checks the cap between iterations
+    res = orc.plan(op, seed, cfg.B, cfg.K, cfg.tree_capacity, 1, time_budget_ms=budget_ms)
     dt = time.perf_counter() - t0
-    return dict(value=res["children"] / dt, seconds=dt, children=res["children"], iterations=res["iterations"],
-                first_solution_ms=res["first_solution_ms"], cost=res["cost"])
+    return dict(seconds=dt, children=res["children"], iterations=res["iterations"], solved=res["outcome"],
+                nodes=int(res["replan_nodes"][0]), first_solution_ms=res["first_solution_ms"], cost=res["cost"],
+                phase_ms=res["phase_ms"], core=core)
 
 
-def run_reference(args, problem, cfg):
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+def oracle_baseline(name: str, budget_s: float, fanout: bool, seed: int = 0) -> dict:
+    """-> cpu_baseline object for workload `name`."""
+    from oracle import pakr_oracle as orc
+    orc.build()  # before the children race to build it
+    cores = sorted(os.sched_getaffinity(0))
+    ctx = mp.get_context("spawn")
+    with ctx.Pool(1) as pool:
+        one = pool.map(_oracle_worker, [(name, seed, budget_s * 1e3, cores[0])])[0]
+    ph = one["phase_ms"]
+    tot = sum(ph) or 1.0
+    how = ("to its first solution" if one["solved"] else f"cut off by the {budget_s:.0f} s cap")
+    out = {"value": one["children"] / one["seconds"], "unit": UNIT, "cores": 1, "kind": "oracle",
+           "pinned_core": one["core"],
+           "sample": f"replan 0 of {name}, planner seed {seed}, {how}: {one['iterations']} iterations, "
+                     f"{one['children']} children, tree {one['nodes']} nodes in {one['seconds']:.1f} s",
+           "phase_share": {"nn": ph[0] / tot, "propagate_validity_prune": ph[1] / tot, "insert": ph[2] / tot},
+           "first_solution_ms": one["first_solution_ms"] if one["solved"] else None}
+    if fanout and len(cores) > 1:
+        t0 = time.perf_counter()
+        with ctx.Pool(len(cores)) as pool:
+            rows = pool.map(_oracle_worker, [(name, seed + 1 + i, budget_s * 1e3, c) for i, c in enumerate(cores)], 1)
+        wall = time.perf_counter() - t0
+        out["all_cores"] = {"cores": len(cores), "value": sum(r["children"] for r in rows) / max(r["seconds"] for r in rows),
+                            "unit": UNIT, "sample": f"{len(cores)} pinned single-thread replicas, planner seeds "
+                                                    f"{seed + 1}..{seed + len(cores)}, same cap; wall {wall:.1f} s"}
+    return out
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the box's host cores, same metric and config (tier rule)."""
+    if int(os.environ.get("RANK", "0")) != 0:
         return
-    for i in range(args.warmup):
-        oracle_sample(problem, cfg, 1000 + i) if i == 0 else None  # one untimed pass warms the library
-    t_total, children, firsts = 0.0, 0, []
-    for i in range(args.steps):
-        r = oracle_sample(problem, cfg, i)
-        t_total += r["seconds"]
-        children += r["children"]
-        firsts.append(r["first_solution_ms"])
-    value = children / t_total
-    sample = f"replan 0 (first solution) of {WORKLOAD} per step, planner seeds 0..{args.steps - 1}"
+    problem, cfg = _workload(args.workload)
+    budget_s = 12.0
+    steps = max(1, min(args.steps, 8))  # ~12 s of CPU per step: the whole run stays within minutes
+    ctx = mp.get_context("spawn")
+    cores = sorted(os.sched_getaffinity(0))
+    from oracle import pakr_oracle as orc
+    orc.build()
+    rows = []
+    with ctx.Pool(1) as pool:
+        for i in range(min(args.warmup, 1)):
+            pool.map(_oracle_worker, [(args.workload, 1000 + i, 2e3, cores[0])])  # one short untimed pass
+        for i in range(steps):
+            rows += pool.map(_oracle_worker, [(args.workload, i, budget_s * 1e3, cores[0])])
+    t_total = sum(r["seconds"] for r in rows)
+    value = sum(r["children"] for r in rows) / t_total
+    sample = (f"per step: replan 0 of {args.workload} under a {budget_s:.0f} s wall-clock cap, planner seed = step; "
+              f"one pinned core")
+    firsts = [r["first_solution_ms"] for r in rows if r["solved"]]
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_total / args.steps,
+            "steps": steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_total / steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": WORKLOAD, "dynamics": problem.name, "B": cfg.B, "K": cfg.K,
-                       "tree_capacity": cfg.tree_capacity, "n_replans": cfg.n_replans,
-                       "sampled": "replan 0 only (the oracle needs ~3 s per replan-0, minutes for all 20)"},
+            "config": {"workload": args.workload, "dynamics": problem.name, "B": cfg.B, "K": cfg.K,
+                       "tree_capacity": cfg.tree_capacity, "n_replans": cfg.n_replans, "sampled": sample},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "first_solution_ms_median": statistics.median(firsts)}
+            "first_solution_ms_median": statistics.median(firsts) if firsts else None,
+            "solved": len(firsts)}
     print(json.dumps(line), flush=True)
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    args = ap.parse_args()
-    problem, cfg = wl.CONFIGS[WORKLOAD]()
-    if args.impl == "reference":
-        if args.steps > 8:
-            args.steps = 8  # ~10 s of CPU per step: keep the whole run within minutes
-        return run_reference(args, problem, cfg)
+# ---------------------------------------------------------------------------------------------------------
+def time_plans(torch, pl, cfg, seeds, flush, n_replans=None):
+    """Times one pakr_plan per seed: CUDA events on the launching stream (device) and the host clock around the
+    same call (end to end: HOST buffers in, HOST result out).  L2 is flushed between steps, outside the events."""
+    R = cfg.n_replans if n_replans is None else n_replans
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in seeds]
+    results, wall = [], []
+    for i, s in enumerate(seeds):
+        flush.fill_(i & 0xFF)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ev[i][0].record()
+        res = pl.plan(s, cfg.B, cfg.K, cfg.tree_capacity, R)
+        ev[i][1].record()
+        torch.cuda.synchronize()
+        wall.append(time.perf_counter() - t0)
+        results.append(res)
+    return results, [a.elapsed_time(b) for a, b in ev], wall
 
+
+def roofline_of(problem, results, dev_ms, sm_max_mhz, measured_peak) -> dict:
+    ops = [algorithmic_ops(problem, r["nn_pairs"], r["children"]) for r in results]
+    alg = sum(o["nn"] + o["prop"] for o in ops)
+    launch_s = sum(dev_ms) * 1e-3
+    peak = NOMINAL_LANES * sm_max_mhz * 1e6 / 1e12
+    achieved = alg / launch_s / 1e12
+    out = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tlaneop/s (fp32 lane-instructions)",
+           "frac": achieved / peak, "traffic": None,
+           "avg_launch_ms": 1e3 * launch_s / len(results), "kernel_ms_by_globaltimer": float(np.mean([r["device_ms"] for r in results])),
+           "algorithmic_ops_per_launch": alg / len(results), "nn_ops_per_pair": ops[0]["nn_per_pair"],
+           "prop_ops_per_child": ops[0]["per_child"], "nn_share_of_ops": sum(o["nn"] for o in ops) / alg,
+           "peak_basis": f"nominal: 148 SM x 4 schedulers x 32 lanes x {sm_max_mhz:.0f} MHz (clocks.max.sm)"}
+    if measured_peak:
+        out["peak_measured_ffma"] = measured_peak["ffma_lane_ops_per_s"] / 1e12
+        out["frac_vs_measured_ffma"] = achieved / out["peak_measured_ffma"]
+    ev = sum(r.get("nn_pairs_evaluated", r["nn_pairs"]) for r in results)
+    tot = sum(r["nn_pairs"] for r in results)
+    if ev != tot:  # the NN index answered with fewer distance evaluations than the B*n of the definition
+        exe = (ev * ops[0]["nn_per_pair"] + sum(o["prop"] for o in ops)) / launch_s / 1e12
+        out["nn_pairs_evaluated_share"] = ev / tot
+        out["executed_frac"] = exe / peak
+    return out
+
+
+def summarize(results, dev_ms, wall):
+    first = [r["first_solution_ms"] for r in results if r["first_solution_ms"] >= 0]
+    kern = sum(r["device_ms"] for r in results)
+    return {"first_solution_ms_median": statistics.median(first) if first else None,
+            "final_cost_median": statistics.median(r["cost"] for r in results),
+            "iterations_per_step": float(np.mean([r["iterations"] for r in results])),
+            "replans_solved_per_step": float(np.mean([r["replans_solved"] for r in results])),
+            "replans_run_per_step": float(np.mean([r["replans_run"] for r in results])),
+            "phase_share": {k: sum(r["phase_ms"][i] for r in results) / kern
+                            for i, k in enumerate(("nn_scan_phases", "propagate_and_nn_lookahead", "insert_phases"))},
+            "inserted_nodes_per_s": sum(r["inserted"] for r in results) / (sum(dev_ms) * 1e-3),
+            "solved": sum(r["outcome"] for r in results)}
+
+
+def run_bench(args):
     import torch
     import torch.distributed as dist
     from paper_2607_03987_b200 import pakr
@@ -152,8 +275,9 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
     pakr.lib()  # fails loudly if the CUDA extension is missing
+    problem, cfg = _workload(args.workload)
     pl = pakr.Planner(problem, local)
-    ws = pl.workspace(cfg.B, cfg.K, cfg.tree_capacity)
+    ws = pl.workspace(cfg.B, cfg.K, cfg.tree_capacity)  # noqa: F841  (allocated before the timed region)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{local}")  # > 126 MB L2
 
     def barrier():
@@ -162,85 +286,283 @@ def main():
         torch.cuda.synchronize()
 
     # replicas only: rank r plans seeds r, r + world, ...
-    seeds = replicas.replica_seeds(rank, world, args.warmup + args.steps)
-    for s in seeds[:max(args.warmup, 3)]:
+    W = max(args.warmup, 3)
+    seeds = replicas.replica_seeds(rank, world, W + args.steps)
+    for s in seeds[:W]:
         pl.plan(s, cfg.B, cfg.K, cfg.tree_capacity, cfg.n_replans)
     sampler = ClockSampler(local)
     barrier()
     sampler.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    results, wall = [], []
     barrier()
-    for i, s in enumerate(seeds[args.warmup:]):
-        flush.fill_(i & 0xFF)  # L2 flush between timed steps (outside the events)
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        ev[i][0].record()
-        res = pl.plan(s, cfg.B, cfg.K, cfg.tree_capacity, cfg.n_replans)  # HOST result buffers filled inside
-        ev[i][1].record()
-        torch.cuda.synchronize()
-        wall.append(time.perf_counter() - t0)
-        results.append(res)
+    results, dev_ms, wall = time_plans(torch, pl, cfg, seeds[W:], flush)
     barrier()
     clocks = sampler.finish()
-    dev_ms = [a.elapsed_time(b) for a, b in ev]
-    kern_ms = [r["device_ms"] for r in results]
     agg = replicas.aggregate(sum(dev_ms), sum(wall) * 1e3, float(sum(r["children"] for r in results)),
                              dist=dist if world > 1 else None, device=f"cuda:{local}")
-    value, e2e = agg["value"], agg["e2e"]
-    ms_per_step = agg["device_ms"] / args.steps
 
     if rank == 0:
-        # roofline of the one kernel (ALU-bound: DESIGN.md "Roofline")
-        ops = [algorithmic_ops(problem, r["nn_pairs"], r["children"]) for r in results]
-        alg = sum(o["nn"] + o["prop"] for o in ops)
-        launch_s = sum(kern_ms) * 1e-3
         sm_max = clocks["sm_max_mhz"] or 1965.0
-        peak = 148 * 128 * sm_max * 1e6 / 1e12
-        achieved = alg / launch_s / 1e12
-        first = [r["first_solution_ms"] for r in results if r["first_solution_ms"] >= 0]
+        measured = pakr.measure_fp32_peak(local)
+        roof = roofline_of(problem, results, dev_ms, sm_max, measured)
+        roof["traffic"] = NCU_TRAFFIC_BYTES_PER_LAUNCH
+        roof["kernel"] = f"pakr_loop_kernel ({problem.name})"
+        if clocks["sm_mhz"]:
+            roof["frac_at_sampled_clock"] = roof["achieved"] / (NOMINAL_LANES * clocks["sm_mhz"] * 1e6 / 1e12)
         # best cost at 100 ms (BASELINE metric, part 3): unlimited replans under a device time budget
         best100 = [pl.plan(s, cfg.B, cfg.K, cfg.tree_capacity, 4096, time_budget_ms=100.0)["cost"] for s in range(5)]
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+            "metric": METRIC, "value": agg["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": W, "ms_per_step": agg["device_ms"] / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": WORKLOAD, "dynamics": problem.name, "B": cfg.B, "K": cfg.K,
+            "config": {"workload": args.workload, "dynamics": problem.name, "B": cfg.B, "K": cfg.K,
                        "tree_capacity": cfg.tree_capacity, "n_replans": cfg.n_replans,
                        "seeds": f"rank + {world} * step", "l2": "flushed between timed steps (256 MiB fill)",
                        "parallelism": f"replicas x{world}"},
             "clocks": clocks,
-            "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 4 * pl.Dp + 4,
-                    "d2h_bytes_per_step": int(np.mean([1700 + 4 * r["path_len"] * (1 + pl.D + pl.m) for r in results]))},
+            "e2e": {"value": agg["e2e"], "unit": UNIT,  # bytes as counted by pakr_plan itself (pakr_stats)
+                    "h2d_bytes_per_step": int(np.mean([r["h2d_bytes"] for r in results])),
+                    "d2h_bytes_per_step": int(np.mean([r["d2h_bytes"] for r in results]))},
             "gpu_launches": args.steps,
-            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tlaneop/s (fp32 lane-instructions)",
-                         "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
-                         "kernel": "pakr_loop_kernel<DI3,BOX>", "avg_launch_ms": 1e3 * launch_s / args.steps,
-                         "algorithmic_ops_per_launch": alg / args.steps,
-                         "nn_share_of_ops": sum(o["nn"] for o in ops) / alg,
-                         "nn_fma_pipe_frac": sum(r["nn_pairs"] for r in results) * 2 * problem.state_dim / launch_s / 1e12 / peak,
-                         "peak_basis": f"148 SM x 4 schedulers x 32 lanes x {sm_max:.0f} MHz issue slots (= FMA-pipe lane-ops/s)",
-                         "frac_at_measured_clock": (achieved / (148 * 128 * clocks['sm_mhz'] * 1e6 / 1e12))
-                         if clocks["sm_mhz"] else None},
-            "first_solution_ms_median": statistics.median(first) if first else None,
+            "roofline": roof,
             "best_cost_at_100ms_median": statistics.median(best100),
-            "final_cost_median": statistics.median(r["cost"] for r in results),
-            "iterations_per_step": float(np.mean([r["iterations"] for r in results])),
-            "phase_share": {k: sum(r["phase_ms"][i] for r in results) / sum(kern_ms)
-                            for i, k in enumerate(("nn_tail_scan", "propagate_and_nn_lookahead", "insert_and_fused_tail"))},
-            "inserted_nodes_per_s": sum(r["inserted"] for r in results) / (sum(dev_ms) * 1e-3),
-            "solved": sum(r["outcome"] for r in results),
         }
+        line.update(summarize(results, dev_ms, wall))
+        pl.close()
+        if not args.no_extras and world == 1:
+            line["other_workloads"] = {}
+            for name in ("C1", "C2", "C3", "C5"):
+                p2, c2 = _workload(name)
+                pl2 = pakr.Planner(p2, local)
+                pl2.plan(999, c2.B, c2.K, c2.tree_capacity, c2.n_replans)
+                res2, dev2, wall2 = time_plans(torch, pl2, c2, list(range(3)), flush)
+                row = {"B": c2.B, "K": c2.K, "n_replans": c2.n_replans, "steps": 3,
+                       "value": sum(r["children"] for r in res2) / (sum(dev2) * 1e-3), "unit": UNIT,
+                       "e2e": sum(r["children"] for r in res2) / sum(wall2), "ms_per_step": sum(dev2) / 3}
+                row.update(summarize(res2, dev2, wall2))
+                rf = roofline_of(p2, res2, dev2, sm_max, measured)
+                row["roofline_frac"] = rf["frac"]
+                row["roofline_frac_vs_measured_ffma"] = rf.get("frac_vs_measured_ffma")
+                if "executed_frac" in rf:
+                    row["executed_frac"] = rf["executed_frac"]
+                if not args.no_cpu_baseline:
+                    row["cpu_baseline"] = oracle_baseline(name, 4.0, fanout=False)
+                line["other_workloads"]["C5 (B=%d, K=%d)" % C5_POINT if name == "C5" else name] = row
+                pl2.close()
         if not args.no_cpu_baseline and world == 1:
-            cb = oracle_sample(problem, cfg, 0)
-            line["cpu_baseline"] = {"value": cb["value"], "unit": UNIT, "cores": 1, "kind": "oracle",
-                                    "sample": f"replan 0 (first solution) of {WORKLOAD}, planner seed 0: "
-                                              f"{cb['iterations']} iterations, {cb['children']} children in {cb['seconds']:.1f} s",
-                                    "first_solution_ms": cb["first_solution_ms"]}
+            line["cpu_baseline"] = oracle_baseline(args.workload, 12.0, fanout=True)
         print(json.dumps(line), flush=True)
-    pl.close()
+    else:
+        pl.close()
     if world > 1:
         dist.destroy_process_group()
+
+
+def run_peak(args):
+    """Measured fp32 peaks: the denominators beside the nominal one in `roofline`."""
+    from paper_2607_03987_b200 import pakr
+    m = pakr.measure_fp32_peak(0)
+    nominal = NOMINAL_LANES * m["sm_clock_mhz"] * 1e6
+    print(json.dumps({"what": "peak", "nominal_lane_ops_per_s": nominal, **m,
+                      "ffma_frac_of_nominal": m["ffma_lane_ops_per_s"] / nominal,
+                      "ffma2_frac_of_nominal": m["ffma2_lane_ops_per_s"] / nominal,
+                      "scan_mix_frac_of_nominal": m["scan_mix_lane_ops_per_s"] / nominal}), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# --what phases: one pakr_expand_step on a synthetic tree of n uniform-in-bounds nodes is one iteration whose
+# phases the kernel times itself (pakr_read_stats: phase_ms[0] = NN scan of the whole tree, [1] = propagate
+# (+ insert when B*K is small), [2] = insert as a phase of its own; each includes its grid barrier, ~1.2 us).
+# ---------------------------------------------------------------------------------------------------------
+def measure_phase(torch, pl, problem, n, B, K, reps, flush, nn_mode=0):
+    host = wl.random_tree(problem, n, seed=n % 1000 + B, flat=True)
+    cap = n + B * K
+    tree = pl.new_tree(cap, host)
+    ws = pl.workspace(B, K, cap)
+    out = []
+    for rep in range(reps + 1):
+        tree["n_nodes"][0] = n
+        if flush is not None:
+            flush.fill_(rep)  # tree out of L2
+        torch.cuda.synchronize()
+        pl.expand_step(tree, 0, 0, rep, B, K, debug=False, workspace=ws, nn_mode=nn_mode)
+        st = pl.read_stats(B, K, cap, workspace=ws)
+        if rep:  # first call is the warm-up
+            out.append(st["phase_ms"])
+    return np.median(np.array(out), axis=0)
+
+
+def run_phases(args):
+    import torch
+    from paper_2607_03987_b200 import pakr
+    pakr.lib()
+    peak = NOMINAL_LANES * 1.965e9
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    reps = 3 if args.quick else 7
+    nn_points = [("C2", 1 << 16, 1024), ("C2", 1 << 20, 1024), ("C5", 1 << 20, 16384), ("C3", 1 << 20, 2048),
+                 ("C4", 1 << 18, 4096), ("C4", 1 << 22, 4096)]
+    if args.quick:
+        nn_points = nn_points[1:3] + nn_points[5:]
+    for name, n, B in (nn_points if args.only in ("", "nn") else []):
+        p, _ = wl.CONFIGS[name]()
+        pl = pakr.Planner(p)
+        ph = measure_phase(torch, pl, p, n, B, 1, reps, None, nn_mode=pakr.NN_SCAN)
+        t = ph[0] * 1e-3
+        ops = nn_ops_per_pair(p)
+        print(json.dumps({"phase": "nn", "workload": name, "D": p.state_dim, "n": n, "B": B, "ms": ph[0],
+                          "pairs_per_s": B * n / t, "alg_lane_ops_per_pair": ops,
+                          "alu_frac": B * n * ops / t / peak,
+                          "fma_pipe_frac": B * n * 2 * p.state_dim / t / peak,
+                          "tree_GBps": 4 * p.state_dim * n / t / 1e9}), flush=True)
+        pl.close()
+    # HBM-bound regime: few queries share one pass over a tree > L2.  Algorithmic bytes = 4 * D * n (SURVEY 8(d)).
+    for name, B in ((("C2", 8), ("C4", 8), ("C4", 4)) if args.only in ("", "stream") else ()):
+        p, _ = wl.CONFIGS[name]()
+        pl = pakr.Planner(p)
+        n = 1 << 23
+        ph = measure_phase(torch, pl, p, n, B, 1, reps, flush, nn_mode=pakr.NN_SCAN)
+        t = ph[0] * 1e-3
+        print(json.dumps({"phase": "stream", "workload": name, "D": p.state_dim, "n": n, "B": B, "ms": ph[0],
+                          "algorithmic_GBps": 4 * p.state_dim * n / t / 1e9,
+                          "hbm_frac_of_measured_6446": 4 * p.state_dim * n / t / 6446.3e9,
+                          "row_bytes_in_memory": 4 * p.state_stride, "l2": "flushed before every call"}), flush=True)
+        pl.close()
+    for name, B, K in ((("C2", 1024, 8), ("C3", 2048, 8), ("C4", 4096, 16), ("C5", 16384, 64)) if args.only in ("", "prop") else ()):
+        if args.quick and name in ("C3",):
+            continue
+        p, _ = wl.CONFIGS[name]()
+        pl = pakr.Planner(p)
+        ph = measure_phase(torch, pl, p, 4096, B, K, reps, None)
+        t = ph[1] * 1e-3
+        ops = prop_ops_per_child(p)
+        print(json.dumps({"phase": "prop", "workload": name, "children": B * K, "ms": ph[1], "insert_ms": ph[2],
+                          "children_per_s": B * K / t, "alg_lane_ops_per_child": ops,
+                          "alu_frac": B * K * ops / t / peak}), flush=True)
+        pl.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# --what sweep | c5 | pathlen: BASELINE.json metrics over planner seeds (medians), one JSON line per row.
+# ---------------------------------------------------------------------------------------------------------
+def med(v):
+    v = [x for x in v if x is not None]
+    return statistics.median(v) if v else None
+
+
+def run_sweep_configs(pakr, seeds, path_length=False):
+    for name in (("C1", "C2") if path_length else ("C1", "C2", "C3", "C4", "N1", "N2", "N3")):
+        p, cfg = wl.CONFIGS[name]()
+        if path_length:  # the paper's convergence metric (Table II, Fig. 2: cost = distance travelled, PAPER.md:180)
+            p = dataclasses.replace(p, cost_mode=wl.COST_PATH_LENGTH, heuristic_speed=1.0, name=p.name + "-pathlen")
+        pl = pakr.Planner(p)
+        pl.plan(1000, cfg.B, cfg.K, cfg.tree_capacity, 1)  # warm-up
+        first, nodes1, cost1, costf, ms_all, iters, solved, rate = [], [], [], [], [], [], 0, []
+        curve_c, curve_t = [], []
+        for s in range(seeds):
+            r = pl.plan(s, cfg.B, cfg.K, cfg.tree_capacity, cfg.n_replans)
+            solved += r["outcome"]
+            if r["first_solution_ms"] >= 0:
+                k = int((r["replan_cost"] < float("inf")).argmax())
+                first.append(r["first_solution_ms"])
+                nodes1.append(int(r["replan_nodes"][k]))
+                cost1.append(float(r["replan_cost"][k]))
+            costf.append(r["cost"])
+            curve_c.append([float(v) if v < float("inf") else None for v in r["replan_cost"]])
+            curve_t.append([float(v) for v in r["replan_end_ms"]])
+            ms_all.append(r["device_ms"])
+            iters.append(r["iterations"])
+            rate.append(r["children"] / (r["device_ms"] * 1e-3))
+        best100 = [pl.plan(s, cfg.B, cfg.K, cfg.tree_capacity, 4096, time_budget_ms=100.0)["cost"]
+                   for s in range(min(seeds, 10))]
+        print(json.dumps({"row": "config", "workload": p.name if path_length else name, "B": cfg.B, "K": cfg.K,
+                          "replans": cfg.n_replans, "seeds": seeds, "solved": solved,
+                          "first_solution_ms_median": med(first), "first_solution_nodes_median": med(nodes1),
+                          "first_cost_median": med(cost1), "final_cost_median": med(costf),
+                          "all_replans_ms_median": med(ms_all), "iterations_median": med(iters),
+                          "expanded_nodes_per_s_median": med(rate), "best_cost_at_100ms_median": med(best100),
+                          # cost-vs-time curve of AO-x (PAPER.md:180 Table II, Fig. 2): median over seeds of c_best
+                          # and of the device time at the end of each replan
+                          "cost_after_replan_median": [med(c) for c in zip(*curve_c)],
+                          "ms_at_end_of_replan_median": [med(t) for t in zip(*curve_t)]}), flush=True)
+        pl.close()
+
+
+def run_sweep_c5(pakr, seeds):
+    """BASELINE config 5: expansions/s, NN-scan HBM GB/s and time-to-first-solution at every (B, K)."""
+    p, _ = wl.config5()
+    pl = pakr.Planner(p)
+    for B in (256, 1024, 4096, 16384):
+        for K in (1, 4, 16, 64):
+            cap = 1 << 23 if B * K >= (1 << 18) else 1 << 21
+            pl.plan(1000, B, K, cap, 1)
+            first, nodes, iters, rate, nn_share, gbps, solved = [], [], [], [], [], [], 0
+            for s in range(seeds):
+                r = pl.plan(s, B, K, cap, 1)
+                solved += r["outcome"]
+                if r["outcome"]:
+                    first.append(r["first_solution_ms"])
+                nodes.append(r["final_tree_nodes"])
+                iters.append(r["iterations"])
+                rate.append(r["children"] / (r["device_ms"] * 1e-3))
+                nn_ms = r["phase_ms"][0] + r["phase_ms"][1]
+                nn_share.append(nn_ms / r["device_ms"])
+                # every iteration's NN reads its snapshot once: sum_i 4 D n_i = 4 D nn_pairs / B algorithmic bytes
+                gbps.append(4 * p.state_dim * r["nn_pairs"] / B / (nn_ms * 1e-3) / 1e9 if nn_ms > 0 else None)
+            print(json.dumps({"row": "c5", "B": B, "K": K, "children_per_iter": B * K, "tree_capacity": cap,
+                              "seeds": seeds, "solved": solved, "first_solution_ms_median": med(first),
+                              "iterations_median": med(iters), "nodes_median": med(nodes),
+                              "expanded_nodes_per_s_median": med(rate),
+                              "nn_scan_tree_GBps_median": med(gbps),
+                              "share_of_time_in_scan_and_propagate_phases": med(nn_share)}), flush=True)
+    pl.close()
+
+
+def run_sweep(args):
+    from paper_2607_03987_b200 import pakr
+    pakr.lib()
+    if args.what == "sweep":
+        run_sweep_configs(pakr, args.seeds)
+    elif args.what == "pathlen":
+        run_sweep_configs(pakr, args.seeds, path_length=True)
+    elif args.what == "c5":
+        run_sweep_c5(pakr, args.seeds)
+
+
+def spawn_ranks(args) -> int:
+    """`python bench.py --gpus N` started by hand: launch the N ranks exactly as the driver would."""
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--what", default="bench", choices=["bench", "peak", "phases", "sweep", "c5", "pathlen"])
+    ap.add_argument("--workload", default=WORKLOAD, choices=["C1", "C2", "C3", "C4", "C5"],
+                    help="headline workload of --what bench (default: the largest single-GPU config)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the other_workloads rows")
+    ap.add_argument("--seeds", type=int, default=10, help="--what sweep|c5|pathlen: planner seeds per row")
+    ap.add_argument("--quick", action="store_true", help="--what phases: fewer points and repetitions")
+    ap.add_argument("--only", default="", help="--what phases: nn | stream | prop")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.what == "peak":
+        return run_peak(args)
+    if args.what == "phases":
+        return run_phases(args)
+    if args.what in ("sweep", "c5", "pathlen"):
+        return run_sweep(args)
+    if args.gpus > 1 and "RANK" not in os.environ:
+        sys.exit(spawn_ranks(args))
+    return run_bench(args)
 
 
 if __name__ == "__main__":

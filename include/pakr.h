@@ -143,7 +143,9 @@ typedef struct {
   int64_t iterations;      /* inner-loop trips over all replans */
   int64_t children;        /* = iterations * B * K propagated and checked ("expanded nodes") */
   int64_t inserted;        /* nodes appended over all replans */
-  int64_t nn_pairs;        /* sum over iterations of B * n: (query, node) distance evaluations */
+  int64_t nn_pairs;        /* sum over iterations of B * n: the (query, node) pairs of the NN definition */
+  int64_t h2d_bytes, d2h_bytes; /* bytes pakr_plan copied host->device (root node) and device->host (control
+                                   block, path) in this call; kernel parameters (~1.3 KB) not counted */
   int32_t replans_run, replans_solved;
   int32_t termination;     /* 0 all replans run, 1 time budget */
   int32_t replan_stats_truncated; /* 1 if replans_run > PAKR_MAX_REPLAN_STATS: the per-replan arrays hold the first 64 */
@@ -213,6 +215,19 @@ pakr_status pakr_expand_step(pakr_planner* planner, const pakr_step_args* args, 
  * when the children are few), [2] = insert as a phase of its own, each including its grid barrier. */
 pakr_status pakr_read_stats(pakr_planner* planner, int32_t B, int32_t K, int64_t tree_capacity,
                             void* d_workspace, size_t workspace_bytes, void* cuda_stream, pakr_stats* out);
+
+/* Measurement support, not on the planning path: sustained fp32 rates of `cuda_device`, the denominators of the ALU
+ * roofline (the measured FFMA rate stands beside the nominal SMs x 128 lanes x clock).  Runs three
+ * register-only kernels for a few milliseconds each on the default stream and synchronises.  A lane-op is one fp32
+ * add, multiply or fused multiply-add on one lane; a packed f32x2 instruction counts two per lane.  *out is HOST. */
+typedef struct {
+  double ffma_lane_ops_per_s;     /* scalar fma.rn.f32 (SASS FFMA)                                    */
+  double ffma2_lane_ops_per_s;    /* packed fma.rn.f32x2 (SASS FFMA2), the NN scan's arithmetic       */
+  double scan_mix_lane_ops_per_s; /* one packed subtract per packed fma: the NN scan's own mix        */
+  double sm_clock_mhz;            /* the device's reported peak SM clock                              */
+  int32_t sm_count;
+} pakr_fp32_peak;
+pakr_status pakr_measure_fp32_peak(int cuda_device, pakr_fp32_peak* out);
 
 #ifdef __cplusplus
 }

@@ -364,6 +364,8 @@ extern "C" int32_t orc_expand_iteration(const orc_problem* P, orc_tree* T, uint6
   std::vector<double> x_rand((size_t)B * D), xs((size_t)BK * D), us((size_t)BK * m), cs(BK);
   std::vector<int64_t> nn(B);
   std::vector<int32_t> flags(BK);
+  using clk = std::chrono::steady_clock;  // timing only (bench.py's cpu_baseline reports per-phase shares)
+  const auto t_begin = clk::now();
 
   // l.6  X_rand <- SampleStates(B)
   for (int s = 0; s < B; ++s) orc_sample_state(P, seed, r, it, (uint32_t)s, &x_rand[(size_t)s * D]);
@@ -375,6 +377,7 @@ extern "C" int32_t orc_expand_iteration(const orc_problem* P, orc_tree* T, uint6
     if (dbg && dbg->nn_d2) dbg->nn_d2[s] = d2;
   }
   if (dbg && dbg->x_rand) std::memcpy(dbg->x_rand, x_rand.data(), sizeof(double) * B * D);
+  const auto t_nn = clk::now();
   // l.8  U <- SampleControls(B, K);  l.9  X_new, C_new <- Propagate(X_near, U, dt)
   for (int s = 0; s < B; ++s) {
     for (int k = 0; k < K; ++k) {
@@ -397,6 +400,7 @@ extern "C" int32_t orc_expand_iteration(const orc_problem* P, orc_tree* T, uint6
       if (dbg && dbg->goal_margin) dbg->goal_margin[c] = gm;
     }
   }
+  const auto t_prop = clk::now();
   // l.13  T <- T u {(x_new, u, c_new)} in ascending child index while n < cap (P20)
   int64_t inserted = 0, goal_node = -1;
   double goal_cost = kInf;
@@ -424,6 +428,10 @@ extern "C" int32_t orc_expand_iteration(const orc_problem* P, orc_tree* T, uint6
     dbg->n_inserted = inserted;
     dbg->goal_node = goal_node;
     dbg->new_c_best = goal_node >= 0 ? goal_cost : c_best;
+    const auto t_end = clk::now();
+    dbg->phase_ms[0] = std::chrono::duration<double, std::milli>(t_nn - t_begin).count();
+    dbg->phase_ms[1] = std::chrono::duration<double, std::milli>(t_prop - t_nn).count();
+    dbg->phase_ms[2] = std::chrono::duration<double, std::milli>(t_end - t_prop).count();
   }
   return goal_node >= 0 ? 1 : 0;
 }
@@ -464,6 +472,7 @@ extern "C" int32_t orc_plan(const orc_problem* P, const orc_plan_opts* O, orc_tr
   R->iterations = R->children = R->inserted = 0;
   R->replans_run = R->replans_solved = 0;
   R->first_solution_ms = -1.0;
+  R->phase_ms[0] = R->phase_ms[1] = R->phase_ms[2] = 0.0;
   int32_t status = 0;
   for (int32_t r = 0; r < O->n_replans; ++r) {  // l.3 (P22: a failed replan counts against R)
     if (O->time_budget_ms > 0 && ms_since() >= O->time_budget_ms) break;
@@ -478,6 +487,7 @@ extern "C" int32_t orc_plan(const orc_problem* P, const orc_plan_opts* O, orc_tr
       R->iterations += 1;
       R->children += BK;
       R->inserted += dbg.n_inserted;
+      for (int ph = 0; ph < 3; ++ph) R->phase_ms[ph] += dbg.phase_ms[ph];
       if (goal) {  // l.14-17
         c_best = dbg.new_c_best;
         if (extract_path(P, T, dbg.goal_node, R)) status = 1;

@@ -115,6 +115,8 @@ typedef struct {
   int64_t n_inserted;   /* out */
   int64_t goal_node;    /* out: node id of the winner or -1 */
   double new_c_best;    /* out: c_best after the iteration */
+  double phase_ms[3];   /* out: wall time of this trip spent in l.6-7 (sample + nearest neighbour), l.8-12 (controls,
+                           propagate, validity, prune, goal test), l.13-15 (insert, goal winner); timing only */
 } orc_iter_debug;
 
 void orc_tree_reset(const orc_problem* P, orc_tree* T);            /* Alg. 1 l.4 */
@@ -140,6 +142,7 @@ typedef struct {
   double* replan_cost;  /* [n_replans] c_best after each replan (inf if none) or NULL */
   int64_t* replan_nodes;/* [n_replans] tree size at the end of each replan or NULL    */
   int64_t* replan_iters;/* [n_replans] or NULL */
+  double phase_ms[3];   /* sums of orc_iter_debug.phase_ms over every iteration of the call */
 } orc_plan_result;
 
 int32_t orc_plan(const orc_problem* P, const orc_plan_opts* O, orc_tree* T, orc_plan_result* R);

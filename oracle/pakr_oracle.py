@@ -57,7 +57,8 @@ class _IterDebug(C.Structure):
     _fields_ = [("x_rand", _dp), ("nn_idx", _ip), ("nn_d2", _dp), ("child_state", _dp),
                 ("child_ctrl", _dp), ("child_cost", _dp), ("child_flags", _ip),
                 ("child_margin", _dp), ("prune_margin", _dp), ("goal_margin", _dp),
-                ("n_inserted", C.c_int64), ("goal_node", C.c_int64), ("new_c_best", C.c_double)]
+                ("n_inserted", C.c_int64), ("goal_node", C.c_int64), ("new_c_best", C.c_double),
+                ("phase_ms", C.c_double * 3)]
 
 
 class _PlanOpts(C.Structure):
@@ -74,7 +75,7 @@ class _PlanResult(C.Structure):
                 ("iterations", C.c_int64), ("children", C.c_int64), ("inserted", C.c_int64),
                 ("replans_run", C.c_int32), ("replans_solved", C.c_int32),
                 ("first_solution_ms", C.c_double), ("total_ms", C.c_double),
-                ("replan_cost", _dp), ("replan_nodes", _lp), ("replan_iters", _lp)]
+                ("replan_cost", _dp), ("replan_nodes", _lp), ("replan_iters", _lp), ("phase_ms", C.c_double * 3)]
 
 
 F_VALID, F_INBOUNDS, F_COLLFREE, F_NOTPRUNED, F_GOAL, F_INSERTED = 1, 2, 4, 8, 16, 32
@@ -251,7 +252,7 @@ def expand_iteration(op: OracleProblem, tree: OracleTree, seed: int, r: int, it:
     dbg = _IterDebug(_ptr(out["x_rand"]), _ptr(out["nn_idx"], _ip), _ptr(out["nn_d2"]),
                      _ptr(out["child_state"]), _ptr(out["child_ctrl"]), _ptr(out["child_cost"]),
                      _ptr(out["child_flags"], _ip), _ptr(out["child_margin"]), _ptr(out["prune_margin"]),
-                     _ptr(out["goal_margin"]), 0, -1, 0.0)
+                     _ptr(out["goal_margin"]), 0, -1, 0.0, (C.c_double * 3)())
     goal = lib().orc_expand_iteration(op.ref, tree.ref, C.c_uint64(seed), C.c_uint32(r), C.c_uint32(it),
                                       C.c_int32(B), C.c_int32(K), C.c_double(c_best), C.byref(dbg))
     out.update(goal=bool(goal), n_inserted=int(dbg.n_inserted), goal_node=int(dbg.goal_node),
@@ -272,7 +273,7 @@ def plan(op: OracleProblem, seed: int, B: int, K: int, tree_capacity: int, n_rep
     ri = np.zeros(n_replans, np.int64)
     opts = _PlanOpts(seed, B, K, tree_capacity, n_replans, time_budget_ms, max_iters_per_replan, initial_cost_bound)
     res = _PlanResult(_ptr(nodes, _ip), _ptr(states), _ptr(ctrls), path_capacity, 0, 0.0, 0, 0, 0, 0, 0, 0,
-                      0.0, 0.0, _ptr(rc), _ptr(rn, _lp), _ptr(ri, _lp))
+                      0.0, 0.0, _ptr(rc), _ptr(rn, _lp), _ptr(ri, _lp), (C.c_double * 3)())
     status = lib().orc_plan(op.ref, C.byref(opts), tree.ref, C.byref(res))
     L = res.path_len if status == 0 else 0
     return dict(status=status, outcome=int(res.outcome), cost=float(res.cost), path_len=int(res.path_len),
@@ -280,7 +281,8 @@ def plan(op: OracleProblem, seed: int, B: int, K: int, tree_capacity: int, n_rep
                 path_controls=ctrls[:max(L - 1, 0)].copy(), iterations=int(res.iterations),
                 children=int(res.children), inserted=int(res.inserted), replans_run=int(res.replans_run),
                 replans_solved=int(res.replans_solved), first_solution_ms=float(res.first_solution_ms),
-                total_ms=float(res.total_ms), replan_cost=rc, replan_nodes=rn, replan_iters=ri, tree=tree)
+                total_ms=float(res.total_ms), replan_cost=rc, replan_nodes=rn, replan_iters=ri, tree=tree,
+                phase_ms=[float(v) for v in res.phase_ms])
 
 
 def philox4x32_10(ctr, key) -> np.ndarray:

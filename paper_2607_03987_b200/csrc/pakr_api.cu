@@ -529,6 +529,8 @@ extern "C" pakr_status pakr_plan(pakr_planner* pl, const pakr_plan_opts* o, void
   CUDA_TRY(pl, cudaStreamSynchronize(stream));
   // results
   fill_stats(hc, BK, &out->stats);
+  out->stats.h2d_bytes = (int64_t)pl->DP * 4 + 4;
+  out->stats.d2h_bytes = (int64_t)sizeof(Ctrl);
   out->final_tree_nodes = hc->n_nodes;
   out->outcome = hc->solved ? PAKR_SOLVED : PAKR_NO_SOLUTION;
   out->cost = hc->solved ? (double)hc->best_cost : (double)INFINITY;
@@ -559,6 +561,8 @@ extern "C" pakr_status pakr_plan(pakr_planner* pl, const pakr_plan_opts* o, void
   if (out->path_controls && Lp > 1)
     CUDA_TRY(pl, cudaMemcpyAsync(h_ctrls, P.path_controls, (size_t)(Lp - 1) * pl->M * 4, cudaMemcpyDeviceToHost, stream));
   CUDA_TRY(pl, cudaStreamSynchronize(stream));
+  out->stats.d2h_bytes += (out->path_nodes ? (int64_t)Lp * 4 : 0) + (out->path_states ? (int64_t)Lp * pl->D * 4 : 0) +
+                          (out->path_controls && Lp > 1 ? (int64_t)(Lp - 1) * pl->M * 4 : 0);
   if (out->path_nodes) std::memcpy(out->path_nodes, h_nodes, (size_t)Lp * 4);
   if (out->path_states) std::memcpy(out->path_states, h_states, (size_t)Lp * pl->D * 4);
   if (out->path_controls && Lp > 1) std::memcpy(out->path_controls, h_ctrls, (size_t)(Lp - 1) * pl->M * 4);

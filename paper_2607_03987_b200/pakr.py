@@ -16,7 +16,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "libpakr.so")
 _CSRC = os.path.join(_HERE, "csrc")
-_SOURCES = ["pakr_api.cu", "pakr_kernel_inst.cu", "pakr_kernel.cuh", "pakr_device.cuh"]
+_SOURCES = ["pakr_api.cu", "pakr_kernel_inst.cu", "pakr_peak.cu", "pakr_kernel.cuh", "pakr_device.cuh"]
 
 F_VALID, F_INBOUNDS, F_COLLFREE, F_NOTPRUNED, F_GOAL, F_INSERTED = 1, 2, 4, 8, 16, 32
 NN_AUTO, NN_SCAN, NN_INDEX = 0, 1, 2
@@ -50,7 +50,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             stale = True
     if force or stale:
         tag = f".{os.getpid()}.tmp"
-        units = [("pakr_api.cu", [], "api")]
+        units = [("pakr_api.cu", [], "api"), ("pakr_peak.cu", [], "peak")]
         for tier, part in ((0, 0), (0, 1), (1, 0), (1, 1), (2, 0)):
             units.append(("pakr_kernel_inst.cu", [f"-DPAKR_STREAM_TIER={tier}", f"-DPAKR_PART={part}"], f"t{tier}p{part}"))
         objs, procs = [], []
@@ -110,6 +110,7 @@ class _PlanOpts(C.Structure):
 
 class _Stats(C.Structure):
     _fields_ = [("iterations", C.c_int64), ("children", C.c_int64), ("inserted", C.c_int64), ("nn_pairs", C.c_int64),
+                ("h2d_bytes", C.c_int64), ("d2h_bytes", C.c_int64),
                 ("replans_run", C.c_int32), ("replans_solved", C.c_int32), ("termination", C.c_int32),
                 ("replan_stats_truncated", C.c_int32), ("path_truncated", C.c_int32),
                 ("first_solution_ms", C.c_double), ("device_ms", C.c_double), ("phase_ms", C.c_double * 3),
@@ -134,8 +135,13 @@ class _StepArgs(C.Structure):
                 ("n_inserted", C.c_void_p), ("goal_node", C.c_void_p), ("new_c_best", C.c_void_p)]
 
 
+class _Fp32Peak(C.Structure):
+    _fields_ = [("ffma_lane_ops_per_s", C.c_double), ("ffma2_lane_ops_per_s", C.c_double),
+                ("scan_mix_lane_ops_per_s", C.c_double), ("sm_clock_mhz", C.c_double), ("sm_count", C.c_int32)]
+
+
 EXPORTS = ["pakr_create", "pakr_destroy", "pakr_last_error", "pakr_workspace_bytes", "pakr_get_tree_layout",
-           "pakr_plan", "pakr_expand_step", "pakr_read_stats"]
+           "pakr_plan", "pakr_expand_step", "pakr_read_stats", "pakr_measure_fp32_peak"]
 
 _lib = None
 
@@ -163,8 +169,19 @@ def lib():
         L.pakr_read_stats.restype = C.c_int
         L.pakr_read_stats.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.c_size_t, C.c_void_p,
                                       C.POINTER(_Stats)]
+        L.pakr_measure_fp32_peak.restype = C.c_int
+        L.pakr_measure_fp32_peak.argtypes = [C.c_int, C.POINTER(_Fp32Peak)]
         _lib = L
     return _lib
+
+
+def measure_fp32_peak(device: int = 0) -> dict:
+    """pakr_measure_fp32_peak: sustained FFMA / FFMA2 / scan-mix lane-ops per second of the device."""
+    out = _Fp32Peak()
+    st = lib().pakr_measure_fp32_peak(device, C.byref(out))
+    if st != 0:
+        raise PakrError(st, "pakr_measure_fp32_peak failed")
+    return {k: getattr(out, k) for k, _ in _Fp32Peak._fields_}
 
 
 def _f32(a) -> np.ndarray:
@@ -260,7 +277,8 @@ class Planner:
         return dict(outcome=int(res.outcome), cost=float(res.cost), path_len=L, path_nodes=nodes[:L].copy(),
                     path_states=states[:L].copy(), path_controls=ctrls[:max(L - 1, 0)].copy(),
                     final_tree_nodes=int(res.final_tree_nodes), iterations=int(s.iterations), children=int(s.children),
-                    inserted=int(s.inserted), nn_pairs=int(s.nn_pairs), replans_run=int(s.replans_run), replans_solved=int(s.replans_solved),
+                    inserted=int(s.inserted), nn_pairs=int(s.nn_pairs), h2d_bytes=int(s.h2d_bytes),
+                    d2h_bytes=int(s.d2h_bytes), replans_run=int(s.replans_run), replans_solved=int(s.replans_solved),
                     termination=int(s.termination), first_solution_ms=float(s.first_solution_ms),
                     device_ms=float(s.device_ms), phase_ms=[float(v) for v in s.phase_ms], replan_cost=np.array(s.replan_cost[:R], np.float32),
                     replan_nodes=np.array(s.replan_nodes[:R], np.int64), replan_iters=np.array(s.replan_iters[:R], np.int64),

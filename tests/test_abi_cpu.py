@@ -16,7 +16,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def _declared_functions():
     text = open(os.path.join(ROOT, "include", "pakr.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(pakr_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(pakr_[a-z0-9_]+)\s*\(", text)))
 
 
 def test_library_exports_every_declared_symbol():
@@ -39,7 +39,8 @@ def test_sass_is_sm100a_with_tma():
 
 
 _STRUCTS = {"pakr_problem": "_Problem", "pakr_tree_layout": "_TreeLayout", "pakr_plan_opts": "_PlanOpts",
-            "pakr_stats": "_Stats", "pakr_result": "_Result", "pakr_step_args": "_StepArgs"}
+            "pakr_stats": "_Stats", "pakr_result": "_Result", "pakr_step_args": "_StepArgs",
+            "pakr_fp32_peak": "_Fp32Peak"}
 
 
 def _header_fields(name):
