@@ -258,7 +258,8 @@ def summarize(results, dev_ms, wall):
             "replans_solved_per_step": float(np.mean([r["replans_solved"] for r in results])),
             "replans_run_per_step": float(np.mean([r["replans_run"] for r in results])),
             "phase_share": {k: sum(r["phase_ms"][i] for r in results) / kern
-                            for i, k in enumerate(("nn_scan_phases", "propagate_and_nn_lookahead", "insert_phases"))},
+                            for i, k in enumerate(("nn_phases", "propagate_and_nn_lookahead", "insert_phases",
+                                                   "nn_index_rebuilds"))},
             "inserted_nodes_per_s": sum(r["inserted"] for r in results) / (sum(dev_ms) * 1e-3),
             "solved": sum(r["outcome"] for r in results)}
 

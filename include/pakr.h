@@ -144,6 +144,8 @@ typedef struct {
   int64_t children;        /* = iterations * B * K propagated and checked ("expanded nodes") */
   int64_t inserted;        /* nodes appended over all replans */
   int64_t nn_pairs;        /* sum over iterations of B * n: the (query, node) pairs of the NN definition */
+  int64_t nn_pairs_evaluated; /* distances actually evaluated: = nn_pairs under the scan tiers, fewer when the NN
+                              index answered (it scores only rows whose bounding box can beat the running best) */
   int64_t h2d_bytes, d2h_bytes; /* bytes pakr_plan copied host->device (root node) and device->host (control
                                    block, path) in this call; kernel parameters (~1.3 KB) not counted */
   int32_t replans_run, replans_solved;
@@ -153,9 +155,10 @@ typedef struct {
                               but could not be extracted; pakr_result then holds the last path that fit and ITS cost */
   double first_solution_ms;/* device time from kernel start to the end of the first solved replan; -1 if none */
   double device_ms;        /* device time of the whole loop (%globaltimer) */
-  double phase_ms[3];      /* CTA 0's time in: separate NN (tail) scan phases / the propagate phase (with the next
-                              iteration's NN look-ahead scan beside it and, when children are few, the insert
-                              inside it) / insert phases of their own; each incl. its grid barrier */
+  double phase_ms[4];      /* CTA 0's time in: NN phases of their own (whole-tree NN at the head of an iteration, scans
+                              of rows added since the look-ahead) / the propagate phase (with the next iteration's NN
+                              look-ahead beside it and, when children are few, the insert inside it) / insert phases
+                              of their own / rebuilds of the NN index; each incl. its grid barriers */
   /* first PAKR_MAX_REPLAN_STATS replans: */
   float replan_cost[PAKR_MAX_REPLAN_STATS];   /* c_best after the replan (+INF before any solution) */
   int32_t replan_nodes[PAKR_MAX_REPLAN_STATS];/* tree size at its end */

@@ -41,6 +41,7 @@ extern "C" const void* pakr_select_kernel_t0_1(int dyn, int obs);
 extern "C" const void* pakr_select_kernel_t1_0(int dyn, int obs);
 extern "C" const void* pakr_select_kernel_t1_1(int dyn, int obs);
 extern "C" const void* pakr_select_kernel_t2_0(int dyn, int obs);
+extern "C" const void* pakr_select_kernel_t2_1(int dyn, int obs);
 
 static const void* pakr_select_kernel_tiled(int dyn, int obs) {
   const void* k = pakr_select_kernel_t0_0(dyn, obs);
@@ -50,7 +51,10 @@ static const void* pakr_select_kernel_stream(int dyn, int obs) {
   const void* k = pakr_select_kernel_t1_0(dyn, obs);
   return k ? k : pakr_select_kernel_t1_1(dyn, obs);
 }
-static const void* pakr_select_kernel_index(int dyn, int obs) { return pakr_select_kernel_t2_0(dyn, obs); }
+static const void* pakr_select_kernel_index(int dyn, int obs) {
+  const void* k = pakr_select_kernel_t2_0(dyn, obs);
+  return k ? k : pakr_select_kernel_t2_1(dyn, obs);
+}
 
 namespace {
 
@@ -59,7 +63,8 @@ size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
   size_t states, actions, parents, costs, nn_key, unit_count, scr_state, scr_ctrl, scr_cost, scr_parent,
-      scr_flags, idx_ids, idx_start, idx_cnt, ctrl, path_rev, path_nodes, path_states, path_controls, total;
+      scr_flags, idx_keys, idx_ids, idx_hist, idx_ctasum, idx_tile_ids, idx_rows, idx_tlo, idx_thi, idx_slo, idx_shi,
+      ctrl, path_rev, path_nodes, path_states, path_controls, total;
 };
 
 Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap) {
@@ -73,9 +78,22 @@ Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap) {
   L.costs = take((size_t)cap * 4);
   L.nn_key = take((size_t)B * 16);  // two iterations in flight
   L.unit_count = take(std::max<size_t>(U, kFuseUnits + 8) * 4);
-  L.idx_ids = take((size_t)cap * 4);
-  L.idx_start = take((size_t)(kIdxMaxCells + 1) * 4);
-  L.idx_cnt = take((size_t)kIdxMaxCells * 4);
+  {  // NN index; nothing when the problem cannot be indexed
+    const size_t on = pl->index_ok ? 1 : 0;
+    const IdxDims G = idx_dims((int)cap);
+    const size_t grid_warps = (size_t)pl->num_sms * kCtasPerSm * kWarps;
+    const size_t sort_warps = std::min<size_t>(grid_warps, (size_t)cap / kIdxChunkMin + 1);
+    L.idx_keys = take(on * 2 * cap * 4);
+    L.idx_ids = take(on * 2 * cap * 4);
+    L.idx_hist = take(on * kIdxBins * sort_warps * 4);
+    L.idx_ctasum = take(on * pl->num_sms * kCtasPerSm * 4);
+    L.idx_tile_ids = take(on * (size_t)G.n_super * 1024 * 4);
+    L.idx_rows = take(on * (size_t)G.n_super * 1024 * pl->D * 4);
+    L.idx_tlo = take(on * (size_t)G.n_super * pl->D * 32 * 4);
+    L.idx_thi = take(on * (size_t)G.n_super * pl->D * 32 * 4);
+    L.idx_slo = take(on * (size_t)G.n_groups * pl->D * 32 * 4);
+    L.idx_shi = take(on * (size_t)G.n_groups * pl->D * 32 * 4);
+  }
   L.scr_state = take(slots * pl->DP * 4);
   L.scr_ctrl = take(slots * 16);
   L.scr_cost = take(slots * 4);
@@ -174,6 +192,44 @@ HostGrid build_grid(const pakr_problem* p, int obs_kind) {
     return g;
   }
   return g;
+}
+
+// Morton key layout of the NN index: 30 key bits are dealt out one at a time, always to the dimension whose weighted
+// cell (hi - lo) sqrt(w) / 2^bits is widest at that moment -- the split order of a kd-tree over the weighted state
+// box.  Keyed: non-angle dimensions with a finite box of positive width and a positive weight.  Returns false if
+// no dimension can be keyed (the index tier is then unavailable for the problem).
+bool idx_key_layout(DevProblem& pb, int D, int angle_dim) {
+  double cell[kMaxD];
+  int bits[kMaxD] = {0};
+  bool any = false;
+  for (int d = 0; d < D; ++d) {
+    const bool ok = d != angle_dim && std::isfinite(pb.lo[d]) && std::isfinite(pb.hi[d]) && pb.hi[d] > pb.lo[d] && pb.w[d] > 0.0f;
+    cell[d] = ok ? ((double)pb.hi[d] - pb.lo[d]) * std::sqrt((double)pb.w[d]) : 0.0;
+    any = any || ok;
+  }
+  if (!any) return false;
+  int order[kIdxDigitBits * kIdxPasses];
+  int total = 0;
+  for (; total < kIdxDigitBits * kIdxPasses; ++total) {
+    int best = -1;
+    for (int d = 0; d < D; ++d)
+      if (cell[d] > 0.0 && bits[d] < 16 && (best < 0 || cell[d] > cell[best])) best = d;
+    if (best < 0) break;
+    order[total] = best;
+    ++bits[best];
+    cell[best] *= 0.5;
+  }
+  int taken[kMaxD] = {0};
+  for (int i = 0; i < total; ++i) {  // i-th dealt bit: key position total-1-i, the dimension's next bit from its top
+    const int d = order[i];
+    pb.idx_pos[d][bits[d] - 1 - taken[d]] = (uint8_t)(total - 1 - i);
+    ++taken[d];
+  }
+  for (int d = 0; d < D; ++d) {
+    pb.idx_bits[d] = (uint8_t)bits[d];
+    pb.idx_scale[d] = bits[d] ? (float)((double)(1 << bits[d]) / ((double)pb.hi[d] - pb.lo[d])) : 0.0f;
+  }
+  return true;
 }
 
 pakr_status fail(pakr_planner* pl, pakr_status st, const std::string& msg) {
@@ -308,12 +364,7 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
   pb.dt = p->dt; pb.S = p->steps_per_edge; pb.integrator = p->integrator; pb.cost_mode = p->cost_mode;
   pb.inv_hspeed = std::isinf(p->heuristic_speed) ? 0.0f : 1.0f / p->heuristic_speed;
   pb.unit_weights = unit ? 1 : 0;
-  {
-    bool ok = true;
-    for (int a = 0; a < PD; ++a)
-      ok = ok && std::isfinite(pb.lo[a]) && std::isfinite(pb.hi[a]) && pb.hi[a] > pb.lo[a] && pb.w[a] > 0.0f;
-    pl->index_ok = ok;  // the tier itself is chosen per call (pakr_plan_opts.nn_mode / pakr_step_args.nn_mode)
-  }
+  pl->index_ok = idx_key_layout(pb, D, angle);  // the tier is chosen per call (pakr_plan_opts.nn_mode)
   pb.n_obs = p->n_obstacles;
 
   // obstacle table in the kernel's shared-memory row format
@@ -420,9 +471,16 @@ void fill_common(const pakr_planner* pl, Params& P, const Layout& L, char* ws, i
   P.pb = pl->pb;
   P.nn_key = reinterpret_cast<unsigned long long*>(ws + L.nn_key);
   P.unit_count = reinterpret_cast<unsigned*>(ws + L.unit_count);
+  P.idx_keys = reinterpret_cast<unsigned*>(ws + L.idx_keys);
   P.idx_ids = reinterpret_cast<int*>(ws + L.idx_ids);
-  P.idx_start = reinterpret_cast<int*>(ws + L.idx_start);
-  P.idx_cnt = reinterpret_cast<int*>(ws + L.idx_cnt);
+  P.idx_hist = reinterpret_cast<unsigned*>(ws + L.idx_hist);
+  P.idx_ctasum = reinterpret_cast<unsigned*>(ws + L.idx_ctasum);
+  P.idx_tile_ids = reinterpret_cast<int*>(ws + L.idx_tile_ids);
+  P.idx_rows = reinterpret_cast<float*>(ws + L.idx_rows);
+  P.idx_tlo = reinterpret_cast<float*>(ws + L.idx_tlo);
+  P.idx_thi = reinterpret_cast<float*>(ws + L.idx_thi);
+  P.idx_slo = reinterpret_cast<float*>(ws + L.idx_slo);
+  P.idx_shi = reinterpret_cast<float*>(ws + L.idx_shi);
   P.scr_state = reinterpret_cast<float*>(ws + L.scr_state);
   P.scr_ctrl = reinterpret_cast<float*>(ws + L.scr_ctrl);
   P.scr_cost = reinterpret_cast<float*>(ws + L.scr_cost);
@@ -443,7 +501,8 @@ void fill_stats(const Ctrl* hc, int64_t BK, pakr_stats* out) {
   s.children = hc->iterations * BK;
   s.inserted = hc->inserted;
   s.nn_pairs = hc->nn_pairs;
-  for (int i = 0; i < 3; ++i) s.phase_ms[i] = (double)hc->phase_ns[i] * 1e-6;
+  s.nn_pairs_evaluated = hc->nn_pairs - hc->nn_idx_covered + (int64_t)hc->nn_scored;
+  for (int i = 0; i < 4; ++i) s.phase_ms[i] = (double)hc->phase_ns[i] * 1e-6;
   s.replans_run = hc->replans_run;
   s.replans_solved = hc->replans_solved;
   s.termination = hc->termination;
@@ -463,7 +522,7 @@ void fill_stats(const Ctrl* hc, int64_t BK, pakr_stats* out) {
 // nn_mode (PAKR_NN_*) -> Params::nn_index
 bool set_nn_mode(pakr_planner* pl, Params& P, int nn_mode) {
   if (nn_mode != PAKR_NN_AUTO && nn_mode != PAKR_NN_SCAN && nn_mode != PAKR_NN_INDEX) return false;
-  constexpr int kAutoIndex = 0;  // what PAKR_NN_AUTO means for the index: 0 never, 1 when B*n is large
+  constexpr int kAutoIndex = 1;  // what PAKR_NN_AUTO means for the index: 1 = when B*n is large enough to pay
   P.nn_index = !pl->index_ok ? 0 : nn_mode == PAKR_NN_INDEX ? 2 : nn_mode == PAKR_NN_AUTO ? kAutoIndex : 0;
   return true;
 }

@@ -54,6 +54,10 @@ struct DevProblem {
   int g_cells, g_list;                 // number of cells, total list entries
   const uint32_t* grid_cells;          // DEVICE [g_cells]: cell words, see cell_margin()
   const uint16_t* grid_list;           // DEVICE [g_list] obstacle ids
+  // NN index: Morton key layout over the weighted state box (pakr_api.cu: idx_key_layout)
+  float idx_scale[kMaxD];              // quantised coordinate = floor((x - lo) * scale), 0 .. 2^bits - 1
+  uint8_t idx_bits[kMaxD];             // key bits of every dimension (0: not keyed)
+  uint8_t idx_pos[kMaxD][16];          // key position of bit b of the dimension's quantised coordinate
 };
 
 // ---- Philox4x32-10 ---------------------------------------------------------------------------

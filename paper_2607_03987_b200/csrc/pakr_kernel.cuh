@@ -29,9 +29,10 @@ constexpr int kThreads = 256;    // 256 x 2 CTAs per SM measured 1.4x faster in 
 constexpr int kCtasPerSm = 2;
 constexpr int kWarps = kThreads / 32;
 constexpr int kQ = 4;            // queries per lane in the NN scan
-constexpr int kIdxMaxCells = 16384;  // cells of the NN index (resolution chosen from the tree size at every rebuild)
-constexpr int kIdxMinRows = 4096;    // smaller trees are scanned
-constexpr long long kIdxMinPairs = 120000000ll;  // ... and so are iterations whose scan (B*n pairs) takes < ~60 us
+constexpr int kIdxMinRows = 4096;    // NN index: smaller trees are scanned
+constexpr long long kIdxMinPairs = 60000000ll;  // ... and so are iterations whose scan (B*n pairs) takes < ~30 us
+constexpr long long kIdxRebuildWork = 400000000ll;  // rebuild once scanning the rows added since the last rebuild costs
+                                                    // about as much as rebuilding: B * rows * D lane-ops (~50 us)
 constexpr int kPathMax = 8192;   // longest path the device buffers hold
 constexpr int kStatsMax = 64;
 constexpr unsigned long long kKeyNone = ~0ull;
@@ -45,11 +46,14 @@ struct Ctrl {  // device control block (in the workspace)
   unsigned long long goal_key[kSlots];  // min (cost bits, node) over the goal children inserted in the iteration
   unsigned long long t_start_ns, t_first_ns, t_end_ns;
   long long iterations, inserted, nn_pairs;
-  unsigned long long phase_ns[3];  // leader's time in NN / propagate / insert incl. the grid sync after each
+  unsigned long long nn_scored;  // (query, row) pairs the NN index tier scored, summed over its warps
+  long long nn_idx_covered;      // sum over iterations of B * (rows the index answered for): pairs NOT scanned
+  unsigned long long phase_ns[4];  // leader's time in NN / propagate / insert (incl. the grid sync after each) / index rebuilds
   int n_nodes;
   int stop[kSlots];        // 1: the time budget ran out during the iteration (written by the leader every iteration)
   unsigned pbar;           // arrival counter of the barrier among the propagate CTAs (insert inside phase X)
   int iter_total[kSlots];  // survivors of the iteration, published by CTA 0 when the insert ran inside phase X
+  int idx_query[2][kSlots];// NN index tier: next query to hand out ([0] whole-tree NN of the iteration, [1] look-ahead)
   int path_len, solved;
   int path_overflow;       // a solved replan's path was longer than kPathMax and was not extracted
   float path_cost;         // cost of the path held in the path buffers
@@ -69,9 +73,14 @@ struct Params {
   unsigned long long* nn_key;  // [2][B] (d2 bits << 32) | node, combined with atomicMin; two iterations in flight
   // NN cell index (exact spatial pruning): tree rows [0, n_sorted) bucketed by position cell
   int nn_index;                // 0: scan tiers only; 1: index when B*n is large; 2: index whenever n >= 256 (tests)
-  int* idx_ids;                // [cap] row ids ordered by cell
-  int* idx_start;              // [kIdxMaxCells + 1] first slot of every cell
-  int* idx_cnt;                // [kIdxMaxCells] histogram / scatter cursors
+  unsigned* idx_keys;          // [2][cap] Morton keys (radix-sort ping-pong)
+  int* idx_ids;                // [2][cap] row ids, sorted together with the keys
+  unsigned* idx_hist;          // [kIdxBins][sorting warps] digit histogram / scatter offsets
+  unsigned* idx_ctasum;        // [CTAs] partial sums of the histogram scan
+  int* idx_tile_ids;           // [tiles][32] row id of every tile slot (-1: padding)
+  float* idx_rows;             // [tiles][D][32] the sorted rows, dimension-major inside a tile
+  float* idx_tlo; float* idx_thi;  // [super-tiles][D][32] boxes of the tiles
+  float* idx_slo; float* idx_shi;  // [groups][D][32] boxes of the super-tiles
   unsigned* unit_count;        // [ceil(B*K/32)] survivors per warp unit
   float* scr_state; float* scr_ctrl; float* scr_cost; int* scr_parent; int* scr_flags;
   Ctrl* ctrl;
@@ -337,154 +346,35 @@ __device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, u
 }
 
 // ---- NN index tier: exact nearest neighbour with spatial pruning ----------
-// Tree rows [0, n_sorted) are bucketed by a uniform grid over the POSITION dims (counting sort, rebuilt when the
-// tree has grown by an eighth).  A warp answers one query: it visits the cells of growing Chebyshev rings around
-// the query's cell, lanes gather rows by id and evaluate the same distance as the scan tiers, and it stops after
-// ring r as soon as best d2 < min_a w_a (r * cell_a)^2: every row outside the visited cube differs by more than
-// r cells on some position axis, so none can be nearer (exact; ties go to the lowest node id through the
-// (d2, id) key as everywhere).  Rows appended since the last rebuild are scanned by the tiled tier.
-struct IdxGeom {
-  int g[3];          // cells per position axis (g[2] = 1 in 2-D)
-  float inv[3];      // cells per unit length
-  float lb[3];       // w_a * (cell_a * (1 - 1e-4))^2: lower-bound coefficient per axis
-  int cells;
+// RRT trees are strongly clustered, so the structure is BALANCED: tree rows [0, n_sorted) are sorted by a Morton
+// key over the weighted state box (the host decides how many bits every dimension gets: always the dimension whose
+// weighted cell is widest next, DevProblem::idx_*) and cut into tiles of 32 consecutive rows; a tile knows the
+// bounding box of its rows over every non-angle dimension, 32 tiles form a super-tile with the box of their union.
+// Dense regions get many small boxes, empty space gets none.
+//   rebuild  keys -> LSD radix sort (3 passes of 10 bits: per-warp histograms, grid-wide exclusive scan, stable
+//            per-warp scatter) -> tiles: rows copied as [tile][dim][32] so that a lane reads its row with
+//            coalesced loads -> tile boxes -> super-tile boxes.  Runs when the tree has grown by a sixteenth.
+//   search   one warp per query.  A lower bound of the weighted squared distance from the query to a box is
+//            sum_d w_d max(0, lo_d - q_d, q_d - hi_d)^2.  Pass A walks the super-tile boxes (one per lane), descends
+//            into the nearest one and scores its nearest tile: the exact distance of a real row, an upper bound ub.
+//            Pass B walks the super-tile boxes again and opens only boxes whose bound (shrunk by 1e-5 against
+//            fp32 rounding) does not exceed ub; every scored tile tightens ub.  A row is skipped only if its box
+//            bound is strictly above the final minimum, so the result -- min over (d2 bits, row id) with the same
+//            dist2() arithmetic as the scan tiers -- is bit-identical to the brute-force scan, ties included.
+// Rows appended since the last rebuild are scanned by the tiled tier; atomicMin merges the two partial results.
+constexpr int kIdxDigitBits = 10, kIdxBins = 1 << kIdxDigitBits, kIdxPasses = 3;  // 30-bit keys
+constexpr int kIdxChunkMin = 512;    // rows per sorting warp at least (keeps the histogram table <= 2n entries)
+constexpr float kIdxShrink = 1.0f - 1e-5f;
+
+struct IdxDims {  // sizes of the index over n rows
+  int n_tiles, n_super, n_groups;
 };
-
-template <int PD>
-__device__ __forceinline__ IdxGeom idx_geometry(const DevProblem& pb, int n) {
-  IdxGeom G;
-  // about 12 rows per cell, at most kIdxMaxCells cells
-  int target = max(n / 12, 64);
-  if (target > kIdxMaxCells) target = kIdxMaxCells;
-  int side = 2;
-  if (PD == 2) { while ((side + 1) * (side + 1) <= target) ++side; }
-  else { while ((side + 1) * (side + 1) * (side + 1) <= target) ++side; }
-  G.cells = 1;
-#pragma unroll
-  for (int a = 0; a < 3; ++a) {
-    G.g[a] = a < PD ? side : 1;
-    const float ext = a < PD ? (pb.hi[a] - pb.lo[a]) : 1.0f;
-    G.inv[a] = (float)G.g[a] / ext;
-    const float cs = ext / (float)G.g[a] * 0.9999f;
-    G.lb[a] = a < PD ? pb.w[a] * cs * cs : __int_as_float(0x7f800000);
-    G.cells *= G.g[a];
-  }
-  return G;
-}
-
-template <int PD>
-__device__ __forceinline__ void idx_cell_coords(const DevProblem& pb, const IdxGeom& G, const float* pos, int (&c)[3]) {
-#pragma unroll
-  for (int a = 0; a < 3; ++a) {
-    int v = a < PD ? __float2int_rd((pos[a] - pb.lo[a]) * G.inv[a]) : 0;
-    c[a] = min(max(v, 0), G.g[a] - 1);
-  }
-}
-
-// Counting sort of rows [0, n) by cell; four grid-wide steps.  Within a cell the order is whatever the atomics
-// give: the search reduces with the (d2, id) key, so results do not depend on it.
-template <int DYN>
-__device__ __forceinline__ void idx_rebuild(const Params& P, const IdxGeom& G, int n, cg::grid_group& grid, int* sm_scan) {
-  using T = DynTraits<DYN>;
-  const int tid = blockIdx.x * kThreads + threadIdx.x, nth = gridDim.x * kThreads;
-  for (int c = tid; c < G.cells; c += nth) P.idx_cnt[c] = 0;
-  grid.sync();
-  for (int row = tid; row < n; row += nth) {
-    float pos[3] = {0.f, 0.f, 0.f};
-    const float4 a = __ldcg(reinterpret_cast<const float4*>(P.states + (size_t)row * T::DP));
-    pos[0] = a.x; pos[1] = a.y; pos[2] = a.z;
-    int c[3];
-    idx_cell_coords<T::PD>(P.pb, G, pos, c);
-    atomicAdd(&P.idx_cnt[c[0] + G.g[0] * (c[1] + G.g[1] * c[2])], 1);
-  }
-  grid.sync();
-  if (blockIdx.x == 0) {  // exclusive scan of the histogram by one CTA (<= 16384 cells)
-    const int per = (G.cells + kThreads - 1) / kThreads;
-    const int c0 = threadIdx.x * per, c1 = min(G.cells, c0 + per);
-    int sum = 0;
-    for (int c = c0; c < c1; ++c) sum += __ldcg(&P.idx_cnt[c]);
-    sm_scan[threadIdx.x] = sum;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      int run = 0;
-      for (int t = 0; t < kThreads; ++t) { const int v = sm_scan[t]; sm_scan[t] = run; run += v; }
-      P.idx_start[G.cells] = run;
-    }
-    __syncthreads();
-    int run = sm_scan[threadIdx.x];
-    for (int c = c0; c < c1; ++c) {
-      const int v = __ldcg(&P.idx_cnt[c]);
-      P.idx_start[c] = run;
-      P.idx_cnt[c] = run;  // scatter cursor
-      run += v;
-    }
-  }
-  __threadfence();
-  grid.sync();
-  for (int row = tid; row < n; row += nth) {
-    float pos[3] = {0.f, 0.f, 0.f};
-    const float4 a = __ldcg(reinterpret_cast<const float4*>(P.states + (size_t)row * T::DP));
-    pos[0] = a.x; pos[1] = a.y; pos[2] = a.z;
-    int c[3];
-    idx_cell_coords<T::PD>(P.pb, G, pos, c);
-    const int slot = atomicAdd(&P.idx_cnt[c[0] + G.g[0] * (c[1] + G.g[1] * c[2])], 1);
-    P.idx_ids[slot] = row;
-  }
-  __threadfence();
-  grid.sync();
-}
-
-// Scores the rows of up to 32 contiguous slices of idx_ids (one slice per lane: beg, cnt) against q.  Four 32-row
-// batches are in flight at a time (ids first, then rows), so the dependent L2 round trips overlap.
-template <int DYN, bool UNIT_W>
-__device__ __forceinline__ void idx_score_slices(const Params& P, const float (&q)[DynTraits<DYN>::D], int beg, int cnt,
-                                                 unsigned long long& best) {
-  constexpr int DP = DynTraits<DYN>::DP;
-  const int lane = threadIdx.x & 31;
-  int incl = cnt;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    const int t = __shfl_up_sync(0xffffffffu, incl, o);
-    if (lane >= o) incl += t;
-  }
-  const int total = __shfl_sync(0xffffffffu, incl, 31);
-  for (int j0 = 0; j0 < total; j0 += 128) {
-    int slot[4];
-#pragma unroll
-    for (int b = 0; b < 4; ++b) {
-      const int k = j0 + b * 32 + lane;
-      int lo = 0, hi = 31;  // owner = first lane whose inclusive count exceeds k
-#pragma unroll
-      for (int step = 0; step < 5; ++step) {
-        const int mid = (lo + hi) >> 1;
-        const int v = __shfl_sync(0xffffffffu, incl, mid);
-        if (v > k) hi = mid; else lo = mid + 1;
-      }
-      const int o_incl = __shfl_sync(0xffffffffu, incl, lo), o_cnt = __shfl_sync(0xffffffffu, cnt, lo),
-                o_beg = __shfl_sync(0xffffffffu, beg, lo);
-      slot[b] = k < total ? o_beg + (k - (o_incl - o_cnt)) : -1;
-    }
-    int id[4];
-#pragma unroll
-    for (int b = 0; b < 4; ++b) id[b] = slot[b] >= 0 ? __ldcg(&P.idx_ids[slot[b]]) : -1;
-    float4 rowv[4][DP / 4];
-#pragma unroll
-    for (int b = 0; b < 4; ++b) {
-      const float4* sp = reinterpret_cast<const float4*>(P.states + (size_t)max(id[b], 0) * DP);
-#pragma unroll
-      for (int v = 0; v < DP / 4; ++v) rowv[b][v] = __ldcg(sp + v);
-    }
-#pragma unroll
-    for (int b = 0; b < 4; ++b) {
-      float p[DP];
-#pragma unroll
-      for (int v = 0; v < DP / 4; ++v) {
-        p[4 * v] = rowv[b][v].x; p[4 * v + 1] = rowv[b][v].y; p[4 * v + 2] = rowv[b][v].z; p[4 * v + 3] = rowv[b][v].w;
-      }
-      const float d2 = dist2<DYN, UNIT_W>(P.pb, q, p);
-      if (id[b] >= 0) best = min(best, ((unsigned long long)__float_as_uint(d2) << 32) | (unsigned)id[b]);
-    }
-  }
+__host__ __device__ __forceinline__ IdxDims idx_dims(int n) {
+  IdxDims d;
+  d.n_tiles = (n + 31) / 32;
+  d.n_super = (d.n_tiles + 31) / 32;
+  d.n_groups = (d.n_super + 31) / 32;
+  return d;
 }
 
 __device__ __forceinline__ unsigned long long warp_min_key(unsigned long long m) {
@@ -493,77 +383,334 @@ __device__ __forceinline__ unsigned long long warp_min_key(unsigned long long m)
   return m;
 }
 
-// One warp, one query (all lanes hold the same q): exact NN over the indexed rows.
-//   stage 1: the query's cell and its neighbours (Chebyshev radius 1); if nothing is there, 64 rows spread evenly
-//            over the cell-ordered id list stand in.  Either way `best` is now the exact distance of a real row:
-//            an upper bound.
-//   stage 2: only rows with |p_a - q_a| <= sqrt(best / w_a) on every position axis can beat it, i.e. rows in the
-//            box of cells within ceil(sqrt(best / w_a) / cell_a) of the query's cell.  That box is visited in one
-//            pass, (y, z) column by column; cells being x-fastest, a column is ONE contiguous slice of idx_ids.
-template <int DYN, bool UNIT_W>
-__device__ __forceinline__ unsigned long long idx_search(const Params& P, const IdxGeom& G, int n_sorted,
-                                                         const float (&q)[DynTraits<DYN>::D]) {
-  using T = DynTraits<DYN>;
-  constexpr int DP = T::DP, PD = T::PD;
-  const int lane = threadIdx.x & 31;
-  int qc[3];
-  {
-    float pos[3] = {q[0], q[1], PD == 3 ? q[2] : 0.0f};
-    idx_cell_coords<PD>(P.pb, G, pos, qc);
-  }
-  unsigned long long best = kKeyNone;
-  int rad[3] = {1, 1, PD == 3 ? 1 : 0};  // half-widths of the box of cells, per axis
-  for (int stage = 0; stage < 2; ++stage) {
-    const int y0 = max(qc[1] - rad[1], 0), y1 = min(qc[1] + rad[1], G.g[1] - 1);
-    const int z0 = max(qc[2] - rad[2], 0), z1 = min(qc[2] + rad[2], G.g[2] - 1);
-    const int x0 = max(qc[0] - rad[0], 0), x1 = min(qc[0] + rad[0], G.g[0] - 1);
-    const int ny = y1 - y0 + 1, cols = ny * (z1 - z0 + 1);
-    for (int base = 0; base < cols; base += 32) {
-      const int idx = base + lane;
-      int beg = 0, cnt = 0;
-      if (idx < cols) {
-        const int cy = y0 + idx % ny, cz = z0 + idx / ny;
-        const int rowbase = G.g[0] * (cy + G.g[1] * cz);
-        beg = __ldcg(&P.idx_start[rowbase + x0]);
-        cnt = __ldcg(&P.idx_start[rowbase + x1 + 1]) - beg;
-      }
-      idx_score_slices<DYN, UNIT_W>(P, q, beg, cnt, best);
-    }
-    best = warp_min_key(best);
-    if (stage == 1) break;
-    if (best == kKeyNone) {  // empty neighbourhood: take the bound from 64 rows spread over the whole index
-      const int k0 = (int)(((long long)n_sorted * (2 * lane)) >> 6), k1 = (int)(((long long)n_sorted * (2 * lane + 1)) >> 6);
-      idx_score_slices<DYN, UNIT_W>(P, q, k0, 1, best);
-      idx_score_slices<DYN, UNIT_W>(P, q, k1, 1, best);
-      best = warp_min_key(best);
-    }
-    // box that can still hold a nearer row; done if it is inside what stage 1 covered
-    const float ub = __uint_as_float((unsigned)(best >> 32));
-    bool inside = true;
+// Morton key of a row: per keyed dimension a quantised coordinate, its bits dealt to the key positions the host chose.
+template <int DYN>
+__device__ __forceinline__ unsigned idx_key(const DevProblem& pb, const float (&x)[DynTraits<DYN>::DP]) {
+  unsigned key = 0;
 #pragma unroll
-    for (int a = 0; a < PD; ++a) {
-      // rows beyond r cells differ by more than r * cell_a * 0.9999 on axis a; need w_a * that^2 > ub to exclude them
-      const float cells_f = sqrtf(ub / G.lb[a]);  // G.lb[a] = w_a * (0.9999 cell_a)^2
-      const int r = min((int)cells_f + 1, G.g[a]);
-      inside = inside && (r <= 1);
-      rad[a] = r;
-    }
-    if (inside) break;
+  for (int d = 0; d < DynTraits<DYN>::D; ++d) {
+    const int nb = pb.idx_bits[d];
+    if (nb == 0) continue;
+    int q = __float2int_rd((x[d] - pb.lo[d]) * pb.idx_scale[d]);
+    q = min(max(q, 0), (1 << nb) - 1);
+    for (int b = 0; b < nb; ++b) key |= (unsigned)((q >> b) & 1) << pb.idx_pos[d][b];
   }
-  return best;
+  return key;
 }
 
+// Grid-wide rebuild over rows [0, n).  sm_hist: kWarps * kIdxBins words (the TMA tile buffers, idle here);
+// sm_scan: kThreads + kWarps + 8 words.
+template <int DYN>
+__device__ __forceinline__ void idx_rebuild(const Params& P, int n, cg::grid_group& grid, unsigned* sm_hist, int* sm_scan) {
+  using T = DynTraits<DYN>;
+  constexpr int D = T::D, DP = T::DP;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int NB = gridDim.x, W = NB * kWarps;
+  // sorting warps: warp 0 of every CTA first, then the warps 1, ... (spread over the SMs when few take part)
+  const int pj = warp * NB + (int)blockIdx.x;
+  int chunk = ((n + W - 1) / W + 31) & ~31;
+  if (chunk < kIdxChunkMin) chunk = kIdxChunkMin;
+  const int Wp = (n + chunk - 1) / chunk;
+  const int cb = min(n, pj * chunk), ce = min(n, cb + chunk);
+  unsigned* h = sm_hist + warp * kIdxBins;
+  // keys of the chunk (buffer 0): the same lanes read them back below, no barrier needed
+  for (int i = cb + lane; i < ce; i += 32) {
+    float x[DP];
+    const float4* sp = reinterpret_cast<const float4*>(P.states + (size_t)i * DP);
+#pragma unroll
+    for (int v = 0; v < DP / 4; ++v) {
+      const float4 a = __ldcg(sp + v);
+      x[4 * v] = a.x; x[4 * v + 1] = a.y; x[4 * v + 2] = a.z; x[4 * v + 3] = a.w;
+    }
+    P.idx_keys[i] = idx_key<DYN>(P.pb, x);
+    P.idx_ids[i] = i;
+  }
+  const int E = kIdxBins * Wp;                                      // histogram table [bin][sorting warp]
+  const int per = (E + NB * kThreads - 1) / (NB * kThreads);        // entries per thread in the scan
+  for (int pass = 0; pass < kIdxPasses; ++pass) {
+    const unsigned* ksrc = P.idx_keys + (size_t)(pass & 1) * P.cap;
+    const int* isrc = P.idx_ids + (size_t)(pass & 1) * P.cap;
+    unsigned* kdst = P.idx_keys + (size_t)((pass & 1) ^ 1) * P.cap;
+    int* idst = P.idx_ids + (size_t)((pass & 1) ^ 1) * P.cap;
+    const int shift = pass * kIdxDigitBits;
+    // 1. per-warp digit histogram
+    if (pj < Wp) {
+      for (int b = lane; b < kIdxBins; b += 32) h[b] = 0;
+      __syncwarp();
+      for (int i = cb + lane; i < ce; i += 32) atomicAdd(&h[(__ldcg(&ksrc[i]) >> shift) & (kIdxBins - 1)], 1u);
+      __syncwarp();
+      for (int b = lane; b < kIdxBins; b += 32) P.idx_hist[(size_t)b * Wp + pj] = h[b];
+    }
+    __threadfence();
+    grid.sync();
+    // 2. exclusive scan of the table: thread sums -> CTA totals -> (barrier) -> offsets written in place
+    const int e0 = min(E, ((int)blockIdx.x * kThreads + (int)threadIdx.x) * per), e1 = min(E, e0 + per);
+    unsigned mine = 0;
+    for (int e = e0; e < e1; ++e) mine += __ldcg(&P.idx_hist[e]);
+    unsigned incl = mine;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned t = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += t;
+    }
+    __syncthreads();
+    if (lane == 31) sm_scan[kThreads + warp] = (int)incl;
+    __syncthreads();
+    unsigned wbase = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < kWarps; ++w) {
+      const unsigned t = (unsigned)sm_scan[kThreads + w];
+      if (w < warp) wbase += t;
+      total += t;
+    }
+    if (threadIdx.x == 0) P.idx_ctasum[blockIdx.x] = total;
+    __threadfence();
+    grid.sync();
+    unsigned before = 0;  // sum of the totals of the CTAs before this one
+    for (int c = (int)threadIdx.x; c < (int)blockIdx.x; c += kThreads) before += __ldcg(&P.idx_ctasum[c]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) before += __shfl_xor_sync(0xffffffffu, before, o);
+    __syncthreads();
+    if (lane == 0) sm_scan[kThreads + warp] = (int)before;
+    __syncthreads();
+    unsigned cta_before = 0;
+#pragma unroll
+    for (int w = 0; w < kWarps; ++w) cta_before += (unsigned)sm_scan[kThreads + w];
+    unsigned run = cta_before + wbase + incl - mine;
+    for (int e = e0; e < e1; ++e) {
+      const unsigned v = __ldcg(&P.idx_hist[e]);
+      P.idx_hist[e] = run;
+      run += v;
+    }
+    __threadfence();
+    grid.sync();
+    // 3. stable scatter: the warp walks its chunk in order, 32 keys at a time
+    if (pj < Wp) {
+      for (int b = lane; b < kIdxBins; b += 32) h[b] = __ldcg(&P.idx_hist[(size_t)b * Wp + pj]);
+      __syncwarp();
+      for (int i0 = cb; i0 < ce; i0 += 32) {
+        const int i = i0 + lane;
+        const bool on = i < ce;
+        const unsigned act = __ballot_sync(0xffffffffu, on);
+        if (on) {
+          const unsigned key = __ldcg(&ksrc[i]);
+          const int id = __ldcg(&isrc[i]);
+          const unsigned dg = (key >> shift) & (kIdxBins - 1);
+          const unsigned m = __match_any_sync(act, dg);
+          const unsigned base = h[dg];
+          const unsigned pos = base + __popc(m & ((1u << lane) - 1u));
+          __syncwarp(act);
+          if ((m >> lane) == 1u) h[dg] = base + __popc(m);  // highest lane of the group
+          kdst[pos] = key;
+          idst[pos] = id;
+        }
+        __syncwarp();
+      }
+    }
+    __threadfence();
+    grid.sync();
+  }
+  // sorted ids are in buffer (kIdxPasses & 1).  Tiles: rows as [tile][dim][32], ids padded with -1, boxes.
+  const int* sorted = P.idx_ids + (size_t)(kIdxPasses & 1) * P.cap;
+  const IdxDims G = idx_dims(n);
+  const int gw = (int)blockIdx.x * kWarps + warp;
+  const float inf = __int_as_float(0x7f800000);
+  for (int t = gw; t < G.n_super * 32; t += W) {
+    const int pos = t * 32 + lane;
+    const int id = pos < n ? __ldcg(&sorted[pos]) : -1;
+    float x[DP];
+    const float4* sp = reinterpret_cast<const float4*>(P.states + (size_t)max(id, 0) * DP);
+#pragma unroll
+    for (int v = 0; v < DP / 4; ++v) {
+      const float4 a = __ldcg(sp + v);
+      x[4 * v] = a.x; x[4 * v + 1] = a.y; x[4 * v + 2] = a.z; x[4 * v + 3] = a.w;
+    }
+    P.idx_tile_ids[pos] = id;
+    float mylo = inf, myhi = -inf;
+#pragma unroll
+    for (int d = 0; d < D; ++d) {
+      P.idx_rows[((size_t)t * D + d) * 32 + lane] = id >= 0 ? x[d] : 0.0f;
+      float lo = id >= 0 ? x[d] : inf, hi = id >= 0 ? x[d] : -inf;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        lo = fminf(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+        hi = fmaxf(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+      }
+      if (lane == d) { mylo = lo; myhi = hi; }
+    }
+    if (lane < D) {
+      const size_t at = ((size_t)(t >> 5) * D + lane) * 32 + (t & 31);
+      P.idx_tlo[at] = mylo;
+      P.idx_thi[at] = myhi;
+    }
+  }
+  __threadfence();
+  grid.sync();
+  for (int s = gw; s < G.n_groups * 32; s += W) {
+    float mylo = inf, myhi = -inf;
+#pragma unroll
+    for (int d = 0; d < D; ++d) {
+      float lo = inf, hi = -inf;
+      if (s < G.n_super) {
+        lo = __ldcg(&P.idx_tlo[((size_t)s * D + d) * 32 + lane]);
+        hi = __ldcg(&P.idx_thi[((size_t)s * D + d) * 32 + lane]);
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        lo = fminf(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+        hi = fmaxf(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+      }
+      if (lane == d) { mylo = lo; myhi = hi; }
+    }
+    if (lane < D) {
+      const size_t at = ((size_t)(s >> 5) * D + lane) * 32 + (s & 31);
+      P.idx_slo[at] = mylo;
+      P.idx_shi[at] = myhi;
+    }
+  }
+  __threadfence();
+  __syncthreads();
+  fence_proxy_async();  // the histogram words live in the TMA tile buffers: order them before the next bulk copy
+  grid.sync();
+}
 
-// All indexed rows against every query of iteration `it`: warps of the CTAs vb = 0..vbcount-1 take the queries
-// round-robin, each draws its query itself (Alg. 1 l.6).
+// lower bound of the weighted squared distance from q to box `j` of a [group][dim][32] box table (lane-private j)
+template <int DYN>
+__device__ __forceinline__ float idx_box_bound(const DevProblem& pb, const float* __restrict__ lo,
+                                               const float* __restrict__ hi, size_t group, int j,
+                                               const float (&q)[DynTraits<DYN>::D]) {
+  constexpr int D = DynTraits<DYN>::D;
+  float acc = 0.0f;
+#pragma unroll
+  for (int d = 0; d < D; ++d) {
+    if (d == DynTraits<DYN>::ANGLE) continue;  // wrapped dims take no part in the bound (they add >= 0)
+    const float l = __ldcg(&lo[(group * D + d) * 32 + j]), h = __ldcg(&hi[(group * D + d) * 32 + j]);
+    const float e = fmaxf(fmaxf(l - q[d], q[d] - h), 0.0f);
+    acc = fmaf(e * pb.w[d], e, acc);
+  }
+  return acc * kIdxShrink;
+}
+
+// Scores up to NT tiles (32 rows each, one per lane; t[a] < 0: none) against q with all their loads in flight
+// together; returns the tightened upper bound.
+template <int DYN, bool UNIT_W, int NT>
+__device__ __forceinline__ float idx_score_tiles(const Params& P, const int (&t)[NT], const float (&q)[DynTraits<DYN>::D],
+                                                 unsigned long long& best, float ub) {
+  constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
+  const int lane = threadIdx.x & 31;
+  int id[NT];
+  float p[NT][DP];
+#pragma unroll
+  for (int a = 0; a < NT; ++a) {
+    if (t[a] >= 0) {  // warp-uniform
+      id[a] = __ldcg(&P.idx_tile_ids[(size_t)t[a] * 32 + lane]);
+#pragma unroll
+      for (int d = 0; d < DP; ++d) p[a][d] = d < D ? __ldcg(&P.idx_rows[((size_t)t[a] * D + d) * 32 + lane]) : 0.0f;
+    }
+  }
+  unsigned bits = 0x7f800000u;
+#pragma unroll
+  for (int a = 0; a < NT; ++a) {
+    if (t[a] >= 0) {
+      const float d2 = dist2<DYN, UNIT_W>(P.pb, q, p[a]);
+      if (id[a] >= 0) {
+        const unsigned b = __float_as_uint(d2);  // d2 >= 0: uint order == float order
+        best = min(best, ((unsigned long long)b << 32) | (unsigned)id[a]);
+        bits = min(bits, b);
+      }
+    }
+  }
+  return fminf(ub, __uint_as_float(__reduce_min_sync(0xffffffffu, bits)));
+}
+
+// Pops the candidate with the smallest bound out of the lane mask `cand` (lane j holds bound `lb`): returns its lane,
+// or -1 -- and empties the mask -- once the smallest remaining bound is above ub.
+__device__ __forceinline__ int idx_pop_nearest(unsigned& cand, float lb, float ub) {
+  const int lane = threadIdx.x & 31;
+  const unsigned mine = ((cand >> lane) & 1u) ? __float_as_uint(lb) : 0xffffffffu;  // lb >= 0
+  const unsigned mb = __reduce_min_sync(0xffffffffu, mine);
+  if (!(__uint_as_float(mb) <= ub)) { cand = 0; return -1; }  // also taken when cand was already empty (mb all ones = NaN)
+  const int j = __ffs(__ballot_sync(0xffffffffu, mine == mb)) - 1;
+  cand &= ~(1u << j);
+  return j;
+}
+
+// One warp, one query (all lanes hold the same q): exact NN over the indexed rows [0, n_sorted).
+// Boxes are opened nearest-first inside every group of 32, so ub tightens early and most boxes are never opened.
 template <int DYN, bool UNIT_W>
-__device__ __forceinline__ void idx_phase(const Params& P, const IdxGeom& G, int n_sorted, uint32_t r, uint32_t it,
-                                          unsigned long long* key, int vb, int vbcount) {
+__device__ __forceinline__ unsigned long long idx_search(const Params& P, const IdxDims& G,
+                                                         const float (&q)[DynTraits<DYN>::D], long long& scored) {
+  constexpr int NT = DynTraits<DYN>::DP <= 8 ? 4 : 2;  // tiles scored together (register budget)
+  const int lane = threadIdx.x & 31;
+  const float inf = __int_as_float(0x7f800000);
+  unsigned long long best = kKeyNone;
+  float ub = inf;
+  int s_near = -1, t_near = -1;
+  if (G.n_super > 32) {
+    // pass A (several groups of super-tiles): the globally nearest super-tile box, its nearest tile box, that
+    // tile's rows -> the exact distance of a real row
+    unsigned long long near = kKeyNone;
+    for (int s0 = 0; s0 < G.n_super; s0 += 32) {
+      const int s = s0 + lane;
+      const float lb = s < G.n_super ? idx_box_bound<DYN>(P.pb, P.idx_slo, P.idx_shi, (size_t)(s0 >> 5), lane, q) : inf;
+      near = min(near, ((unsigned long long)__float_as_uint(lb) << 32) | (unsigned)s);
+    }
+    s_near = (int)(unsigned)(warp_min_key(near) & 0xffffffffu);
+    const int t = s_near * 32 + lane;
+    const float lb = t < G.n_tiles ? idx_box_bound<DYN>(P.pb, P.idx_tlo, P.idx_thi, (size_t)s_near, lane, q) : inf;
+    t_near = (int)(unsigned)(warp_min_key(((unsigned long long)__float_as_uint(lb) << 32) | (unsigned)t) & 0xffffffffu);
+    int one[NT];
+#pragma unroll
+    for (int a = 0; a < NT; ++a) one[a] = a == 0 ? t_near : -1;
+    ub = idx_score_tiles<DYN, UNIT_W, NT>(P, one, q, best, ub);
+    scored += 32;
+  }
+  // pass B: every box that can still hold a row at distance <= ub
+  for (int s0 = 0; s0 < G.n_super; s0 += 32) {
+    const int s_mine = s0 + lane;
+    const float lb = s_mine < G.n_super ? idx_box_bound<DYN>(P.pb, P.idx_slo, P.idx_shi, (size_t)(s0 >> 5), lane, q) : inf;
+    unsigned cand = __ballot_sync(0xffffffffu, s_mine < G.n_super && lb <= ub);
+    for (;;) {
+      const int j = idx_pop_nearest(cand, lb, ub);
+      if (j < 0) break;
+      const int s = s0 + j;
+      const int t_mine = s * 32 + lane;
+      const float lbt = t_mine < G.n_tiles ? idx_box_bound<DYN>(P.pb, P.idx_tlo, P.idx_thi, (size_t)s, lane, q) : inf;
+      unsigned tc = __ballot_sync(0xffffffffu, t_mine < G.n_tiles && lbt <= ub);
+      if (s == s_near) tc &= ~(1u << (t_near & 31));  // scored in pass A
+      while (tc) {
+        int t[NT];
+        int cnt = 0;
+#pragma unroll
+        for (int a = 0; a < NT; ++a) {
+          const int k = tc ? idx_pop_nearest(tc, lbt, ub) : -1;
+          t[a] = k >= 0 ? s * 32 + k : -1;
+          cnt += k >= 0;
+        }
+        if (cnt == 0) break;
+        ub = idx_score_tiles<DYN, UNIT_W, NT>(P, t, q, best, ub);
+        scored += 32 * cnt;
+      }
+    }
+  }
+  return warp_min_key(best);
+}
+
+// All indexed rows against every query of iteration `it` (Alg. 1 l.6-7).  The warps of the CTAs vb = 0..vbcount-1
+// take queries off a shared counter (far queries open many more boxes than near ones: static shares would leave
+// most warps waiting for the unlucky ones); each draws its query itself.
+template <int DYN, bool UNIT_W>
+__device__ __forceinline__ void idx_phase(const Params& P, int n_sorted, uint32_t r, uint32_t it,
+                                          unsigned long long* key, int vb, int* counter, long long& scored) {
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
   if (vb < 0) return;
   const int lane = threadIdx.x & 31;
-  const int W = vbcount * kWarps, gw = vb * kWarps + (threadIdx.x >> 5);
-  for (int s = gw; s < P.B; s += W) {
+  const IdxDims G = idx_dims(n_sorted);
+  for (;;) {
+    int s = 0;
+    if (lane == 0) s = atomicAdd(counter, 1);
+    s = __shfl_sync(0xffffffffu, s, 0);
+    if (s >= P.B) break;
     float q[D];
     sample_state<D>(P.pb, P.seed, r, it, (uint32_t)s, q);
     if (lane == 0) {
@@ -572,7 +719,7 @@ __device__ __forceinline__ void idx_phase(const Params& P, const IdxGeom& G, int
         if (P.dbg_x_rand) P.dbg_x_rand[(size_t)s * DP + d] = d < D ? q[d] : 0.0f;
       }
     }
-    const unsigned long long kv = idx_search<DYN, UNIT_W>(P, G, n_sorted, q);
+    const unsigned long long kv = idx_search<DYN, UNIT_W>(P, G, q, scored);
     if (lane == 0 && kv != kKeyNone) atomicMin(&key[s], kv);
   }
 }
@@ -1120,7 +1267,6 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
   // insert inside phase X by the propagate CTAs (one grid barrier per iteration) when the children are few
   const bool xins = split && U_prop <= kFuseUnits;
   unsigned pgen = 0;
-  IdxGeom G = idx_geometry<T::PD>(P.pb, kIdxMinRows);  // dead unless INDEX
   unsigned long long* const key0 = P.nn_key;
   unsigned long long* const key1 = P.nn_key + P.B;
 
@@ -1131,7 +1277,9 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
   int n = P.n_nodes_io ? __ldcg(P.n_nodes_io) : 1;
   int solved_any = 0, replans_solved = 0, replans_run = 0, termination = 0;
   long long iterations = 0, inserted = 0, nn_pairs = 0;
-  unsigned long long ph0 = 0, ph1 = 0, ph2 = 0, tp = t_start;
+  long long nn_scored = 0;       // per warp: pairs the index tier scored (lane 0 reports at the end)
+  long long nn_idx_covered = 0;  // uniform: pairs of the NN definition the index answered without a scan
+  unsigned long long ph0 = 0, ph1 = 0, ph2 = 0, ph3 = 0, tp = t_start;
   bool stop = false;
   int cur = 0;  // key buffer of the current iteration
 
@@ -1141,28 +1289,39 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
     int iters = 0;
     int goal_node = -1;
     int n_scanned = 0;  // NN(it) already covers tree rows [0, n_scanned)
-    int n_sorted = 0;   // rows [0, n_sorted) are in the NN cell index
+    int n_sorted = 0;   // rows [0, n_sorted) are in the NN index
+    int cov_cur = 0, cov_next = 0;  // rows of NN(it) / NN(it+1) the index answered for
     for (;;) {
       unsigned long long* const kcur = cur ? key1 : key0;
       unsigned long long* const knext = cur ? key0 : key1;
       // a fresh tree is the root alone: every query's nearest node is node 0, no scan needed
       const bool root_only = (n == 1) && !P.n_nodes_io;
-      // NN index: (re)build once the tree has outgrown it by an eighth
+      // NN index tier: used once B*n is large; rebuilt when scanning the rows added since the last rebuild would
+      // cost about as much as rebuilding.  When every warp both propagates and searches (no split of the CTAs) the
+      // whole NN of the iteration runs at its head, right after the rebuild, instead of one iteration ahead: the
+      // rows of the previous batch are then inside the index and need no brute-force pass of their own.
       bool idx_use = false;
       if constexpr (INDEX) idx_use = P.nn_index == 2 ? n >= 256 : (n >= kIdxMinRows && (long long)P.B * n >= kIdxMinPairs);
       if (!idx_use) n_sorted = 0;
-      if (idx_use && n - n_sorted > max(n_sorted >> 3, P.nn_index == 2 ? 64 : 1024)) {
-        G = idx_geometry<T::PD>(P.pb, n);
-        idx_rebuild<DYN>(P, G, n, grid, sm_pref);
-        n_sorted = n;
+      const bool idx_head = idx_use && !split;
+      if constexpr (INDEX) {
+        const bool grown = P.nn_index == 2 ? n - n_sorted > 64
+                                           : (long long)P.B * (n - n_sorted) * T::D >= kIdxRebuildWork;
+        if (idx_use && (n_sorted == 0 || grown) && (n_scanned == 0 || !idx_head)) {
+          idx_rebuild<DYN>(P, n, grid, reinterpret_cast<unsigned*>(sm_tiles), sm_pref);
+          n_sorted = n;
+          if (leader) { const unsigned long long t = globaltimer_ns(); ph3 += t - tp; tp = t; }
+        }
       }
       // phase A': rows appended since the look-ahead scan
       if (!root_only && n_scanned < n) {
         int a_beg = n_scanned;
         if (idx_use && n_sorted > 0 && n_scanned == 0) {  // whole-tree NN (first call on a given tree): index + rest
-          if (P.pb.unit_weights) idx_phase<DYN, true>(P, G, n_sorted, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB);
-          else idx_phase<DYN, false>(P, G, n_sorted, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB);
+          int* qc = &P.ctrl->idx_query[0][iterations % kSlots];
+          if (P.pb.unit_weights) idx_phase<DYN, true>(P, n_sorted, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, qc, nn_scored);
+          else idx_phase<DYN, false>(P, n_sorted, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, qc, nn_scored);
           a_beg = n_sorted;
+          cov_cur = n_sorted;
         }
         if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1);
         else nn_phase<DYN, false, STREAM>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1);
@@ -1170,7 +1329,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       }
       if (leader) { const unsigned long long t = globaltimer_ns(); ph0 += t - tp; tp = t; }
       // phase X: propagate(it) and, meanwhile, NN(it+1) over the frozen snapshot [0, n)
-      const bool ahead = (iters + 1 < P.max_iters);
+      const bool ahead = (iters + 1 < P.max_iters) && !idx_head;
       prop_phase<DYN, OBS>(P, (uint32_t)r, (uint32_t)it, c_best, kcur, root_only, x_pw, x_pcnt, sm_obs, sm_cells, sm_list);
       // slots rotate over the whole launch (not per replan); see kSlots
       const int slot = (int)(iterations % kSlots);
@@ -1196,15 +1355,19 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       if (ahead) {
         int x_beg = 0;
         if (idx_use && n_sorted > 0) {
-          if (P.pb.unit_weights) idx_phase<DYN, true>(P, G, n_sorted, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt);
-          else idx_phase<DYN, false>(P, G, n_sorted, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt);
+          int* qc = &P.ctrl->idx_query[1][slot];
+          if (P.pb.unit_weights) idx_phase<DYN, true>(P, n_sorted, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, qc, nn_scored);
+          else idx_phase<DYN, false>(P, n_sorted, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, qc, nn_scored);
           x_beg = n_sorted;
+          cov_next = n_sorted;
         }
         if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1);
         else nn_phase<DYN, false, STREAM>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1);
       }
       if (leader) {
         P.ctrl->goal_key[slot_next] = kKeyNone;
+        P.ctrl->idx_query[0][slot_next] = 0;
+        P.ctrl->idx_query[1][slot_next] = 0;
         if (xins) P.ctrl->stop[slot] = (P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) ? 1 : 0;
       }
       fence_proxy_async();  // scratch rows written with st.global may be read by TMA in the insert phase
@@ -1228,6 +1391,9 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       }
       const int added = min(total, P.cap - n);
       nn_pairs += (long long)P.B * n;  // (query, node) pairs of this iteration's NN
+      nn_idx_covered += (long long)P.B * cov_cur;
+      cov_cur = cov_next;
+      cov_next = 0;
       n_scanned = ahead ? (fused ? n + added : n) : 0;  // fused: NN(it+1) already covers the new rows
       n += added;
       inserted += added;
@@ -1264,13 +1430,15 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
     }
     if (stop) termination = 1;
   }
+  if (lane == 0 && nn_scored) atomicAdd(&P.ctrl->nn_scored, (unsigned long long)nn_scored);
   if (leader) {
     Ctrl* c = P.ctrl;
     c->t_end_ns = globaltimer_ns();
     c->iterations = iterations;
     c->inserted = inserted;
     c->nn_pairs = nn_pairs;
-    c->phase_ns[0] = ph0; c->phase_ns[1] = ph1; c->phase_ns[2] = ph2;
+    c->nn_idx_covered = nn_idx_covered;
+    c->phase_ns[0] = ph0; c->phase_ns[1] = ph1; c->phase_ns[2] = ph2; c->phase_ns[3] = ph3;
     c->n_nodes = n;
     c->solved = solved_any;
     c->best_cost = c_best;

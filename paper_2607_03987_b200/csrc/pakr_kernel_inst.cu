@@ -1,7 +1,7 @@
 // pakr_kernel_inst.cu -- instantiates the persistent kernel of pakr_kernel.cuh for (dynamics, obstacle kind).
 // Compiled once per (tier, part) so that the sets build in parallel and a rarely used tier costs the common one
 // no registers:  -DPAKR_STREAM_TIER=0 tiled NN scan (the normal case), =1 streaming NN tier for B <= 16,
-// =2 tiled scan + opt-in NN cell index (double integrators and unicycle-2 only);
+// =2 tiled scan + NN index tier;
 // -DPAKR_PART=0 double integrators and unicycles, =1 quadrotors and the Dubins airplane.
 #include "pakr_kernel.cuh"
 
@@ -32,10 +32,8 @@ extern "C" const void* PAKR_SELECT_NAME(PAKR_STREAM_TIER, PAKR_PART)(int dyn, in
     case DYN_DI3 * 2 + OBS_BOX: return kernel_ptr<DYN_DI3, OBS_BOX>();
     case DYN_UNI2 * 2 + OBS_CIRCLE: return kernel_ptr<DYN_UNI2, OBS_CIRCLE>();
     case DYN_UNI2 * 2 + OBS_BOX: return kernel_ptr<DYN_UNI2, OBS_BOX>();
-#if PAKR_STREAM_TIER != 2
     case DYN_UNI1 * 2 + OBS_CIRCLE: return kernel_ptr<DYN_UNI1, OBS_CIRCLE>();
     case DYN_UNI1 * 2 + OBS_BOX: return kernel_ptr<DYN_UNI1, OBS_BOX>();
-#endif
 #else
     case DYN_QUAD * 2 + OBS_CIRCLE: return kernel_ptr<DYN_QUAD, OBS_CIRCLE>();
     case DYN_QUAD * 2 + OBS_BOX: return kernel_ptr<DYN_QUAD, OBS_BOX>();

@@ -51,7 +51,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale:
         tag = f".{os.getpid()}.tmp"
         units = [("pakr_api.cu", [], "api"), ("pakr_peak.cu", [], "peak")]
-        for tier, part in ((0, 0), (0, 1), (1, 0), (1, 1), (2, 0)):
+        for tier, part in ((0, 0), (0, 1), (1, 0), (1, 1), (2, 0), (2, 1)):
             units.append(("pakr_kernel_inst.cu", [f"-DPAKR_STREAM_TIER={tier}", f"-DPAKR_PART={part}"], f"t{tier}p{part}"))
         objs, procs = [], []
         for src, defs, name in units:
@@ -110,10 +110,10 @@ class _PlanOpts(C.Structure):
 
 class _Stats(C.Structure):
     _fields_ = [("iterations", C.c_int64), ("children", C.c_int64), ("inserted", C.c_int64), ("nn_pairs", C.c_int64),
-                ("h2d_bytes", C.c_int64), ("d2h_bytes", C.c_int64),
+                ("nn_pairs_evaluated", C.c_int64), ("h2d_bytes", C.c_int64), ("d2h_bytes", C.c_int64),
                 ("replans_run", C.c_int32), ("replans_solved", C.c_int32), ("termination", C.c_int32),
                 ("replan_stats_truncated", C.c_int32), ("path_truncated", C.c_int32),
-                ("first_solution_ms", C.c_double), ("device_ms", C.c_double), ("phase_ms", C.c_double * 3),
+                ("first_solution_ms", C.c_double), ("device_ms", C.c_double), ("phase_ms", C.c_double * 4),
                 ("replan_cost", C.c_float * MAX_REPLAN_STATS), ("replan_nodes", C.c_int32 * MAX_REPLAN_STATS),
                 ("replan_iters", C.c_int32 * MAX_REPLAN_STATS), ("replan_end_ms", C.c_double * MAX_REPLAN_STATS)]
 
@@ -277,7 +277,8 @@ class Planner:
         return dict(outcome=int(res.outcome), cost=float(res.cost), path_len=L, path_nodes=nodes[:L].copy(),
                     path_states=states[:L].copy(), path_controls=ctrls[:max(L - 1, 0)].copy(),
                     final_tree_nodes=int(res.final_tree_nodes), iterations=int(s.iterations), children=int(s.children),
-                    inserted=int(s.inserted), nn_pairs=int(s.nn_pairs), h2d_bytes=int(s.h2d_bytes),
+                    inserted=int(s.inserted), nn_pairs=int(s.nn_pairs), nn_pairs_evaluated=int(s.nn_pairs_evaluated),
+                    h2d_bytes=int(s.h2d_bytes),
                     d2h_bytes=int(s.d2h_bytes), replans_run=int(s.replans_run), replans_solved=int(s.replans_solved),
                     termination=int(s.termination), first_solution_ms=float(s.first_solution_ms),
                     device_ms=float(s.device_ms), phase_ms=[float(v) for v in s.phase_ms], replan_cost=np.array(s.replan_cost[:R], np.float32),
@@ -311,7 +312,7 @@ class Planner:
         self._check(lib().pakr_read_stats(self._h, B, K, tree_capacity, C.c_void_p(ws.data_ptr()), ws.numel(),
                                           C.c_void_p(self._stream()), C.byref(st)))
         return dict(iterations=int(st.iterations), children=int(st.children), inserted=int(st.inserted),
-                    nn_pairs=int(st.nn_pairs), device_ms=float(st.device_ms), phase_ms=[float(v) for v in st.phase_ms])
+                    nn_pairs=int(st.nn_pairs), nn_pairs_evaluated=int(st.nn_pairs_evaluated), device_ms=float(st.device_ms), phase_ms=[float(v) for v in st.phase_ms])
 
     # ---- pakr_expand_step ----
     def new_tree(self, capacity: int, host: Optional[dict] = None) -> dict:

@@ -116,6 +116,22 @@ def test_plan_seeds_c5_point_and_first_solution_time(pakr, orc):
     pl.close()
 
 
+@pytest.mark.parametrize("B,K", [(16384, 16), (4096, 64)])
+def test_plan_c5_large_batches(pakr, orc, B, K):
+    """Config 5's corner points: B*K = 262,144 children per iteration (insert's large-batch path, K = 64,
+    multi-hundred-thousand-node trees); the plan is re-propagated by the oracle and the tree checked."""
+    p, cfg = wl.config5(B=B, K=K)
+    pl = pakr.Planner(p)
+    res = pl.plan(1, B, K, cfg.tree_capacity, 1)
+    op = _check_plan(orc, p, res)
+    assert res["children"] == res["iterations"] * B * K and res["final_tree_nodes"] > 100000
+    tree = pl.read_tree(B, K, cfg.tree_capacity, res["final_tree_nodes"])
+    _check_tree(orc, op, p, tree, cfg.tree_capacity, n_samples=200)
+    res2 = pl.plan(1, B, K, cfg.tree_capacity, 1)
+    np.testing.assert_array_equal(res["path_states"], res2["path_states"])
+    pl.close()
+
+
 def test_plan_time_budget_and_no_solution(pakr, orc):
     p, cfg = wl.config2()
     pl = pakr.Planner(p)
@@ -230,11 +246,11 @@ def test_plan_initial_cost_bound(pakr, orc):
     pl.close()
 
 
-@pytest.mark.parametrize("name,iters", [("C2", 9), ("C3", 6), ("C1", 12)])
+@pytest.mark.parametrize("name,iters", [("C2", 9), ("C3", 6), ("C1", 12), ("C4", 5), ("N1", 8), ("C5", 4)])
 def test_plan_loop_with_nn_index_equals_scan(pakr, name, iters):
     """Inside the device loop the index is rebuilt as the tree grows and the rows added since are scanned:
-    the tree must be bit-identical to the one the scan tiers build."""
-    p, cfg = wl.CONFIGS[name]()
+    the tree must be bit-identical to the one the scan tiers build (C5: the B = 4096, K = 64 sweep point)."""
+    p, cfg = wl.config5(B=4096, K=64) if name == "C5" else wl.CONFIGS[name]()
     cap = 1 + iters * cfg.B * cfg.K
     trees = {}
     pl = pakr.Planner(p)

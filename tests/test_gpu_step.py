@@ -45,6 +45,11 @@ _CASES = [
     ("N2", 20000, 1024, 8),
     ("N3", 2500, 384, 16),  # quadcopter with body-frame velocities, PAPER.md:174 (NEXT-2)
     ("N3", 15000, 1024, 8),
+    # B*K > 65,536 (more than 2048 warp units: the insert's per-thread-chunk prefix) and K = 64, as config 5 runs them
+    ("C2", 5000, 2048, 64),   # B*K = 131,072
+    ("C5", 5000, 4096, 64),   # B*K = 262,144, 128 boxes
+    ("C2", 3000, 16384, 64),  # B*K = 2^20
+    ("C4", 4000, 8192, 16),   # B*K = 131,072 on the 12-D model
 ]
 
 
@@ -162,20 +167,36 @@ def test_teacher_forced_run_c2(pakr, orc):
     pl.close()
 
 
-@pytest.mark.parametrize("name,n0", [("C2", 300000), ("C3", 200000), ("C4", 150000), ("C5", 120000)])
-def test_full_size_sampled(pakr, orc, name, n0):
-    """BASELINE configs at full B, K (C2 is the bench launch configuration) on a large tree: NN checked on
-    sampled queries (oracle one by one), children of those queries checked exactly."""
+@pytest.mark.parametrize("name,n0,B,finite", [
+    ("C2", 300000, None, False), ("C3", 200000, None, True), ("C4", 150000, None, True), ("C5", 120000, None, False),
+    # tree sizes of the NN microbenchmarks (SURVEY.md 7 stage 4: 2^20; bench.py --what phases: 2^20 .. 2^23)
+    ("C2", 1 << 20, None, True), ("C4", 1 << 22, None, False), ("C5", 1 << 20, 16384, False),
+    ("C2", 1 << 23, 8, False), ("C4", 1 << 23, 4, False),   # streaming tier at the size its roofline is quoted on
+])
+def test_full_size_sampled(pakr, orc, name, n0, B, finite):
+    """BASELINE configs at full B, K (C4 is the bench launch configuration) on large trees: NN checked on
+    sampled queries (oracle one by one), children of those queries checked exactly -- validity, and under a
+    finite c_best the prune and goal bits too; the insert is checked over ALL children (bit-exact copy_if)."""
     p, cfg = wl.CONFIGS[name]()
     pl = pakr.Planner(p)
     op = orc.OracleProblem(p)
     host = wl.random_tree(p, n0, seed=77, flat=True)
-    B, K = cfg.B, cfg.K
+    B, K = B or cfg.B, cfg.K
+    edge = float(np.float32(p.steps_per_edge) * np.float32(p.dt))
+    # every node of the flat tree costs one edge: children cost two; a bound at 2 edges + the median heuristic of
+    # the box prunes roughly half of them
+    c_best = float("inf")
+    if finite:
+        rs = np.random.default_rng(5)
+        lo, hi = p.state_lo[:p.pos_dim].astype(np.float64), p.state_hi[:p.pos_dim].astype(np.float64)
+        hs = [op.heuristic(np.r_[rs.uniform(lo, hi), np.zeros(p.state_dim - p.pos_dim)]) for _ in range(400)]
+        c_best = 2 * edge + float(np.median(hs))
     tree = pl.new_tree(n0 + B * K, host)
-    out = pl.expand_step(tree, 0, 0, 40, B, K)
+    out = pl.expand_step(tree, 0, 0, 40, B, K, c_best=c_best)
     tree64 = host["states"].astype(np.float64)
     rng = np.random.default_rng(1)
-    for s in rng.choice(B, 24, replace=False):
+    n_pruned = 0
+    for s in rng.choice(B, min(24, B), replace=False):
         q = op.sample_state(0, 0, 40, int(s))
         np.testing.assert_array_equal(out["x_rand"][s].astype(np.float64), q)
         i, d2 = op.nearest(tree64, q)
@@ -186,17 +207,45 @@ def test_full_size_sampled(pakr, orc, name, n0):
             u = op.sample_control(0, 0, 40, int(s), k)
             np.testing.assert_array_equal(out["child_ctrl"][c].astype(np.float64), u)
             x, fl, fb, mm, ec = op.propagate(tree64[out["nn_idx"][s]], u)
+            gf = int(out["child_flags"][c])
             if mm > 1e-5:
-                assert (out["child_flags"][c] & 1) == (fl & 1)
-            if fl & 1 and out["child_flags"][c] & 1:
+                assert (gf & 1) == (fl & 1)
+            if fl & 1 and gf & 1:
                 err = np.abs(out["child_state"][c] - x)
                 ang = p.dim_kind == 1
                 err[ang] = np.minimum(err[ang], 2 * np.pi - err[ang])
                 assert err.max() < 1e-4
+                # Alg. 1 l.11 and l.14 on this child (the flat tree's nodes all cost one edge)
+                g = float(host["costs"][out["nn_idx"][s]]) + ec
+                assert out["child_cost"][c] == pytest.approx(g, rel=1e-6)
+                f = g + op.heuristic(x)
+                notpruned = f < c_best
+                if abs(f - c_best) > 1e-5:
+                    assert bool(gf & 8) == notpruned
+                    n_pruned += not notpruned
+                    ing, gm = op.in_goal(x)
+                    if gm > 1e-5:
+                        assert bool(gf & 16) == (notpruned and ing)
+    if finite:
+        assert n_pruned > 0 and 0.05 < float(((out["child_flags"] & 8) != 0).mean()) < 0.95
     # properties that hold at any size
     assert out["nn_idx"].min() >= 0 and out["nn_idx"].max() < n0
-    keep = (out["child_flags"] & 9) == 9
-    assert out["n_inserted"] == int(keep.sum()) == int(tree["n_nodes"][0].item()) - n0
+    keep = np.nonzero((out["child_flags"] & 9) == 9)[0]
+    n1 = int(tree["n_nodes"][0].item())
+    assert out["n_inserted"] == len(keep) == n1 - n0
+    # insert order over ALL children: bit-exact copy_if of the kept children, in child order (P20)
+    D, m = p.state_dim, p.control_dim
+    np.testing.assert_array_equal(tree["states"][n0:n1, :D].cpu().numpy(), out["child_state"][keep])
+    np.testing.assert_array_equal(tree["actions"][n0:n1, :m].cpu().numpy(), out["child_ctrl"][keep])
+    np.testing.assert_array_equal(tree["costs"][n0:n1].cpu().numpy(), out["child_cost"][keep])
+    np.testing.assert_array_equal(tree["parents"][n0:n1].cpu().numpy(), out["nn_idx"][keep // K])
+    np.testing.assert_array_equal(np.nonzero((out["child_flags"] & 32) != 0)[0], keep)
+    g = keep[(out["child_flags"][keep] & 16) != 0]
+    if len(g):
+        best = g[np.argmin(out["child_cost"][g])]
+        assert out["goal_node"] == n0 + int(np.nonzero(keep == best)[0][0])
+    else:
+        assert out["goal_node"] == -1
     pl.close()
 
 
@@ -236,7 +285,9 @@ def test_nn_tiers_agree_bit_for_bit(pakr, name):
 
 
 @pytest.mark.parametrize("name,n0,B,K", [("C2", 20000, 512, 2), ("C3", 9000, 300, 3), ("C3", 40000, 257, 2),
-                                         ("C1", 700, 64, 4), ("C5", 60000, 1024, 1)])
+                                         ("C1", 700, 64, 4), ("C5", 60000, 1024, 1), ("C4", 30000, 512, 2),
+                                         ("C4", 1025, 300, 1), ("N1", 5000, 256, 2), ("N2", 33000, 400, 2),
+                                         ("N3", 70000, 256, 1), ("C2", 300000, 2048, 1)])
 def test_nn_index_tier_equals_scan_tier(pakr, orc, name, n0, B, K):
     """The NN index (exact spatial pruning) must return bit-identical NN indices
     and distances to the brute-force scan, on clustered trees too (queries far from every node search wide),
