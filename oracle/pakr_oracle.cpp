@@ -131,7 +131,7 @@ extern "C" int64_t orc_nearest(const orc_problem* P, const double* states, int64
   return best;
 }
 
-/* Eq. (1) xdot = f(x,u) for the three model families of the configs. */
+/* Eq. (1) xdot = f(x,u) for the model families of the configs and of PAPER.md Sec. V. */
 extern "C" void orc_f(const orc_problem* P, const double* x, const double* u, double* xd) {
   switch (P->dynamics_id) {
     case ORC_DYN_DOUBLE_INTEGRATOR: {  // [p, pdot], control = accelerations
@@ -219,6 +219,34 @@ extern "C" void orc_f(const orc_problem* P, const double* x, const double* u, do
       xd[9] = (u[1] - (Izz - Iyy) * q * r) / Ixx;
       xd[10] = (u[2] - (Ixx - Izz) * p * r) / Iyy;
       xd[11] = (u[3] - (Iyy - Ixx) * p * q) / Izz;
+      break;
+    }
+    case ORC_DYN_ACROBOT: {
+      // state [theta1, theta2, theta1_dot, theta2_dot], two-link pendulum actuated at the elbow,
+      // control = elbow torque.  The paper prints no equations (it points to DynoBench); reading P35:
+      // the planar double pendulum of rigid links from Lagrange's equations, theta1 measured from the downward
+      // vertical, theta2 relative to link 1, I1 and I2 about each link's centre of mass:
+      //   T = 1/2 qd^T D(q) qd,   V = -m1 g lc1 cos(th1) - m2 g (l1 cos(th1) + lc2 cos(th1 + th2))
+      //   D(q) qdd + c(q, qd) = -dV/dq + (0, tau)
+      const double m1 = P->dyn_params[0], m2 = P->dyn_params[1], l1 = P->dyn_params[2], lc1 = P->dyn_params[3],
+                   lc2 = P->dyn_params[4], I1 = P->dyn_params[5], I2 = P->dyn_params[6], g = P->dyn_params[7];
+      const double th1 = x[0], th2 = x[1], w1 = x[2], w2 = x[3];
+      const double c2 = std::cos(th2), s2 = std::sin(th2);
+      const double d11 = I1 + I2 + m1 * lc1 * lc1 + m2 * (l1 * l1 + lc2 * lc2 + 2.0 * l1 * lc2 * c2);
+      const double d12 = I2 + m2 * (lc2 * lc2 + l1 * lc2 * c2);
+      const double d22 = I2 + m2 * lc2 * lc2;
+      const double hh = m2 * l1 * lc2 * s2;
+      const double cor1 = -hh * (2.0 * w1 * w2 + w2 * w2);  // Coriolis / centrifugal terms c(q, qd)
+      const double cor2 = hh * w1 * w1;
+      const double grav1 = -(m1 * lc1 + m2 * l1) * g * std::sin(th1) - m2 * lc2 * g * std::sin(th1 + th2);  // -dV/dth1
+      const double grav2 = -m2 * lc2 * g * std::sin(th1 + th2);                                              // -dV/dth2
+      const double r1 = grav1 - cor1;
+      const double r2 = grav2 - cor2 + u[0];
+      const double det = d11 * d22 - d12 * d12;
+      xd[0] = w1;
+      xd[1] = w2;
+      xd[2] = (d22 * r1 - d12 * r2) / det;
+      xd[3] = (d11 * r2 - d12 * r1) / det;
       break;
     }
     default:
@@ -318,9 +346,17 @@ extern "C" int32_t orc_propagate(const orc_problem* P, const double* x0, const d
   return flags;
 }
 
+/* Euclidean distance to the goal centre over the goal dims (default: the position dims), the difference wrapped on
+ * angle dims (P18; Acrobot's goal lives in angle space, "swing-up"). */
 static double goal_distance(const orc_problem* P, const double* x) {
   double s = 0.0;
-  for (int a = 0; a < P->pos_dim; ++a) s += (x[a] - P->goal_center[a]) * (x[a] - P->goal_center[a]);
+  const int ng = P->goal_n_dims > 0 ? P->goal_n_dims : P->pos_dim;
+  for (int i = 0; i < ng; ++i) {
+    const int d = P->goal_n_dims > 0 ? P->goal_dims[i] : i;
+    double delta = x[d] - P->goal_center[i];
+    if (P->dim_kind[d] == ORC_DIM_ANGLE) delta = orc_wrap_pi(delta);
+    s += delta * delta;
+  }
   return std::sqrt(s);
 }
 

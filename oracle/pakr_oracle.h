@@ -28,7 +28,7 @@ extern "C" {
 #endif
 
 enum { ORC_DYN_DOUBLE_INTEGRATOR = 0, ORC_DYN_UNICYCLE2 = 1, ORC_DYN_QUADROTOR = 2,
-       ORC_DYN_DUBINS_AIRPLANE = 3, ORC_DYN_UNICYCLE1 = 4, ORC_DYN_QUADROTOR_BODY = 5 };
+       ORC_DYN_DUBINS_AIRPLANE = 3, ORC_DYN_UNICYCLE1 = 4, ORC_DYN_QUADROTOR_BODY = 5, ORC_DYN_ACROBOT = 6 };
 enum { ORC_INT_EULER = 0, ORC_INT_RK4 = 1 };
 enum { ORC_OBS_CIRCLE2D = 0, ORC_OBS_AABB = 1, ORC_OBS_ZCYLINDER = 2 };
 enum { ORC_COST_DURATION = 0, ORC_COST_PATH_LENGTH = 1 };
@@ -48,17 +48,21 @@ enum {
  * All arrays are caller-owned, fp64 (fp32 inputs widened by the caller). */
 typedef struct {
   int32_t dynamics_id, integrator, state_dim, control_dim, pos_dim;
-  const double* dyn_params; int32_t n_dyn_params;    /* quadrotor: m, Ixx, Iyy, Izz, g */
+  const double* dyn_params; int32_t n_dyn_params;    /* quadrotor: m, Ixx, Iyy, Izz, g; acrobot: m1, m2, l1, lc1,
+                                                        lc2, I1, I2, g (I about each link's centre of mass) */
   const double* state_lo; const double* state_hi;    /* [D]; +-inf = unbounded          */
   const uint8_t* dim_kind;                           /* [D] ORC_DIM_*                   */
   const double* nn_weight;                           /* [D] >= 0                        */
   const double* control_lo; const double* control_hi;/* [m]                             */
   int32_t obstacle_type; const double* obstacles; int32_t n_obstacles;
   const double* start;                               /* [D]                             */
-  const double* goal_center; double goal_radius;     /* [pos_dim], ball in position     */
+  const double* goal_center; double goal_radius;     /* ball over the goal dims (below) */
   int32_t goal_angle_dim; double goal_angle, goal_angle_tol; /* -1 = no heading test    */
   double dt; int32_t steps_per_edge;
   int32_t cost_mode; double heuristic_speed;         /* h = max(0,|p-g|-r)/speed        */
+  /* X_goal = { x : sqrt(sum_{i} delta_i^2) <= goal_radius }, delta_i = x[goal_dims[i]] - goal_center[i], wrapped to
+   * [-pi, pi) when that dim is an angle dim.  goal_n_dims = 0: the first pos_dim dims (goal_center[pos_dim]). */
+  int32_t goal_n_dims; const int32_t* goal_dims;     /* [goal_n_dims] state indices     */
 } orc_problem;
 
 /* Tree of PAPER.md:140: four buffers + a scalar count.  Node-major (states[i*D+d]). */

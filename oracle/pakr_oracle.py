@@ -45,6 +45,7 @@ class _Problem(C.Structure):
         ("goal_angle_dim", C.c_int32), ("goal_angle", C.c_double), ("goal_angle_tol", C.c_double),
         ("dt", C.c_double), ("steps_per_edge", C.c_int32),
         ("cost_mode", C.c_int32), ("heuristic_speed", C.c_double),
+        ("goal_n_dims", C.c_int32), ("goal_dims", _ip),
     ]
 
 
@@ -130,7 +131,8 @@ class OracleProblem:
             kind=np.ascontiguousarray(p.dim_kind, dtype=np.uint8), w=_d(p.nn_weight),
             ulo=_d(p.control_lo), uhi=_d(p.control_hi),
             obs=_d(p.obstacles.reshape(-1) if p.n_obstacles else [0.0]), start=_d(p.start),
-            goal=_d(p.goal_center))
+            goal=_d(p.goal_center),
+            gdims=np.ascontiguousarray(p.goal_dims if p.goal_dims is not None else [0], dtype=np.int32))
         k = self._keep
         self.c = _Problem(
             p.dynamics_id, p.integrator, p.state_dim, p.control_dim, p.pos_dim,
@@ -138,7 +140,7 @@ class OracleProblem:
             _ptr(k["w"]), _ptr(k["ulo"]), _ptr(k["uhi"]), p.obstacle_type, _ptr(k["obs"]),
             p.n_obstacles, _ptr(k["start"]), _ptr(k["goal"]), f32(p.goal_radius), p.goal_angle_dim,
             f32(p.goal_angle), f32(p.goal_angle_tol), f32(p.dt), p.steps_per_edge, p.cost_mode,
-            f32(p.heuristic_speed))
+            f32(p.heuristic_speed), 0 if p.goal_dims is None else len(p.goal_dims), _ptr(k["gdims"], _ip))
         self.ref = C.byref(self.c)
 
     # ---- building blocks ----

@@ -22,7 +22,7 @@ import numpy as np
 # ABI constants (numeric values documented in DESIGN.md; restated in include/pakr.h and
 # oracle/pakr_oracle.h independently).
 DYN_DOUBLE_INTEGRATOR, DYN_UNICYCLE2, DYN_QUADROTOR, DYN_DUBINS_AIRPLANE, DYN_UNICYCLE1 = 0, 1, 2, 3, 4
-DYN_QUADROTOR_BODY = 5
+DYN_QUADROTOR_BODY, DYN_ACROBOT = 5, 6
 INT_EULER, INT_RK4 = 0, 1
 OBS_CIRCLE2D, OBS_AABB, OBS_ZCYLINDER = 0, 1, 2
 COST_DURATION, COST_PATH_LENGTH = 0, 1
@@ -57,6 +57,7 @@ class Problem:
     steps_per_edge: int
     cost_mode: int
     heuristic_speed: float
+    goal_dims: Optional[np.ndarray] = None   # int32 state indices the goal ball spans; None = the position dims
 
     @property
     def n_obstacles(self) -> int:
@@ -288,7 +289,28 @@ def config8(env_seed: int = 404) -> tuple[Problem, PlanConfig]:
     return p, cfg
 
 
-CONFIGS = {"C1": config1, "C2": config2, "C3": config3, "C4": config4, "C5": config5, "N1": config6, "N2": config7, "N3": config8}
+def config9() -> tuple[Problem, PlanConfig]:
+    """N4 (NEXT-2, not a BASELINE config): Acrobot swing-up -- state [theta1, theta2, theta1_dot,
+    theta2_dot], elbow torque; both angles are angle dims, no obstacles, start hanging at rest, goal a ball in angle
+    space around the upright pose (theta1 = pi, theta2 = 0), velocities free like every other goal here (P18).
+    Uniform unit rods (P35): m = 1, l = 1, lc = 0.5, I = m l^2 / 12, g = 9.81."""
+    pi = math.pi
+    wmax = 10.0
+    p = Problem(
+        name="N4-acrobot", dynamics_id=DYN_ACROBOT, integrator=INT_RK4, state_dim=4, control_dim=1, pos_dim=2,
+        dyn_params=_f32([1.0, 1.0, 1.0, 0.5, 0.5, 1.0 / 12.0, 1.0 / 12.0, 9.81]),
+        state_lo=_f32([-pi, -pi, -wmax, -wmax]), state_hi=_f32([pi, pi, wmax, wmax]),
+        dim_kind=np.array([1, 1, 0, 0], np.uint8), nn_weight=_f32([1, 1, 0.1, 0.1]),
+        control_lo=_f32([-10.0]), control_hi=_f32([10.0]), obstacle_type=OBS_CIRCLE2D,
+        obstacles=np.zeros((0, 3), np.float32), start=_f32([0, 0, 0, 0]), goal_center=_f32([pi, 0.0]),
+        goal_radius=0.3, goal_angle_dim=-1, goal_angle=0.0, goal_angle_tol=0.0, dt=0.02, steps_per_edge=10,
+        cost_mode=COST_DURATION, heuristic_speed=math.sqrt(2.0) * wmax,
+        goal_dims=np.array([0, 1], np.int32))
+    return p, PlanConfig(B=1024, K=8, tree_capacity=1 << 20, n_replans=10)
+
+
+CONFIGS = {"C1": config1, "C2": config2, "C3": config3, "C4": config4, "C5": config5, "N1": config6, "N2": config7, "N3": config8,
+           "N4": config9}
 
 
 def random_tree(problem: Problem, n: int, seed: int, flat: bool = False) -> dict[str, np.ndarray]:
