@@ -46,15 +46,15 @@ typedef enum {
 } pakr_status;
 
 enum { PAKR_DYN_DOUBLE_INTEGRATOR = 0, PAKR_DYN_UNICYCLE2 = 1, PAKR_DYN_QUADROTOR = 2,
-       PAKR_DYN_DUBINS_AIRPLANE = 3, PAKR_DYN_UNICYCLE1 = 4, PAKR_DYN_QUADROTOR_BODY = 5 };
+       PAKR_DYN_DUBINS_AIRPLANE = 3, PAKR_DYN_UNICYCLE1 = 4, PAKR_DYN_QUADROTOR_BODY = 5, PAKR_DYN_ACROBOT = 6 };
 enum { PAKR_INT_EULER = 0, PAKR_INT_RK4 = 1 };
 enum { PAKR_OBS_CIRCLE2D = 0, PAKR_OBS_AABB = 1, PAKR_OBS_ZCYLINDER = 2 };
 enum { PAKR_COST_DURATION = 0, PAKR_COST_PATH_LENGTH = 1 };
 enum { PAKR_DIM_REAL = 0, PAKR_DIM_ANGLE = 1 };
 enum { PAKR_NO_SOLUTION = 0, PAKR_SOLVED = 1 }; /* "no solution" is not an error */
 /* nearest-neighbour tier (pakr_plan_opts.nn_mode, pakr_step_args.nn_mode) */
-enum { PAKR_NN_AUTO = 0,  /* the library picks: brute-force scan tiers while the tree is small, the spatial index
-                             once B*n is large enough to pay for building it */
+enum { PAKR_NN_AUTO = 0,  /* the library picks: brute-force scan tiers, and from B = 4096 queries up the spatial index
+                             once the tree is large enough to pay for building it */
        PAKR_NN_SCAN = 1,  /* brute-force scan tiers only (tiled; streaming when B <= 16) */
        PAKR_NN_INDEX = 2  /* spatial index on every tree of >= 256 nodes (tests) */ };
 
@@ -76,33 +76,45 @@ typedef struct {
                           psi) ZYX, (p,q,r)] with control (T, tau) (BASELINE.json config 4), Dubins airplane
                           [x,y,z,yaw,pitch,v] with control (yaw rate, pitch rate, acceleration),
                           first-order unicycle [x,y,theta] with control (v, omega), quadcopter with
-                          body-frame velocities [p, (phi,theta,psi), (u,v,w) body, (p,q,r)] exactly as PAPER.md:174 */
+                          body-frame velocities [p, (phi,theta,psi), (u,v,w) body, (p,q,r)] exactly as PAPER.md:174,
+                          Acrobot [theta1, theta2, theta1_dot, theta2_dot] with the elbow torque as control
+                          (theta1 from the downward vertical, theta2 relative to link 1) */
   int32_t integrator;  /* PAKR_INT_*: forward Euler or classical RK4 */
   int32_t state_dim, control_dim, pos_dim; /* must match dynamics_id: DI (2*pos_dim, pos_dim,
-                          2|3), unicycle2 (5,2,2), both quadrotors (12,4,3), Dubins airplane (6,3,3), unicycle1 (3,2,2) */
-  const float* dyn_params; int32_t n_dyn_params; /* quadrotors: m, Ixx, Iyy, Izz, g; else 0 */
+                          2|3), unicycle2 (5,2,2), both quadrotors (12,4,3), Dubins airplane (6,3,3), unicycle1 (3,2,2),
+                          Acrobot (4,1,2: its "position" dims are the two joint angles) */
+  const float* dyn_params; int32_t n_dyn_params; /* quadrotors: m, Ixx, Iyy, Izz, g; Acrobot: m1, m2, l1, lc1, lc2, I1,
+                          I2, g (link masses, length of link 1, distances joint -> centre of mass, inertias about the
+                          centres of mass); else 0 */
   const float* state_lo; const float* state_hi;  /* [D]; +-INF = unbounded; box-tested every step */
-  const uint8_t* dim_kind; /* [D] PAKR_DIM_*; angle dims (unicycle theta, quadrotor psi, airplane yaw) are wrapped
-                          to [-pi,pi) and never bounds-tested; must match the dynamics */
+  const uint8_t* dim_kind; /* [D] PAKR_DIM_*; angle dims (unicycle theta, quadrotor psi, airplane yaw, both Acrobot
+                          joint angles) are wrapped to [-pi,pi) and never bounds-tested; must match the dynamics */
   const float* nn_weight;  /* [D] >= 0, d^2 = sum_d w_d delta_d^2; 0 drops a dim */
   const float* control_lo; const float* control_hi; /* [m] */
   int32_t obstacle_type;   /* PAKR_OBS_*: circle/cylinder rows (cx, cy, r); box rows (lo[pos_dim],
                           hi[pos_dim]).  Closed sets, point robot. */
-  const float* obstacles; int32_t n_obstacles;   /* n_obstacles <= 1024 */
+  const float* obstacles; int32_t n_obstacles;   /* n_obstacles <= 1024; the Acrobot takes none (its position dims are
+                          angles: UNSUPPORTED with n_obstacles > 0) */
   const float* start;       /* [D] x_init */
-  const float* goal_center; /* [pos_dim] */
-  float goal_radius;        /* X_goal = closed position ball ... */
+  const float* goal_center; /* [pos_dim], or [goal_n_dims] when goal_dims is given */
+  float goal_radius;        /* X_goal = closed ball over the goal dims (default: the position dims) ... */
   int32_t goal_angle_dim; float goal_angle, goal_angle_tol; /* ... and |wrap(x[dim]-angle)| <= tol; -1 = none */
   float dt; int32_t steps_per_edge; /* every edge is exactly steps_per_edge steps of dt */
   int32_t cost_mode;      /* PAKR_COST_DURATION (J = T) or PAKR_COST_PATH_LENGTH */
   float heuristic_speed;  /* h(x) = max(0, |p - goal| - r) / heuristic_speed; +INF => h = 0 */
+  /* Goal region over listed state dims (PAPER.md:67 X_goal; the Acrobot's swing-up goal lives in angle space,
+   * PAPER.md:209,:212): X_goal = { x : sqrt(sum_i delta_i^2) <= goal_radius }, delta_i = x[goal_dims[i]] -
+   * goal_center[i], wrapped to [-pi,pi) on angle dims.  goal_n_dims = 0 / goal_dims = NULL: the first pos_dim dims.
+   * The heuristic uses the same distance; it stays admissible only if heuristic_speed bounds the rate of change of that
+   * distance (with velocity dims in the ball, pass +INF). */
+  int32_t goal_n_dims; const int32_t* goal_dims; /* [goal_n_dims] distinct state indices, HOST */
 } pakr_problem;
 
 /* Validates and copies the problem; selects the compiled kernel variant; binds `cuda_device` (the caller's current
  * device is restored before returning, here and in every other call).
  * INVALID_ARG: NULL, dims that do not match the dynamics, lo > hi, NaN, weight < 0, a sampled
- * real dim (weight > 0) with an infinite bound, dt <= 0, steps < 1.  UNSUPPORTED: unknown ids,
- * dim_kind not the dynamics' own.  CUDA: device not usable (no sm_100 device). */
+ * real dim (weight > 0) with an infinite bound, dt <= 0, steps < 1, goal_dims out of range or repeated.
+ * UNSUPPORTED: unknown ids, dim_kind not the dynamics' own, obstacles with the Acrobot.  CUDA: device not usable (no sm_100 device). */
 pakr_status pakr_create(const pakr_problem* problem, int cuda_device, pakr_planner** out);
 void pakr_destroy(pakr_planner* planner);
 /* Text of the last failure on this planner ("" if none); valid until the next call on it.

@@ -198,12 +198,12 @@ HostGrid build_grid(const pakr_problem* p, int obs_kind) {
 // cell (hi - lo) sqrt(w) / 2^bits is widest at that moment -- the split order of a kd-tree over the weighted state
 // box.  Keyed: non-angle dimensions with a finite box of positive width and a positive weight.  Returns false if
 // no dimension can be keyed (the index tier is then unavailable for the problem).
-bool idx_key_layout(DevProblem& pb, int D, int angle_dim) {
+bool idx_key_layout(DevProblem& pb, int D, unsigned angle_mask) {
   double cell[kMaxD];
   int bits[kMaxD] = {0};
   bool any = false;
   for (int d = 0; d < D; ++d) {
-    const bool ok = d != angle_dim && std::isfinite(pb.lo[d]) && std::isfinite(pb.hi[d]) && pb.hi[d] > pb.lo[d] && pb.w[d] > 0.0f;
+    const bool ok = !((angle_mask >> d) & 1u) && std::isfinite(pb.lo[d]) && std::isfinite(pb.hi[d]) && pb.hi[d] > pb.lo[d] && pb.w[d] > 0.0f;
     cell[d] = ok ? ((double)pb.hi[d] - pb.lo[d]) * std::sqrt((double)pb.w[d]) : 0.0;
     any = any || ok;
   }
@@ -292,6 +292,18 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
     if (p->pos_dim != 2 || p->state_dim != 3 || p->control_dim != 2)
       return fail(nullptr, PAKR_ERR_INVALID_ARG, "unicycle1 needs (D,m,pos)=(3,2,2)");
     dyn = DYN_UNI1;
+  } else if (p->dynamics_id == PAKR_DYN_ACROBOT) {
+    if (p->pos_dim != 2 || p->state_dim != 4 || p->control_dim != 1)
+      return fail(nullptr, PAKR_ERR_INVALID_ARG, "acrobot needs (D,m,pos)=(4,1,2)");
+    if (p->n_dyn_params < 8 || !p->dyn_params)
+      return fail(nullptr, PAKR_ERR_INVALID_ARG, "acrobot needs dyn_params m1,m2,l1,lc1,lc2,I1,I2,g");
+    for (int i = 0; i < 7; ++i)
+      if (!(p->dyn_params[i] > 0.0f) || !std::isfinite(p->dyn_params[i]))
+        return fail(nullptr, PAKR_ERR_INVALID_ARG, "acrobot masses, lengths and inertias must be finite and > 0");
+    if (!std::isfinite(p->dyn_params[7])) return fail(nullptr, PAKR_ERR_INVALID_ARG, "acrobot g must be finite");
+    if (p->n_obstacles > 0)
+      return fail(nullptr, PAKR_ERR_UNSUPPORTED, "the acrobot takes no obstacles (its position dims are angles)");
+    dyn = DYN_ACRO;
   } else {
     return fail(nullptr, PAKR_ERR_UNSUPPORTED, "unknown dynamics_id");
   }
@@ -303,6 +315,7 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
   if (p->obstacle_type == PAKR_OBS_CIRCLE2D || p->obstacle_type == PAKR_OBS_ZCYLINDER) obs = OBS_CIRCLE;
   else if (p->obstacle_type == PAKR_OBS_AABB) obs = OBS_BOX;
   else return fail(nullptr, PAKR_ERR_UNSUPPORTED, "unknown obstacle_type");
+  if (dyn == DYN_ACRO) obs = OBS_CIRCLE;  // no obstacles: one kernel variant
   if (p->n_obstacles < 0 || p->n_obstacles > 1024 || (p->n_obstacles > 0 && !p->obstacles))
     return fail(nullptr, PAKR_ERR_INVALID_ARG, "n_obstacles must be in [0,1024] with a non-null array");
   const int D = p->state_dim, M = p->control_dim, PD = p->pos_dim;
@@ -311,17 +324,20 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
     for (int i = 0; i < p->n_obstacles * per; ++i)
       if (!std::isfinite(p->obstacles[i])) return fail(nullptr, PAKR_ERR_INVALID_ARG, "obstacle coordinates must be finite");
   }
-  const int angle = dyn == DYN_UNI2 ? 2 : dyn == DYN_QUAD ? 8 : dyn == DYN_DA ? 3 : dyn == DYN_UNI1 ? 2 : dyn == DYN_QUADB ? 5 : -1;
+  const unsigned angles = dyn == DYN_UNI2 ? DynTraits<DYN_UNI2>::ANGLES : dyn == DYN_QUAD ? DynTraits<DYN_QUAD>::ANGLES
+                        : dyn == DYN_DA ? DynTraits<DYN_DA>::ANGLES : dyn == DYN_UNI1 ? DynTraits<DYN_UNI1>::ANGLES
+                        : dyn == DYN_QUADB ? DynTraits<DYN_QUADB>::ANGLES : dyn == DYN_ACRO ? DynTraits<DYN_ACRO>::ANGLES : 0u;
+  auto angle_dim = [&](int d) { return ((angles >> d) & 1u) != 0; };
   for (int d = 0; d < D; ++d) {
-    const bool is_angle = p->dim_kind[d] == PAKR_DIM_ANGLE;
-    if (p->dim_kind[d] > 1 || is_angle != (d == angle))
-      return fail(nullptr, PAKR_ERR_UNSUPPORTED, "dim_kind must mark exactly the dynamics' own angle dim");
+    const bool marked = p->dim_kind[d] == PAKR_DIM_ANGLE;
+    if (p->dim_kind[d] > 1 || marked != angle_dim(d))
+      return fail(nullptr, PAKR_ERR_UNSUPPORTED, "dim_kind must mark exactly the dynamics' own angle dims");
     if (std::isnan(p->state_lo[d]) || std::isnan(p->state_hi[d]) || std::isnan(p->nn_weight[d]) ||
         std::isnan(p->start[d]))
       return fail(nullptr, PAKR_ERR_INVALID_ARG, "NaN in state bounds, weights or start");
     if (p->state_lo[d] > p->state_hi[d]) return fail(nullptr, PAKR_ERR_INVALID_ARG, "state_lo > state_hi");
     if (p->nn_weight[d] < 0.0f) return fail(nullptr, PAKR_ERR_INVALID_ARG, "nn_weight < 0");
-    if (!is_angle && p->nn_weight[d] > 0.0f && (std::isinf(p->state_lo[d]) || std::isinf(p->state_hi[d])))
+    if (!marked && p->nn_weight[d] > 0.0f && (std::isinf(p->state_lo[d]) || std::isinf(p->state_hi[d])))
       return fail(nullptr, PAKR_ERR_INVALID_ARG, "a sampled dim (weight > 0) needs finite bounds");
   }
   for (int j = 0; j < M; ++j) {
@@ -332,12 +348,22 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
     return fail(nullptr, PAKR_ERR_INVALID_ARG, "dt must be > 0 and steps_per_edge >= 1");
   if (!(p->goal_radius >= 0.0f) || !(p->heuristic_speed > 0.0f))
     return fail(nullptr, PAKR_ERR_INVALID_ARG, "goal_radius >= 0 and heuristic_speed > 0 required");
-  if (p->goal_angle_dim != -1 && p->goal_angle_dim != angle)
-    return fail(nullptr, PAKR_ERR_INVALID_ARG, "goal_angle_dim must be -1 or the dynamics' angle dim");
+  if (p->goal_angle_dim != -1 && (p->goal_angle_dim < 0 || p->goal_angle_dim >= D || !angle_dim(p->goal_angle_dim)))
+    return fail(nullptr, PAKR_ERR_INVALID_ARG, "goal_angle_dim must be -1 or one of the dynamics' angle dims");
   if (p->goal_angle_dim != -1 && (!std::isfinite(p->goal_angle) || !std::isfinite(p->goal_angle_tol) || p->goal_angle_tol < 0.0f))
     return fail(nullptr, PAKR_ERR_INVALID_ARG, "goal_angle must be finite and goal_angle_tol finite and >= 0");
-  for (int a = 0; a < p->pos_dim; ++a)
-    if (!std::isfinite(p->goal_center[a])) return fail(nullptr, PAKR_ERR_INVALID_ARG, "goal_center must be finite");
+  // goal ball: listed dims, or the position dims
+  if (p->goal_n_dims < 0 || p->goal_n_dims > D || (p->goal_n_dims > 0 && !p->goal_dims))
+    return fail(nullptr, PAKR_ERR_INVALID_ARG, "goal_n_dims must be in [0, state_dim] with a non-null goal_dims");
+  const int n_goal = p->goal_n_dims > 0 ? p->goal_n_dims : p->pos_dim;
+  int goal_dim[kMaxD];
+  for (int i = 0; i < n_goal; ++i) {
+    goal_dim[i] = p->goal_n_dims > 0 ? p->goal_dims[i] : i;
+    if (goal_dim[i] < 0 || goal_dim[i] >= D) return fail(nullptr, PAKR_ERR_INVALID_ARG, "goal_dims entry out of range");
+    for (int j = 0; j < i; ++j)
+      if (goal_dim[j] == goal_dim[i]) return fail(nullptr, PAKR_ERR_INVALID_ARG, "goal_dims entries must be distinct");
+    if (!std::isfinite(p->goal_center[i])) return fail(nullptr, PAKR_ERR_INVALID_ARG, "goal_center must be finite");
+  }
 
   auto* pl = new pakr_planner();
   pl->device = cuda_device;
@@ -350,21 +376,31 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
   for (int d = 0; d < D; ++d) {
     pb.lo[d] = p->state_lo[d]; pb.hi[d] = p->state_hi[d]; pb.w[d] = p->nn_weight[d]; pb.start[d] = p->start[d];
     if (pb.w[d] != 1.0f) unit = false;
-    if (d == angle) { pb.samp_lo[d] = -kPiF; pb.samp_span[d] = kPiF - (-kPiF); }
+    if (angle_dim(d)) { pb.samp_lo[d] = -kPiF; pb.samp_span[d] = kPiF - (-kPiF); }
     else if (std::isfinite(pb.lo[d]) && std::isfinite(pb.hi[d])) { pb.samp_lo[d] = pb.lo[d]; pb.samp_span[d] = pb.hi[d] - pb.lo[d]; }
     else { pb.samp_lo[d] = 0.0f; pb.samp_span[d] = 0.0f; }
   }
   for (int j = 0; j < M; ++j) { pb.ulo[j] = p->control_lo[j]; pb.uhi[j] = p->control_hi[j]; pb.uspan[j] = pb.uhi[j] - pb.ulo[j]; }
-  for (int a = 0; a < PD; ++a) pb.goal[a] = p->goal_center[a];
+  for (int i = 0; i < n_goal; ++i) { pb.goal_c[goal_dim[i]] = p->goal_center[i]; pb.goal_m[goal_dim[i]] = 1.0f; }
   pb.goal_r = p->goal_radius; pb.goal_angle = p->goal_angle; pb.goal_angle_tol = p->goal_angle_tol;
   pb.goal_angle_dim = p->goal_angle_dim;
-  for (int i = 0; i < 5 && i < p->n_dyn_params; ++i) pb.dyn[i] = p->dyn_params[i];
+  if (dyn == DYN_ACRO) {  // the lumped constants dyn_f<DYN_ACRO> reads (P35)
+    const double m1 = p->dyn_params[0], m2 = p->dyn_params[1], l1 = p->dyn_params[2], lc1 = p->dyn_params[3],
+                 lc2 = p->dyn_params[4], I1 = p->dyn_params[5], I2 = p->dyn_params[6], g = p->dyn_params[7];
+    pb.dyn[0] = (float)(I1 + I2 + m1 * lc1 * lc1 + m2 * (l1 * l1 + lc2 * lc2));
+    pb.dyn[1] = (float)(m2 * l1 * lc2);
+    pb.dyn[2] = (float)(I2 + m2 * lc2 * lc2);
+    pb.dyn[3] = (float)((m1 * lc1 + m2 * l1) * g);
+    pb.dyn[4] = (float)(m2 * lc2 * g);
+  } else {
+    for (int i = 0; i < 5 && i < p->n_dyn_params; ++i) pb.dyn[i] = p->dyn_params[i];
+  }
   if (dyn == DYN_QUAD || dyn == DYN_QUADB)
     for (int i = 0; i < 4; ++i) pb.dyn[5 + i] = 1.0f / p->dyn_params[i];
   pb.dt = p->dt; pb.S = p->steps_per_edge; pb.integrator = p->integrator; pb.cost_mode = p->cost_mode;
   pb.inv_hspeed = std::isinf(p->heuristic_speed) ? 0.0f : 1.0f / p->heuristic_speed;
   pb.unit_weights = unit ? 1 : 0;
-  pl->index_ok = idx_key_layout(pb, D, angle);  // the tier is chosen per call (pakr_plan_opts.nn_mode)
+  pl->index_ok = idx_key_layout(pb, D, angles);  // the tier is chosen per call (pakr_plan_opts.nn_mode)
   pb.n_obs = p->n_obstacles;
 
   // obstacle table in the kernel's shared-memory row format
@@ -522,8 +558,11 @@ void fill_stats(const Ctrl* hc, int64_t BK, pakr_stats* out) {
 // nn_mode (PAKR_NN_*) -> Params::nn_index
 bool set_nn_mode(pakr_planner* pl, Params& P, int nn_mode) {
   if (nn_mode != PAKR_NN_AUTO && nn_mode != PAKR_NN_SCAN && nn_mode != PAKR_NN_INDEX) return false;
-  constexpr int kAutoIndex = 1;  // what PAKR_NN_AUTO means for the index: 1 = when B*n is large enough to pay
-  P.nn_index = !pl->index_ok ? 0 : nn_mode == PAKR_NN_INDEX ? 2 : nn_mode == PAKR_NN_AUTO ? kAutoIndex : 0;
+  // PAKR_NN_AUTO: the index kernel only from B = 4096 queries up.  Below that the brute-force scan wins on every
+  // measured tree (config 5 sweep): the index kernel carries more live state through its
+  // 128 registers, so its own scan loop is ~20 % slower, and a rebuild costs as much as scanning ~10^8 pairs.
+  constexpr int kAutoIndexMinB = 4096;
+  P.nn_index = !pl->index_ok ? 0 : nn_mode == PAKR_NN_INDEX ? 2 : (nn_mode == PAKR_NN_AUTO && P.B >= kAutoIndexMinB) ? 1 : 0;
   return true;
 }
 

@@ -16,17 +16,20 @@ constexpr float kPiF = 3.14159274101257324f;   // (float)pi
 constexpr float kTwoPiF = 6.28318548202514648f;
 
 // ---- compile-time description of a dynamics model -------------------------------------------
-enum DynKind { DYN_DI2 = 0, DYN_DI3 = 1, DYN_UNI2 = 2, DYN_QUAD = 3, DYN_DA = 4, DYN_UNI1 = 5, DYN_QUADB = 6 };
+enum DynKind { DYN_DI2 = 0, DYN_DI3 = 1, DYN_UNI2 = 2, DYN_QUAD = 3, DYN_DA = 4, DYN_UNI1 = 5, DYN_QUADB = 6, DYN_ACRO = 7 };
 enum ObsKind { OBS_CIRCLE = 0, OBS_BOX = 1 };
 
+// ANGLES: bit d set = state dim d is an angle (wrapped to [-pi, pi), never bounds-tested; P13)
 template <int DYN> struct DynTraits;
-template <> struct DynTraits<DYN_DI2> { static constexpr int D = 4, M = 2, PD = 2, DP = 4, ANGLE = -1; };
-template <> struct DynTraits<DYN_DI3> { static constexpr int D = 6, M = 3, PD = 3, DP = 8, ANGLE = -1; };
-template <> struct DynTraits<DYN_UNI2> { static constexpr int D = 5, M = 2, PD = 2, DP = 8, ANGLE = 2; };
-template <> struct DynTraits<DYN_QUAD> { static constexpr int D = 12, M = 4, PD = 3, DP = 12, ANGLE = 8; };
-template <> struct DynTraits<DYN_DA> { static constexpr int D = 6, M = 3, PD = 3, DP = 8, ANGLE = 3; };
-template <> struct DynTraits<DYN_UNI1> { static constexpr int D = 3, M = 2, PD = 2, DP = 4, ANGLE = 2; };
-template <> struct DynTraits<DYN_QUADB> { static constexpr int D = 12, M = 4, PD = 3, DP = 12, ANGLE = 5; };
+template <> struct DynTraits<DYN_DI2> { static constexpr int D = 4, M = 2, PD = 2, DP = 4; static constexpr unsigned ANGLES = 0u; };
+template <> struct DynTraits<DYN_DI3> { static constexpr int D = 6, M = 3, PD = 3, DP = 8; static constexpr unsigned ANGLES = 0u; };
+template <> struct DynTraits<DYN_UNI2> { static constexpr int D = 5, M = 2, PD = 2, DP = 8; static constexpr unsigned ANGLES = 1u << 2; };
+template <> struct DynTraits<DYN_QUAD> { static constexpr int D = 12, M = 4, PD = 3, DP = 12; static constexpr unsigned ANGLES = 1u << 8; };
+template <> struct DynTraits<DYN_DA> { static constexpr int D = 6, M = 3, PD = 3, DP = 8; static constexpr unsigned ANGLES = 1u << 3; };
+template <> struct DynTraits<DYN_UNI1> { static constexpr int D = 3, M = 2, PD = 2, DP = 4; static constexpr unsigned ANGLES = 1u << 2; };
+template <> struct DynTraits<DYN_QUADB> { static constexpr int D = 12, M = 4, PD = 3, DP = 12; static constexpr unsigned ANGLES = 1u << 5; };
+template <> struct DynTraits<DYN_ACRO> { static constexpr int D = 4, M = 1, PD = 2, DP = 4; static constexpr unsigned ANGLES = 3u; };
+template <int DYN> __host__ __device__ constexpr bool is_angle(int d) { return (DynTraits<DYN>::ANGLES >> d) & 1u; }
 
 // Problem constants, passed by value in the kernel parameter block.
 struct DevProblem {
@@ -35,10 +38,11 @@ struct DevProblem {
   float samp_lo[kMaxD], samp_span[kMaxD];  // sampling: fmaf(u, span, lo), span = fl32(hi - lo)
   float ulo[kMaxM], uhi[kMaxM], uspan[kMaxM];
   float start[kMaxD];
-  float goal[3];
+  float goal_c[kMaxD], goal_m[kMaxD];  // goal ball: centre per state dim, mask 1 on the goal dims (0 elsewhere)
   float goal_r, goal_angle, goal_angle_tol;
   int goal_angle_dim;
   float dyn[12];                       // quadrotor: m, Ixx, Iyy, Izz, g, then 1/m, 1/Ixx, 1/Iyy, 1/Izz
+                                       // Acrobot: the five lumped constants of dyn_f (set by the host)
   float dt;
   int S;
   int integrator;                      // 0 Euler, 1 RK4
@@ -186,6 +190,24 @@ __device__ __forceinline__ void dyn_f(const DevProblem& pb, const float (&x)[Dyn
     xd[9] = (u[1] - (Izz - Iyy) * q * r) * pb.dyn[6];
     xd[10] = (u[2] - (Ixx - Izz) * p * r) * pb.dyn[7];
     xd[11] = (u[3] - (Iyy - Ixx) * p * q) * pb.dyn[8];
+  } else if constexpr (DYN == DYN_ACRO) {
+    // PAPER.md:209 (P35): D(q) qdd + c(q, qd) = -dV/dq + (0, tau), theta1 from the downward vertical.
+    // Host-lumped constants: A = I1 + I2 + m1 lc1^2 + m2 (l1^2 + lc2^2), Bc = m2 l1 lc2, C = I2 + m2 lc2^2,
+    // Ga = (m1 lc1 + m2 l1) g, Gb = m2 lc2 g.
+    const float A = pb.dyn[0], Bc = pb.dyn[1], C = pb.dyn[2], Ga = pb.dyn[3], Gb = pb.dyn[4];
+    float s2, c2;
+    sincosf(x[1], &s2, &c2);
+    const float s1 = sinf(x[0]), s12 = sinf(x[0] + x[1]);
+    const float w1 = x[2], w2 = x[3];
+    const float d11 = fmaf(2.0f * Bc, c2, A), d12 = fmaf(Bc, c2, C), d22 = C;
+    const float hh = Bc * s2;
+    const float r1 = fmaf(hh * w2, fmaf(2.0f, w1, w2), -fmaf(Ga, s1, Gb * s12));  // -dV/dth1 - c1
+    const float r2 = u[0] - fmaf(hh * w1, w1, Gb * s12);                         // tau - dV/dth2 - c2
+    const float idet = __frcp_rn(fmaf(d11, d22, -d12 * d12));
+    xd[0] = w1;
+    xd[1] = w2;
+    xd[2] = (d22 * r1 - d12 * r2) * idet;
+    xd[3] = (d11 * r2 - d12 * r1) * idet;
   } else {
     const float Ixx = pb.dyn[1], Iyy = pb.dyn[2], Izz = pb.dyn[3], g = pb.dyn[4];
     float sphi, cphi, sth, cth, spsi, cpsi;
@@ -280,7 +302,7 @@ __device__ __forceinline__ float bounds_margin(const DevProblem& pb, const float
   float m0 = __int_as_float(0x7f800000), m1 = m0;
 #pragma unroll
   for (int d = 0; d < DynTraits<DYN>::D; ++d)
-    if (d != DynTraits<DYN>::ANGLE) {
+    if (!is_angle<DYN>(d)) {
       m0 = fminf(m0, x[d] - pb.lo[d]);
       m1 = fminf(m1, pb.hi[d] - x[d]);
     }
@@ -384,11 +406,17 @@ __device__ __forceinline__ float cell_margin(uint32_t hdr, const uint16_t* __res
   return m;
 }
 
-template <int PD>
-__device__ __forceinline__ float goal_dist(const DevProblem& pb, const float* x) {
+// Distance to the goal centre over the goal dims (mask 1; a masked-out dim adds an exact +0), wrapped on angle dims.
+// `x` has its angle dims already wrapped to [-pi, pi).
+template <int DYN>
+__device__ __forceinline__ float goal_dist(const DevProblem& pb, const float (&x)[DynTraits<DYN>::D]) {
   float s = 0.0f;
 #pragma unroll
-  for (int a = 0; a < PD; ++a) { const float d = x[a] - pb.goal[a]; s = fmaf(d, d, s); }
+  for (int d = 0; d < DynTraits<DYN>::D; ++d) {
+    float e = x[d] - pb.goal_c[d];
+    if (is_angle<DYN>(d)) e = wrap_pi(e);
+    s = fmaf(e * pb.goal_m[d], e, s);
+  }
   return sqrtf(s);
 }
 

@@ -30,7 +30,8 @@ constexpr int kCtasPerSm = 2;
 constexpr int kWarps = kThreads / 32;
 constexpr int kQ = 4;            // queries per lane in the NN scan
 constexpr int kIdxMinRows = 4096;    // NN index: smaller trees are scanned
-constexpr long long kIdxMinPairs = 60000000ll;  // ... and so are iterations whose scan (B*n pairs) takes < ~30 us
+constexpr long long kIdxMinWork = 2400000000ll;  // ... and so are iterations whose scan (B*n*D) takes less than ~250 us:
+                                                 // measured crossover of scan vs rebuilds + search on config 5's trees
 constexpr long long kIdxRebuildWork = 400000000ll;  // rebuild once scanning the rows added since the last rebuild costs
                                                     // about as much as rebuilding: B * rows * D lane-ops (~50 us)
 constexpr int kPathMax = 8192;   // longest path the device buffers hold
@@ -164,7 +165,7 @@ __device__ __forceinline__ float dist2(const DevProblem& pb, const float (&q)[Dy
   float acc = 0.0f;
 #pragma unroll
   for (int d = 0; d < D; ++d) {
-    const float delta = (d == DynTraits<DYN>::ANGLE) ? angle_absdiff(q[d], p[d]) : (q[d] - p[d]);
+    const float delta = is_angle<DYN>(d) ? angle_absdiff(q[d], p[d]) : (q[d] - p[d]);
     if (UNIT_W) acc = fmaf(delta, delta, acc);
     else acc = fmaf(delta * pb.w[d], delta, acc);
   }
@@ -207,7 +208,7 @@ __device__ __forceinline__ void dist2x2(const DevProblem& pb, const f32x2 (&q2)[
 #pragma unroll
   for (int d = 0; d < D; ++d) {
     f32x2 delta;
-    if (d == DynTraits<DYN>::ANGLE) {
+    if (is_angle<DYN>(d)) {
       float qa, qb;
       unpack2(q2[d], qa, qb);
       delta = pack2(angle_absdiff(qa, p[d]), angle_absdiff(qb, p[d]));
@@ -583,7 +584,7 @@ __device__ __forceinline__ float idx_box_bound(const DevProblem& pb, const float
   float acc = 0.0f;
 #pragma unroll
   for (int d = 0; d < D; ++d) {
-    if (d == DynTraits<DYN>::ANGLE) continue;  // wrapped dims take no part in the bound (they add >= 0)
+    if (is_angle<DYN>(d)) continue;  // wrapped dims take no part in the bound (they add >= 0)
     const float l = __ldcg(&lo[(group * D + d) * 32 + j]), h = __ldcg(&hi[(group * D + d) * 32 + j]);
     const float e = fmaxf(fmaxf(l - q[d], q[d] - h), 0.0f);
     acc = fmaf(e * pb.w[d], e, acc);
@@ -947,14 +948,18 @@ __device__ __forceinline__ void prop_phase(const Params& P, uint32_t r, uint32_t
     for (int d = 0; d < D; ++d) finite = finite & (fabsf(x[d]) <= 3.4e38f);
     const bool inb = (bm >= 0.0f) & finite;  // closed box (P12); a non-finite state is out of bounds
     const bool cf = om > 0.0f;               // closed obstacles (P11)
-    if (T::ANGLE >= 0) x[T::ANGLE >= 0 ? T::ANGLE : 0] = wrap_pi(x[T::ANGLE >= 0 ? T::ANGLE : 0]);
+#pragma unroll
+    for (int d = 0; d < D; ++d)
+      if (is_angle<DYN>(d)) x[d] = wrap_pi(x[d]);
     const float edge = (pb.cost_mode == 1) ? length : (float)pb.S * pb.dt;
     const float c_new = parent_cost + edge;
-    const float gd = goal_dist<PD>(pb, x);
+    const float gd = goal_dist<DYN>(pb, x);
     const float h = fmaxf(0.0f, gd - pb.goal_r) * pb.inv_hspeed;
     const bool notpruned = (c_new + h) < c_best;
     bool ing = gd <= pb.goal_r;
-    if (pb.goal_angle_dim >= 0) ing = ing && (fabsf(wrap_pi(x[T::ANGLE >= 0 ? T::ANGLE : 0] - pb.goal_angle)) <= pb.goal_angle_tol);
+#pragma unroll
+    for (int d = 0; d < D; ++d)  // optional heading tolerance on one of the angle dims
+      if (is_angle<DYN>(d) && d == pb.goal_angle_dim) ing = ing && (fabsf(wrap_pi(x[d] - pb.goal_angle)) <= pb.goal_angle_tol);
     const bool valid = inb && cf;
     const bool keep = valid && notpruned;
     const int flags = (valid ? 1 : 0) | (inb ? 2 : 0) | (cf ? 4 : 0) | (notpruned ? 8 : 0) | ((keep && ing) ? 16 : 0);
@@ -1301,7 +1306,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       // whole NN of the iteration runs at its head, right after the rebuild, instead of one iteration ahead: the
       // rows of the previous batch are then inside the index and need no brute-force pass of their own.
       bool idx_use = false;
-      if constexpr (INDEX) idx_use = P.nn_index == 2 ? n >= 256 : (n >= kIdxMinRows && (long long)P.B * n >= kIdxMinPairs);
+      if constexpr (INDEX) idx_use = P.nn_index == 2 ? n >= 256 : (n >= kIdxMinRows && (long long)P.B * n * T::D >= kIdxMinWork);
       if (!idx_use) n_sorted = 0;
       const bool idx_head = idx_use && !split;
       if constexpr (INDEX) {

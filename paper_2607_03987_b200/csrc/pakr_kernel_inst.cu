@@ -2,7 +2,7 @@
 // Compiled once per (tier, part) so that the sets build in parallel and a rarely used tier costs the common one
 // no registers:  -DPAKR_STREAM_TIER=0 tiled NN scan (the normal case), =1 streaming NN tier for B <= 16,
 // =2 tiled scan + NN index tier;
-// -DPAKR_PART=0 double integrators and unicycles, =1 quadrotors and the Dubins airplane.
+// -DPAKR_PART=0 double integrators, unicycles and the Acrobot, =1 quadrotors and the Dubins airplane.
 #include "pakr_kernel.cuh"
 
 #ifndef PAKR_STREAM_TIER
@@ -34,6 +34,7 @@ extern "C" const void* PAKR_SELECT_NAME(PAKR_STREAM_TIER, PAKR_PART)(int dyn, in
     case DYN_UNI2 * 2 + OBS_BOX: return kernel_ptr<DYN_UNI2, OBS_BOX>();
     case DYN_UNI1 * 2 + OBS_CIRCLE: return kernel_ptr<DYN_UNI1, OBS_CIRCLE>();
     case DYN_UNI1 * 2 + OBS_BOX: return kernel_ptr<DYN_UNI1, OBS_BOX>();
+    case DYN_ACRO * 2 + OBS_CIRCLE: return kernel_ptr<DYN_ACRO, OBS_CIRCLE>();  // no obstacles: one variant
 #else
     case DYN_QUAD * 2 + OBS_CIRCLE: return kernel_ptr<DYN_QUAD, OBS_CIRCLE>();
     case DYN_QUAD * 2 + OBS_BOX: return kernel_ptr<DYN_QUAD, OBS_BOX>();

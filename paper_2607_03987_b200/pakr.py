@@ -94,6 +94,7 @@ class _Problem(C.Structure):
         ("goal_angle_dim", C.c_int32), ("goal_angle", C.c_float), ("goal_angle_tol", C.c_float),
         ("dt", C.c_float), ("steps_per_edge", C.c_int32),
         ("cost_mode", C.c_int32), ("heuristic_speed", C.c_float),
+        ("goal_n_dims", C.c_int32), ("goal_dims", _ip),
     ]
 
 
@@ -197,12 +198,14 @@ def make_problem_struct(p):
     keep = dict(dyn=_f32(p.dyn_params if len(p.dyn_params) else [0.0]), lo=_f32(p.state_lo), hi=_f32(p.state_hi),
                 kind=np.ascontiguousarray(p.dim_kind, dtype=np.uint8), w=_f32(p.nn_weight), ulo=_f32(p.control_lo),
                 uhi=_f32(p.control_hi), obs=_f32(p.obstacles.reshape(-1) if p.n_obstacles else [0.0]),
-                start=_f32(p.start), goal=_f32(p.goal_center))
+                start=_f32(p.start), goal=_f32(p.goal_center),
+                gdims=np.ascontiguousarray(p.goal_dims if p.goal_dims is not None else [0], dtype=np.int32))
     s = _Problem(p.dynamics_id, p.integrator, p.state_dim, p.control_dim, p.pos_dim, _ptr(keep["dyn"]),
                  len(p.dyn_params), _ptr(keep["lo"]), _ptr(keep["hi"]), _ptr(keep["kind"], _up), _ptr(keep["w"]),
                  _ptr(keep["ulo"]), _ptr(keep["uhi"]), p.obstacle_type, _ptr(keep["obs"]), p.n_obstacles,
                  _ptr(keep["start"]), _ptr(keep["goal"]), p.goal_radius, p.goal_angle_dim, p.goal_angle,
-                 p.goal_angle_tol, p.dt, p.steps_per_edge, p.cost_mode, p.heuristic_speed)
+                 p.goal_angle_tol, p.dt, p.steps_per_edge, p.cost_mode, p.heuristic_speed,
+                 0 if p.goal_dims is None else len(p.goal_dims), _ptr(keep["gdims"], _ip))
     return s, keep
 
 

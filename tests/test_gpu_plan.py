@@ -61,7 +61,7 @@ def _check_tree(orc, op, p, tree, cap, n_samples=300):
         assert d.max() < 1e-4
 
 
-@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "N1", "N2", "N3"])
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "N1", "N2", "N3", "N4"])
 def test_plan_configs(pakr, orc, name):
     p, cfg = wl.CONFIGS[name]()
     pl = pakr.Planner(p)
@@ -170,14 +170,27 @@ def test_abi_errors(pakr):
     # invalid problems never reach the device
     import dataclasses
     for bad in (dataclasses.replace(p, state_dim=5), dataclasses.replace(p, dt=0.0),
-                dataclasses.replace(p, state_lo=p.state_hi + 1), dataclasses.replace(p, dynamics_id=9)):
+                dataclasses.replace(p, state_lo=p.state_hi + 1), dataclasses.replace(p, dynamics_id=9),
+                dataclasses.replace(p, goal_dims=np.array([0, 4], np.int32)),      # goal dim out of range
+                dataclasses.replace(p, goal_dims=np.array([1, 1], np.int32))):     # repeated goal dim
         with pytest.raises(pakr.PakrError) as e:
             pakr.Planner(bad)
         assert e.value.status in (1, 2)
     pl.close()
+    # the Acrobot takes no obstacles (its position dims are angles) and needs its eight parameters
+    a, _ = wl.CONFIGS["N4"]()
+    with pytest.raises(pakr.PakrError) as e:
+        pakr.Planner(dataclasses.replace(a, obstacles=np.array([[0.0, 0.0, 0.5]], np.float32)))
+    assert e.value.status == 2
+    with pytest.raises(pakr.PakrError) as e:
+        pakr.Planner(dataclasses.replace(a, dyn_params=a.dyn_params[:5]))
+    assert e.value.status == 1
+    with pytest.raises(pakr.PakrError) as e:
+        pakr.Planner(dataclasses.replace(a, dim_kind=np.array([1, 0, 0, 0], np.uint8)))
+    assert e.value.status == 2
 
 
-@pytest.mark.parametrize("name,iters", [("C1", 12), ("C2", 9), ("C3", 6), ("N1", 7), ("N2", 8)])
+@pytest.mark.parametrize("name,iters", [("C1", 12), ("C2", 9), ("C3", 6), ("N1", 7), ("N2", 8), ("N4", 8)])
 def test_plan_loop_equals_chain_of_single_steps(pakr, name, iters):
     """The device-resident loop (NN look-ahead scan, fused tail scan, two key buffers) must build exactly
     the tree that `iters` separate pakr_expand_step calls build (no look-ahead there): bit-exact."""
@@ -206,7 +219,7 @@ def test_plan_loop_equals_chain_of_single_steps(pakr, name, iters):
     pl.close()
 
 
-@pytest.mark.parametrize("name,seeds", [("C1", 12), ("C2", 8), ("N2", 6)])
+@pytest.mark.parametrize("name,seeds", [("C1", 12), ("C2", 8), ("N2", 6), ("N4", 6)])
 def test_plan_many_seeds_validated(pakr, orc, name, seeds):
     """Every returned plan of a spread of planner seeds is re-propagated by the oracle (north_star end-to-end bar)."""
     p, cfg = wl.CONFIGS[name]()

@@ -45,6 +45,9 @@ _CASES = [
     ("N2", 20000, 1024, 8),
     ("N3", 2500, 384, 16),  # quadcopter with body-frame velocities, PAPER.md:174 (NEXT-2)
     ("N3", 15000, 1024, 8),
+    ("N4", 1, 64, 4),       # Acrobot, PAPER.md:209 (NEXT-2): two angle dims, goal ball in angle space
+    ("N4", 4097, 300, 5),
+    ("N4", 20000, 1024, 8),
     # B*K > 65,536 (more than 2048 warp units: the insert's per-thread-chunk prefix) and K = 64, as config 5 runs them
     ("C2", 5000, 2048, 64),   # B*K = 131,072
     ("C5", 5000, 4096, 64),   # B*K = 262,144, 128 boxes
@@ -124,6 +127,42 @@ def test_step_prune_goal_and_overflow(pakr, orc):
             assert st["n_inserted"] == 0 and after["n"] == n0
         if cap == n0 + 37:
             assert after["n"] == cap
+    pl.close()
+
+
+def test_step_goal_ball_over_listed_dims(pakr, orc):
+    """pakr_problem.goal_dims: (i) the Acrobot's ball in (theta1, theta2) around (pi, 0) with nodes parked on both
+    sides of the +-pi seam, so the wrapped difference decides; (ii) a double integrator whose goal ball spans a
+    position AND a velocity dim (h = 0).  Goal flags, winner and c_best must match the oracle."""
+    from parity_util import check_iteration, run_both
+    p, _ = wl.CONFIGS["N4"]()
+    rng = np.random.default_rng(3)
+    n0, B, K = 600, 256, 4
+    host = wl.random_tree(p, n0, seed=4)
+    side = np.where(rng.random(n0 - 1) < 0.5, 1.0, -1.0)
+    host["states"][1:, 0] = (side * (np.pi - rng.uniform(0.02, 0.5, n0 - 1))).astype(np.float32)
+    host["states"][1:, 1] = rng.uniform(-0.5, 0.5, n0 - 1).astype(np.float32)
+    host["states"][1:, 2:] = rng.uniform(-1.0, 1.0, (n0 - 1, 2)).astype(np.float32)
+    pl = pakr.Planner(p)
+    op = orc.OracleProblem(p)
+    for c_best in (float("inf"), 3.0):
+        out, after, ref, _ = run_both(pl, orc, op, p, host, seed=2, r=0, it=3, B=B, K=K, c_best=c_best)
+        st = check_iteration(orc, op, p, host, out, after, ref, B, K, n0 + B * K)
+        if c_best == float("inf"):
+            assert st["n_goal"] > 5
+            goal_rows = after["states"][n0:][(out["child_flags"][(out["child_flags"] & 32) != 0] & 16) != 0]
+            assert (goal_rows[:, 0] > 2.5).any() and (goal_rows[:, 0] < -2.5).any()  # both sides of the seam
+    pl.close()
+    p1, _ = wl.config1()
+    p1 = dataclasses.replace(p1, obstacles=p1.obstacles[:2], goal_dims=np.array([1, 2], np.int32),
+                             goal_center=np.array([9.0, 0.25], np.float32), goal_radius=0.6, heuristic_speed=float("inf"))
+    host = wl.random_tree(p1, 400, seed=9)
+    host["states"][1:, 1] = rng.uniform(8.0, 9.8, 399).astype(np.float32)
+    pl = pakr.Planner(p1)
+    op = orc.OracleProblem(p1)
+    out, after, ref, _ = run_both(pl, orc, op, p1, host, seed=5, r=1, it=0, B=B, K=K)
+    st = check_iteration(orc, op, p1, host, out, after, ref, B, K, 400 + B * K)
+    assert 3 < st["n_goal"] < st["n_inserted"]
     pl.close()
 
 
@@ -287,7 +326,7 @@ def test_nn_tiers_agree_bit_for_bit(pakr, name):
 @pytest.mark.parametrize("name,n0,B,K", [("C2", 20000, 512, 2), ("C3", 9000, 300, 3), ("C3", 40000, 257, 2),
                                          ("C1", 700, 64, 4), ("C5", 60000, 1024, 1), ("C4", 30000, 512, 2),
                                          ("C4", 1025, 300, 1), ("N1", 5000, 256, 2), ("N2", 33000, 400, 2),
-                                         ("N3", 70000, 256, 1), ("C2", 300000, 2048, 1)])
+                                         ("N3", 70000, 256, 1), ("C2", 300000, 2048, 1), ("N4", 9000, 300, 2)])
 def test_nn_index_tier_equals_scan_tier(pakr, orc, name, n0, B, K):
     """The NN index (exact spatial pruning) must return bit-identical NN indices
     and distances to the brute-force scan, on clustered trees too (queries far from every node search wide),
