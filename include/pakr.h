@@ -53,10 +53,12 @@ enum { PAKR_COST_DURATION = 0, PAKR_COST_PATH_LENGTH = 1 };
 enum { PAKR_DIM_REAL = 0, PAKR_DIM_ANGLE = 1 };
 enum { PAKR_NO_SOLUTION = 0, PAKR_SOLVED = 1 }; /* "no solution" is not an error */
 /* nearest-neighbour tier (pakr_plan_opts.nn_mode, pakr_step_args.nn_mode) */
-enum { PAKR_NN_AUTO = 0,  /* the library picks: brute-force scan tiers, and from B = 4096 queries up the spatial index
-                             once the tree is large enough to pay for building it */
-       PAKR_NN_SCAN = 1,  /* brute-force scan tiers only (tiled; streaming when B <= 16) */
-       PAKR_NN_INDEX = 2  /* spatial index on every tree of >= 256 nodes (tests) */ };
+enum { PAKR_NN_AUTO = 0,  /* the library picks: the brute-force fp32 scan below B = 4096 queries; from there up the
+                             tensor-core filter for 12-D models and the spatial index otherwise */
+       PAKR_NN_SCAN = 1,  /* brute-force fp32 scan tiers only (tiled; streaming when B <= 16) */
+       PAKR_NN_INDEX = 2, /* spatial index on every tree of >= 256 nodes (tests) */
+       PAKR_NN_FILTER = 3 /* tensor-core coarse filter (fp16 hi/lo mma.sync, fp32 accumulate) on every scan of >= 4096
+                             rows that is long enough to pay, exact fp32 rescoring of its candidates */ };
 
 /* child flag bits written by pakr_expand_step (Alg. 1 l.10-14) */
 enum {
@@ -156,8 +158,10 @@ typedef struct {
   int64_t children;        /* = iterations * B * K propagated and checked ("expanded nodes") */
   int64_t inserted;        /* nodes appended over all replans */
   int64_t nn_pairs;        /* sum over iterations of B * n: the (query, node) pairs of the NN definition */
-  int64_t nn_pairs_evaluated; /* distances actually evaluated: = nn_pairs under the scan tiers, fewer when the NN
-                              index answered (it scores only rows whose bounding box can beat the running best) */
+  int64_t nn_pairs_evaluated; /* fp32 distances actually evaluated: = nn_pairs under the plain scan tiers; fewer when the
+                              NN index answered (it scores only rows whose bounding box can beat the running best) or
+                              the tensor-core filter did (only the rows of its candidate ranges are rescored exactly) */
+  int64_t nn_pairs_filtered;  /* pairs answered by the tensor-core coarse filter (fp16 hi/lo mma, fp32 accumulate) */
   int64_t h2d_bytes, d2h_bytes; /* bytes pakr_plan copied host->device (root node) and device->host (control
                                    block, path) in this call; kernel parameters (~1.3 KB) not counted */
   int32_t replans_run, replans_solved;

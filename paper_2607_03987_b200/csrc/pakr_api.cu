@@ -24,11 +24,13 @@ struct pakr_planner {
   uint32_t* d_grid_cells = nullptr;
   uint16_t* d_grid_list = nullptr;
   int num_sms = 0, blocks_per_sm = 0;
+  bool filter_ok = false; // tensor-core NN filter usable: every feature fits fp16 (pakr_nn_filter.cuh)
   bool index_ok = false;  // NN spatial index usable: finite position box, positive position weights, kernel built
   size_t smem_bytes = 0;
   const void* kernel = nullptr;         // tiled NN scan
   const void* kernel_stream = nullptr;  // streaming NN tier (B <= kStreamB)
-  const void* kernel_index = nullptr;   // tiled scan + NN cell index (only when nn_index != 0)
+  const void* kernel_index = nullptr;   // tiled scan + NN index (only when nn_index != 0)
+  const void* kernel_filter = nullptr;  // tiled scan + tensor-core coarse filter
   void* h_pinned = nullptr;  // Ctrl + path staging
   std::string err;
 };
@@ -42,6 +44,8 @@ extern "C" const void* pakr_select_kernel_t1_0(int dyn, int obs);
 extern "C" const void* pakr_select_kernel_t1_1(int dyn, int obs);
 extern "C" const void* pakr_select_kernel_t2_0(int dyn, int obs);
 extern "C" const void* pakr_select_kernel_t2_1(int dyn, int obs);
+extern "C" const void* pakr_select_kernel_t3_0(int dyn, int obs);
+extern "C" const void* pakr_select_kernel_t3_1(int dyn, int obs);
 
 static const void* pakr_select_kernel_tiled(int dyn, int obs) {
   const void* k = pakr_select_kernel_t0_0(dyn, obs);
@@ -56,13 +60,18 @@ static const void* pakr_select_kernel_index(int dyn, int obs) {
   return k ? k : pakr_select_kernel_t2_1(dyn, obs);
 }
 
+static const void* pakr_select_kernel_filter(int dyn, int obs) {
+  const void* k = pakr_select_kernel_t3_0(dyn, obs);
+  return k ? k : pakr_select_kernel_t3_1(dyn, obs);
+}
+
 namespace {
 
 constexpr size_t kAlign = 256;
 size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-  size_t states, actions, parents, costs, nn_key, unit_count, scr_state, scr_ctrl, scr_cost, scr_parent,
+  size_t states, actions, parents, costs, nn_key, frow, chunkmin, unit_count, scr_state, scr_ctrl, scr_cost, scr_parent,
       scr_flags, idx_keys, idx_ids, idx_hist, idx_ctasum, idx_tile_ids, idx_rows, idx_tlo, idx_thi, idx_slo, idx_shi,
       ctrl, path_rev, path_nodes, path_states, path_controls, total;
 };
@@ -77,6 +86,8 @@ Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap) {
   L.parents = take((size_t)cap * 4);
   L.costs = take((size_t)cap * 4);
   L.nn_key = take((size_t)B * 16);  // two iterations in flight
+  L.frow = take(((size_t)cap + 8) * 96);                            // filter rows: K <= 48 halves
+  L.chunkmin = take((size_t)B * kFilterMaxChunks * 4);
   L.unit_count = take(std::max<size_t>(U, kFuseUnits + 8) * 4);
   {  // NN index; nothing when the problem cannot be indexed
     const size_t on = pl->index_ok ? 1 : 0;
@@ -400,7 +411,34 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
   pb.dt = p->dt; pb.S = p->steps_per_edge; pb.integrator = p->integrator; pb.cost_mode = p->cost_mode;
   pb.inv_hspeed = std::isinf(p->heuristic_speed) ? 0.0f : 1.0f / p->heuristic_speed;
   pb.unit_weights = unit ? 1 : 0;
-  pl->index_ok = idx_key_layout(pb, D, angles);  // the tier is chosen per call (pakr_plan_opts.nn_mode)
+  pl->index_ok = idx_key_layout(pb, D, angles);
+  {
+    // tensor-core NN filter: features u_d = sqrt(w_d) (x_d - centre_d) of the real dims, sqrt(w) (cos, sin) of the
+    // angle dims, |u_real|^2.  S_max bounds sum_i |c_i u_i| over the state box (c = (-2 v, 1)): |u|^2 <= sum U_d^2,
+    // 2 |v.u| <= 2 sum U_d^2, 2 w per angle dim; U_d = sqrt(w_d) (hi_d - lo_d) / 2.
+    double sum_u2 = 0.0, w_ang = 0.0;
+    bool ok = true;
+    for (int d = 0; d < D; ++d) {
+      pb.f_scale[d] = std::sqrt(pb.w[d]);
+      if (angle_dim(d)) { w_ang += pb.w[d]; pb.f_ctr[d] = 0.0f; continue; }
+      if (pb.w[d] > 0.0f) {  // finite box (validated above)
+        pb.f_ctr[d] = 0.5f * pb.lo[d] + 0.5f * pb.hi[d];
+        const double U = std::sqrt((double)pb.w[d]) * 0.5 * ((double)pb.hi[d] - pb.lo[d]);
+        sum_u2 += U * U;
+      } else {
+        pb.f_ctr[d] = 0.0f;  // weight 0: the feature is 0 whatever the coordinate
+      }
+    }
+    const double s_max = 3.0 * sum_u2 + 2.0 * w_ang;
+    if (!(sum_u2 < 3.0e4) || !(s_max > 0.0)) ok = false;  // |u|^2 and every coefficient must fit fp16
+    // An angle dim enters through the lower bound w (2 - 2 cos delta) <= w delta^2, loose by up to w (pi^2 - 4): with a
+    // heavy angle weight (unicycle heading, Acrobot joints) nearly every chunk stays a candidate, so those problems keep
+    // the fp32 scan.  (Exact alternative, not built: two shifted copies of the query per angle dim.)
+    if (w_ang > 0.1) ok = false;
+    pb.f_qn_ang = (float)(2.0 * w_ang);
+    pb.f_band = (float)(s_max * (1.0 / 131072.0));
+    pl->filter_ok = ok;
+  }  // the tier is chosen per call (pakr_plan_opts.nn_mode)
   pb.n_obs = p->n_obstacles;
 
   // obstacle table in the kernel's shared-memory row format
@@ -453,19 +491,25 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
   pl->kernel_stream = pakr_select_kernel_stream(dyn, obs);
   pl->kernel_index = pakr_select_kernel_index(dyn, obs);
   if (!pl->kernel_index) { pl->kernel_index = pl->kernel; pl->index_ok = false; }  // no index tier for this model
+  pl->kernel_filter = pakr_select_kernel_filter(dyn, obs);
+  if (!pl->kernel_filter) { pl->kernel_filter = pl->kernel; pl->filter_ok = false; }
   pl->smem_bytes = smem_for(pl);
   e = cudaFuncSetAttribute(pl->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes);
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute(pl->kernel_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes);
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute(pl->kernel_index, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(pl->kernel_filter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem_bytes);
   if (e != cudaSuccess) return bail(PAKR_ERR_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&pl->blocks_per_sm, pl->kernel, kThreads, pl->smem_bytes);
   int occ_stream = 0;
   if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_stream, pl->kernel_stream, kThreads, pl->smem_bytes);
   int occ_index = 0;
   if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_index, pl->kernel_index, kThreads, pl->smem_bytes);
-  pl->blocks_per_sm = std::min(pl->blocks_per_sm, std::min(occ_stream, occ_index));  // one grid size for all tiers
+  int occ_filter = 0;
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_filter, pl->kernel_filter, kThreads, pl->smem_bytes);
+  pl->blocks_per_sm = std::min(std::min(pl->blocks_per_sm, occ_filter), std::min(occ_stream, occ_index));  // one grid size for all tiers
   if (e != cudaSuccess || pl->blocks_per_sm < 1)
     return bail(PAKR_ERR_CUDA, "kernel does not fit on an SM (occupancy 0)");
   e = cudaMallocHost(&pl->h_pinned, sizeof(Ctrl) + (size_t)kPathMax * (4 + kMaxD * 4 + kMaxM * 4));
@@ -507,6 +551,8 @@ void fill_common(const pakr_planner* pl, Params& P, const Layout& L, char* ws, i
   P.pb = pl->pb;
   P.nn_key = reinterpret_cast<unsigned long long*>(ws + L.nn_key);
   P.unit_count = reinterpret_cast<unsigned*>(ws + L.unit_count);
+  P.frow = reinterpret_cast<__half*>(ws + L.frow);
+  P.chunkmin = reinterpret_cast<float*>(ws + L.chunkmin);
   P.idx_keys = reinterpret_cast<unsigned*>(ws + L.idx_keys);
   P.idx_ids = reinterpret_cast<int*>(ws + L.idx_ids);
   P.idx_hist = reinterpret_cast<unsigned*>(ws + L.idx_hist);
@@ -537,7 +583,8 @@ void fill_stats(const Ctrl* hc, int64_t BK, pakr_stats* out) {
   s.children = hc->iterations * BK;
   s.inserted = hc->inserted;
   s.nn_pairs = hc->nn_pairs;
-  s.nn_pairs_evaluated = hc->nn_pairs - hc->nn_idx_covered + (int64_t)hc->nn_scored;
+  s.nn_pairs_evaluated = hc->nn_pairs - hc->nn_idx_covered + (int64_t)hc->nn_scored - hc->nn_filtered + (int64_t)hc->nn_rescored;
+  s.nn_pairs_filtered = hc->nn_filtered;
   for (int i = 0; i < 4; ++i) s.phase_ms[i] = (double)hc->phase_ns[i] * 1e-6;
   s.replans_run = hc->replans_run;
   s.replans_solved = hc->replans_solved;
@@ -557,12 +604,24 @@ void fill_stats(const Ctrl* hc, int64_t BK, pakr_stats* out) {
 // memset of the control words + one cooperative launch; everything on `stream`
 // nn_mode (PAKR_NN_*) -> Params::nn_index
 bool set_nn_mode(pakr_planner* pl, Params& P, int nn_mode) {
-  if (nn_mode != PAKR_NN_AUTO && nn_mode != PAKR_NN_SCAN && nn_mode != PAKR_NN_INDEX) return false;
-  // PAKR_NN_AUTO: the index kernel only from B = 4096 queries up.  Below that the brute-force scan wins on every
-  // measured tree (config 5 sweep): the index kernel carries more live state through its
-  // 128 registers, so its own scan loop is ~20 % slower, and a rebuild costs as much as scanning ~10^8 pairs.
-  constexpr int kAutoIndexMinB = 4096;
-  P.nn_index = !pl->index_ok ? 0 : nn_mode == PAKR_NN_INDEX ? 2 : (nn_mode == PAKR_NN_AUTO && P.B >= kAutoIndexMinB) ? 1 : 0;
+  if (nn_mode != PAKR_NN_AUTO && nn_mode != PAKR_NN_SCAN && nn_mode != PAKR_NN_INDEX && nn_mode != PAKR_NN_FILTER) return false;
+  // PAKR_NN_AUTO (measured on the config 5 sweep and C1-C4): below B = 4096 queries the plain scan
+  // kernel -- the trees those batches grow are too small for either accelerator to repay its fixed costs, and both
+  // accelerated kernels carry more live state through the 128 registers, so their own scan loop is slower.  From
+  // B = 4096 up: the tensor-core filter for 12-D models (weighted 12-D distances are where the fp32 scan is slowest
+  // and bounding boxes prune least), the spatial index otherwise.
+  constexpr int kAutoMinB = 4096;
+  const bool big = nn_mode == PAKR_NN_AUTO && P.B >= kAutoMinB;
+  P.nn_filter = pl->filter_ok && (nn_mode == PAKR_NN_FILTER || (big && pl->DP == 12)) ? 1 : 0;
+  P.nn_index = !pl->index_ok || P.nn_filter ? 0 : nn_mode == PAKR_NN_INDEX ? 2 : big ? 1 : 0;
+  P.filter_min_work = kFilterMinWork;
+  P.filter_give_up = kFilterGiveUp;
+  if (const char* e = getenv("PAKR_X_FMINWORK")) P.filter_min_work = atoll(e);  // EXPERIMENT ONLY -- remove
+  if (const char* e = getenv("PAKR_X_FGIVEUP")) P.filter_give_up = atoi(e);     // EXPERIMENT ONLY -- remove
+  P.idx_min_work = kIdxMinWork;
+  P.idx_rebuild_work = kIdxRebuildWork;
+  if (const char* e = getenv("PAKR_X_MINWORK")) P.idx_min_work = atoll(e);      // EXPERIMENT ONLY -- remove
+  if (const char* e = getenv("PAKR_X_REBUILD")) P.idx_rebuild_work = atoll(e);  // EXPERIMENT ONLY -- remove
   return true;
 }
 
@@ -573,7 +632,7 @@ pakr_status launch(pakr_planner* pl, Params& P, cudaStream_t stream) {
   CUDA_TRY(pl, cudaMemsetAsync(P.ctrl, 0xFF, sizeof(unsigned long long) * kSlots, stream));  // goal_key[] = none
   void* args[] = {&P};
   const dim3 grid(pl->num_sms * std::min(pl->blocks_per_sm, kCtasPerSm)), block(kThreads);
-  const void* kernel = P.B <= kStreamB ? pl->kernel_stream : (P.nn_index ? pl->kernel_index : pl->kernel);
+  const void* kernel = P.B <= kStreamB ? pl->kernel_stream : P.nn_filter ? pl->kernel_filter : P.nn_index ? pl->kernel_index : pl->kernel;
   CUDA_TRY(pl, cudaLaunchCooperativeKernel(kernel, grid, block, args, pl->smem_bytes, stream));
   return PAKR_OK;
 }

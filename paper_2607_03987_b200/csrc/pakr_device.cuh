@@ -58,6 +58,10 @@ struct DevProblem {
   int g_cells, g_list;                 // number of cells, total list entries
   const uint32_t* grid_cells;          // DEVICE [g_cells]: cell words, see cell_margin()
   const uint16_t* grid_list;           // DEVICE [g_list] obstacle ids
+  // tensor-core NN filter (pakr_nn_filter.cuh): feature u_d = (x_d - f_ctr[d]) * f_scale[d], f_scale = sqrt(w)
+  float f_ctr[kMaxD], f_scale[kMaxD];
+  float f_qn_ang;                      // 2 * sum of the angle dims' weights
+  float f_band;                        // bound of |approximate key - true key| (host: 2^-17 * S_max)
   // NN index: Morton key layout over the weighted state box (pakr_api.cu: idx_key_layout)
   float idx_scale[kMaxD];              // quantised coordinate = floor((x - lo) * scale), 0 .. 2^bits - 1
   uint8_t idx_bits[kMaxD];             // key bits of every dimension (0: not keyed)

@@ -20,6 +20,8 @@
 #pragma once
 #include <cooperative_groups.h>
 
+#include <cuda_fp16.h>
+
 #include "pakr_device.cuh"
 
 namespace pakr {
@@ -49,10 +51,14 @@ struct Ctrl {  // device control block (in the workspace)
   long long iterations, inserted, nn_pairs;
   unsigned long long nn_scored;  // (query, row) pairs the NN index tier scored, summed over its warps
   long long nn_idx_covered;      // sum over iterations of B * (rows the index answered for): pairs NOT scanned
+  long long nn_filtered;         // (query, row) pairs the tensor-core filter answered approximately
+  unsigned long long nn_rescored;         // ... and the rows its second phase rescored exactly, summed over the launch
+  unsigned long long f_rescored[kSlots];  // the same per iteration (slot rotation as goal_key)
   unsigned long long phase_ns[4];  // leader's time in NN / propagate / insert (incl. the grid sync after each) / index rebuilds
   int n_nodes;
   int stop[kSlots];        // 1: the time budget ran out during the iteration (written by the leader every iteration)
   unsigned pbar;           // arrival counter of the barrier among the propagate CTAs (insert inside phase X)
+  unsigned sbar;           // ... and of the one among the scan CTAs (between the two phases of the tensor-core NN filter)
   int iter_total[kSlots];  // survivors of the iteration, published by CTA 0 when the insert ran inside phase X
   int idx_query[2][kSlots];// NN index tier: next query to hand out ([0] whole-tree NN of the iteration, [1] look-ahead)
   int path_len, solved;
@@ -74,6 +80,8 @@ struct Params {
   unsigned long long* nn_key;  // [2][B] (d2 bits << 32) | node, combined with atomicMin; two iterations in flight
   // NN cell index (exact spatial pruning): tree rows [0, n_sorted) bucketed by position cell
   int nn_index;                // 0: scan tiers only; 1: index when B*n is large; 2: index whenever n >= 256 (tests)
+  long long idx_min_work, idx_rebuild_work;  // thresholds of nn_index == 1 (kIdxMinWork, kIdxRebuildWork)
+  long long filter_min_work; int filter_give_up;  // kFilterMinWork, kFilterGiveUp
   unsigned* idx_keys;          // [2][cap] Morton keys (radix-sort ping-pong)
   int* idx_ids;                // [2][cap] row ids, sorted together with the keys
   unsigned* idx_hist;          // [kIdxBins][sorting warps] digit histogram / scatter offsets
@@ -82,6 +90,10 @@ struct Params {
   float* idx_rows;             // [tiles][D][32] the sorted rows, dimension-major inside a tile
   float* idx_tlo; float* idx_thi;  // [super-tiles][D][32] boxes of the tiles
   float* idx_slo; float* idx_shi;  // [groups][D][32] boxes of the super-tiles
+  // tensor-core NN filter (pakr_nn_filter.cuh)
+  int nn_filter;               // host: 1 = launch the filter tier's kernel
+  __half* frow;                // [cap + 8][K halves] filter rows of the tree
+  float* chunkmin;             // [B][kFilterMaxChunks] minimum approximate key per (query, row range)
   unsigned* unit_count;        // [ceil(B*K/32)] survivors per warp unit
   float* scr_state; float* scr_ctrl; float* scr_cost; int* scr_parent; int* scr_flags;
   Ctrl* ctrl;
@@ -151,6 +163,7 @@ __device__ __forceinline__ void cta_group_barrier(unsigned* ctr, unsigned target
   __syncthreads();
 }
 
+constexpr int kTileBufFloats = 1024;  // every TMA tile buffer is 4 KB (two per warp)
 template <int DYN> struct TileCfg {  // nodes per TMA tile: <= 4 KB per buffer
   static constexpr int DP = DynTraits<DYN>::DP;
   static constexpr int TILE = ((DP == 4) ? 256 : (DP == 8) ? 128 : 64) ; 
@@ -592,33 +605,44 @@ __device__ __forceinline__ float idx_box_bound(const DevProblem& pb, const float
   return acc * kIdxShrink;
 }
 
-// Scores up to NT tiles (32 rows each, one per lane; t[a] < 0: none) against q with all their loads in flight
-// together; returns the tightened upper bound.
+// Scores the first `cnt` (1..NT, warp-uniform) of the tiles t[] (32 rows each, one per lane) against q and returns the
+// tightened upper bound.  The distance is accumulated dimension by dimension over all NT tiles at once -- NT
+// independent coalesced loads per dimension, so a warp keeps NT..2NT cache lines in flight instead of one tile's --
+// with the operations and the order of dist2(), hence bit-identical keys.  Slots past cnt re-read tile t[0].
 template <int DYN, bool UNIT_W, int NT>
-__device__ __forceinline__ float idx_score_tiles(const Params& P, const int (&t)[NT], const float (&q)[DynTraits<DYN>::D],
-                                                 unsigned long long& best, float ub) {
-  constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
+__device__ __forceinline__ float idx_score_tiles(const Params& P, const int (&t)[NT], int cnt,
+                                                 const float (&q)[DynTraits<DYN>::D], unsigned long long& best, float ub) {
+  constexpr int D = DynTraits<DYN>::D;
   const int lane = threadIdx.x & 31;
   int id[NT];
-  float p[NT][DP];
+  unsigned off[NT];
+  float acc[NT];
 #pragma unroll
   for (int a = 0; a < NT; ++a) {
-    if (t[a] >= 0) {  // warp-uniform
-      id[a] = __ldcg(&P.idx_tile_ids[(size_t)t[a] * 32 + lane]);
+    const int ta = a < cnt ? t[a] : t[0];
+    id[a] = __ldcg(&P.idx_tile_ids[(size_t)ta * 32 + lane]);
+    off[a] = (unsigned)ta * (D * 32) + lane;
+    acc[a] = 0.0f;
+  }
 #pragma unroll
-      for (int d = 0; d < DP; ++d) p[a][d] = d < D ? __ldcg(&P.idx_rows[((size_t)t[a] * D + d) * 32 + lane]) : 0.0f;
+  for (int d = 0; d < D; ++d) {
+    float v[NT];
+#pragma unroll
+    for (int a = 0; a < NT; ++a) v[a] = __ldcg(&P.idx_rows[(size_t)off[a] + d * 32]);
+#pragma unroll
+    for (int a = 0; a < NT; ++a) {
+      const float delta = is_angle<DYN>(d) ? angle_absdiff(q[d], v[a]) : (q[d] - v[a]);
+      if (UNIT_W) acc[a] = fmaf(delta, delta, acc[a]);
+      else acc[a] = fmaf(delta * P.pb.w[d], delta, acc[a]);
     }
   }
   unsigned bits = 0x7f800000u;
 #pragma unroll
   for (int a = 0; a < NT; ++a) {
-    if (t[a] >= 0) {
-      const float d2 = dist2<DYN, UNIT_W>(P.pb, q, p[a]);
-      if (id[a] >= 0) {
-        const unsigned b = __float_as_uint(d2);  // d2 >= 0: uint order == float order
-        best = min(best, ((unsigned long long)b << 32) | (unsigned)id[a]);
-        bits = min(bits, b);
-      }
+    if (a < cnt && id[a] >= 0) {
+      const unsigned b = __float_as_uint(acc[a]);  // d2 >= 0: uint order == float order
+      best = min(best, ((unsigned long long)b << 32) | (unsigned)id[a]);
+      bits = min(bits, b);
     }
   }
   return fminf(ub, __uint_as_float(__reduce_min_sync(0xffffffffu, bits)));
@@ -637,11 +661,14 @@ __device__ __forceinline__ int idx_pop_nearest(unsigned& cand, float lb, float u
 }
 
 // One warp, one query (all lanes hold the same q): exact NN over the indexed rows [0, n_sorted).
-// Boxes are opened nearest-first inside every group of 32, so ub tightens early and most boxes are never opened.
+// Super-tile boxes are opened nearest-first, so ub tightens early and most boxes are never opened.  Inside a
+// super-tile the nearest tile goes first and the others follow in key order; tiles wait in a small warp-uniform
+// queue that is scored NT at a time (across super-tiles), and what is left of a super-tile is re-filtered against
+// the tightened ub after every batch.  Scoring a tile the final ub would have excluded costs time, never exactness.
 template <int DYN, bool UNIT_W>
 __device__ __forceinline__ unsigned long long idx_search(const Params& P, const IdxDims& G,
                                                          const float (&q)[DynTraits<DYN>::D], long long& scored) {
-  constexpr int NT = DynTraits<DYN>::DP <= 8 ? 4 : 2;  // tiles scored together (register budget)
+  constexpr int NT = 8;  // tiles scored together
   const int lane = threadIdx.x & 31;
   const float inf = __int_as_float(0x7f800000);
   unsigned long long best = kKeyNone;
@@ -660,12 +687,14 @@ __device__ __forceinline__ unsigned long long idx_search(const Params& P, const 
     const int t = s_near * 32 + lane;
     const float lb = t < G.n_tiles ? idx_box_bound<DYN>(P.pb, P.idx_tlo, P.idx_thi, (size_t)s_near, lane, q) : inf;
     t_near = (int)(unsigned)(warp_min_key(((unsigned long long)__float_as_uint(lb) << 32) | (unsigned)t) & 0xffffffffu);
-    int one[NT];
-#pragma unroll
-    for (int a = 0; a < NT; ++a) one[a] = a == 0 ? t_near : -1;
-    ub = idx_score_tiles<DYN, UNIT_W, NT>(P, one, q, best, ub);
+    const int one[1] = {t_near};
+    ub = idx_score_tiles<DYN, UNIT_W, 1>(P, one, 1, q, best, ub);
     scored += 32;
   }
+  int pend[NT];  // warp-uniform queue of tiles waiting to be scored
+  int np = 0;
+#pragma unroll
+  for (int a = 0; a < NT; ++a) pend[a] = 0;
   // pass B: every box that can still hold a row at distance <= ub
   for (int s0 = 0; s0 < G.n_super; s0 += 32) {
     const int s_mine = s0 + lane;
@@ -679,20 +708,37 @@ __device__ __forceinline__ unsigned long long idx_search(const Params& P, const 
       const float lbt = t_mine < G.n_tiles ? idx_box_bound<DYN>(P.pb, P.idx_tlo, P.idx_thi, (size_t)s, lane, q) : inf;
       unsigned tc = __ballot_sync(0xffffffffu, t_mine < G.n_tiles && lbt <= ub);
       if (s == s_near) tc &= ~(1u << (t_near & 31));  // scored in pass A
+      bool first = true;
       while (tc) {
-        int t[NT];
-        int cnt = 0;
-#pragma unroll
-        for (int a = 0; a < NT; ++a) {
-          const int k = tc ? idx_pop_nearest(tc, lbt, ub) : -1;
-          t[a] = k >= 0 ? s * 32 + k : -1;
-          cnt += k >= 0;
+        int k;
+        if (first) {  // nearest tile of the super-tile first
+          k = idx_pop_nearest(tc, lbt, ub);
+          first = false;
+          if (k < 0) break;
+        } else {
+          k = __ffs(tc) - 1;
+          tc &= tc - 1;
         }
-        if (cnt == 0) break;
-        ub = idx_score_tiles<DYN, UNIT_W, NT>(P, t, q, best, ub);
-        scored += 32 * cnt;
+#pragma unroll
+        for (int a = 0; a < NT; ++a)
+          if (a == np) pend[a] = s * 32 + k;
+        if (++np == NT) {
+          ub = idx_score_tiles<DYN, UNIT_W, NT>(P, pend, NT, q, best, ub);
+          scored += 32 * NT;
+          np = 0;
+          tc &= __ballot_sync(0xffffffffu, lbt <= ub);  // the rest of this super-tile against the tightened bound
+        }
+      }
+      if (np > 0 && ub == inf) {  // no real row scored yet (small index, no pass A): get a bound before opening more
+        ub = idx_score_tiles<DYN, UNIT_W, NT>(P, pend, np, q, best, ub);
+        scored += 32 * np;
+        np = 0;
       }
     }
+  }
+  if (np > 0) {
+    ub = idx_score_tiles<DYN, UNIT_W, NT>(P, pend, np, q, best, ub);
+    scored += 32 * np;
   }
   return warp_min_key(best);
 }
@@ -725,17 +771,22 @@ __device__ __forceinline__ void idx_phase(const Params& P, int n_sorted, uint32_
   }
 }
 
+}  // namespace pakr
+#include "pakr_nn_filter.cuh"
+namespace pakr {
+
 // ---- NN scan of tree rows [nbeg, nend) for the queries of iteration `it` (Alg. 1 l.6-7) ----
 // CTAs vb = 0..vbcount-1 take part (vb < 0: this CTA sits out; the call is CTA-uniform).  Work units are
 // (query group of 128, node range); a CTA takes kWarps consecutive units per round, one per warp.  The
 // sampled states of the (at most two) query groups a CTA touches in a round are drawn once by the CTA into
 // shared memory (Alg. 1 l.6) instead of once per warp.  Partial minima are merged into key[s] with a 64-bit
 // atomicMin, so any split of the rows over warps / phases gives the same result.
-template <int DYN, bool UNIT_W, bool STREAM>
+template <int DYN, bool UNIT_W, bool STREAM, bool FILTER>
 __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, uint32_t r, uint32_t it,
                                          unsigned long long* key, int vb, int vbcount, float* sm_tile,
                                          uint64_t* sm_bar, float* sm_q, unsigned long long* sm_keys, uint32_t& par0,
-                                         uint32_t& par1) {
+                                         uint32_t& par1, cg::grid_group& grid, unsigned& sgen,
+                                         bool filter_live, unsigned long long* f_slot, long long& filtered) {
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
   constexpr int TILE = TileCfg<DYN>::TILE, TF = TileCfg<DYN>::TILE_FLOATS;
   constexpr int QG = 32 * kQ;  // queries per group
@@ -745,6 +796,23 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
   if constexpr (STREAM) {  // few queries (B <= kStreamB, chosen by the host): HBM-bound streaming tier
     nn_stream<DYN, UNIT_W>(P, nbeg, nend, r, it, key, vb, vbcount, sm_q, sm_tile, sm_bar, par0, par1);
     return;
+  } else if constexpr (FILTER) {
+   if (filter_live && n >= kFilterMinRows && (long long)P.B * n * D >= P.filter_min_work) {
+    // long row ranges: tensor-core coarse filter, then exact rescoring of the few candidate chunks (same result)
+    const FilterPlan fp = filter_plan<DYN>(P.B, n, vbcount * kWarps);
+    nn_filter_scan<DYN>(P, nbeg, nend, r, it, vb, vbcount, fp, sm_tile, sm_bar, reinterpret_cast<__half*>(sm_q),
+                        reinterpret_cast<float*>(sm_keys), par0, par1);
+    if (vbcount == (int)gridDim.x) {
+      __threadfence();
+      grid.sync();
+    } else {
+      ++sgen;
+      cta_group_barrier(&P.ctrl->sbar, (unsigned)vbcount * sgen);
+    }
+    nn_filter_refine<DYN, UNIT_W>(P, nbeg, nend, r, it, key, vb, vbcount, fp, f_slot);
+    filtered += (long long)P.B * n;
+    return;
+   }
   }
   const int W = vbcount * kWarps;
   const int G = (P.B + QG - 1) / QG;  // query groups
@@ -757,10 +825,10 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
   for (int ub = vb * kWarps; ub < U; ub += W) {
     const int u = ub + warp;
     const bool has = u < U;
-    const int g = has ? u / Reff : 0, rr = u - g * Reff;
+    const int g_lo = ub / Reff, g_hi = min(U - 1, ub + kWarps - 1) / Reff;
+    const int g = has ? u / Reff : g_lo, rr = has ? u - g * Reff : 0;  // idle warps still read group g_lo's queries
     const int beg = nbeg + rr * len;
     const int end = min(nend, beg + len);
-    const int g_lo = ub / Reff, g_hi = min(U - 1, ub + kWarps - 1) / Reff;
     const bool shared_q = (g_hi - g_lo) <= 1;  // CTA-uniform
     f32x2 q2[kQ / 2][D];  // queries 2h and 2h+1 of this lane, packed per dimension
     float best[kQ];
@@ -1086,7 +1154,7 @@ __device__ __forceinline__ void tail_scan_rounds(const Params& P, int n, int U, 
 
 // The first `npcta` CTAs take part (all of them when the insert is a phase of its own; only the propagate CTAs
 // when it runs inside phase X).  tail_mode: 0 none, 2 CTA rounds (r, it_next) when the insert runs inside phase X.
-template <int DYN>
+template <int DYN, bool FILTER>
 __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, unsigned long long* key_done,
                                             int tail_mode, unsigned long long* key_next, uint32_t r, uint32_t it_next,
                                             int npcta, int* sm_pref, int* sm_upre, float* sm_qt, float* sm_tile,
@@ -1163,8 +1231,19 @@ __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, u
       const int node = n + pos;
       const float4* src = reinterpret_cast<const float4*>(P.scr_state + slot * DP);
       float4* dst = reinterpret_cast<float4*>(P.states + (size_t)node * DP);
+      float xr[DP];
 #pragma unroll
-      for (int v = 0; v < DP / 4; ++v) dst[v] = __ldcg(src + v);
+      for (int v = 0; v < DP / 4; ++v) {
+        const float4 a = __ldcg(src + v);
+        dst[v] = a;
+        xr[4 * v] = a.x; xr[4 * v + 1] = a.y; xr[4 * v + 2] = a.z; xr[4 * v + 3] = a.w;
+      }
+      if constexpr (FILTER) {
+        float xd[T::D];
+#pragma unroll
+        for (int d = 0; d < T::D; ++d) xd[d] = xr[d];
+        filter_write_row<DYN>(P.pb, P.frow, (size_t)node, xd);
+      }
       reinterpret_cast<float4*>(P.actions)[node] = __ldcg(reinterpret_cast<const float4*>(P.scr_ctrl) + slot);
       const float cost = __ldcg(&P.scr_cost[slot]);
       P.costs[node] = cost;
@@ -1174,6 +1253,10 @@ __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, u
         atomicMin(&P.ctrl->goal_key[gslot], ((unsigned long long)__float_as_uint(cost) << 32) | (unsigned)node);
       if (P.dbg_child_flags) P.dbg_child_flags[u * cpw + (fl >> 8)] |= 32;
     }
+  }
+  if constexpr (FILTER) if (blockIdx.x == 0 && threadIdx.x < 8) {  // filter rows up to the next multiple of 8: far away
+    const int n_new = n + min(total, room), row = n_new + (int)threadIdx.x;
+    if (row < ((n_new + 7) & ~7)) filter_write_sentinel<DYN>(P.frow, (size_t)row);
   }
   // fused tail scan of the next iteration's NN (every survivor inserted)
   {
@@ -1218,10 +1301,10 @@ __device__ __forceinline__ void extract_path(const Params& P, int goal_node, flo
   }
 }
 
-// TIER: 0 tiled NN scan, 1 streaming NN scan (B <= kStreamB), 2 tiled scan + NN cell index (opt-in)
+// TIER: 0 tiled NN scan, 1 streaming NN scan (B <= kStreamB), 2 tiled scan + NN index, 3 tiled scan + tensor-core filter
 template <int DYN, int OBS, int TIER>
 __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const __grid_constant__ Params P) {
-  constexpr bool STREAM = TIER == 1, INDEX = TIER == 2;
+  constexpr bool STREAM = TIER == 1, INDEX = TIER == 2, FILTER = TIER == 3;
   using T = DynTraits<DYN>;
   constexpr int OS = (OBS == OBS_CIRCLE) ? 4 : 8;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -1229,7 +1312,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
   // [merge keys: kWarps * 128 x u64]
   // [obstacles][grid cells][grid lists]
   float* sm_tiles = reinterpret_cast<float*>(smem_raw);
-  uint64_t* sm_bars = reinterpret_cast<uint64_t*>(sm_tiles + kWarps * 2 * TileCfg<DYN>::TILE_FLOATS);
+  uint64_t* sm_bars = reinterpret_cast<uint64_t*>(sm_tiles + kWarps * 2 * kTileBufFloats);
   int* sm_pref = reinterpret_cast<int*>(sm_bars + kWarps * 2);
   float* sm_q = reinterpret_cast<float*>(sm_pref + kThreads + kWarps + 8);
   unsigned long long* sm_keys = reinterpret_cast<unsigned long long*>(sm_q + kMaxD * 2 * 32 * kQ);
@@ -1252,7 +1335,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   fence_proxy_async();
   __syncthreads();
-  float* my_tile = sm_tiles + warp * 2 * TileCfg<DYN>::TILE_FLOATS;
+  float* my_tile = sm_tiles + warp * 2 * kTileBufFloats;
   uint64_t* my_bar = sm_bars + warp * 2;
   uint32_t par0 = 0, par1 = 0;
 
@@ -1271,10 +1354,28 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
   const int x_vbcnt = split ? NB - NPB : NB;
   // insert inside phase X by the propagate CTAs (one grid barrier per iteration) when the children are few
   const bool xins = split && U_prop <= kFuseUnits;
-  unsigned pgen = 0;
+  unsigned pgen = 0, sgen = 0;
   unsigned long long* const key0 = P.nn_key;
   unsigned long long* const key1 = P.nn_key + P.B;
 
+  if constexpr (FILTER) {
+    // filter rows of what is already in the tree: the root (pakr_plan) or a caller's whole tree (pakr_expand_step),
+    // plus far-away rows up to the next multiple of 8.  A hand-over cost, taken before the clock starts.
+    const int n0 = P.n_nodes_io ? __ldcg(P.n_nodes_io) : 1;
+    for (int i = blockIdx.x * kThreads + threadIdx.x; i < ((n0 + 7) & ~7); i += gridDim.x * kThreads) {
+      if (i < n0) {
+        float xd[T::D];
+#pragma unroll
+        for (int d = 0; d < T::D; ++d) xd[d] = __ldcg(&P.states[(size_t)i * T::DP + d]);
+        filter_write_row<DYN>(P.pb, P.frow, (size_t)i, xd);
+      } else {
+        filter_write_sentinel<DYN>(P.frow, (size_t)i);
+      }
+    }
+    __threadfence();
+    fence_proxy_async();
+    grid.sync();
+  }
   unsigned long long t_start = 0;
   if (leader) { t_start = globaltimer_ns(); P.ctrl->t_start_ns = t_start; }
 
@@ -1284,6 +1385,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
   long long iterations = 0, inserted = 0, nn_pairs = 0;
   long long nn_scored = 0;       // per warp: pairs the index tier scored (lane 0 reports at the end)
   long long nn_idx_covered = 0;  // uniform: pairs of the NN definition the index answered without a scan
+  long long nn_filtered = 0;
+  unsigned long long nn_rescored = 0;  // uniform (read back from the per-iteration slots)
   unsigned long long ph0 = 0, ph1 = 0, ph2 = 0, ph3 = 0, tp = t_start;
   bool stop = false;
   int cur = 0;  // key buffer of the current iteration
@@ -1296,9 +1399,15 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
     int n_scanned = 0;  // NN(it) already covers tree rows [0, n_scanned)
     int n_sorted = 0;   // rows [0, n_sorted) are in the NN index
     int cov_cur = 0, cov_next = 0;  // rows of NN(it) / NN(it+1) the index answered for
+    bool filter_live = FILTER;            // tensor-core NN filter in use (per replan)
+    long long filt_ahead = 0;             // pairs it took on for the NEXT iteration's NN (credited when that NN is used)
     for (;;) {
       unsigned long long* const kcur = cur ? key1 : key0;
       unsigned long long* const knext = cur ? key0 : key1;
+      // per-iteration control words live in slots that rotate over the whole launch (not per replan); see kSlots
+      const int slot = (int)(iterations % kSlots);
+      const int slot_next = (slot + 1) % kSlots;
+      long long filt_head = 0, filt_x = 0;  // pairs the tensor-core filter took on for NN(it) now / for NN(it+1) (uniform)
       // a fresh tree is the root alone: every query's nearest node is node 0, no scan needed
       const bool root_only = (n == 1) && !P.n_nodes_io;
       // NN index tier: used once B*n is large; rebuilt when scanning the rows added since the last rebuild would
@@ -1306,12 +1415,12 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       // whole NN of the iteration runs at its head, right after the rebuild, instead of one iteration ahead: the
       // rows of the previous batch are then inside the index and need no brute-force pass of their own.
       bool idx_use = false;
-      if constexpr (INDEX) idx_use = P.nn_index == 2 ? n >= 256 : (n >= kIdxMinRows && (long long)P.B * n * T::D >= kIdxMinWork);
+      if constexpr (INDEX) idx_use = P.nn_index == 2 ? n >= 256 : (n >= kIdxMinRows && (long long)P.B * n * T::D >= P.idx_min_work);
       if (!idx_use) n_sorted = 0;
       const bool idx_head = idx_use && !split;
       if constexpr (INDEX) {
         const bool grown = P.nn_index == 2 ? n - n_sorted > 64
-                                           : (long long)P.B * (n - n_sorted) * T::D >= kIdxRebuildWork;
+                                           : (long long)P.B * (n - n_sorted) * T::D >= P.idx_rebuild_work;
         if (idx_use && (n_sorted == 0 || grown) && (n_scanned == 0 || !idx_head)) {
           idx_rebuild<DYN>(P, n, grid, reinterpret_cast<unsigned*>(sm_tiles), sm_pref);
           n_sorted = n;
@@ -1328,17 +1437,14 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
           a_beg = n_sorted;
           cov_cur = n_sorted;
         }
-        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1);
-        else nn_phase<DYN, false, STREAM>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1);
+        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM, FILTER>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_head);
+        else nn_phase<DYN, false, STREAM, FILTER>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_head);
         grid.sync();
       }
       if (leader) { const unsigned long long t = globaltimer_ns(); ph0 += t - tp; tp = t; }
       // phase X: propagate(it) and, meanwhile, NN(it+1) over the frozen snapshot [0, n)
       const bool ahead = (iters + 1 < P.max_iters) && !idx_head;
       prop_phase<DYN, OBS>(P, (uint32_t)r, (uint32_t)it, c_best, kcur, root_only, x_pw, x_pcnt, sm_obs, sm_cells, sm_list);
-      // slots rotate over the whole launch (not per replan); see kSlots
-      const int slot = (int)(iterations % kSlots);
-      const int slot_next = (slot + 1) % kSlots;
       bool fused = false;
       int total = 0;
       if (xins) {
@@ -1349,7 +1455,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
           ++pgen;
           cta_group_barrier(&P.ctrl->pbar, (unsigned)NPB * pgen);
           fence_proxy_async();
-          total = insert_phase<DYN>(P, n, slot, kcur, ahead ? 2 : 0, knext, (uint32_t)r, (uint32_t)(it + 1), NPB, sm_pref,
+          total = insert_phase<DYN, FILTER>(P, n, slot, kcur, ahead ? 2 : 0, knext, (uint32_t)r, (uint32_t)(it + 1), NPB, sm_pref,
                                     reinterpret_cast<int*>(sm_q), reinterpret_cast<float*>(sm_keys), my_tile, my_bar, par0,
                                     fused);
           if (leader) P.ctrl->iter_total[slot] = total;
@@ -1366,11 +1472,12 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
           x_beg = n_sorted;
           cov_next = n_sorted;
         }
-        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1);
-        else nn_phase<DYN, false, STREAM>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1);
+        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM, FILTER>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_x);
+        else nn_phase<DYN, false, STREAM, FILTER>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_x);
       }
       if (leader) {
         P.ctrl->goal_key[slot_next] = kKeyNone;
+        P.ctrl->f_rescored[slot_next] = 0ull;
         P.ctrl->idx_query[0][slot_next] = 0;
         P.ctrl->idx_query[1][slot_next] = 0;
         if (xins) P.ctrl->stop[slot] = (P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) ? 1 : 0;
@@ -1384,7 +1491,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
         fused = ahead && total <= P.cap - n && total <= kXTailRows;
       } else {
         // phase C: insert as a phase of its own (every CTA takes part)
-        total = insert_phase<DYN>(P, n, slot, kcur, 0, knext, (uint32_t)r, (uint32_t)(it + 1), NB, sm_pref,
+        total = insert_phase<DYN, FILTER>(P, n, slot, kcur, 0, knext, (uint32_t)r, (uint32_t)(it + 1), NB, sm_pref,
                                   reinterpret_cast<int*>(sm_q), reinterpret_cast<float*>(sm_keys), my_tile, my_bar, par0,
                                   fused);
         if (leader) P.ctrl->stop[slot] = (P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) ? 1 : 0;
@@ -1405,6 +1512,17 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       ++iterations;
       ++iters;
       cur ^= 1;
+      nn_filtered += filt_ahead + filt_head;  // what NN(it) got from the filter (its look-ahead ran one iteration ago)
+      filt_ahead = filt_x;
+      const long long filt_iter = filt_head + filt_x;  // the filter's work inside this iteration
+      if (filt_iter > 0) {
+        // The filter pays only while its second phase rescans few rows: dense, clustered trees put many rows within the
+        // rounding band of the nearest one.  Once it does not, the rest of the replan uses the exact scan (the tree only
+        // gets denser).  Every thread reads the same counter after the same barrier: the decision is grid-uniform.
+        const unsigned long long rsc = __ldcg(&P.ctrl->f_rescored[slot]);
+        nn_rescored += rsc;
+        if ((long long)rsc * P.filter_give_up > filt_iter) filter_live = false;
+      }
       const unsigned long long gk = __ldcg(&P.ctrl->goal_key[slot]);
       stop = __ldcg(&P.ctrl->stop[slot]) != 0;
       ++it;
@@ -1443,6 +1561,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
     c->inserted = inserted;
     c->nn_pairs = nn_pairs;
     c->nn_idx_covered = nn_idx_covered;
+    c->nn_filtered = nn_filtered;
+    c->nn_rescored = nn_rescored;
     c->phase_ns[0] = ph0; c->phase_ns[1] = ph1; c->phase_ns[2] = ph2; c->phase_ns[3] = ph3;
     c->n_nodes = n;
     c->solved = solved_any;

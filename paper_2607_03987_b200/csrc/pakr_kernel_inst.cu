@@ -1,7 +1,7 @@
 // pakr_kernel_inst.cu -- instantiates the persistent kernel of pakr_kernel.cuh for (dynamics, obstacle kind).
 // Compiled once per (tier, part) so that the sets build in parallel and a rarely used tier costs the common one
 // no registers:  -DPAKR_STREAM_TIER=0 tiled NN scan (the normal case), =1 streaming NN tier for B <= 16,
-// =2 tiled scan + NN index tier;
+// =2 tiled scan + NN index tier, =3 tiled scan + tensor-core coarse filter;
 // -DPAKR_PART=0 double integrators, unicycles and the Acrobot, =1 quadrotors and the Dubins airplane.
 #include "pakr_kernel.cuh"
 

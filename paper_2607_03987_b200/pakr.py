@@ -16,10 +16,11 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "libpakr.so")
 _CSRC = os.path.join(_HERE, "csrc")
-_SOURCES = ["pakr_api.cu", "pakr_kernel_inst.cu", "pakr_peak.cu", "pakr_kernel.cuh", "pakr_device.cuh"]
+_SOURCES = ["pakr_api.cu", "pakr_kernel_inst.cu", "pakr_peak.cu", "pakr_kernel.cuh", "pakr_device.cuh",
+            "pakr_nn_filter.cuh"]
 
 F_VALID, F_INBOUNDS, F_COLLFREE, F_NOTPRUNED, F_GOAL, F_INSERTED = 1, 2, 4, 8, 16, 32
-NN_AUTO, NN_SCAN, NN_INDEX = 0, 1, 2
+NN_AUTO, NN_SCAN, NN_INDEX, NN_FILTER = 0, 1, 2, 3
 MAX_REPLAN_STATS = 64
 MAX_PATH_NODES = 8192
 _STATUS = {0: "PAKR_OK", 1: "PAKR_ERR_INVALID_ARG", 2: "PAKR_ERR_UNSUPPORTED", 3: "PAKR_ERR_WORKSPACE_TOO_SMALL",
@@ -34,7 +35,7 @@ class PakrError(RuntimeError):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """nvcc -gencode arch=compute_100a,code=sm_100a -> paper_2607_03987_b200/libpakr.so (in-tree).
-    Six translation units (host API; kernels per NN tier and model group) compile in parallel."""
+    Ten translation units (host API; peak microbenchmark; kernels per NN tier and model group) compile in parallel."""
     srcs = [os.path.join(_CSRC, s) for s in _SOURCES] + [os.path.join(_HERE, "..", "include", "pakr.h")]
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     flags = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
@@ -51,7 +52,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale:
         tag = f".{os.getpid()}.tmp"
         units = [("pakr_api.cu", [], "api"), ("pakr_peak.cu", [], "peak")]
-        for tier, part in ((0, 0), (0, 1), (1, 0), (1, 1), (2, 0), (2, 1)):
+        for tier, part in ((0, 0), (0, 1), (1, 0), (1, 1), (2, 0), (2, 1), (3, 0), (3, 1)):
             units.append(("pakr_kernel_inst.cu", [f"-DPAKR_STREAM_TIER={tier}", f"-DPAKR_PART={part}"], f"t{tier}p{part}"))
         objs, procs = [], []
         for src, defs, name in units:
@@ -111,7 +112,7 @@ class _PlanOpts(C.Structure):
 
 class _Stats(C.Structure):
     _fields_ = [("iterations", C.c_int64), ("children", C.c_int64), ("inserted", C.c_int64), ("nn_pairs", C.c_int64),
-                ("nn_pairs_evaluated", C.c_int64), ("h2d_bytes", C.c_int64), ("d2h_bytes", C.c_int64),
+                ("nn_pairs_evaluated", C.c_int64), ("nn_pairs_filtered", C.c_int64), ("h2d_bytes", C.c_int64), ("d2h_bytes", C.c_int64),
                 ("replans_run", C.c_int32), ("replans_solved", C.c_int32), ("termination", C.c_int32),
                 ("replan_stats_truncated", C.c_int32), ("path_truncated", C.c_int32),
                 ("first_solution_ms", C.c_double), ("device_ms", C.c_double), ("phase_ms", C.c_double * 4),
@@ -281,6 +282,7 @@ class Planner:
                     path_states=states[:L].copy(), path_controls=ctrls[:max(L - 1, 0)].copy(),
                     final_tree_nodes=int(res.final_tree_nodes), iterations=int(s.iterations), children=int(s.children),
                     inserted=int(s.inserted), nn_pairs=int(s.nn_pairs), nn_pairs_evaluated=int(s.nn_pairs_evaluated),
+                    nn_pairs_filtered=int(s.nn_pairs_filtered),
                     h2d_bytes=int(s.h2d_bytes),
                     d2h_bytes=int(s.d2h_bytes), replans_run=int(s.replans_run), replans_solved=int(s.replans_solved),
                     termination=int(s.termination), first_solution_ms=float(s.first_solution_ms),
@@ -315,7 +317,8 @@ class Planner:
         self._check(lib().pakr_read_stats(self._h, B, K, tree_capacity, C.c_void_p(ws.data_ptr()), ws.numel(),
                                           C.c_void_p(self._stream()), C.byref(st)))
         return dict(iterations=int(st.iterations), children=int(st.children), inserted=int(st.inserted),
-                    nn_pairs=int(st.nn_pairs), nn_pairs_evaluated=int(st.nn_pairs_evaluated), device_ms=float(st.device_ms), phase_ms=[float(v) for v in st.phase_ms])
+                    nn_pairs=int(st.nn_pairs), nn_pairs_evaluated=int(st.nn_pairs_evaluated),
+                    nn_pairs_filtered=int(st.nn_pairs_filtered), device_ms=float(st.device_ms), phase_ms=[float(v) for v in st.phase_ms])
 
     # ---- pakr_expand_step ----
     def new_tree(self, capacity: int, host: Optional[dict] = None) -> dict:

@@ -299,3 +299,21 @@ def test_plan_small_b_stream_tier_and_no_obstacles(pakr, orc):
     res = pl.plan(0, 512, 8, 1 << 18, 2)
     _check_plan(orc, p0, res)
     pl.close()
+
+
+@pytest.mark.parametrize("name,B,K,iters", [("C4", 4096, 16, 6), ("C5", 4096, 64, 4), ("N3", 2048, 16, 8), ("C2", 16384, 8, 4)])
+def test_plan_loop_with_nn_filter_equals_scan(pakr, name, B, K, iters):
+    """Inside the device loop the filter rows are written at insert time and the filter answers the look-ahead NN and
+    the scans of freshly appended rows: the tree must be bit-identical to the one the fp32 scan builds."""
+    p, cfg = wl.config5(B=B, K=K) if name == "C5" else wl.CONFIGS[name]()
+    cap = 1 + iters * B * K
+    trees = {}
+    pl = pakr.Planner(p)
+    for mode in (pakr.NN_SCAN, pakr.NN_FILTER):
+        res = pl.plan(7, B, K, cap, 1, max_iters_per_replan=iters, nn_mode=mode)
+        trees[mode] = (res["final_tree_nodes"], pl.read_tree(B, K, cap, res["final_tree_nodes"]), res["nn_pairs_filtered"])
+    pl.close()
+    assert trees[pakr.NN_SCAN][0] == trees[pakr.NN_FILTER][0] > B
+    assert trees[pakr.NN_SCAN][2] == 0 and trees[pakr.NN_FILTER][2] > 0
+    for k in ("states", "actions", "parents", "costs"):
+        np.testing.assert_array_equal(trees[pakr.NN_SCAN][1][k], trees[pakr.NN_FILTER][1][k])

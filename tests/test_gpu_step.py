@@ -351,3 +351,45 @@ def test_nn_index_tier_equals_scan_tier(pakr, orc, name, n0, B, K):
     pl.close()
     for k in ("x_rand", "nn_idx", "nn_d2", "child_state"):
         np.testing.assert_array_equal(outs[pakr.NN_SCAN][k], outs[pakr.NN_INDEX][k])
+
+
+@pytest.mark.parametrize("name,n0,B,K,clustered", [
+    ("C2", 70000, 1024, 2, False), ("C2", 300000, 2048, 1, True), ("C5", 1 << 20, 512, 1, False),
+    ("C4", 60000, 4096, 1, False), ("C4", 200000, 1024, 2, True), ("N3", 90000, 2048, 1, False),
+    ("C3", 150000, 2048, 1, False), ("C3", 150000, 2048, 1, True),      # heading weight 1: the cosine bound is loose
+    ("N4", 120000, 1024, 1, False), ("N1", 200000, 1024, 1, True), ("N2", 200000, 1024, 1, False),
+    ("C1", 65000, 2048, 1, True), ("C2", 4096, 20000, 1, False)])
+def test_nn_filter_tier_equals_scan_tier(pakr, orc, name, n0, B, K, clustered):
+    """The tensor-core coarse filter (pakr_nn_filter.cuh: fp16 hi/lo mma, fp32 accumulate, exact rescoring of the
+    candidate chunks) must return bit-identical NN indices and distances to the brute-force fp32 scan -- on uniform
+    trees, on trees squeezed into a corner with duplicated rows (many rows inside the rounding band: ties, lowest index
+    wins) -- and meets the oracle bar on sampled queries.  Problems with heavy angle weights (C3, N1, N2, N4) silently
+    keep the fp32 scan under PAKR_NN_FILTER; B = 20000 on a 4096-node tree is the shape that exposed an out-of-range
+    shared-memory read of idle warps in the scan's last round."""
+    p, _ = wl.CONFIGS[name]()
+    host = wl.random_tree(p, n0, seed=n0 % 977, flat=True)
+    if clustered:
+        pd = p.pos_dim
+        host["states"][n0 // 3:, :pd] = (p.state_lo[:pd] + 0.05 * (host["states"][n0 // 3:, :pd] - p.state_lo[:pd]))
+        host["states"][n0 - 3000:] = host["states"][100:3100]       # exact duplicates, far apart in index
+        host["states"][n0 // 2:n0 // 2 + 3000] = host["states"][100:3100] + np.float32(1e-4)  # near-duplicates inside the band
+    outs = {}
+    pl = pakr.Planner(p)
+    for mode in (pakr.NN_SCAN, pakr.NN_FILTER):
+        tree = pl.new_tree(n0 + B * K, host)
+        outs[mode] = pl.expand_step(tree, 5, 1, 4, B, K, nn_mode=mode)
+        st = pl.read_stats(B, K, n0 + B * K)
+        heavy_angles = float(p.nn_weight[p.dim_kind == 1].sum()) > 0.1   # those problems keep the fp32 scan
+        if mode == pakr.NN_FILTER and B * n0 * p.state_dim >= 4e8 and not heavy_angles:
+            assert st["nn_pairs_filtered"] == B * n0, "the filter did not run"
+    pl.close()
+    for k in ("x_rand", "nn_idx", "nn_d2", "child_state", "child_flags"):
+        np.testing.assert_array_equal(outs[pakr.NN_SCAN][k], outs[pakr.NN_FILTER][k])
+    op = orc.OracleProblem(p)
+    tree64 = host["states"].astype(np.float64)
+    rng = np.random.default_rng(2)
+    for s_ in rng.choice(B, 12, replace=False):
+        q = op.sample_state(5, 1, 4, int(s_))
+        i, d2 = op.nearest(tree64, q)
+        j = int(outs[pakr.NN_FILTER]["nn_idx"][s_])
+        assert j == i or op.dist2(q, tree64[j]) <= (1 + 1e-6) * d2
