@@ -53,12 +53,13 @@ enum { PAKR_COST_DURATION = 0, PAKR_COST_PATH_LENGTH = 1 };
 enum { PAKR_DIM_REAL = 0, PAKR_DIM_ANGLE = 1 };
 enum { PAKR_NO_SOLUTION = 0, PAKR_SOLVED = 1 }; /* "no solution" is not an error */
 /* nearest-neighbour tier (pakr_plan_opts.nn_mode, pakr_step_args.nn_mode) */
-enum { PAKR_NN_AUTO = 0,  /* the library picks: the brute-force fp32 scan below B = 4096 queries; from there up the
-                             tensor-core filter for 12-D models and the spatial index otherwise */
+enum { PAKR_NN_AUTO = 0,  /* the library picks: the brute-force fp32 scan below B = 4096 queries, the spatial index (once
+                             the tree is large enough to pay for building it) from there up */
        PAKR_NN_SCAN = 1,  /* brute-force fp32 scan tiers only (tiled; streaming when B <= 16) */
        PAKR_NN_INDEX = 2, /* spatial index on every tree of >= 256 nodes (tests) */
        PAKR_NN_FILTER = 3 /* tensor-core coarse filter (fp16 hi/lo mma.sync, fp32 accumulate) on every scan of >= 4096
-                             rows that is long enough to pay, exact fp32 rescoring of its candidates */ };
+                             rows that is long enough to pay, exact fp32 rescoring of its candidates; problems whose
+                             angle dims weigh more than 0.1 in total keep the fp32 scan */ };
 
 /* child flag bits written by pakr_expand_step (Alg. 1 l.10-14) */
 enum {
@@ -174,7 +175,9 @@ typedef struct {
   double phase_ms[4];      /* CTA 0's time in: NN phases of their own (whole-tree NN at the head of an iteration, scans
                               of rows added since the look-ahead) / the propagate phase (with the next iteration's NN
                               look-ahead beside it and, when children are few, the insert inside it) / insert phases
-                              of their own / rebuilds of the NN index; each incl. its grid barriers */
+                              of their own / rebuilds of the NN index (index tier) or the exact rescoring phase of the
+                              tensor-core filter when every CTA takes part in it (filter tier; the filter's first phase
+                              is counted with the phase it runs in); each incl. its grid barriers */
   /* first PAKR_MAX_REPLAN_STATS replans: */
   float replan_cost[PAKR_MAX_REPLAN_STATS];   /* c_best after the replan (+INF before any solution) */
   int32_t replan_nodes[PAKR_MAX_REPLAN_STATS];/* tree size at its end */

@@ -436,7 +436,7 @@ extern "C" pakr_status pakr_create(const pakr_problem* p, int cuda_device, pakr_
     // the fp32 scan.  (Exact alternative, not built: two shifted copies of the query per angle dim.)
     if (w_ang > 0.1) ok = false;
     pb.f_qn_ang = (float)(2.0 * w_ang);
-    pb.f_band = (float)(s_max * (1.0 / 131072.0));
+    pb.f_eps = (float)(1.0 / 131072.0);
     pl->filter_ok = ok;
   }  // the tier is chosen per call (pakr_plan_opts.nn_mode)
   pb.n_obs = p->n_obstacles;
@@ -608,20 +608,15 @@ bool set_nn_mode(pakr_planner* pl, Params& P, int nn_mode) {
   // PAKR_NN_AUTO (measured on the config 5 sweep and C1-C4): below B = 4096 queries the plain scan
   // kernel -- the trees those batches grow are too small for either accelerator to repay its fixed costs, and both
   // accelerated kernels carry more live state through the 128 registers, so their own scan loop is slower.  From
-  // B = 4096 up: the tensor-core filter for 12-D models (weighted 12-D distances are where the fp32 scan is slowest
-  // and bounding boxes prune least), the spatial index otherwise.
+  // B = 4096 up the spatial index.  The tensor-core filter beats the plain scan from ~10^5 rows up but not the index on
+  // the planner's own trees, so it is chosen only explicitly (PAKR_NN_FILTER).
   constexpr int kAutoMinB = 4096;
-  const bool big = nn_mode == PAKR_NN_AUTO && P.B >= kAutoMinB;
-  P.nn_filter = pl->filter_ok && (nn_mode == PAKR_NN_FILTER || (big && pl->DP == 12)) ? 1 : 0;
-  P.nn_index = !pl->index_ok || P.nn_filter ? 0 : nn_mode == PAKR_NN_INDEX ? 2 : big ? 1 : 0;
+  P.nn_filter = pl->filter_ok && nn_mode == PAKR_NN_FILTER ? 1 : 0;
+  P.nn_index = !pl->index_ok ? 0 : nn_mode == PAKR_NN_INDEX ? 2 : (nn_mode == PAKR_NN_AUTO && P.B >= kAutoMinB) ? 1 : 0;
   P.filter_min_work = kFilterMinWork;
   P.filter_give_up = kFilterGiveUp;
-  if (const char* e = getenv("PAKR_X_FMINWORK")) P.filter_min_work = atoll(e);  // EXPERIMENT ONLY -- remove
-  if (const char* e = getenv("PAKR_X_FGIVEUP")) P.filter_give_up = atoi(e);     // EXPERIMENT ONLY -- remove
   P.idx_min_work = kIdxMinWork;
   P.idx_rebuild_work = kIdxRebuildWork;
-  if (const char* e = getenv("PAKR_X_MINWORK")) P.idx_min_work = atoll(e);      // EXPERIMENT ONLY -- remove
-  if (const char* e = getenv("PAKR_X_REBUILD")) P.idx_rebuild_work = atoll(e);  // EXPERIMENT ONLY -- remove
   return true;
 }
 

@@ -61,7 +61,7 @@ struct DevProblem {
   // tensor-core NN filter (pakr_nn_filter.cuh): feature u_d = (x_d - f_ctr[d]) * f_scale[d], f_scale = sqrt(w)
   float f_ctr[kMaxD], f_scale[kMaxD];
   float f_qn_ang;                      // 2 * sum of the angle dims' weights
-  float f_band;                        // bound of |approximate key - true key| (host: 2^-17 * S_max)
+  float f_eps;                         // |approximate key - true key| <= f_eps * sum_i |c_i u_i| (host: 2^-17)
   // NN index: Morton key layout over the weighted state box (pakr_api.cu: idx_key_layout)
   float idx_scale[kMaxD];              // quantised coordinate = floor((x - lo) * scale), 0 .. 2^bits - 1
   uint8_t idx_bits[kMaxD];             // key bits of every dimension (0: not keyed)

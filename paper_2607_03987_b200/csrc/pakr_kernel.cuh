@@ -786,7 +786,8 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
                                          unsigned long long* key, int vb, int vbcount, float* sm_tile,
                                          uint64_t* sm_bar, float* sm_q, unsigned long long* sm_keys, uint32_t& par0,
                                          uint32_t& par1, cg::grid_group& grid, unsigned& sgen,
-                                         bool filter_live, unsigned long long* f_slot, long long& filtered) {
+                                         bool filter_live, unsigned long long* f_slot, long long& filtered,
+                                         unsigned long long& ph_outer, unsigned long long& ph_refine, unsigned long long& tp) {
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
   constexpr int TILE = TileCfg<DYN>::TILE, TF = TileCfg<DYN>::TILE_FLOATS;
   constexpr int QG = 32 * kQ;  // queries per group
@@ -809,7 +810,10 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
       ++sgen;
       cta_group_barrier(&P.ctrl->sbar, (unsigned)vbcount * sgen);
     }
-    nn_filter_refine<DYN, UNIT_W>(P, nbeg, nend, r, it, key, vb, vbcount, fp, f_slot);
+    const bool timer = blockIdx.x == (unsigned)(gridDim.x - vbcount) && threadIdx.x == 0;  // first participating CTA
+    if (timer && blockIdx.x == 0) { const unsigned long long t = globaltimer_ns(); ph_outer += t - tp; tp = t; }
+    nn_filter_refine<DYN, UNIT_W>(P, nbeg, nend, r, it, key, vb, vbcount, fp, f_slot, reinterpret_cast<int*>(sm_tile - (threadIdx.x >> 5) * 2 * kTileBufFloats));
+    if (timer && blockIdx.x == 0) { const unsigned long long t = globaltimer_ns(); ph_refine += t - tp; tp = t; }
     filtered += (long long)P.B * n;
     return;
    }
@@ -1437,8 +1441,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
           a_beg = n_sorted;
           cov_cur = n_sorted;
         }
-        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM, FILTER>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_head);
-        else nn_phase<DYN, false, STREAM, FILTER>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_head);
+        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM, FILTER>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_head, ph0, ph3, tp);
+        else nn_phase<DYN, false, STREAM, FILTER>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_head, ph0, ph3, tp);
         grid.sync();
       }
       if (leader) { const unsigned long long t = globaltimer_ns(); ph0 += t - tp; tp = t; }
@@ -1472,8 +1476,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
           x_beg = n_sorted;
           cov_next = n_sorted;
         }
-        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM, FILTER>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_x);
-        else nn_phase<DYN, false, STREAM, FILTER>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_x);
+        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM, FILTER>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_x, ph1, ph3, tp);
+        else nn_phase<DYN, false, STREAM, FILTER>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_x, ph1, ph3, tp);
       }
       if (leader) {
         P.ctrl->goal_key[slot_next] = kKeyNone;

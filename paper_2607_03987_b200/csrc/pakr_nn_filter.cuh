@@ -18,9 +18,10 @@
 //     upper bound UB, then every other range whose minimum is <= UB - qn + band, tightening UB as it goes.
 // Exactness: the true nearest row p* has a(p*) <= d2(p*) - qn + band <= UB - qn + band at all times, so its range is
 // always rescanned; ranges are rescanned with the exact arithmetic, so the result is bit-identical to the brute-force
-// scan tiers (ties included).  band = 2^-17 * S_max, S_max >= sum |c_i u_i| over the state box (host, pakr_api.cu), covers
-// the fp16 hi/lo truncation (3 * 2^-22 S), the tensor core's fp32 accumulation (K * 2^-24 S) and the fp32 feature
-// arithmetic; rows are assumed to lie inside the state box (tree rows do; pakr_expand_step documents it).
+// scan tiers (ties included).  band = 2^-17 * S with S >= sum |c_i u_i| of the pair, bounded per query by
+// 3 V^2 + 4 V sqrt(UB) + UB (V = |v|; rows that matter have |u| <= V + sqrt(UB)); 2^-17 covers the fp16 hi/lo
+// truncation (3 * 2^-22 S), the tensor core's fp32 accumulation (K * 2^-24 S) and the fp32 feature arithmetic with a
+// margin of ~5.
 //
 // Why mma.sync and not tcgen05 here: the epilogue must look at EVERY accumulator (a min over the row axis), and K is
 // only 32..48.  tcgen05.mma would finish a 128 x 256 x 32 tile in ~256 cycles but draining its 128 KB of accumulators
@@ -56,7 +57,7 @@ struct FilterPlan {
   int G;     // query groups of 64
   int CH;    // rows per chunk: the granularity of chunkmin and of the exact rescoring (a whole number of TMA tiles)
   int NC;    // chunks over the scanned rows
-  int CPR;   // chunks per work range (1, 2 or 4)
+  int CPR;   // chunks per work range (1, 2, 4, 8 or 16)
   int Reff;  // work ranges per query group
   int U;     // work units of phase 1: (query group, row range)
 };
@@ -72,7 +73,7 @@ __host__ __device__ __forceinline__ FilterPlan filter_plan(int B, int n, int W) 
   int R0 = W / f.G;  // ranges per group that fill the machine once
   if (R0 < 8) R0 = 8;
   const int cpr = f.NC / R0;
-  f.CPR = cpr >= 4 ? 4 : cpr >= 2 ? 2 : 1;
+  f.CPR = cpr >= 16 ? 16 : cpr >= 8 ? 8 : cpr >= 4 ? 4 : cpr >= 2 ? 2 : 1;
   f.Reff = (f.NC + f.CPR - 1) / f.CPR;
   f.U = f.G * f.Reff;
   return f;
@@ -289,25 +290,30 @@ __device__ __noinline__ void nn_filter_scan(const Params& P, int nbeg, int nend,
             float v = m[mt][h];
             v = fminf(v, __shfl_xor_sync(0xffffffffu, v, 1));
             v = fminf(v, __shfl_xor_sync(0xffffffffu, v, 2));
-            if (t4 == 0) my_cm[(mt * 16 + gq + 8 * h) * 4 + j] = v;
+            if (t4 == 0) my_cm[(mt * 16 + gq + 8 * h) * 4 + (j & 3)] = v;
             m[mt][h] = inf;
           }
         }
-      }
-    }
-    __syncwarp();
-    // the range's CPR chunk minima of every query in one store (slots past the last chunk hold +inf, never read)
+        if ((j & 3) == 3 || t + 1 == ntiles) {
+          // four chunk minima (or the range's CPR < 4) of every query in one store; slots past the last chunk hold
+          // +inf and are never read
+          __syncwarp();
 #pragma unroll
-    for (int h = 0; h < 2; ++h) {
-      const int qi = lane + 32 * h, s = g * kFilterQ + qi;
-      if (s < P.B) {
-        float* dst = &P.chunkmin[(size_t)s * kFilterMaxChunks + c_first];  // c_first is a multiple of CPR
-        if (fp.CPR == 4) __stcg(reinterpret_cast<float4*>(dst), *reinterpret_cast<const float4*>(&my_cm[qi * 4]));
-        else if (fp.CPR == 2) __stcg(reinterpret_cast<float2*>(dst), *reinterpret_cast<const float2*>(&my_cm[qi * 4]));
-        else __stcg(dst, my_cm[qi * 4]);
+          for (int h = 0; h < 2; ++h) {
+            const int qi = lane + 32 * h, s = g * kFilterQ + qi;
+            if (s < P.B) {
+              float* dst = &P.chunkmin[(size_t)s * kFilterMaxChunks + c_first + (j & ~3)];  // c_first: a multiple of CPR
+              if (fp.CPR >= 4) __stcg(reinterpret_cast<float4*>(dst), *reinterpret_cast<const float4*>(&my_cm[qi * 4]));
+              else if (fp.CPR == 2) __stcg(reinterpret_cast<float2*>(dst), *reinterpret_cast<const float2*>(&my_cm[qi * 4]));
+              else __stcg(dst, my_cm[qi * 4]);
+            }
+          }
+          __syncwarp();
+          for (int i = lane; i < 4 * kFilterQ; i += 32) my_cm[i] = inf;
+          __syncwarp();
+        }
       }
     }
-    __syncwarp();
   }
 }
 
@@ -339,16 +345,20 @@ __device__ __forceinline__ unsigned float_orderable(float v) {  // monotone floa
   return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
 }
 
-// ---- phase 2: exact rescoring of the candidate ranges, one warp per query -------------------------------------------
+// ---- phase 2: exact rescoring of the candidate chunks, one warp per query -------------------------------------------
+// sm_list: kWarps * kFilterList ints (a warp's pending candidate chunks).
+constexpr int kFilterList = 64;
+
 template <int DYN, bool UNIT_W>
 __device__ __noinline__ void nn_filter_refine(const Params& P, int nbeg, int nend, uint32_t r, uint32_t it,
-                                                 unsigned long long* key, int vb, int vbcount, const FilterPlan& fp,
-                                                 unsigned long long* rescored) {
+                                              unsigned long long* key, int vb, int vbcount, const FilterPlan& fp,
+                                              unsigned long long* rescored, int* sm_list) {
   using C = FilterCfg<DYN>;
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int Wp = vbcount * kWarps;
   const float inf = __int_as_float(0x7f800000);
+  int* list = sm_list + warp * kFilterList;
   int rows = 0;  // rows this warp rescanned (warp-uniform)
   for (int s = vb * kWarps + warp; s < P.B; s += Wp) {
     float q[D];
@@ -360,8 +370,15 @@ __device__ __noinline__ void nn_filter_refine(const Params& P, int nbeg, int nen
     float f[C::NF];
     filter_features<DYN>(P.pb, q, f);
     const float qn = f[C::NF - 1] + P.pb.f_qn_ang;
+    // Rounding band of THIS query: |approximate - true key| <= eps * sum_i |c_i u_i| <= eps (|u|^2 + 2 |v| |u|) with
+    // |u| <= |v| + sqrt(d2) for the rows that matter (d2 <= UB): eps (3 V^2 + 4 V sqrt(UB) + UB), V^2 = qn / ... >= |v|^2.
+    // f_eps = 2^-17 carries the same margin over the nominal 2^-19.5 as the box-wide band did.
+    const float v2 = f[C::NF - 1] + 0.5f * P.pb.f_qn_ang, vn = sqrtf(v2);
+    auto threshold = [&](float ub) {
+      return ub < inf ? ub - qn + P.pb.f_eps * (3.0f * v2 + 4.0f * vn * sqrtf(ub) + ub) : inf;
+    };
     const float* cm = P.chunkmin + (size_t)s * kFilterMaxChunks;
-    // the range with the smallest approximate key first: its exact minimum is a real upper bound
+    // the chunk with the smallest approximate key first: its exact minimum is a real upper bound
     unsigned long long near = kKeyNone;
     for (int c = lane; c < fp.NC; c += 32)
       near = min(near, ((unsigned long long)float_orderable(__ldcg(&cm[c])) << 32) | (unsigned)c);
@@ -370,20 +387,44 @@ __device__ __noinline__ void nn_filter_refine(const Params& P, int nbeg, int nen
     unsigned long long best = filter_rescan<DYN, UNIT_W>(P, nbeg + c0 * fp.CH, min(nend, nbeg + (c0 + 1) * fp.CH), q);
     float ub = best != kKeyNone ? __uint_as_float((unsigned)(best >> 32)) : inf;
     rows += fp.CH;
+    // every other chunk whose minimum could still hide a nearer row: collected into a list, rescored together (the
+    // loads of different chunks are independent), the bound tightened between batches
+    int cnt = 0;
+    unsigned long long mine = kKeyNone;  // this lane's best over the batch
+    auto flush = [&]() {
+      __syncwarp();
+      for (int e = 0; e < cnt; ++e) {
+        const int cc = list[e];
+        const int rb = nbeg + cc * fp.CH, re = min(nend, rb + fp.CH);
+        for (int i = rb + lane; i < re; i += 32) {
+          float p[DP];
+          const float4* sp = reinterpret_cast<const float4*>(P.states + (size_t)i * DP);
+#pragma unroll
+          for (int v = 0; v < DP / 4; ++v) {
+            const float4 a = __ldcg(sp + v);
+            p[4 * v] = a.x; p[4 * v + 1] = a.y; p[4 * v + 2] = a.z; p[4 * v + 3] = a.w;
+          }
+          const float d2 = dist2<DYN, UNIT_W>(P.pb, q, p);
+          if (d2 >= 0.0f) mine = min(mine, ((unsigned long long)__float_as_uint(d2) << 32) | (unsigned)i);
+        }
+      }
+      rows += cnt * fp.CH;
+      cnt = 0;
+      best = min(best, warp_min_key(mine));
+      if (best != kKeyNone) ub = __uint_as_float((unsigned)(best >> 32));
+      __syncwarp();
+    };
     for (int cb = 0; cb < fp.NC; cb += 32) {
       const int c = cb + lane;
       const float v = c < fp.NC ? __ldcg(&cm[c]) : inf;
-      unsigned cand = __ballot_sync(0xffffffffu, c < fp.NC && c != c0 && v <= ub - qn + P.pb.f_band);
-      while (cand) {
-        const int j = __ffs(cand) - 1;
-        cand &= cand - 1;
-        const int cc = cb + j;
-        best = min(best, filter_rescan<DYN, UNIT_W>(P, nbeg + cc * fp.CH, min(nend, nbeg + (cc + 1) * fp.CH), q));
-        if (best != kKeyNone) ub = __uint_as_float((unsigned)(best >> 32));
-        rows += fp.CH;
-        cand &= __ballot_sync(0xffffffffu, v <= ub - qn + P.pb.f_band);  // the rest against the tightened bound
-      }
+      const bool is = c < fp.NC && c != c0 && v <= threshold(ub);
+      const unsigned cand = __ballot_sync(0xffffffffu, is);
+      if (cand == 0) continue;
+      if (cnt + __popc(cand) > kFilterList) flush();  // keeps `is` as decided with the older, looser bound: still exact
+      if (is) list[cnt + __popc(cand & ((1u << lane) - 1u))] = c;
+      cnt += __popc(cand);
     }
+    if (cnt > 0) flush();
     if (lane == 0 && best != kKeyNone) atomicMin(&key[s], best);
   }
   if (lane == 0 && rows) atomicAdd(rescored, (unsigned long long)rows);
