@@ -9,7 +9,7 @@ planner seed = step index.  metric = expanded nodes/s = children propagated and 
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
   python bench.py --what peak                 measured FFMA / FFMA2 rates (the ALU roofline's denominators)
-  python bench.py --what phases [--only nn|stream|prop] [--quick]      single phases through pakr_expand_step
+  python bench.py --what phases [--only nn|filter|stream|prop] [--quick]   single phases through pakr_expand_step
   python bench.py --what sweep|c5|pathlen [--seeds N]                  BASELINE metrics over seeds, config 5 sweep
 
 With --gpus N > 1 and no RANK in the environment it starts the N ranks itself (torch.distributed.run, one
@@ -366,7 +366,10 @@ def run_peak(args):
     print(json.dumps({"what": "peak", "nominal_lane_ops_per_s": nominal, **m,
                       "ffma_frac_of_nominal": m["ffma_lane_ops_per_s"] / nominal,
                       "ffma2_frac_of_nominal": m["ffma2_lane_ops_per_s"] / nominal,
-                      "scan_mix_frac_of_nominal": m["scan_mix_lane_ops_per_s"] / nominal}), flush=True)
+                      "scan_mix_frac_of_nominal": m["scan_mix_lane_ops_per_s"] / nominal,
+                      "mma_f16_mac_per_clk_per_sm": m["mma_f16_mac_per_s"] / (m["sm_clock_mhz"] * 1e6) / m["sm_count"],
+                      "mma_f16_minfold_mac_per_clk_per_sm": m["mma_f16_minfold_mac_per_s"] / (m["sm_clock_mhz"] * 1e6) / m["sm_count"]}),
+          flush=True)
 
 
 # ---------------------------------------------------------------------------------------------------------
@@ -398,22 +401,37 @@ def run_phases(args):
     pakr.lib()
     peak = NOMINAL_LANES * 1.965e9
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    hbm_peak_gbs = 6446.3  # fallback: the copy bandwidth measured on this pool in round 1
+    try:
+        hbm_peak_gbs = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
+    except Exception:
+        pass
     reps = 3 if args.quick else 7
     nn_points = [("C2", 1 << 16, 1024), ("C2", 1 << 20, 1024), ("C5", 1 << 20, 16384), ("C3", 1 << 20, 2048),
                  ("C4", 1 << 18, 4096), ("C4", 1 << 22, 4096)]
     if args.quick:
         nn_points = nn_points[1:3] + nn_points[5:]
-    for name, n, B in (nn_points if args.only in ("", "nn") else []):
+    for name, n, B in (nn_points if args.only in ("", "nn", "filter") else []):
         p, _ = wl.CONFIGS[name]()
         pl = pakr.Planner(p)
-        ph = measure_phase(torch, pl, p, n, B, 1, reps, None, nn_mode=pakr.NN_SCAN)
-        t = ph[0] * 1e-3
         ops = nn_ops_per_pair(p)
-        print(json.dumps({"phase": "nn", "workload": name, "D": p.state_dim, "n": n, "B": B, "ms": ph[0],
-                          "pairs_per_s": B * n / t, "alg_lane_ops_per_pair": ops,
-                          "alu_frac": B * n * ops / t / peak,
-                          "fma_pipe_frac": B * n * 2 * p.state_dim / t / peak,
-                          "tree_GBps": 4 * p.state_dim * n / t / 1e9}), flush=True)
+        heavy_angles = float(p.nn_weight[p.dim_kind == 1].sum()) > 0.1  # such problems keep the fp32 scan (pakr.h)
+        tiers = [("fp32 scan", pakr.NN_SCAN)] if args.only != "filter" else []
+        if args.only in ("", "filter") and not heavy_angles:
+            tiers.append(("tensor-core filter + exact rescoring", pakr.NN_FILTER))
+        for tier, mode in tiers:
+            ph = measure_phase(torch, pl, p, n, B, 1, reps, None, nn_mode=mode)
+            t = (ph[0] + ph[3]) * 1e-3  # [3]: the filter's rescoring phase (0 for the scan)
+            row = {"phase": "nn", "tier": tier, "workload": name, "D": p.state_dim, "n": n, "B": B, "ms": ph[0] + ph[3],
+                   "pairs_per_s": B * n / t, "alg_lane_ops_per_pair": ops, "alu_frac": B * n * ops / t / peak,
+                   "fma_pipe_frac": B * n * 2 * p.state_dim / t / peak, "tree_GBps": 4 * p.state_dim * n / t / 1e9}
+            if mode == pakr.NN_FILTER:
+                K = 32 if 3 * (p.state_dim + int((p.dim_kind == 1).sum()) + 1) <= 32 else 48
+                row.update({"rescoring_ms": ph[3], "filter_K": K,
+                            # tensor roofline of the first phase: K multiply-accumulates per pair against the measured
+                            # mma.sync rate with the min-fold epilogue (bench.py --what peak)
+                            "mma_mac_per_s": B * n * K / (ph[0] * 1e-3)})
+            print(json.dumps(row), flush=True)
         pl.close()
     # HBM-bound regime: few queries share one pass over a tree > L2.  Algorithmic bytes = 4 * D * n.
     for name, B in ((("C2", 8), ("C4", 8), ("C4", 4)) if args.only in ("", "stream") else ()):
@@ -424,8 +442,9 @@ def run_phases(args):
         t = ph[0] * 1e-3
         print(json.dumps({"phase": "stream", "workload": name, "D": p.state_dim, "n": n, "B": B, "ms": ph[0],
                           "algorithmic_GBps": 4 * p.state_dim * n / t / 1e9,
-                          "hbm_frac_of_measured_6446": 4 * p.state_dim * n / t / 6446.3e9,
-                          "row_bytes_in_memory": 4 * p.state_stride, "l2": "flushed before every call"}), flush=True)
+                          "hbm_frac_of_measured": 4 * p.state_dim * n / t / (hbm_peak_gbs * 1e9), "hbm_peak_GBps": hbm_peak_gbs,
+                          "alu_frac": B * n * nn_ops_per_pair(p) / t / peak,
+                          "row_bytes_in_memory": 4 * p.state_dim, "l2": "flushed before every call"}), flush=True)
         pl.close()
     for name, B, K in ((("C2", 1024, 8), ("C3", 2048, 8), ("C4", 4096, 16), ("C5", 16384, 64)) if args.only in ("", "prop") else ()):
         if args.quick and name in ("C3",):
@@ -551,7 +570,7 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the other_workloads rows")
     ap.add_argument("--seeds", type=int, default=10, help="--what sweep|c5|pathlen: planner seeds per row")
     ap.add_argument("--quick", action="store_true", help="--what phases: fewer points and repetitions")
-    ap.add_argument("--only", default="", help="--what phases: nn | stream | prop")
+    ap.add_argument("--only", default="", help="--what phases: nn | filter | stream | prop")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

@@ -71,7 +71,7 @@ constexpr size_t kAlign = 256;
 size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-  size_t states, actions, parents, costs, nn_key, frow, chunkmin, unit_count, scr_state, scr_ctrl, scr_cost, scr_parent,
+  size_t states, actions, parents, costs, nn_key, prow, frow, chunkmin, unit_count, scr_state, scr_ctrl, scr_cost, scr_parent,
       scr_flags, idx_keys, idx_ids, idx_hist, idx_ctasum, idx_tile_ids, idx_rows, idx_tlo, idx_thi, idx_slo, idx_shi,
       ctrl, path_rev, path_nodes, path_states, path_controls, total;
 };
@@ -86,6 +86,7 @@ Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap) {
   L.parents = take((size_t)cap * 4);
   L.costs = take((size_t)cap * 4);
   L.nn_key = take((size_t)B * 16);  // two iterations in flight
+  L.prow = take(B <= kStreamB ? ((size_t)cap + 4) * pl->D * 4 : 0); // streaming tier: packed rows
   L.frow = take(((size_t)cap + 8) * 96);                            // filter rows: K <= 48 halves
   L.chunkmin = take((size_t)B * kFilterMaxChunks * 4);
   L.unit_count = take(std::max<size_t>(U, kFuseUnits + 8) * 4);
@@ -551,6 +552,7 @@ void fill_common(const pakr_planner* pl, Params& P, const Layout& L, char* ws, i
   P.pb = pl->pb;
   P.nn_key = reinterpret_cast<unsigned long long*>(ws + L.nn_key);
   P.unit_count = reinterpret_cast<unsigned*>(ws + L.unit_count);
+  P.prow = reinterpret_cast<float*>(ws + L.prow);
   P.frow = reinterpret_cast<__half*>(ws + L.frow);
   P.chunkmin = reinterpret_cast<float*>(ws + L.chunkmin);
   P.idx_keys = reinterpret_cast<unsigned*>(ws + L.idx_keys);

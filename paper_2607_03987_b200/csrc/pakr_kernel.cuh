@@ -90,6 +90,7 @@ struct Params {
   float* idx_rows;             // [tiles][D][32] the sorted rows, dimension-major inside a tile
   float* idx_tlo; float* idx_thi;  // [super-tiles][D][32] boxes of the tiles
   float* idx_slo; float* idx_shi;  // [groups][D][32] boxes of the super-tiles
+  float* prow;                 // streaming tier: [cap + 4][D] the tree rows packed without pad lanes
   // tensor-core NN filter (pakr_nn_filter.cuh)
   int nn_filter;               // host: 1 = launch the filter tier's kernel
   __half* frow;                // [cap + 8][K halves] filter rows of the tree
@@ -292,15 +293,19 @@ __device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, u
     }
   }
   __syncthreads();
-  constexpr int TILE = TileCfg<DYN>::TILE, TF = TileCfg<DYN>::TILE_FLOATS;
+  // The rows come from the PACKED copy of the tree (D floats per row, no pad lanes): every byte that crosses HBM is a
+  // coordinate, 4 D n per pass -- the algorithmic figure of SURVEY.md 8(d).  Tiles are whole rows; a tile starts at a
+  // multiple of 4 rows and carries a multiple of 4 rows so that every bulk copy is 16-byte aligned and sized.
+  constexpr int TILE = TileCfg<DYN>::TILE, TF = TILE * D;
   const int W = vbcount * kWarps, gw = vb * kWarps + warp;
   // every warp streams ONE contiguous chunk of rows through its double-buffered TMA tiles; inside a tile
   // lane l scores rows l, l+32, ... (ascending per lane)
-  const int span = nend - nbeg;
+  const int base = nbeg & ~3;
+  const int span = nend - base;
   const int chunk = ((span + W - 1) / W + 31) & ~31;
-  const int cb = nbeg + min(span, gw * chunk), ce = nbeg + min(span, (gw + 1) * chunk);
+  const int cb = base + min(span, gw * chunk), ce = base + min(span, (gw + 1) * chunk);
   const int ntiles = (ce - cb + TILE - 1) / TILE;
-  const float* src = P.states + (size_t)cb * DP;
+  const float* src = P.prow + (size_t)cb * D;
   for (int q0 = 0; q0 < P.B; q0 += QS) {
     f32x2 q2[QS / 2][D];
     float best[QS];
@@ -314,7 +319,7 @@ __device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, u
 #pragma unroll
     for (int j = 0; j < QS; ++j) { best[j] = __int_as_float(0x7f800000); bidx[j] = 0x7fffffff; }
     if (ntiles > 0 && lane == 0) {
-      const uint32_t bytes = (uint32_t)min(TILE, ce - cb) * DP * 4;
+      const uint32_t bytes = (uint32_t)((min(TILE, ce - cb) + 3) & ~3) * D * 4;
       mbar_expect_tx(&sm_bar[0], bytes);
       tma_load_1d(sm_tile, src, bytes, &sm_bar[0]);
     }
@@ -322,22 +327,28 @@ __device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, u
       const int cnt = min(TILE, ce - cb - t * TILE);
       if (t + 1 < ntiles && lane == 0) {  // prefetch the next tile into the other buffer
         const int nb = (t + 1) & 1;
-        const uint32_t bytes = (uint32_t)min(TILE, ce - cb - (t + 1) * TILE) * DP * 4;
+        const uint32_t bytes = (uint32_t)((min(TILE, ce - cb - (t + 1) * TILE) + 3) & ~3) * D * 4;
         mbar_expect_tx(&sm_bar[nb], bytes);
-        tma_load_1d(sm_tile + nb * TF, src + (size_t)(t + 1) * TF, bytes, &sm_bar[nb]);
+        tma_load_1d(sm_tile + nb * kTileBufFloats, src + (size_t)(t + 1) * TF, bytes, &sm_bar[nb]);
       }
       if (t & 1) { mbar_wait(&sm_bar[1], par1); par1 ^= 1; }
       else { mbar_wait(&sm_bar[0], par0); par0 ^= 1; }
-      const float4* tp = reinterpret_cast<const float4*>(sm_tile + (t & 1) * TF);
+      const float* tp = sm_tile + (t & 1) * kTileBufFloats;
 #pragma unroll 2
       for (int i = lane; i < cnt; i += 32) {
         float p[DP];
+        if constexpr (D % 2 == 0) {  // 8-byte aligned rows: LDS.64, conflict-free per half-warp (row stride D words)
+          const float2* rp = reinterpret_cast<const float2*>(tp + i * D);
 #pragma unroll
-        for (int v = 0; v < DP / 4; ++v) {
-          const float4 a = tp[i * (DP / 4) + v];
-          p[4 * v] = a.x; p[4 * v + 1] = a.y; p[4 * v + 2] = a.z; p[4 * v + 3] = a.w;
+          for (int v = 0; v < D / 2; ++v) { const float2 a = rp[v]; p[2 * v] = a.x; p[2 * v + 1] = a.y; }
+        } else {                      // odd row stride: scalar loads are conflict-free
+#pragma unroll
+          for (int d = 0; d < D; ++d) p[d] = tp[i * D + d];
         }
+#pragma unroll
+        for (int d = D; d < DP; ++d) p[d] = 0.0f;
         const int row = cb + t * TILE + i;
+        if (row < nbeg) continue;  // the chunk of warp 0 starts at the aligned row below nbeg
 #pragma unroll
         for (int h = 0; h < QS / 2; ++h) {
           float da, db;
@@ -667,7 +678,8 @@ __device__ __forceinline__ int idx_pop_nearest(unsigned& cand, float lb, float u
 // the tightened ub after every batch.  Scoring a tile the final ub would have excluded costs time, never exactness.
 template <int DYN, bool UNIT_W>
 __device__ __forceinline__ unsigned long long idx_search(const Params& P, const IdxDims& G,
-                                                         const float (&q)[DynTraits<DYN>::D], long long& scored) {
+                                                         const float (&q)[DynTraits<DYN>::D], long long& scored,
+                                                         int part, int nparts, const unsigned long long* shared_key) {
   constexpr int NT = 8;  // tiles scored together
   const int lane = threadIdx.x & 31;
   const float inf = __int_as_float(0x7f800000);
@@ -688,8 +700,10 @@ __device__ __forceinline__ unsigned long long idx_search(const Params& P, const 
     const float lb = t < G.n_tiles ? idx_box_bound<DYN>(P.pb, P.idx_tlo, P.idx_thi, (size_t)s_near, lane, q) : inf;
     t_near = (int)(unsigned)(warp_min_key(((unsigned long long)__float_as_uint(lb) << 32) | (unsigned)t) & 0xffffffffu);
     const int one[1] = {t_near};
-    ub = idx_score_tiles<DYN, UNIT_W, 1>(P, one, 1, q, best, ub);
+    unsigned long long near_best = kKeyNone;
+    ub = idx_score_tiles<DYN, UNIT_W, 1>(P, one, 1, q, near_best, ub);
     scored += 32;
+    if (part == 0) best = near_best;  // every part scores this tile for its bound; part 0 reports it
   }
   int pend[NT];  // warp-uniform queue of tiles waiting to be scored
   int np = 0;
@@ -699,8 +713,13 @@ __device__ __forceinline__ unsigned long long idx_search(const Params& P, const 
   for (int s0 = 0; s0 < G.n_super; s0 += 32) {
     const int s_mine = s0 + lane;
     const float lb = s_mine < G.n_super ? idx_box_bound<DYN>(P.pb, P.idx_slo, P.idx_shi, (size_t)(s0 >> 5), lane, q) : inf;
-    unsigned cand = __ballot_sync(0xffffffffu, s_mine < G.n_super && lb <= ub);
+    // this part's super-tiles: every nparts-th one (spatially spread, so the parts cost about the same)
+    unsigned cand = __ballot_sync(0xffffffffu, s_mine < G.n_super && s_mine % nparts == part && lb <= ub);
     for (;;) {
+      if (nparts > 1) {  // what the other parts of this query have found so far tightens the bound
+        const unsigned long long kv = __ldcg(shared_key);
+        if (kv != kKeyNone) ub = fminf(ub, __uint_as_float((unsigned)(kv >> 32)));
+      }
       const int j = idx_pop_nearest(cand, lb, ub);
       if (j < 0) break;
       const int s = s0 + j;
@@ -744,29 +763,39 @@ __device__ __forceinline__ unsigned long long idx_search(const Params& P, const 
 }
 
 // All indexed rows against every query of iteration `it` (Alg. 1 l.6-7).  The warps of the CTAs vb = 0..vbcount-1
-// take queries off a shared counter (far queries open many more boxes than near ones: static shares would leave
-// most warps waiting for the unlucky ones); each draws its query itself.
+// take work off a shared counter (far queries open many more boxes than near ones: static shares would leave most
+// warps waiting for the unlucky ones).  A unit is (query, part): the super-tiles of a query are dealt to kIdxParts
+// units, handed out part by part, so that one expensive query is four medium units instead of one long tail, and the
+// later parts start from the bound the earlier ones left in key[s] -- but only while queries are scarce (fewer than ~8
+// per warp): with many queries the balance is there already and the repeated first pass would only cost.
+// Each unit draws its query itself.
+constexpr int kIdxParts = 4;
+
 template <int DYN, bool UNIT_W>
 __device__ __forceinline__ void idx_phase(const Params& P, int n_sorted, uint32_t r, uint32_t it,
-                                          unsigned long long* key, int vb, int* counter, long long& scored) {
+                                          unsigned long long* key, int vb, int vbcount, int* counter, long long& scored) {
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
   if (vb < 0) return;
   const int lane = threadIdx.x & 31;
   const IdxDims G = idx_dims(n_sorted);
+  const int want = 8 * vbcount * kWarps / P.B;  // parts that bring the units to ~8 per warp
+  const int nparts = G.n_super < 4 * kIdxParts ? 1 : want >= 4 ? kIdxParts : want >= 2 ? 2 : 1;
+  const int units = P.B * nparts;
   for (;;) {
-    int s = 0;
-    if (lane == 0) s = atomicAdd(counter, 1);
-    s = __shfl_sync(0xffffffffu, s, 0);
-    if (s >= P.B) break;
+    int u = 0;
+    if (lane == 0) u = atomicAdd(counter, 1);
+    u = __shfl_sync(0xffffffffu, u, 0);
+    if (u >= units) break;
+    const int part = u / P.B, s = u - part * P.B;
     float q[D];
     sample_state<D>(P.pb, P.seed, r, it, (uint32_t)s, q);
-    if (lane == 0) {
+    if (lane == 0 && part == 0) {
 #pragma unroll
       for (int d = 0; d < DP; ++d) {
         if (P.dbg_x_rand) P.dbg_x_rand[(size_t)s * DP + d] = d < D ? q[d] : 0.0f;
       }
     }
-    const unsigned long long kv = idx_search<DYN, UNIT_W>(P, G, q, scored);
+    const unsigned long long kv = idx_search<DYN, UNIT_W>(P, G, q, scored, part, nparts, &key[s]);
     if (lane == 0 && kv != kKeyNone) atomicMin(&key[s], kv);
   }
 }
@@ -1158,7 +1187,7 @@ __device__ __forceinline__ void tail_scan_rounds(const Params& P, int n, int U, 
 
 // The first `npcta` CTAs take part (all of them when the insert is a phase of its own; only the propagate CTAs
 // when it runs inside phase X).  tail_mode: 0 none, 2 CTA rounds (r, it_next) when the insert runs inside phase X.
-template <int DYN, bool FILTER>
+template <int DYN, bool FILTER, bool STREAM>
 __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, unsigned long long* key_done,
                                             int tail_mode, unsigned long long* key_next, uint32_t r, uint32_t it_next,
                                             int npcta, int* sm_pref, int* sm_upre, float* sm_qt, float* sm_tile,
@@ -1241,6 +1270,10 @@ __device__ __forceinline__ int insert_phase(const Params& P, int n, int gslot, u
         const float4 a = __ldcg(src + v);
         dst[v] = a;
         xr[4 * v] = a.x; xr[4 * v + 1] = a.y; xr[4 * v + 2] = a.z; xr[4 * v + 3] = a.w;
+      }
+      if constexpr (STREAM) {
+#pragma unroll
+        for (int d = 0; d < T::D; ++d) P.prow[(size_t)node * T::D + d] = xr[d];
       }
       if constexpr (FILTER) {
         float xd[T::D];
@@ -1362,6 +1395,17 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
   unsigned long long* const key0 = P.nn_key;
   unsigned long long* const key1 = P.nn_key + P.B;
 
+  if constexpr (STREAM) {
+    // packed rows of what is already in the tree: the root (pakr_plan) or a caller's whole tree (pakr_expand_step)
+    const int n0 = P.n_nodes_io ? __ldcg(P.n_nodes_io) : 1;
+    for (int i = blockIdx.x * kThreads + threadIdx.x; i < n0; i += gridDim.x * kThreads) {
+#pragma unroll
+      for (int d = 0; d < T::D; ++d) P.prow[(size_t)i * T::D + d] = __ldcg(&P.states[(size_t)i * T::DP + d]);
+    }
+    __threadfence();
+    fence_proxy_async();
+    grid.sync();
+  }
   if constexpr (FILTER) {
     // filter rows of what is already in the tree: the root (pakr_plan) or a caller's whole tree (pakr_expand_step),
     // plus far-away rows up to the next multiple of 8.  A hand-over cost, taken before the clock starts.
@@ -1436,8 +1480,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
         int a_beg = n_scanned;
         if (idx_use && n_sorted > 0 && n_scanned == 0) {  // whole-tree NN (first call on a given tree): index + rest
           int* qc = &P.ctrl->idx_query[0][iterations % kSlots];
-          if (P.pb.unit_weights) idx_phase<DYN, true>(P, n_sorted, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, qc, nn_scored);
-          else idx_phase<DYN, false>(P, n_sorted, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, qc, nn_scored);
+          if (P.pb.unit_weights) idx_phase<DYN, true>(P, n_sorted, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, qc, nn_scored);
+          else idx_phase<DYN, false>(P, n_sorted, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, qc, nn_scored);
           a_beg = n_sorted;
           cov_cur = n_sorted;
         }
@@ -1459,7 +1503,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
           ++pgen;
           cta_group_barrier(&P.ctrl->pbar, (unsigned)NPB * pgen);
           fence_proxy_async();
-          total = insert_phase<DYN, FILTER>(P, n, slot, kcur, ahead ? 2 : 0, knext, (uint32_t)r, (uint32_t)(it + 1), NPB, sm_pref,
+          total = insert_phase<DYN, FILTER, STREAM>(P, n, slot, kcur, ahead ? 2 : 0, knext, (uint32_t)r, (uint32_t)(it + 1), NPB, sm_pref,
                                     reinterpret_cast<int*>(sm_q), reinterpret_cast<float*>(sm_keys), my_tile, my_bar, par0,
                                     fused);
           if (leader) P.ctrl->iter_total[slot] = total;
@@ -1471,8 +1515,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
         int x_beg = 0;
         if (idx_use && n_sorted > 0) {
           int* qc = &P.ctrl->idx_query[1][slot];
-          if (P.pb.unit_weights) idx_phase<DYN, true>(P, n_sorted, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, qc, nn_scored);
-          else idx_phase<DYN, false>(P, n_sorted, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, qc, nn_scored);
+          if (P.pb.unit_weights) idx_phase<DYN, true>(P, n_sorted, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, qc, nn_scored);
+          else idx_phase<DYN, false>(P, n_sorted, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, qc, nn_scored);
           x_beg = n_sorted;
           cov_next = n_sorted;
         }
@@ -1495,7 +1539,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
         fused = ahead && total <= P.cap - n && total <= kXTailRows;
       } else {
         // phase C: insert as a phase of its own (every CTA takes part)
-        total = insert_phase<DYN, FILTER>(P, n, slot, kcur, 0, knext, (uint32_t)r, (uint32_t)(it + 1), NB, sm_pref,
+        total = insert_phase<DYN, FILTER, STREAM>(P, n, slot, kcur, 0, knext, (uint32_t)r, (uint32_t)(it + 1), NB, sm_pref,
                                   reinterpret_cast<int*>(sm_q), reinterpret_cast<float*>(sm_keys), my_tile, my_bar, par0,
                                   fused);
         if (leader) P.ctrl->stop[slot] = (P.budget_ns && globaltimer_ns() - t_start >= P.budget_ns) ? 1 : 0;

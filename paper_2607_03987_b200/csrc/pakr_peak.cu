@@ -4,6 +4,8 @@
 //   FFMA            scalar fused multiply-add                         (1 lane-op per lane per instruction)
 //   FFMA2           packed fma.rn.f32x2, the NN scan's instruction    (2 lane-ops per lane per instruction)
 //   FADD2 + FFMA2   the scan's own mix: one packed subtract per packed fma
+//   HMMA            mma.sync.m16n8k16 f16 x f16 -> f32, the tensor-core NN filter's instruction (pakr_nn_filter.cuh),
+//                   alone (accumulating) and with the filter's epilogue: fresh accumulators folded into running minima
 // A lane-op is one fp32 add, multiply or fused multiply-add on one lane.  Not on the planning path.
 #include <algorithm>
 #include <cuda_runtime.h>
@@ -55,6 +57,46 @@ __global__ void __launch_bounds__(kThreads) peak_ffma2(float* out, float a, floa
   out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
+__device__ __forceinline__ void mma_16816(float (&c)[4], const unsigned (&a)[4], const unsigned (&b)[2]) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+               : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+               : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
+}
+constexpr int kMmaChains = 8, kMmaIters = 8192;
+
+template <bool MIN_FOLD>
+__global__ void __launch_bounds__(kThreads) peak_mma(float* out, float a0, float b0) {
+  unsigned a[kMmaChains][4], b[2] = {__float_as_uint(b0) + threadIdx.x, 0x3c003c00u};
+#pragma unroll
+  for (int i = 0; i < kMmaChains; ++i) {
+    a[i][0] = __float_as_uint(a0) + i; a[i][1] = 0x3c003c00u + threadIdx.x; a[i][2] = 0x38003800u; a[i][3] = 0x34003400u + i;
+  }
+  float acc[kMmaChains][4], m[kMmaChains][2];
+#pragma unroll
+  for (int i = 0; i < kMmaChains; ++i) {
+    acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.0f;
+    m[i][0] = m[i][1] = 3.0e38f;
+  }
+  for (int it = 0; it < kMmaIters; ++it) {
+    if (MIN_FOLD) b[0] += 0x00010001u;
+#pragma unroll
+    for (int i = 0; i < kMmaChains; ++i) {
+      if (MIN_FOLD) {
+        float c[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+        mma_16816(c, a[i], b);
+        m[i][0] = fminf(m[i][0], fminf(c[0], c[1]));
+        m[i][1] = fminf(m[i][1], fminf(c[2], c[3]));
+      } else {
+        mma_16816(acc[i], a[i], b);
+      }
+    }
+  }
+  float s = 0.0f;
+#pragma unroll
+  for (int i = 0; i < kMmaChains; ++i) s += acc[i][0] + acc[i][1] + acc[i][2] + acc[i][3] + m[i][0] + m[i][1];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 template <class K>
 cudaError_t time_kernel(K kernel, int sms, float* out, int reps, double lane_ops_per_thread, double* rate) {
   cudaEvent_t e0, e1;
@@ -96,6 +138,10 @@ extern "C" pakr_status pakr_measure_fp32_peak(int cuda_device, pakr_fp32_peak* o
   if (e == cudaSuccess) e = time_kernel(peak_ffma, prop.multiProcessorCount, buf, 5, per_thread, &out->ffma_lane_ops_per_s);
   if (e == cudaSuccess) e = time_kernel(peak_ffma2<false>, prop.multiProcessorCount, buf, 5, 2.0 * per_thread, &out->ffma2_lane_ops_per_s);
   if (e == cudaSuccess) e = time_kernel(peak_ffma2<true>, prop.multiProcessorCount, buf, 5, 2.0 * per_thread, &out->scan_mix_lane_ops_per_s);
+  // one warp instruction = 16 x 8 x 16 multiply-accumulates: 64 per lane
+  const double mma_per_thread = (double)kMmaChains * kMmaIters * 64.0;
+  if (e == cudaSuccess) e = time_kernel(peak_mma<false>, prop.multiProcessorCount, buf, 5, mma_per_thread, &out->mma_f16_mac_per_s);
+  if (e == cudaSuccess) e = time_kernel(peak_mma<true>, prop.multiProcessorCount, buf, 5, mma_per_thread, &out->mma_f16_minfold_mac_per_s);
   if (e == cudaSuccess) {
     out->sm_count = prop.multiProcessorCount;
     int khz = 0;

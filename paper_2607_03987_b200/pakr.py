@@ -139,7 +139,8 @@ class _StepArgs(C.Structure):
 
 class _Fp32Peak(C.Structure):
     _fields_ = [("ffma_lane_ops_per_s", C.c_double), ("ffma2_lane_ops_per_s", C.c_double),
-                ("scan_mix_lane_ops_per_s", C.c_double), ("sm_clock_mhz", C.c_double), ("sm_count", C.c_int32)]
+                ("scan_mix_lane_ops_per_s", C.c_double), ("sm_clock_mhz", C.c_double), ("sm_count", C.c_int32),
+                ("mma_f16_mac_per_s", C.c_double), ("mma_f16_minfold_mac_per_s", C.c_double)]
 
 
 EXPORTS = ["pakr_create", "pakr_destroy", "pakr_last_error", "pakr_workspace_bytes", "pakr_get_tree_layout",
