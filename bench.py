@@ -434,7 +434,7 @@ def run_phases(args):
             print(json.dumps(row), flush=True)
         pl.close()
     # HBM-bound regime: few queries share one pass over a tree > L2.  Algorithmic bytes = 4 * D * n.
-    for name, B in ((("C2", 8), ("C4", 8), ("C4", 4)) if args.only in ("", "stream") else ()):
+    for name, B in ((("C2", 4), ("C2", 8), ("C4", 4), ("C4", 8)) if args.only in ("", "stream") else ()):
         p, _ = wl.CONFIGS[name]()
         pl = pakr.Planner(p)
         n = 1 << 23

@@ -128,7 +128,7 @@ size_t tile_floats(int DP) { return (size_t)TileCfg<DYN_DI2>::TILE * 4; }  // ev
 
 size_t smem_for(const pakr_planner* pl) {
   const int os = pl->obs == OBS_CIRCLE ? 4 : 8;
-  return kWarps * 2 * tile_floats(pl->DP) * 4 + kWarps * 2 * 8 + (kThreads + kWarps + 8) * 4 + kMaxD * 2 * 32 * kQ * 4 + kWarps * 32 * kQ * 8 +
+  return kWarps * 2 * tile_floats(pl->DP) * 4 + kWarps * 4 * 8 + (kThreads + kWarps + 8) * 4 + kMaxD * 2 * 32 * kQ * 4 + kWarps * 32 * kQ * 8 +
          (size_t)((pl->pb.n_obs * os + 3) & ~3) * 4 + (size_t)pl->pb.g_cells * 4 + (size_t)pl->pb.g_list * 2 + 16;
 }
 

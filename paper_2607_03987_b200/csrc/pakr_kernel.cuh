@@ -275,7 +275,7 @@ constexpr int kStreamB = 16;
 template <int DYN, bool UNIT_W>
 __device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, uint32_t r, uint32_t it,
                                        unsigned long long* key, int vb, int vbcount, float* sm_q,
-                                          float* sm_tile, uint64_t* sm_bar, uint32_t& par0, uint32_t& par1) {
+                                          float* sm_tile, uint64_t* sm_bar, uint32_t& par0, uint32_t& par1, uint32_t& parx) {
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
   constexpr int QS = (D <= 8) ? 8 : 4;  // queries held in registers per pass over the rows
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -296,16 +296,25 @@ __device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, u
   // The rows come from the PACKED copy of the tree (D floats per row, no pad lanes): every byte that crosses HBM is a
   // coordinate, 4 D n per pass -- the algorithmic figure of SURVEY.md 8(d).  Tiles are whole rows; a tile starts at a
   // multiple of 4 rows and carries a multiple of 4 rows so that every bulk copy is 16-byte aligned and sized.
-  constexpr int TILE = TileCfg<DYN>::TILE, TF = TILE * D;
-  const int W = vbcount * kWarps, gw = vb * kWarps + warp;
-  // every warp streams ONE contiguous chunk of rows through its double-buffered TMA tiles; inside a tile
-  // lane l scores rows l, l+32, ... (ascending per lane)
+  // A CTA streams ONE contiguous chunk of rows; its warps take the chunk's tiles round robin (warp w: tiles w, w + 8,
+  // ...), so the eight bulk copies a CTA has in flight cover one contiguous 24-32 KB stretch of HBM instead of eight
+  // separate streams.  Tiles hold a multiple of 32 rows (every lane of the row loop busy), at most 4 KB, two buffers
+  // per warp.  Inside a tile lane l scores rows l, l+32, ...: ascending per lane over the whole call.
+  constexpr int NS = 2, BUF = kTileBufFloats;
+  constexpr int TILE = ((BUF / D) & ~31), TF = TILE * D;
   const int base = nbeg & ~3;
   const int span = nend - base;
-  const int chunk = ((span + W - 1) / W + 31) & ~31;
-  const int cb = base + min(span, gw * chunk), ce = base + min(span, (gw + 1) * chunk);
-  const int ntiles = (ce - cb + TILE - 1) / TILE;
+  const int cchunk = ((span + vbcount - 1) / vbcount + TILE - 1) / TILE * TILE;  // rows per CTA: whole tiles
+  const int cb = base + min(span, vb * cchunk), ce = base + min(span, (vb + 1) * cchunk);
+  const int ctiles = (ce - cb + TILE - 1) / TILE;
+  const int ntiles = ctiles > warp ? (ctiles - warp + kWarps - 1) / kWarps : 0;  // this warp's tiles
   const float* src = P.prow + (size_t)cb * D;
+  auto issue = [&](int t) {  // lane 0: bulk copy of this warp's t-th tile into stage t % NS
+    const int st = t % NS, T = t * kWarps + warp;
+    const uint32_t bytes = (uint32_t)((min(TILE, ce - cb - T * TILE) + 3) & ~3) * D * 4;
+    mbar_expect_tx(&sm_bar[st], bytes);
+    tma_load_1d(sm_tile + st * BUF, src + (size_t)T * TF, bytes, &sm_bar[st]);
+  };
   for (int q0 = 0; q0 < P.B; q0 += QS) {
     f32x2 q2[QS / 2][D];
     float best[QS];
@@ -318,22 +327,16 @@ __device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, u
     }
 #pragma unroll
     for (int j = 0; j < QS; ++j) { best[j] = __int_as_float(0x7f800000); bidx[j] = 0x7fffffff; }
-    if (ntiles > 0 && lane == 0) {
-      const uint32_t bytes = (uint32_t)((min(TILE, ce - cb) + 3) & ~3) * D * 4;
-      mbar_expect_tx(&sm_bar[0], bytes);
-      tma_load_1d(sm_tile, src, bytes, &sm_bar[0]);
-    }
+    if (lane == 0)
+      for (int t = 0; t < min(NS - 1, ntiles); ++t) issue(t);
     for (int t = 0; t < ntiles; ++t) {
-      const int cnt = min(TILE, ce - cb - t * TILE);
-      if (t + 1 < ntiles && lane == 0) {  // prefetch the next tile into the other buffer
-        const int nb = (t + 1) & 1;
-        const uint32_t bytes = (uint32_t)((min(TILE, ce - cb - (t + 1) * TILE) + 3) & ~3) * D * 4;
-        mbar_expect_tx(&sm_bar[nb], bytes);
-        tma_load_1d(sm_tile + nb * kTileBufFloats, src + (size_t)(t + 1) * TF, bytes, &sm_bar[nb]);
-      }
-      if (t & 1) { mbar_wait(&sm_bar[1], par1); par1 ^= 1; }
-      else { mbar_wait(&sm_bar[0], par0); par0 ^= 1; }
-      const float* tp = sm_tile + (t & 1) * kTileBufFloats;
+      const int T = t * kWarps + warp;
+      const int cnt = min(TILE, ce - cb - T * TILE);
+      if (t + NS - 1 < ntiles && lane == 0) issue(t + NS - 1);  // into the stage tile t-1 left (syncwarp below)
+      const int st = t % NS;
+      if (st == 0) { mbar_wait(&sm_bar[0], par0); par0 ^= 1; }
+      else { mbar_wait(&sm_bar[1], par1); par1 ^= 1; }
+      const float* tp = sm_tile + st * BUF;
 #pragma unroll 2
       for (int i = lane; i < cnt; i += 32) {
         float p[DP];
@@ -347,8 +350,8 @@ __device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, u
         }
 #pragma unroll
         for (int d = D; d < DP; ++d) p[d] = 0.0f;
-        const int row = cb + t * TILE + i;
-        if (row < nbeg) continue;  // the chunk of warp 0 starts at the aligned row below nbeg
+        const int row = cb + T * TILE + i;
+        if (row < nbeg) continue;  // the first tile starts at the aligned row below nbeg
 #pragma unroll
         for (int h = 0; h < QS / 2; ++h) {
           float da, db;
@@ -357,7 +360,7 @@ __device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, u
           if (db < best[2 * h + 1]) { best[2 * h + 1] = db; bidx[2 * h + 1] = row; }
         }
       }
-      __syncwarp();  // every lane is done with this buffer before lane 0 refills it
+      __syncwarp();  // every lane is done with this stage before lane 0 refills it
     }
 #pragma unroll
     for (int j = 0; j < QS; ++j) {
@@ -816,7 +819,7 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
                                          uint64_t* sm_bar, float* sm_q, unsigned long long* sm_keys, uint32_t& par0,
                                          uint32_t& par1, cg::grid_group& grid, unsigned& sgen,
                                          bool filter_live, unsigned long long* f_slot, long long& filtered,
-                                         unsigned long long& ph_outer, unsigned long long& ph_refine, unsigned long long& tp) {
+                                         unsigned long long& ph_outer, unsigned long long& ph_refine, unsigned long long& tp, uint32_t& parx) {
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
   constexpr int TILE = TileCfg<DYN>::TILE, TF = TileCfg<DYN>::TILE_FLOATS;
   constexpr int QG = 32 * kQ;  // queries per group
@@ -824,7 +827,7 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
   const int n = nend - nbeg;
   if (vb < 0 || n <= 0) return;
   if constexpr (STREAM) {  // few queries (B <= kStreamB, chosen by the host): HBM-bound streaming tier
-    nn_stream<DYN, UNIT_W>(P, nbeg, nend, r, it, key, vb, vbcount, sm_q, sm_tile, sm_bar, par0, par1);
+    nn_stream<DYN, UNIT_W>(P, nbeg, nend, r, it, key, vb, vbcount, sm_q, sm_tile, sm_bar, par0, par1, parx);
     return;
   } else if constexpr (FILTER) {
    if (filter_live && n >= kFilterMinRows && (long long)P.B * n * D >= P.filter_min_work) {
@@ -1345,12 +1348,12 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
   using T = DynTraits<DYN>;
   constexpr int OS = (OBS == OBS_CIRCLE) ? 4 : 8;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  // [tiles: kWarps * 2 * TILE_FLOATS][bars: kWarps * 2][pref: kThreads + kWarps + 8][queries: kMaxD * 256]
+  // [tiles: kWarps * 2 * kTileBufFloats][bars: kWarps * 4][pref: kThreads + kWarps + 8][queries: kMaxD * 256]
   // [merge keys: kWarps * 128 x u64]
   // [obstacles][grid cells][grid lists]
   float* sm_tiles = reinterpret_cast<float*>(smem_raw);
   uint64_t* sm_bars = reinterpret_cast<uint64_t*>(sm_tiles + kWarps * 2 * kTileBufFloats);
-  int* sm_pref = reinterpret_cast<int*>(sm_bars + kWarps * 2);
+  int* sm_pref = reinterpret_cast<int*>(sm_bars + kWarps * 4);
   float* sm_q = reinterpret_cast<float*>(sm_pref + kThreads + kWarps + 8);
   unsigned long long* sm_keys = reinterpret_cast<unsigned long long*>(sm_q + kMaxD * 2 * 32 * kQ);
   float* sm_obs = reinterpret_cast<float*>(sm_keys + kWarps * 32 * kQ);
@@ -1366,15 +1369,15 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
     for (int i = threadIdx.x; i < P.pb.g_list; i += kThreads) sm_list[i] = P.pb.grid_list[i];
   }
   if (lane == 0) {
-    mbar_init(&sm_bars[warp * 2], 1);
-    mbar_init(&sm_bars[warp * 2 + 1], 1);
+#pragma unroll
+    for (int b = 0; b < 4; ++b) mbar_init(&sm_bars[warp * 4 + b], 1);  // [2], [3]: the streaming tier's extra stages
   }
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   fence_proxy_async();
   __syncthreads();
   float* my_tile = sm_tiles + warp * 2 * kTileBufFloats;
-  uint64_t* my_bar = sm_bars + warp * 2;
-  uint32_t par0 = 0, par1 = 0;
+  uint64_t* my_bar = sm_bars + warp * 4;
+  uint32_t par0 = 0, par1 = 0, parx = 0;
 
   // Roles in phase X.  When the children fill at most a quarter of the SMs, the first NPB CTAs only
   // propagate (latency-bound dependent chains, kept away from the issue-bound scan warps) and the other
@@ -1485,8 +1488,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
           a_beg = n_sorted;
           cov_cur = n_sorted;
         }
-        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM, FILTER>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_head, ph0, ph3, tp);
-        else nn_phase<DYN, false, STREAM, FILTER>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_head, ph0, ph3, tp);
+        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM, FILTER>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_head, ph0, ph3, tp, parx);
+        else nn_phase<DYN, false, STREAM, FILTER>(P, a_beg, n, (uint32_t)r, (uint32_t)it, kcur, (int)blockIdx.x, NB, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_head, ph0, ph3, tp, parx);
         grid.sync();
       }
       if (leader) { const unsigned long long t = globaltimer_ns(); ph0 += t - tp; tp = t; }
@@ -1520,8 +1523,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
           x_beg = n_sorted;
           cov_next = n_sorted;
         }
-        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM, FILTER>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_x, ph1, ph3, tp);
-        else nn_phase<DYN, false, STREAM, FILTER>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_x, ph1, ph3, tp);
+        if (P.pb.unit_weights) nn_phase<DYN, true, STREAM, FILTER>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_x, ph1, ph3, tp, parx);
+        else nn_phase<DYN, false, STREAM, FILTER>(P, x_beg, n, (uint32_t)r, (uint32_t)(it + 1), knext, x_vb, x_vbcnt, my_tile, my_bar, sm_q, sm_keys, par0, par1, grid, sgen, filter_live, &P.ctrl->f_rescored[slot], filt_x, ph1, ph3, tp, parx);
       }
       if (leader) {
         P.ctrl->goal_key[slot_next] = kKeyNone;
