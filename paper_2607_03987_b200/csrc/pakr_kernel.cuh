@@ -781,7 +781,7 @@ __device__ __forceinline__ void idx_phase(const Params& P, int n_sorted, uint32_
   if (vb < 0) return;
   const int lane = threadIdx.x & 31;
   const IdxDims G = idx_dims(n_sorted);
-  const int want = 8 * vbcount * kWarps / P.B;  // parts that bring the units to ~8 per warp
+  const int want = 8 * vbcount * kWarps / P.B;  // parts that bring the units to ~8 per warp (8 parts measured slower)
   const int nparts = G.n_super < 4 * kIdxParts ? 1 : want >= 4 ? kIdxParts : want >= 2 ? 2 : 1;
   const int units = P.B * nparts;
   for (;;) {

@@ -27,7 +27,7 @@
 // only 32..48.  tcgen05.mma would finish a 128 x 256 x 32 tile in ~256 cycles but draining its 128 KB of accumulators
 // through tcgen05.ld takes >= 2048 cycles at the measured 64 B/clk/SM (B300_MICROARCH.md "TMEM"); mma.sync leaves the
 // accumulators in registers where the FMNMX fold is free, and sustains 750 MAC/clk/SM with the fold (measured,
-// profiles/r02_mma_sync_rates.md) = 23 (K = 32) / 15 (K = 48) pairs/clk/SM against 10.7 / 3.6 for the FFMA2 scan.
+// profiles/r02_fp32_peak.md) = 23 (K = 32) / 15 (K = 48) pairs/clk/SM against 10.7 / 3.6 for the FFMA2 scan.
 #pragma once
 #include <cuda_fp16.h>
 
