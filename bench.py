@@ -42,14 +42,14 @@ UNIT = "nodes/s"
 C5_POINT = (4096, 16)  # the fixed config-5 point reported beside the headline
 # dram__bytes_read.sum + dram__bytes_write.sum of one pakr_loop_kernel launch on WORKLOAD, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists for the current kernel).
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 51817216  # profiles/r02_ncu_c4_bench.md: 1,700,608 read + 50,116,608 written
 NOMINAL_LANES = 148 * 4 * 32  # SMs x schedulers x lanes: issue slots per clock = fp32 FMA lanes per clock
 
 # Arithmetic of one evaluation of f(x, u), counted on the formulas of DESIGN.md "Readings" Q / P33 / P34 with every
 # multiply-add fused (one lane-op each), a sine/cosine pair as 2, a reciprocal as 1 (DESIGN.md "Measurement" has
 # the count line by line).
 F_DYN = {wl.DYN_DOUBLE_INTEGRATOR: 0, wl.DYN_UNICYCLE2: 4, wl.DYN_QUADROTOR: 37, wl.DYN_DUBINS_AIRPLANE: 8,
-         wl.DYN_UNICYCLE1: 4, wl.DYN_QUADROTOR_BODY: 59}
+         wl.DYN_UNICYCLE1: 4, wl.DYN_QUADROTOR_BODY: 59, wl.DYN_ACROBOT: 24}
 
 
 def nn_ops_per_pair(problem) -> int:
@@ -246,6 +246,9 @@ def roofline_of(problem, results, dev_ms, sm_max_mhz, measured_peak) -> dict:
         exe = (ev * ops[0]["nn_per_pair"] + sum(o["prop"] for o in ops)) / launch_s / 1e12
         out["nn_pairs_evaluated_share"] = ev / tot
         out["executed_frac"] = exe / peak
+        out["note"] = ("achieved counts the ALGORITHMIC lane-ops of the B*n-pair NN definition (SURVEY.md 8(d)); the NN index / "
+                       "tensor-core filter answered it with nn_pairs_evaluated_share of the fp32 distance evaluations, so frac "
+                       "can exceed 1; executed_frac = lane-ops actually executed / peak")
     return out
 
 
@@ -469,7 +472,7 @@ def med(v):
 
 
 def run_sweep_configs(pakr, seeds, path_length=False):
-    for name in (("C1", "C2") if path_length else ("C1", "C2", "C3", "C4", "N1", "N2", "N3")):
+    for name in (("C1", "C2") if path_length else ("C1", "C2", "C3", "C4", "N1", "N2", "N3", "N4")):
         p, cfg = wl.CONFIGS[name]()
         if path_length:  # the paper's convergence metric (Table II, Fig. 2: cost = distance travelled)
             p = dataclasses.replace(p, cost_mode=wl.COST_PATH_LENGTH, heuristic_speed=1.0, name=p.name + "-pathlen")

@@ -866,6 +866,12 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
     const int beg = nbeg + rr * len;
     const int end = min(nend, beg + len);
     const bool shared_q = (g_hi - g_lo) <= 1;  // CTA-uniform
+    const float* src = P.states + (size_t)beg * DP;
+    if (has && lane == 0) {  // the first tile is on its way while the queries are drawn
+      const uint32_t bytes = (uint32_t)min(TILE, end - beg) * DP * 4;
+      mbar_expect_tx(&sm_bar[0], bytes);
+      tma_load_1d(sm_tile, src, bytes, &sm_bar[0]);
+    }
     f32x2 q2[kQ / 2][D];  // queries 2h and 2h+1 of this lane, packed per dimension
     float best[kQ];
     int bidx[kQ];
@@ -911,12 +917,6 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
     }
     if (has) {
     const int ntiles = (end - beg + TILE - 1) / TILE;
-    const float* src = P.states + (size_t)beg * DP;
-    if (lane == 0) {
-      const uint32_t bytes = (uint32_t)min(TILE, end - beg) * DP * 4;
-      mbar_expect_tx(&sm_bar[0], bytes);
-      tma_load_1d(sm_tile, src, bytes, &sm_bar[0]);
-    }
     for (int t = 0; t < ntiles; ++t) {
       const int cnt = min(TILE, end - beg - t * TILE);
       if (t + 1 < ntiles && lane == 0) {  // prefetch the next tile into the other buffer
