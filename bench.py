@@ -449,15 +449,18 @@ def run_phases(args):
                           "alu_frac": B * n * nn_ops_per_pair(p) / t / peak,
                           "row_bytes_in_memory": 4 * p.state_dim, "l2": "flushed before every call"}), flush=True)
         pl.close()
-    for name, B, K in ((("C2", 1024, 8), ("C3", 2048, 8), ("C4", 4096, 16), ("C5", 16384, 64)) if args.only in ("", "prop") else ()):
-        if args.quick and name in ("C3",):
+    for name, B, K in ((("C2", 1024, 8), ("C3", 2048, 8), ("C4", 4096, 16), ("C5", 16384, 64)) if args.only in ("", "prop", "prop1") else ()):
+        if (args.quick and name in ("C3",)) or (args.only == "prop1" and name != "C4"):
             continue
         p, _ = wl.CONFIGS[name]()
         pl = pakr.Planner(p)
-        ph = measure_phase(torch, pl, p, 4096, B, K, reps, None)
+        # tree of 4096 nodes: the launch also scans 4096 rows; tree of 1 node (--only prop1): the launch is the
+        # propagate + insert alone, which is what an ncu capture of the executed instructions per child needs
+        n_tree = 1 if args.only == "prop1" else 4096
+        ph = measure_phase(torch, pl, p, n_tree, B, K, reps, None, nn_mode=pakr.NN_SCAN)
         t = ph[1] * 1e-3
         ops = prop_ops_per_child(p)
-        print(json.dumps({"phase": "prop", "workload": name, "children": B * K, "ms": ph[1], "insert_ms": ph[2],
+        print(json.dumps({"phase": "prop", "workload": name, "children": B * K, "tree_nodes": n_tree, "ms": ph[1], "insert_ms": ph[2],
                           "children_per_s": B * K / t, "alg_lane_ops_per_child": ops,
                           "alu_frac": B * K * ops / t / peak}), flush=True)
         pl.close()
@@ -573,7 +576,7 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the other_workloads rows")
     ap.add_argument("--seeds", type=int, default=10, help="--what sweep|c5|pathlen: planner seeds per row")
     ap.add_argument("--quick", action="store_true", help="--what phases: fewer points and repetitions")
-    ap.add_argument("--only", default="", help="--what phases: nn | filter | stream | prop")
+    ap.add_argument("--only", default="", help="--what phases: nn | filter | stream | prop | prop1")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

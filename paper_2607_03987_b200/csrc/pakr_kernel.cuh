@@ -1386,15 +1386,17 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
   const int W = NB * kWarps;
   const int gw = blockIdx.x * kWarps + warp;
   const int U_prop = (P.B * P.K + 31) / 32;
-  const int NPB = (U_prop + kWarps - 1) / kWarps;
-  const bool split = NPB * 4 <= NB;
-  const int x_pw = split ? (blockIdx.x < NPB ? gw : -1) : gw;  // propagate warp index, count
-  const int x_pcnt = split ? NPB * kWarps : W;
-  const int x_vb = split ? (int)blockIdx.x - NPB : (int)blockIdx.x;  // scan CTA index (< 0: none), count
-  const int x_vbcnt = split ? NB - NPB : NB;
+  const int NPB1 = (U_prop + kWarps - 1) / kWarps;  // propagate CTAs at one warp unit (32 children) per warp
+  const bool split = NPB1 * 4 <= NB;
   // insert inside phase X by the propagate CTAs (one grid barrier per iteration) when the children are few
   const bool xins = split && U_prop <= kFuseUnits;
-  unsigned pgen = 0, sgen = 0;
+  // Rough per-unit cost of an edge and per-pair cost of the scan (ns / ps, from profiles/r02_phases.jsonl): when the
+  // look-ahead scan of an iteration takes much longer than the edges, the propagate warps take 2 or 4 units each and
+  // the CTAs that frees join the scan.
+  const float unit_ns = 3000.0f + (float)P.pb.S * (P.pb.integrator ? 4.0f : 1.0f) *
+                                      ((DYN == DYN_DI2 || DYN == DYN_DI3) ? 150.0f : (DYN == DYN_QUAD || DYN == DYN_QUADB) ? 460.0f : 360.0f);
+  const float pair_ps = (P.pb.unit_weights ? 0.08f : 0.11f) * (float)T::D;
+  unsigned ptarget = 0, sgen = 0;
   unsigned long long* const key0 = P.nn_key;
   unsigned long long* const key1 = P.nn_key + P.B;
 
@@ -1495,6 +1497,18 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
       if (leader) { const unsigned long long t = globaltimer_ns(); ph0 += t - tp; tp = t; }
       // phase X: propagate(it) and, meanwhile, NN(it+1) over the frozen snapshot [0, n)
       const bool ahead = (iters + 1 < P.max_iters) && !idx_head;
+      // roles of this iteration (uniform: every thread derives them from the same n)
+      int upw = 1;  // warp units per propagate warp
+      if (split && !FILTER && ahead) {
+        const float scan_ns = (float)P.B * (float)n * pair_ps * 1e-3f;
+        upw = 4.0f * unit_ns <= 0.8f * scan_ns ? 4 : 2.0f * unit_ns <= 0.8f * scan_ns ? 2 : 1;
+      }
+      const int NPB = (U_prop + kWarps * upw - 1) / (kWarps * upw);
+      const int x_pw = split ? ((int)blockIdx.x < NPB ? gw : -1) : gw;  // propagate warp index, count
+      const int x_pcnt = split ? NPB * kWarps : W;
+      const int x_vb = split ? (int)blockIdx.x - NPB : (int)blockIdx.x;  // scan CTA index (< 0: none), count
+      const int x_vbcnt = split ? NB - NPB : NB;
+      ptarget += (unsigned)NPB;
       prop_phase<DYN, OBS>(P, (uint32_t)r, (uint32_t)it, c_best, kcur, root_only, x_pw, x_pcnt, sm_obs, sm_cells, sm_list);
       bool fused = false;
       int total = 0;
@@ -1503,8 +1517,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) pakr_loop_kernel(const _
         // barrier of their own, ordered insert, tail of NN(it+1) over the new rows.
         if ((int)blockIdx.x < NPB) {
           fence_proxy_async();  // scratch rows written with st.global are gathered by TMA below
-          ++pgen;
-          cta_group_barrier(&P.ctrl->pbar, (unsigned)NPB * pgen);
+          cta_group_barrier(&P.ctrl->pbar, ptarget);  // running count of arrivals: NPB may change between iterations
           fence_proxy_async();
           total = insert_phase<DYN, FILTER, STREAM>(P, n, slot, kcur, ahead ? 2 : 0, knext, (uint32_t)r, (uint32_t)(it + 1), NPB, sm_pref,
                                     reinterpret_cast<int*>(sm_q), reinterpret_cast<float*>(sm_keys), my_tile, my_bar, par0,
