@@ -124,7 +124,9 @@ void pakr_destroy(pakr_planner* planner);
  * pakr_last_error(NULL) returns the text of the last failed pakr_create in this thread. */
 const char* pakr_last_error(const pakr_planner* planner);
 
-/* Bytes of DEVICE workspace pakr_plan / pakr_expand_step need for (B, K, tree_capacity);
+/* Bytes of DEVICE workspace pakr_plan / pakr_expand_step need for (B, K, tree_capacity), whichever nn_mode is used later
+ * (tree 4*(Dp+6) bytes per node + the tiers' copies: packed rows when B <= 16, index arrays ~(4 D + 20) and filter rows 96
+ * bytes per node where the problem admits them, B * 16 KB of chunk minima for the filter);
  * 0 if an argument is invalid (B < 1, K < 1, K > 4096, B*K > 2^24, capacity < 2 or > 2^30). */
 size_t pakr_workspace_bytes(const pakr_planner* planner, int32_t B, int32_t K, int64_t tree_capacity);
 
@@ -206,7 +208,10 @@ typedef struct {
 pakr_status pakr_plan(pakr_planner* planner, const pakr_plan_opts* opts, void* d_workspace,
                       size_t workspace_bytes, void* cuda_stream, pakr_result* out);
 
-/* One trip of Alg. 1 l.6-17 on caller-visible DEVICE buffers (test hook; same kernels). */
+/* One trip of Alg. 1 l.6-17 on caller-visible DEVICE buffers (test hook; same kernels).  The streaming, index and
+ * filter tiers first build their own copy of the caller's tree rows inside the workspace (a hand-over pass before the
+ * kernel's clock starts).  PAKR_NN_FILTER assumes every row lies inside the state box on the weighted dims (rows the
+ * planner inserted always do): its rounding band is derived from the box. */
 typedef struct {
   uint64_t seed; uint32_t replan, iteration;
   int32_t B, K; int64_t tree_capacity;
