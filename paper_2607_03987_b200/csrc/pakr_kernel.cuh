@@ -272,12 +272,11 @@ __device__ __forceinline__ void scan_rows(const DevProblem& pb, const float4* __
 // (d2, index) ordering as the tiled tier, so both tiers return identical results.
 constexpr int kStreamB = 16;
 
-template <int DYN, bool UNIT_W>
+template <int DYN, bool UNIT_W, int QS>  // QS: query slots held in registers per pass over the rows
 __device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, uint32_t r, uint32_t it,
                                        unsigned long long* key, int vb, int vbcount, float* sm_q,
                                           float* sm_tile, uint64_t* sm_bar, uint32_t& par0, uint32_t& par1, uint32_t& parx) {
   constexpr int D = DynTraits<DYN>::D, DP = DynTraits<DYN>::DP;
-  constexpr int QS = (D <= 8) ? 8 : 4;  // queries held in registers per pass over the rows
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   __syncthreads();  // earlier readers of sm_q are done
   for (int t = threadIdx.x; t < P.B; t += kThreads) {
@@ -827,7 +826,10 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
   const int n = nend - nbeg;
   if (vb < 0 || n <= 0) return;
   if constexpr (STREAM) {  // few queries (B <= kStreamB, chosen by the host): HBM-bound streaming tier
-    nn_stream<DYN, UNIT_W>(P, nbeg, nend, r, it, key, vb, vbcount, sm_q, sm_tile, sm_bar, par0, par1, parx);
+    // 8 query slots when the rows are short (D <= 8) and there are more than 4 queries, else 4: with few queries the
+    // arithmetic per byte stays under the machine balance and the pass is HBM-bound
+    if (D <= 8 && P.B > 4) nn_stream<DYN, UNIT_W, 8>(P, nbeg, nend, r, it, key, vb, vbcount, sm_q, sm_tile, sm_bar, par0, par1, parx);
+    else nn_stream<DYN, UNIT_W, 4>(P, nbeg, nend, r, it, key, vb, vbcount, sm_q, sm_tile, sm_bar, par0, par1, parx);
     return;
   } else if constexpr (FILTER) {
    if (filter_live && n >= kFilterMinRows && (long long)P.B * n * D >= P.filter_min_work) {
