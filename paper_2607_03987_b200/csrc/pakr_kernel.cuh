@@ -688,7 +688,12 @@ __device__ __forceinline__ unsigned long long idx_search(const Params& P, const 
   unsigned long long best = kKeyNone;
   float ub = inf;
   int s_near = -1, t_near = -1;
-  if (G.n_super > 32) {
+  bool have_bound = false;
+  if (part > 0) {  // a later part: what the earlier parts of this query left in key[s] is a real row's distance already
+    const unsigned long long kv = __ldcg(shared_key);
+    if (kv != kKeyNone) { ub = __uint_as_float((unsigned)(kv >> 32)); have_bound = true; }
+  }
+  if (G.n_super > 32 && !have_bound) {
     // pass A (several groups of super-tiles): the globally nearest super-tile box, its nearest tile box, that
     // tile's rows -> the exact distance of a real row
     unsigned long long near = kKeyNone;
