@@ -236,6 +236,39 @@ typedef struct {
 pakr_status pakr_expand_step(pakr_planner* planner, const pakr_step_args* args, void* d_workspace,
                              size_t workspace_bytes, void* cuda_stream);
 
+/* pakr_expand_step for callers that have no device memory to hand over as a workspace and are not allowed to get any.
+ *
+ * Who that is: a planner embedded in a control loop usually reserves all its memory while the robot boots and is
+ * forbidden to allocate afterwards -- cudaMalloc / cudaFree may stall the whole device for an unbounded time, which a
+ * loop with a deadline cannot accept -- and a plug-in inside a host program whose own pool owns the device memory has
+ * nobody to ask for 2 MB more.  Such a caller already holds its tree buffers (inputs and outputs); what it lacks is
+ * the scratch one iteration of Alg. 1 l.6-17 needs on top of them: the NN keys of the B queries, the children
+ * between propagation and the ordered insert (Alg. 1 l.8-13), the control block and the path buffers.
+ *
+ * Here that scratch is a fixed array of PAKR_STATIC_SCRATCH_BYTES that is part of the library image itself (a
+ * file-scope __device__ array): every GPU that loads libpakr.so carries it from then until the process exits,
+ * whether or not this call is ever made.  The call itself performs no cudaMalloc, cudaMallocHost, cudaFree or any other
+ * allocating routine, on the first call or later; it enqueues three small memsets of its own scratch and one
+ * cooperative kernel launch on `cuda_stream` and returns without synchronising.  `planner` comes from pakr_create,
+ * which does allocate a few KB (obstacle tables, a pinned staging block) and therefore belongs to start-up.
+ *
+ * Same arguments, outputs and bit-for-bit results as pakr_expand_step with nn_mode = PAKR_NN_SCAN, except:
+ *   - limit: B * K <= PAKR_STATIC_MAX_CHILDREN.  More is PAKR_ERR_INVALID_ARG ("... exceeds the static scratch ...");
+ *     nothing is launched.  tree_capacity is not limited by the scratch (the tree is the caller's), only by 2^30.
+ *   - args->nn_mode must be PAKR_NN_AUTO or PAKR_NN_SCAN (else PAKR_ERR_UNSUPPORTED): the NN is always the tiled fp32
+ *     scan, also for B <= 16; the streaming, index and filter tiers keep per-node copies that do not fit a fixed array.
+ *   - pakr_read_stats has nothing to read afterwards (it looks inside a caller workspace).
+ * First call on each device: the library looks up that device's address of the array (cudaGetSymbolAddress, with the
+ * planner's device current) and remembers it.  Make one call per device during start-up, before any stream capture
+ * begins; later calls skip the look-up.
+ * Sharing: there is ONE array per device, used by every planner and every thread of the process.  Two calls whose
+ * kernels can run at the same time on one device (different streams, or different host threads) corrupt each other's
+ * results: issue them on one stream, or order them with events.  The array keeps whatever the previous call left;
+ * the words that must start from a known value (NN keys, control block) are reset on `cuda_stream` by each call. */
+#define PAKR_STATIC_MAX_CHILDREN 16384
+#define PAKR_STATIC_SCRATCH_BYTES (2304u * 1024u) /* 2.25 MiB per device */
+pakr_status pakr_expand_step_static(pakr_planner* planner, const pakr_step_args* args, void* cuda_stream);
+
 /* Statistics of the last pakr_plan / pakr_expand_step launch that used this workspace with the same
  * (B, K, tree_capacity): synchronises `cuda_stream`, then copies the device control block into *out (HOST).
  * After pakr_expand_step: iterations = 1, phase_ms[0] = the NN scan of the whole tree, [1] = propagate (+ insert

@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -768,5 +769,114 @@ extern "C" pakr_status pakr_read_stats(pakr_planner* pl, int32_t B, int32_t K, i
   CUDA_TRY(pl, cudaMemcpyAsync(hc, static_cast<char*>(d_ws) + L.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, stream));
   CUDA_TRY(pl, cudaStreamSynchronize(stream));
   fill_stats(hc, (int64_t)B * K, out);
+  return PAKR_OK;
+}
+
+// ---- pakr_expand_step_static: one iteration with the scratch inside the library image (include/pakr.h) ----------------
+//
+// For callers that may not allocate device memory once they are running (control loops with deadlines, plug-ins inside a
+// host whose pool owns the device).  The scratch below is part of libpakr.so's device image: the driver places one copy
+// on every GPU that loads the library and keeps it until the process exits.  Nothing here calls cudaMalloc / cudaFree.
+//
+// g_static_scratch, as host code sees it, is only a handle for the symbol -- NOT a device address.  Passing
+// `g_static_scratch` itself to a kernel would hand it a host pointer (a fault, or on machines where the GPU can reach
+// host memory, silent use of the wrong bytes).  The device address is asked for once per device with
+// cudaGetSymbolAddress while that device is current, and that is the pointer the kernel parameters are built from.
+static __device__ __align__(256) unsigned char g_static_scratch[PAKR_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+void* g_static_ptr[kStaticMaxDevices] = {nullptr};  // device address of g_static_scratch on device i, once known
+
+// Scratch of one tiled-scan iteration, packed from offset 0: what make_layout() reserves minus the tree (the caller's)
+// and minus the per-node copies of the streaming / index / filter tiers (never used here).
+Layout make_static_layout(const pakr_planner* pl, int64_t B, int64_t K) {
+  Layout L{};
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+  const size_t BK = (size_t)B * K, slots = BK + 32;
+  L.nn_key = take((size_t)B * 16);
+  L.unit_count = take(std::max<size_t>(BK, kFuseUnits + 8) * 4);
+  L.scr_state = take(slots * pl->DP * 4);
+  L.scr_ctrl = take(slots * 16);
+  L.scr_cost = take(slots * 4);
+  L.scr_parent = take(slots * 4);
+  L.scr_flags = take(slots * 4);
+  L.ctrl = take(sizeof(Ctrl));
+  L.path_rev = take((size_t)kPathMax * 4);
+  L.path_nodes = take((size_t)kPathMax * 4);
+  L.path_states = take((size_t)kPathMax * kMaxD * 4);
+  L.path_controls = take((size_t)kPathMax * kMaxM * 4);
+  L.total = o;
+  return L;
+}
+
+}  // namespace
+
+extern "C" pakr_status pakr_expand_step_static(pakr_planner* pl, const pakr_step_args* a, void* cuda_stream) {
+  if (!pl) return PAKR_ERR_INVALID_ARG;
+  if (!a) return fail(pl, PAKR_ERR_INVALID_ARG, "null args");
+  if (!sizes_ok(a->B, a->K, a->tree_capacity)) return fail(pl, PAKR_ERR_INVALID_ARG, "B, K or tree_capacity out of range");
+  if ((int64_t)a->B * a->K > PAKR_STATIC_MAX_CHILDREN)
+    return fail(pl, PAKR_ERR_INVALID_ARG,
+                "B*K = " + std::to_string((int64_t)a->B * a->K) + " exceeds the static scratch (PAKR_STATIC_MAX_CHILDREN = " +
+                    std::to_string(PAKR_STATIC_MAX_CHILDREN) + "); use pakr_expand_step with a workspace");
+  if (a->nn_mode != PAKR_NN_AUTO && a->nn_mode != PAKR_NN_SCAN)
+    return fail(pl, PAKR_ERR_UNSUPPORTED, "pakr_expand_step_static runs the tiled fp32 scan only (nn_mode AUTO or SCAN)");
+  if (!a->states || !a->actions || !a->parents || !a->costs || !a->n_nodes)
+    return fail(pl, PAKR_ERR_INVALID_ARG, "null tree pointer");
+  if (std::isnan(a->c_best)) return fail(pl, PAKR_ERR_INVALID_ARG, "c_best is NaN");
+  if (reinterpret_cast<uintptr_t>(a->states) % 16 || reinterpret_cast<uintptr_t>(a->actions) % 16)
+    return fail(pl, PAKR_ERR_INVALID_ARG, "states/actions must be 16-byte aligned");
+  const Layout L = make_static_layout(pl, a->B, a->K);
+  if (L.total > (size_t)PAKR_STATIC_SCRATCH_BYTES)  // cannot happen below PAKR_STATIC_MAX_CHILDREN; kept as the real guard
+    return fail(pl, PAKR_ERR_INVALID_ARG, "scratch for this (B, K) exceeds PAKR_STATIC_SCRATCH_BYTES");
+  if (pl->device < 0 || pl->device >= kStaticMaxDevices)
+    return fail(pl, PAKR_ERR_UNSUPPORTED, "static scratch is tracked for device ordinals 0..63 only");
+  DeviceGuard guard(pl->device);
+  CUDA_TRY(pl, guard.err);
+  char* ws = nullptr;
+  {
+    // set-up, once per device, with that device current: the symbol's address ON THIS DEVICE
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[pl->device]) {
+      void* ptr = nullptr;
+      CUDA_TRY(pl, cudaGetSymbolAddress(&ptr, g_static_scratch));
+      if (!ptr || reinterpret_cast<uintptr_t>(ptr) % kAlign) return fail(pl, PAKR_ERR_CUDA, "static scratch has no usable device address");
+      g_static_ptr[pl->device] = ptr;
+    }
+    ws = static_cast<char*>(g_static_ptr[pl->device]);
+  }
+  Params P;
+  fill_common(pl, P, L, ws, a->B, a->K, a->tree_capacity);
+  // tiers that keep per-node copies are off; their pointers must never be followed
+  P.prow = nullptr; P.frow = nullptr; P.chunkmin = nullptr;
+  P.idx_keys = nullptr; P.idx_ids = nullptr; P.idx_hist = nullptr; P.idx_ctasum = nullptr; P.idx_tile_ids = nullptr;
+  P.idx_rows = nullptr; P.idx_tlo = nullptr; P.idx_thi = nullptr; P.idx_slo = nullptr; P.idx_shi = nullptr;
+  P.nn_index = 0; P.nn_filter = 0;
+  P.filter_min_work = kFilterMinWork; P.filter_give_up = kFilterGiveUp;
+  P.idx_min_work = kIdxMinWork; P.idx_rebuild_work = kIdxRebuildWork;
+  P.states = a->states; P.actions = a->actions; P.parents = a->parents; P.costs = a->costs;
+  P.seed = a->seed;
+  P.n_replans = 1; P.max_iters = 1; P.budget_ns = 0;
+  P.r0 = (int)a->replan; P.it0 = (int)a->iteration;
+  P.c_best0 = a->c_best;
+  P.early_exit = 0;
+  P.n_nodes_io = a->n_nodes;
+  P.dbg_x_rand = a->x_rand; P.dbg_nn_idx = a->nn_idx; P.dbg_nn_d2 = a->nn_d2;
+  P.dbg_child_state = a->child_state; P.dbg_child_ctrl = a->child_ctrl; P.dbg_child_cost = a->child_cost;
+  P.dbg_child_flags = a->child_flags; P.dbg_n_inserted = a->n_inserted; P.dbg_goal_node = a->goal_node;
+  P.dbg_new_c_best = a->new_c_best;
+  // The array holds the previous call's bytes.  What the kernel expects to find reset: NN keys = "none" (all ones),
+  // control block = 0 with its goal keys = "none".  Everything else in the scratch is written before it is read.
+  cudaStream_t stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+  CUDA_TRY(pl, cudaMemsetAsync(P.nn_key, 0xFF, (size_t)P.B * 16, stream));
+  CUDA_TRY(pl, cudaMemsetAsync(P.ctrl, 0, sizeof(Ctrl), stream));
+  CUDA_TRY(pl, cudaMemsetAsync(P.ctrl, 0xFF, sizeof(unsigned long long) * kSlots, stream));
+  void* args[] = {&P};
+  const dim3 grid(pl->num_sms * std::min(pl->blocks_per_sm, kCtasPerSm)), block(kThreads);
+  CUDA_TRY(pl, cudaLaunchCooperativeKernel(pl->kernel, grid, block, args, pl->smem_bytes, stream));  // tiled tier, any B
   return PAKR_OK;
 }

@@ -23,6 +23,8 @@ F_VALID, F_INBOUNDS, F_COLLFREE, F_NOTPRUNED, F_GOAL, F_INSERTED = 1, 2, 4, 8, 1
 NN_AUTO, NN_SCAN, NN_INDEX, NN_FILTER = 0, 1, 2, 3
 MAX_REPLAN_STATS = 64
 MAX_PATH_NODES = 8192
+STATIC_MAX_CHILDREN = 16384          # PAKR_STATIC_MAX_CHILDREN: B*K limit of pakr_expand_step_static
+STATIC_SCRATCH_BYTES = 2304 * 1024   # PAKR_STATIC_SCRATCH_BYTES
 _STATUS = {0: "PAKR_OK", 1: "PAKR_ERR_INVALID_ARG", 2: "PAKR_ERR_UNSUPPORTED", 3: "PAKR_ERR_WORKSPACE_TOO_SMALL",
            4: "PAKR_ERR_BUFFER_TOO_SMALL", 5: "PAKR_ERR_CUDA"}
 
@@ -144,7 +146,7 @@ class _Fp32Peak(C.Structure):
 
 
 EXPORTS = ["pakr_create", "pakr_destroy", "pakr_last_error", "pakr_workspace_bytes", "pakr_get_tree_layout",
-           "pakr_plan", "pakr_expand_step", "pakr_read_stats", "pakr_measure_fp32_peak"]
+           "pakr_plan", "pakr_expand_step", "pakr_expand_step_static", "pakr_read_stats", "pakr_measure_fp32_peak"]
 
 _lib = None
 
@@ -169,6 +171,8 @@ def lib():
                                 C.POINTER(_Result)]
         L.pakr_expand_step.restype = C.c_int
         L.pakr_expand_step.argtypes = [C.c_void_p, C.POINTER(_StepArgs), C.c_void_p, C.c_size_t, C.c_void_p]
+        L.pakr_expand_step_static.restype = C.c_int
+        L.pakr_expand_step_static.argtypes = [C.c_void_p, C.POINTER(_StepArgs), C.c_void_p]
         L.pakr_read_stats.restype = C.c_int
         L.pakr_read_stats.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.c_size_t, C.c_void_p,
                                       C.POINTER(_Stats)]
@@ -373,6 +377,43 @@ class Planner:
         self._check(st)
         if not debug:
             return None
+        torch.cuda.synchronize(self.device)
+        out = {k: v.cpu().numpy() for k, v in dbg.items()}
+        out["x_rand"] = out["x_rand"][:, :self.D]
+        out["child_state"] = out["child_state"][:, :self.D]
+        out["child_ctrl"] = out["child_ctrl"][:, :self.m]
+        for k in ("n_inserted", "goal_node", "new_c_best"):
+            out[k] = out[k][0].item()
+        return out
+
+    # ---- pakr_expand_step_static ----
+    def expand_step_static(self, tree: dict, seed: int, replan: int, iteration: int, B: int, K: int,
+                           c_best: float = float("inf"), nn_mode: int = NN_AUTO) -> dict:
+        """pakr_expand_step_static: one iteration without a workspace, for callers that may not allocate device
+        memory while they run (a deadline-bound control loop, a plug-in whose host owns the pool).  The library's
+        scratch is a fixed 2.25 MiB array inside libpakr.so on each GPU; B*K <= STATIC_MAX_CHILDREN, NN = tiled scan.
+        The C call allocates nothing.  The tree (in/out) and the per-child output tensors are the caller's: this
+        convenience wrapper makes the outputs with torch, exactly as expand_step(debug=True) does, and returns them as
+        numpy.  One array per device is shared by all planners: calls on different streams must not overlap."""
+        torch = self._torch
+        dev = f"cuda:{self.device}"
+        BK = B * K
+        ptr = lambda t: C.c_void_p(t.data_ptr())
+        dbg = dict(x_rand=torch.zeros((B, self.Dp), dtype=torch.float32, device=dev),
+                   nn_idx=torch.zeros(B, dtype=torch.int32, device=dev),
+                   nn_d2=torch.zeros(B, dtype=torch.float32, device=dev),
+                   child_state=torch.zeros((BK, self.Dp), dtype=torch.float32, device=dev),
+                   child_ctrl=torch.zeros((BK, 4), dtype=torch.float32, device=dev),
+                   child_cost=torch.zeros(BK, dtype=torch.float32, device=dev),
+                   child_flags=torch.zeros(BK, dtype=torch.int32, device=dev),
+                   n_inserted=torch.zeros(1, dtype=torch.int32, device=dev),
+                   goal_node=torch.zeros(1, dtype=torch.int32, device=dev),
+                   new_c_best=torch.zeros(1, dtype=torch.float32, device=dev))
+        a = _StepArgs(seed, replan, iteration, B, K, tree["capacity"], c_best, nn_mode, ptr(tree["states"]),
+                      ptr(tree["actions"]), ptr(tree["parents"]), ptr(tree["costs"]), ptr(tree["n_nodes"]),
+                      *[ptr(dbg[k]) for k in ("x_rand", "nn_idx", "nn_d2", "child_state", "child_ctrl", "child_cost",
+                                              "child_flags", "n_inserted", "goal_node", "new_c_best")])
+        self._check(lib().pakr_expand_step_static(self._h, C.byref(a), C.c_void_p(self._stream())))
         torch.cuda.synchronize(self.device)
         out = {k: v.cpu().numpy() for k, v in dbg.items()}
         out["x_rand"] = out["x_rand"][:, :self.D]
