@@ -21,7 +21,8 @@
 // scan tiers (ties included).  band = 2^-17 * S with S >= sum |c_i u_i| of the pair, bounded per query by
 // 3 V^2 + 4 V sqrt(UB) + UB (V = |v|; rows that matter have |u| <= V + sqrt(UB)); 2^-17 covers the fp16 hi/lo
 // truncation (3 * 2^-22 S), the tensor core's fp32 accumulation (K * 2^-24 S) and the fp32 feature arithmetic with a
-// margin of ~5.
+// margin of ~5, plus an absolute floor of 2^-24 (2 + 8 V + 4 R + R^2), R = V + sqrt(UB), for the fp16 subnormal range
+// (see nn_filter_refine).
 //
 // Why mma.sync and not tcgen05 here: the epilogue must look at EVERY accumulator (a min over the row axis), and K is
 // only 32..48.  tcgen05.mma would finish a 128 x 256 x 32 tile in ~256 cycles but draining its 128 KB of accumulators
@@ -373,9 +374,18 @@ __device__ __noinline__ void nn_filter_refine(const Params& P, int nbeg, int nen
     // Rounding band of THIS query: |approximate - true key| <= eps * sum_i |c_i u_i| <= eps (|u|^2 + 2 |v| |u|) with
     // |u| <= |v| + sqrt(d2) for the rows that matter (d2 <= UB): eps (3 V^2 + 4 V sqrt(UB) + UB), V^2 = qn / ... >= |v|^2.
     // f_eps = 2^-17 carries the same margin over the nominal 2^-19.5 as the box-wide band did.
+    // Absolute floor on top of the relative band: a feature or coefficient below 2^-3 has an fp16-SUBNORMAL lo half
+    // (and below 2^-14 a subnormal hi half), whose rounding error is an absolute 2^-25 whatever the value.  That adds at
+    // most 2^-25 (sum_i |c_i| + sum_i |u_i|) to |approximate - true key|, with sum |c_i| <= 1 + 2 sqrt(NF) V and, for the
+    // rows that matter, sum |u_i| <= R^2 + sqrt(NF) R, R = V + sqrt(UB); sqrt(NF) < 4.  Taken with 2^-24.  It matters
+    // for queries near the centre of the box and for state boxes much narrower than 1 in weighted units, where the
+    // relative band alone shrinks below the subnormal spacing.
     const float v2 = f[C::NF - 1] + 0.5f * P.pb.f_qn_ang, vn = sqrtf(v2);
     auto threshold = [&](float ub) {
-      return ub < inf ? ub - qn + P.pb.f_eps * (3.0f * v2 + 4.0f * vn * sqrtf(ub) + ub) : inf;
+      const float su = sqrtf(ub), rr = vn + su;
+      return ub < inf ? ub - qn + P.pb.f_eps * (3.0f * v2 + 4.0f * vn * su + ub) +
+                            5.9604645e-8f * (2.0f + 8.0f * vn + 4.0f * rr + rr * rr)
+                      : inf;
     };
     const float* cm = P.chunkmin + (size_t)s * kFilterMaxChunks;
     // the chunk with the smallest approximate key first: its exact minimum is a real upper bound

@@ -393,3 +393,31 @@ def test_nn_filter_tier_equals_scan_tier(pakr, orc, name, n0, B, K, clustered):
         i, d2 = op.nearest(tree64, q)
         j = int(outs[pakr.NN_FILTER]["nn_idx"][s_])
         assert j == i or op.dist2(q, tree64[j]) <= (1 + 1e-6) * d2
+
+
+@pytest.mark.parametrize("half_width", [0.02, 0.005])
+def test_nn_filter_tier_equals_scan_tier_on_a_tiny_state_box(pakr, half_width):
+    """A state box much narrower than 1 in weighted units puts every filter feature in the fp16 subnormal range of its
+    lo half, where the hi/lo split is only good to an absolute 2^-25: the relative rounding band alone would then drop
+    the chunk of the true nearest row.  With the absolute floor in the band the filter tier must still equal the scan
+    bit for bit (and must really have run)."""
+    p, _ = wl.config2()
+    D = p.state_dim
+    centre = np.full(D, 0.3, np.float32)
+    lo, hi = centre - np.float32(half_width), centre + np.float32(half_width)
+    p = dataclasses.replace(p, state_lo=lo, state_hi=hi, start=centre.copy(), obstacles=p.obstacles[:0],
+                            goal_center=centre[:p.pos_dim] + np.float32(0.5 * half_width),
+                            goal_radius=float(0.1 * half_width), nn_weight=np.ones(D, np.float32))
+    n0, B, K = 200000, 1024, 1
+    host = wl.random_tree(p, n0, seed=17, flat=True)
+    host["states"][n0 - 2000:] = host["states"][100:2100]   # exact duplicates: lowest index must win
+    outs = {}
+    pl = pakr.Planner(p)
+    for mode in (pakr.NN_SCAN, pakr.NN_FILTER):
+        tree = pl.new_tree(n0 + B * K, host)
+        outs[mode] = pl.expand_step(tree, 5, 1, 4, B, K, nn_mode=mode)
+        if mode == pakr.NN_FILTER:
+            assert pl.read_stats(B, K, n0 + B * K)["nn_pairs_filtered"] == B * n0, "the filter did not run"
+    pl.close()
+    for k in ("x_rand", "nn_idx", "nn_d2"):
+        np.testing.assert_array_equal(outs[pakr.NN_SCAN][k], outs[pakr.NN_FILTER][k])
