@@ -56,10 +56,14 @@ enum { PAKR_NO_SOLUTION = 0, PAKR_SOLVED = 1 }; /* "no solution" is not an error
 enum { PAKR_NN_AUTO = 0,  /* the library picks: the brute-force fp32 scan below B = 4096 queries, the spatial index (once
                              the tree is large enough to pay for building it) from there up */
        PAKR_NN_SCAN = 1,  /* brute-force fp32 scan tiers only (tiled; streaming when B <= 16) */
-       PAKR_NN_INDEX = 2, /* spatial index on every tree of >= 256 nodes (tests) */
+       PAKR_NN_INDEX = 2, /* spatial index on every tree of >= 256 nodes (tests).  Not with B <= 16 (see below), not for
+                             problems without a finite, positively weighted real dim, and not for capacities whose
+                             index rows would pass 2^32 floats (~358 M nodes at state_dim 12): those keep the scan */
        PAKR_NN_FILTER = 3 /* tensor-core coarse filter (fp16 hi/lo mma.sync, fp32 accumulate) on every scan of >= 4096
                              rows that is long enough to pay, exact fp32 rescoring of its candidates; problems whose
                              angle dims weigh more than 0.1 in total keep the fp32 scan */ };
+/* B <= 16 queries always run the streaming scan tier, whatever nn_mode says: with so few queries the scan is bound by
+ * reading the tree once, which neither the index nor the filter can beat. */
 
 /* child flag bits written by pakr_expand_step (Alg. 1 l.10-14) */
 enum {

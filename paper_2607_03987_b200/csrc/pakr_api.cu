@@ -616,6 +616,9 @@ bool set_nn_mode(pakr_planner* pl, Params& P, int nn_mode) {
   constexpr int kAutoMinB = 4096;
   P.nn_filter = pl->filter_ok && nn_mode == PAKR_NN_FILTER ? 1 : 0;
   P.nn_index = !pl->index_ok ? 0 : nn_mode == PAKR_NN_INDEX ? 2 : (nn_mode == PAKR_NN_AUTO && P.B >= kAutoMinB) ? 1 : 0;
+  // The index search addresses its tile rows with 32-bit element offsets (tiles x D x 32 floats).  A capacity whose
+  // index would not fit them (~358 M rows at D = 12) keeps the scan tiers: same results, every tier is bit-identical.
+  if ((unsigned long long)idx_dims(P.cap).n_super * 1024ull * (unsigned long long)pl->D >= (1ull << 32)) P.nn_index = 0;
   P.filter_min_work = kFilterMinWork;
   P.filter_give_up = kFilterGiveUp;
   P.idx_min_work = kIdxMinWork;

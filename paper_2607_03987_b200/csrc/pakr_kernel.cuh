@@ -380,7 +380,8 @@ __device__ __forceinline__ void nn_stream(const Params& P, int nbeg, int nend, u
 // Dense regions get many small boxes, empty space gets none.
 //   rebuild  keys -> LSD radix sort (3 passes of 10 bits: per-warp histograms, grid-wide exclusive scan, stable
 //            per-warp scatter) -> tiles: rows copied as [tile][dim][32] so that a lane reads its row with
-//            coalesced loads -> tile boxes -> super-tile boxes.  Runs when the tree has grown by a sixteenth.
+//            coalesced loads -> tile boxes -> super-tile boxes.  Runs when scanning the rows added since the
+//            last rebuild would cost about as much as rebuilding (kIdxRebuildWork).
 //   search   one warp per query.  A lower bound of the weighted squared distance from the query to a box is
 //            sum_d w_d max(0, lo_d - q_d, q_d - hi_d)^2.  Pass A walks the super-tile boxes (one per lane), descends
 //            into the nearest one and scores its nearest tile: the exact distance of a real row, an upper bound ub.
@@ -634,7 +635,7 @@ __device__ __forceinline__ float idx_score_tiles(const Params& P, const int (&t)
   for (int a = 0; a < NT; ++a) {
     const int ta = a < cnt ? t[a] : t[0];
     id[a] = __ldcg(&P.idx_tile_ids[(size_t)ta * 32 + lane]);
-    off[a] = (unsigned)ta * (D * 32) + lane;
+    off[a] = (unsigned)ta * (D * 32) + lane;  // < 2^32: the host keeps larger trees off the index (set_nn_mode)
     acc[a] = 0.0f;
   }
 #pragma unroll
@@ -852,6 +853,8 @@ __device__ __forceinline__ void nn_phase(const Params& P, int nbeg, int nend, ui
     const bool timer = blockIdx.x == (unsigned)(gridDim.x - vbcount) && threadIdx.x == 0;  // first participating CTA
     if (timer && blockIdx.x == 0) { const unsigned long long t = globaltimer_ns(); ph_outer += t - tp; tp = t; }
     nn_filter_refine<DYN, UNIT_W>(P, nbeg, nend, r, it, key, vb, vbcount, fp, f_slot, reinterpret_cast<int*>(sm_tile - (threadIdx.x >> 5) * 2 * kTileBufFloats));
+    fence_proxy_async();  // the candidate lists were written into the TMA tile buffers with ordinary stores; the next
+                          // bulk copy into them belongs to the async proxy (same reuse as after idx_rebuild)
     if (timer && blockIdx.x == 0) { const unsigned long long t = globaltimer_ns(); ph_refine += t - tp; tp = t; }
     filtered += (long long)P.B * n;
     return;
