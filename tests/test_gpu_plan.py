@@ -276,6 +276,53 @@ def test_plan_loop_with_nn_index_equals_scan(pakr, name, iters):
         np.testing.assert_array_equal(trees[pakr.NN_SCAN][1][k], trees[pakr.NN_INDEX][1][k])
 
 
+@pytest.mark.parametrize("name,iters", [("C4", 8), ("C5", 5)])
+def test_plan_loop_auto_policy_equals_scan(pakr, name, iters):
+    """PAKR_NN_AUTO is what bench.py times.  At B = 4096 it searches the index over the rows sorted at the last rebuild
+    and scans the rows added since with the tiled tier, rebuilding only when that remainder has grown enough.  On C4
+    (B = 4096, K = 16) the first batch takes the tree past the engagement size (48.8 k rows), and iterations 3-5 add
+    only 0.5-3 k rows each: they run index + remainder without a rebuild.  C5 (4096, 64) rebuilds every iteration.
+    A wrong (non-nearest) parent would still give a valid plan, so the whole tree must equal the scan's bit for bit --
+    and the index must really have answered (fewer distance evaluations than pairs)."""
+    p, cfg = wl.config5(B=4096, K=64) if name == "C5" else wl.CONFIGS[name]()
+    cap = 1 + iters * cfg.B * cfg.K
+    got = {}
+    pl = pakr.Planner(p)
+    for mode in (pakr.NN_SCAN, pakr.NN_AUTO):
+        res = pl.plan(7, cfg.B, cfg.K, cap, 1, max_iters_per_replan=iters, nn_mode=mode)
+        got[mode] = (res, pl.read_tree(cfg.B, cfg.K, cap, res["final_tree_nodes"]))
+    pl.close()
+    scan, auto = got[pakr.NN_SCAN][0], got[pakr.NN_AUTO][0]
+    assert scan["final_tree_nodes"] == auto["final_tree_nodes"] > 60000
+    assert scan["iterations"] == auto["iterations"] == iters
+    for k in ("states", "actions", "parents", "costs"):
+        np.testing.assert_array_equal(got[pakr.NN_SCAN][1][k], got[pakr.NN_AUTO][1][k])
+    assert scan["nn_pairs"] == auto["nn_pairs"] == scan["nn_pairs_evaluated"]
+    assert auto["nn_pairs_evaluated"] < 0.5 * auto["nn_pairs"], "the index did not engage"
+    assert auto["phase_ms"][3] > 0.0   # at least one rebuild ran inside the loop
+
+
+@pytest.mark.parametrize("seed", [0, 1])
+def test_plan_c1_lockstep_with_oracle_over_all_replans(pakr, orc, seed):
+    """Alg. 1 l.1-4 at the loop level: all 10 replans of BASELINE config 1 against orc.plan --
+    fresh tree and re-keyed draws per replan, c_best carried over.  fp32 vs fp64 may flip a near-tie, so node counts get
+    2 % and iteration counts +-2; costs are multiples of the edge duration and must be equal."""
+    p, cfg = wl.config1()
+    pl = pakr.Planner(p)
+    res = pl.plan(seed, cfg.B, cfg.K, cfg.tree_capacity, cfg.n_replans)
+    op = orc.OracleProblem(p)
+    ref = orc.plan(op, seed, cfg.B, cfg.K, cfg.tree_capacity, cfg.n_replans)
+    pl.close()
+    assert res["replans_run"] == ref["replans_run"] == 10
+    assert res["replans_solved"] == ref["replans_solved"] >= 2
+    for r in range(10):
+        assert abs(int(res["replan_iters"][r]) - int(ref["replan_iters"][r])) <= 2, r
+        assert abs(int(res["replan_nodes"][r]) - int(ref["replan_nodes"][r])) <= 0.02 * ref["replan_nodes"][r], r
+        assert res["replan_cost"][r] == pytest.approx(ref["replan_cost"][r], rel=1e-6), r
+        assert res["replan_nodes"][r] <= 1 + int(res["replan_iters"][r]) * cfg.B * cfg.K, r   # grown from the root alone
+    assert res["cost"] == pytest.approx(ref["cost"], rel=1e-6)
+
+
 def test_plan_small_b_stream_tier_and_no_obstacles(pakr, orc):
     """B <= 16 runs the streaming-tier kernel through the whole device loop (look-ahead, in-phase insert, tail
     rounds): same tree as the chain of single steps; and a problem without obstacles plans fine."""

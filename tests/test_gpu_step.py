@@ -67,7 +67,23 @@ def test_step_matches_oracle(pakr, orc, name, n0, B, K):
     out, after, ref, _ = run_both(pl, orc, op, p, host, seed=11, r=2, it=5, B=B, K=K, cap=cap)
     st = check_iteration(orc, op, p, host, out, after, ref, B, K, cap)
     assert st["nn_equal"] > 0.99
+    _STRICT[(name, n0, B, K)] = st["strict"]
     pl.close()
+
+
+_STRICT = {}
+
+
+def test_step_matches_oracle_compared_the_insert_counts():
+    """check_iteration compares the oracle's insert count and goal node only when every NN index and deciding flag
+    agreed.  That must have been the case on most of the cases above, the smallest ones included: otherwise the
+    oracle's own insert is never looked at."""
+    if not _STRICT:
+        pytest.skip("test_step_matches_oracle did not run in this session")
+    ran = [k for k, v in _STRICT.items() if v]
+    assert len(ran) >= len(_STRICT) // 2, (len(ran), len(_STRICT))
+    small = [k for k in _STRICT if k[2] * k[3] <= 2048]
+    assert small and all(_STRICT[k] for k in small), {k: _STRICT[k] for k in small}
 
 
 def test_step_duplicates_and_ties(pakr, orc):
@@ -421,3 +437,40 @@ def test_nn_filter_tier_equals_scan_tier_on_a_tiny_state_box(pakr, half_width):
     pl.close()
     for k in ("x_rand", "nn_idx", "nn_d2"):
         np.testing.assert_array_equal(outs[pakr.NN_SCAN][k], outs[pakr.NN_FILTER][k])
+
+
+@pytest.mark.parametrize("name", ["C3", "C4"])
+def test_step_on_planner_grown_trees(pakr, orc, name):
+    """SURVEY.md 8(c) "T" on the trees the planner itself grows (every batch sees the frozen snapshot the
+    previous batches left), at BASELINE's B and K: (a) replan 0 cut after 6 iterations, no bound yet; (b) the tree of a
+    late replan (r = 2) grown under a finite c_best -- nodes hugging the corridor the bound leaves open.  The tree is
+    read back, handed to one pakr_expand_step (the library picks the NN tier as it does in the loop) and to the oracle,
+    which checks sampled queries exactly: draw, nearest node, the K children re-propagated from the chosen parent."""
+    from parity_util import check_sampled
+    p, cfg = wl.CONFIGS[name]()
+    B, K, cap = cfg.B, cfg.K, cfg.tree_capacity
+    pl = pakr.Planner(p)
+    op = orc.OracleProblem(p)
+    c0 = pl.plan(3, B, K, cap, 1)["cost"]
+    assert np.isfinite(c0)
+    grown = []
+    res = pl.plan(3, B, K, cap, 1, max_iters_per_replan=6)
+    grown.append((res, 0, int(res["replan_iters"][0]), float("inf")))
+    res = pl.plan(3, B, K, cap, 3, max_iters_per_replan=10, initial_cost_bound=c0)
+    grown.append((res, 2, int(res["replan_iters"][2]), float(min(c0, res["replan_cost"][2]))))
+    rng = np.random.default_rng(11)
+    for res, r, it, c_best in grown:
+        n = res["final_tree_nodes"]
+        assert n > 20000
+        host = pl.read_tree(B, K, cap, n)
+        step_cap = n + B * K
+        tree = pl.new_tree(step_cap, host)
+        out = pl.expand_step(tree, 3, r, it, B, K, c_best=c_best)
+        share = check_sampled(op, p, host, out, 3, r, it, K, c_best, rng.choice(B, 64, replace=False))
+        assert share > 0.95
+        # the insert is the stable compaction of the GPU's own keep flags
+        keep = np.nonzero(((out["child_flags"] & 1) != 0) & ((out["child_flags"] & 8) != 0))[0]
+        assert out["n_inserted"] == len(keep) == int(tree["n_nodes"][0].item()) - n
+        np.testing.assert_array_equal(tree["parents"][n:n + len(keep)].cpu().numpy(), out["nn_idx"][keep // K])
+        np.testing.assert_array_equal(tree["states"][n:n + len(keep), :p.state_dim].cpu().numpy(), out["child_state"][keep])
+    pl.close()
