@@ -128,11 +128,17 @@ void pakr_destroy(pakr_planner* planner);
  * pakr_last_error(NULL) returns the text of the last failed pakr_create in this thread. */
 const char* pakr_last_error(const pakr_planner* planner);
 
-/* Bytes of DEVICE workspace pakr_plan / pakr_expand_step need for (B, K, tree_capacity), whichever nn_mode is used later
- * (tree 4*(Dp+6) bytes per node + the tiers' copies: packed rows when B <= 16, index arrays ~(4 D + 20) and filter rows 96
- * bytes per node where the problem admits them, B * 16 KB of chunk minima for the filter);
- * 0 if an argument is invalid (B < 1, K < 1, K > 4096, B*K > 2^24, capacity < 2 or > 2^30). */
+/* Bytes of DEVICE workspace pakr_plan / pakr_expand_step need for (B, K, tree_capacity), whichever nn_mode is used later:
+ * tree 4*(Dp+6) bytes per node, ~(Dp+7)*4 bytes per child, the control block and path buffers (0.6 MB), plus the buffers
+ * of EVERY tier the problem admits: packed rows when B <= 16; else index arrays ~(4 D + 20) bytes per node, filter rows
+ * 96 bytes per node and B * 16 KB of chunk minima.  0 if an argument is invalid (B < 1, K < 1, K > 4096, B*K > 2^24,
+ * capacity < 2 or > 2^30). */
 size_t pakr_workspace_bytes(const pakr_planner* planner, int32_t B, int32_t K, int64_t tree_capacity);
+/* The same for a caller that knows the nn_mode it will pass: only that mode's tier buffers are counted (AUTO: the index
+ * arrays from B = 4096 up, never the filter's; SCAN: none).  A workspace of this size is accepted by pakr_plan /
+ * pakr_expand_step calls with this nn_mode (and by pakr_read_stats, pakr_get_tree_layout: the tree, the control block and
+ * the path buffers have the same offsets in every mode).  Always <= pakr_workspace_bytes().  0 on invalid arguments. */
+size_t pakr_workspace_bytes_for(const pakr_planner* planner, int32_t B, int32_t K, int64_t tree_capacity, int32_t nn_mode);
 
 /* Where pakr_plan keeps its tree inside the workspace (byte offsets), so a caller can read the
  * tree of the last replan after pakr_plan returns (tests check the tree invariants on it). */

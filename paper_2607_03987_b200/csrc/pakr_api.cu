@@ -77,7 +77,14 @@ struct Layout {
       ctrl, path_rev, path_nodes, path_states, path_controls, total;
 };
 
-Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap) {
+// nn_mode = kLayoutAllTiers reserves the buffers of every tier the problem admits (pakr_workspace_bytes); a PAKR_NN_*
+// value reserves only what that mode can launch (pakr_workspace_bytes_for).  The tree comes first and everything up to
+// the path buffers has the same offset whatever the mode, so pakr_get_tree_layout and pakr_read_stats need not know it;
+// the tiers' own buffers (all rebuilt inside every launch) follow.
+constexpr int kLayoutAllTiers = -1;
+constexpr int kAutoMinB = 4096;  // PAKR_NN_AUTO: the spatial index from this many queries up (set_nn_mode)
+
+Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap, int nn_mode = kLayoutAllTiers) {
   Layout L{};
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
@@ -87,12 +94,27 @@ Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap) {
   L.parents = take((size_t)cap * 4);
   L.costs = take((size_t)cap * 4);
   L.nn_key = take((size_t)B * 16);  // two iterations in flight
-  L.prow = take(B <= kStreamB ? ((size_t)cap + 4) * pl->D * 4 : 0); // streaming tier: packed rows
-  L.frow = take(((size_t)cap + 8) * 96);                            // filter rows: K <= 48 halves
-  L.chunkmin = take((size_t)B * kFilterMaxChunks * 4);
   L.unit_count = take(std::max<size_t>(U, kFuseUnits + 8) * 4);
+  L.scr_state = take(slots * pl->DP * 4);
+  L.scr_ctrl = take(slots * 16);
+  L.scr_cost = take(slots * 4);
+  L.scr_parent = take(slots * 4);
+  L.scr_flags = take(slots * 4);
+  L.ctrl = take(sizeof(Ctrl));
+  L.path_rev = take((size_t)kPathMax * 4);
+  L.path_nodes = take((size_t)kPathMax * 4);
+  L.path_states = take((size_t)kPathMax * kMaxD * 4);
+  L.path_controls = take((size_t)kPathMax * kMaxM * 4);
+  // per-tier buffers; B <= kStreamB always launches the streaming kernel, which uses neither index nor filter
+  const bool stream = B <= kStreamB;
+  const bool all = nn_mode == kLayoutAllTiers;
+  const size_t want_filter = (!stream && pl->filter_ok && (all || nn_mode == PAKR_NN_FILTER)) ? 1 : 0;
+  const size_t want_index = (!stream && pl->index_ok && (all || nn_mode == PAKR_NN_INDEX || (nn_mode == PAKR_NN_AUTO && B >= kAutoMinB))) ? 1 : 0;
+  L.prow = take(stream ? ((size_t)cap + 4) * pl->D * 4 : 0);        // streaming tier: packed rows
+  L.frow = take(want_filter * ((size_t)cap + 8) * 96);              // filter rows: K <= 48 halves
+  L.chunkmin = take(want_filter * (size_t)B * kFilterMaxChunks * 4);
   {  // NN index; nothing when the problem cannot be indexed
-    const size_t on = pl->index_ok ? 1 : 0;
+    const size_t on = want_index;
     const IdxDims G = idx_dims((int)cap);
     const size_t grid_warps = (size_t)pl->num_sms * kCtasPerSm * kWarps;
     const size_t sort_warps = std::min<size_t>(grid_warps, (size_t)cap / kIdxChunkMin + 1);
@@ -107,18 +129,12 @@ Layout make_layout(const pakr_planner* pl, int64_t B, int64_t K, int64_t cap) {
     L.idx_slo = take(on * (size_t)G.n_groups * pl->D * 32 * 4);
     L.idx_shi = take(on * (size_t)G.n_groups * pl->D * 32 * 4);
   }
-  L.scr_state = take(slots * pl->DP * 4);
-  L.scr_ctrl = take(slots * 16);
-  L.scr_cost = take(slots * 4);
-  L.scr_parent = take(slots * 4);
-  L.scr_flags = take(slots * 4);
-  L.ctrl = take(sizeof(Ctrl));
-  L.path_rev = take((size_t)kPathMax * 4);
-  L.path_nodes = take((size_t)kPathMax * 4);
-  L.path_states = take((size_t)kPathMax * kMaxD * 4);
-  L.path_controls = take((size_t)kPathMax * kMaxM * 4);
   L.total = o;
   return L;
+}
+
+bool nn_mode_ok(int nn_mode) {
+  return nn_mode == PAKR_NN_AUTO || nn_mode == PAKR_NN_SCAN || nn_mode == PAKR_NN_INDEX || nn_mode == PAKR_NN_FILTER;
 }
 
 bool sizes_ok(int64_t B, int64_t K, int64_t cap) {
@@ -537,6 +553,11 @@ extern "C" size_t pakr_workspace_bytes(const pakr_planner* pl, int32_t B, int32_
   return make_layout(pl, B, K, cap).total;
 }
 
+extern "C" size_t pakr_workspace_bytes_for(const pakr_planner* pl, int32_t B, int32_t K, int64_t cap, int32_t nn_mode) {
+  if (!pl || !sizes_ok(B, K, cap) || !nn_mode_ok(nn_mode)) return 0;
+  return make_layout(pl, B, K, cap, nn_mode).total;
+}
+
 extern "C" pakr_status pakr_get_tree_layout(const pakr_planner* pl, int32_t B, int32_t K, int64_t cap,
                                             pakr_tree_layout* out) {
   if (!pl || !out || !sizes_ok(B, K, cap)) return PAKR_ERR_INVALID_ARG;
@@ -607,13 +628,12 @@ void fill_stats(const Ctrl* hc, int64_t BK, pakr_stats* out) {
 // memset of the control words + one cooperative launch; everything on `stream`
 // nn_mode (PAKR_NN_*) -> Params::nn_index
 bool set_nn_mode(pakr_planner* pl, Params& P, int nn_mode) {
-  if (nn_mode != PAKR_NN_AUTO && nn_mode != PAKR_NN_SCAN && nn_mode != PAKR_NN_INDEX && nn_mode != PAKR_NN_FILTER) return false;
+  if (!nn_mode_ok(nn_mode)) return false;
   // PAKR_NN_AUTO (measured on the config 5 sweep and C1-C4): below B = 4096 queries the plain scan
   // kernel -- the trees those batches grow are too small for either accelerator to repay its fixed costs, and both
   // accelerated kernels carry more live state through the 128 registers, so their own scan loop is slower.  From
   // B = 4096 up the spatial index.  The tensor-core filter beats the plain scan from ~10^5 rows up but not the index on
   // the planner's own trees, so it is chosen only explicitly (PAKR_NN_FILTER).
-  constexpr int kAutoMinB = 4096;
   P.nn_filter = pl->filter_ok && nn_mode == PAKR_NN_FILTER ? 1 : 0;
   P.nn_index = !pl->index_ok ? 0 : nn_mode == PAKR_NN_INDEX ? 2 : (nn_mode == PAKR_NN_AUTO && P.B >= kAutoMinB) ? 1 : 0;
   // The index search addresses its tile rows with 32-bit element offsets (tiles x D x 32 floats).  A capacity whose
@@ -649,8 +669,9 @@ extern "C" pakr_status pakr_plan(pakr_planner* pl, const pakr_plan_opts* o, void
       std::isnan(o->initial_cost_bound))
     return fail(pl, PAKR_ERR_INVALID_ARG, "B, K, tree_capacity, n_replans or max_iters out of range");
   if (reinterpret_cast<uintptr_t>(d_ws) % kAlign) return fail(pl, PAKR_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
-  const Layout L = make_layout(pl, o->B, o->K, o->tree_capacity);
-  if (ws_bytes < L.total) return fail(pl, PAKR_ERR_WORKSPACE_TOO_SMALL, "workspace smaller than pakr_workspace_bytes()");
+  if (!nn_mode_ok(o->nn_mode)) return fail(pl, PAKR_ERR_INVALID_ARG, "nn_mode must be a PAKR_NN_* value");
+  const Layout L = make_layout(pl, o->B, o->K, o->tree_capacity, o->nn_mode);
+  if (ws_bytes < L.total) return fail(pl, PAKR_ERR_WORKSPACE_TOO_SMALL, "workspace smaller than pakr_workspace_bytes_for() of this nn_mode");
   cudaStream_t stream = reinterpret_cast<cudaStream_t>(cuda_stream);
   char* ws = static_cast<char*>(d_ws);
   Params P;
@@ -738,8 +759,9 @@ extern "C" pakr_status pakr_expand_step(pakr_planner* pl, const pakr_step_args* 
   if (reinterpret_cast<uintptr_t>(d_ws) % kAlign || reinterpret_cast<uintptr_t>(a->states) % 16 ||
       reinterpret_cast<uintptr_t>(a->actions) % 16)
     return fail(pl, PAKR_ERR_INVALID_ARG, "workspace must be 256-byte, states/actions 16-byte aligned");
-  const Layout L = make_layout(pl, a->B, a->K, a->tree_capacity);
-  if (ws_bytes < L.total) return fail(pl, PAKR_ERR_WORKSPACE_TOO_SMALL, "workspace smaller than pakr_workspace_bytes()");
+  if (!nn_mode_ok(a->nn_mode)) return fail(pl, PAKR_ERR_INVALID_ARG, "nn_mode must be a PAKR_NN_* value");
+  const Layout L = make_layout(pl, a->B, a->K, a->tree_capacity, a->nn_mode);
+  if (ws_bytes < L.total) return fail(pl, PAKR_ERR_WORKSPACE_TOO_SMALL, "workspace smaller than pakr_workspace_bytes_for() of this nn_mode");
   Params P;
   fill_common(pl, P, L, static_cast<char*>(d_ws), a->B, a->K, a->tree_capacity);
   if (!set_nn_mode(pl, P, a->nn_mode)) return fail(pl, PAKR_ERR_INVALID_ARG, "nn_mode must be a PAKR_NN_* value");
@@ -763,8 +785,8 @@ extern "C" pakr_status pakr_read_stats(pakr_planner* pl, int32_t B, int32_t K, i
                                        size_t ws_bytes, void* cuda_stream, pakr_stats* out) {
   if (!pl) return PAKR_ERR_INVALID_ARG;
   if (!d_ws || !out || !sizes_ok(B, K, cap)) return fail(pl, PAKR_ERR_INVALID_ARG, "null pointer or sizes out of range");
-  const Layout L = make_layout(pl, B, K, cap);
-  if (ws_bytes < L.total) return fail(pl, PAKR_ERR_WORKSPACE_TOO_SMALL, "workspace smaller than pakr_workspace_bytes()");
+  const Layout L = make_layout(pl, B, K, cap, PAKR_NN_SCAN);  // the control block sits at the same offset in every mode
+  if (ws_bytes < L.total) return fail(pl, PAKR_ERR_WORKSPACE_TOO_SMALL, "workspace smaller than pakr_workspace_bytes_for(PAKR_NN_SCAN)");
   cudaStream_t stream = reinterpret_cast<cudaStream_t>(cuda_stream);
   Ctrl* hc = static_cast<Ctrl*>(pl->h_pinned);
   DeviceGuard guard(pl->device);

@@ -145,7 +145,8 @@ class _Fp32Peak(C.Structure):
                 ("mma_f16_mac_per_s", C.c_double), ("mma_f16_minfold_mac_per_s", C.c_double)]
 
 
-EXPORTS = ["pakr_create", "pakr_destroy", "pakr_last_error", "pakr_workspace_bytes", "pakr_get_tree_layout",
+EXPORTS = ["pakr_create", "pakr_destroy", "pakr_last_error", "pakr_workspace_bytes", "pakr_workspace_bytes_for",
+           "pakr_get_tree_layout",
            "pakr_plan", "pakr_expand_step", "pakr_expand_step_static", "pakr_read_stats", "pakr_measure_fp32_peak"]
 
 _lib = None
@@ -164,6 +165,8 @@ def lib():
         L.pakr_last_error.argtypes = [C.c_void_p]
         L.pakr_workspace_bytes.restype = C.c_size_t
         L.pakr_workspace_bytes.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64]
+        L.pakr_workspace_bytes_for.restype = C.c_size_t
+        L.pakr_workspace_bytes_for.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_int32]
         L.pakr_get_tree_layout.restype = C.c_int
         L.pakr_get_tree_layout.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.POINTER(_TreeLayout)]
         L.pakr_plan.restype = C.c_int
@@ -251,6 +254,10 @@ class Planner:
 
     def workspace_bytes(self, B: int, K: int, cap: int) -> int:
         return int(lib().pakr_workspace_bytes(self._h, B, K, cap))
+
+    def workspace_bytes_for(self, B: int, K: int, cap: int, nn_mode: int) -> int:
+        """pakr_workspace_bytes_for: what calls with this nn_mode need (no buffers of tiers the mode cannot launch)."""
+        return int(lib().pakr_workspace_bytes_for(self._h, B, K, cap, nn_mode))
 
     def workspace(self, B: int, K: int, cap: int):
         """A cached torch.uint8 device tensor of at least pakr_workspace_bytes()."""

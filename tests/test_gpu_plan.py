@@ -364,3 +364,37 @@ def test_plan_loop_with_nn_filter_equals_scan(pakr, name, B, K, iters):
     assert trees[pakr.NN_SCAN][2] == 0 and trees[pakr.NN_FILTER][2] > 0
     for k in ("states", "actions", "parents", "costs"):
         np.testing.assert_array_equal(trees[pakr.NN_SCAN][1][k], trees[pakr.NN_FILTER][1][k])
+
+
+def test_workspace_sized_for_the_nn_mode(pakr):
+    """pakr_workspace_bytes_for: a caller that knows its nn_mode does not pay for the other tiers' buffers (C4 under
+    AUTO: no 96 B/node filter rows).  A workspace of exactly that size runs that mode with the same result as the
+    all-tiers workspace; one byte less is refused before anything is launched."""
+    import torch
+    p, cfg = wl.config4()
+    B, K, cap, iters = cfg.B, cfg.K, 1 + 6 * cfg.B * cfg.K, 6
+    pl = pakr.Planner(p)
+    full = pl.workspace_bytes(B, K, cap)
+    need = {m: pl.workspace_bytes_for(B, K, cap, m) for m in (pakr.NN_AUTO, pakr.NN_SCAN, pakr.NN_INDEX, pakr.NN_FILTER)}
+    assert all(0 < v <= full for v in need.values())
+    assert need[pakr.NN_SCAN] < need[pakr.NN_AUTO] == need[pakr.NN_INDEX] < full
+    assert need[pakr.NN_SCAN] < need[pakr.NN_FILTER] < full
+    assert full - need[pakr.NN_AUTO] >= 96 * cap          # the filter rows are not charged to AUTO
+    assert pl.workspace_bytes_for(B, K, cap, 9) == 0
+    ref = pl.plan(2, B, K, cap, 1, max_iters_per_replan=iters, nn_mode=pakr.NN_SCAN)
+    ref_tree = pl.read_tree(B, K, cap, ref["final_tree_nodes"])
+    for mode, nbytes in need.items():
+        ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        res = pl.plan(2, B, K, cap, 1, max_iters_per_replan=iters, nn_mode=mode, workspace=ws)
+        assert res["final_tree_nodes"] == ref["final_tree_nodes"]
+        tree = pl.read_tree(B, K, cap, res["final_tree_nodes"], workspace=ws)
+        np.testing.assert_array_equal(tree["states"], ref_tree["states"])
+        np.testing.assert_array_equal(tree["parents"], ref_tree["parents"])
+        assert pl.read_stats(B, K, cap, workspace=ws)["iterations"] == iters
+        with pytest.raises(pakr.PakrError) as e:
+            pl.plan(2, B, K, cap, 1, max_iters_per_replan=iters, nn_mode=mode, workspace=ws[:nbytes - 1])
+        assert e.value.status == 3
+    # B <= 16 runs the streaming tier in every mode: packed rows, no index or filter buffers
+    small = {m: pl.workspace_bytes_for(8, 4, 100000, m) for m in need}
+    assert len(set(small.values())) == 1 and small[pakr.NN_AUTO] == pl.workspace_bytes(8, 4, 100000)
+    pl.close()
