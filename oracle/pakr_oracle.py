@@ -13,7 +13,13 @@ from typing import Optional
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "libpakr_oracle.so")
+# PAKR_ORACLE_SANITIZE=1: the same source built with AddressSanitizer + UBSan into a library of its own, for running
+# the oracle's pins under a memory / undefined-behaviour checker.  The interpreter is not instrumented, so the ASan
+# runtime has to be preloaded:
+#   LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 PAKR_ORACLE_SANITIZE=1 \
+#       python -m pytest tests -m "not gpu" -k oracle
+_SANITIZE = os.environ.get("PAKR_ORACLE_SANITIZE", "") not in ("", "0")
+_SO = os.path.join(_HERE, "libpakr_oracle_san.so" if _SANITIZE else "libpakr_oracle.so")
 _SRC = [os.path.join(_HERE, "pakr_oracle.cpp"), os.path.join(_HERE, "pakr_oracle.h")]
 
 
@@ -22,7 +28,9 @@ def build(force: bool = False) -> str:
     stale = (not os.path.exists(_SO)) or any(os.path.getmtime(s) > os.path.getmtime(_SO) for s in _SRC)
     if force or stale:
         tmp = _SO + f".{os.getpid()}.tmp"
-        subprocess.check_call(["g++", "-O2", "-std=c++17", "-Wall", "-shared", "-fPIC", "-o", tmp, _SRC[0]])
+        opt = (["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
+               if _SANITIZE else ["-O2"])
+        subprocess.check_call(["g++"] + opt + ["-std=c++17", "-Wall", "-shared", "-fPIC", "-o", tmp, _SRC[0]])
         os.replace(tmp, _SO)
     return _SO
 
