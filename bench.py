@@ -42,7 +42,7 @@ UNIT = "nodes/s"
 C5_POINT = (4096, 16)  # the fixed config-5 point reported beside the headline
 # dram__bytes_read.sum + dram__bytes_write.sum of one pakr_loop_kernel launch on WORKLOAD, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists for the current kernel).
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 51817216  # profiles/r02_ncu_c4_bench.md: 1,700,608 read + 50,116,608 written
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 79737088  # profiles/r03_ncu_c4_bench.md: 1,630,720 read + 78,106,368 written
 NOMINAL_LANES = 148 * 4 * 32  # SMs x schedulers x lanes: issue slots per clock = fp32 FMA lanes per clock
 
 # Arithmetic of one evaluation of f(x, u), counted on the formulas of DESIGN.md "Readings" Q / P33 / P34 with every
@@ -315,7 +315,7 @@ def run_bench(args):
         roof = roofline_of(problem, results, dev_ms, sm_max, measured)
         roof["traffic"] = NCU_TRAFFIC_BYTES_PER_LAUNCH
         roof["traffic_source"] = ("constant: dram read + written bytes of one launch in the ncu --set full capture "
-                                  "profiles/r02_ncu_c4_bench.md, not measured in this run")
+                                  "profiles/r03_ncu_c4_bench.md, not measured in this run")
         roof["kernel"] = f"pakr_loop_kernel ({problem.name})"
         if clocks["sm_mhz"]:
             roof["frac_at_sampled_clock"] = roof["achieved"] / (NOMINAL_LANES * clocks["sm_mhz"] * 1e6 / 1e12)
@@ -338,6 +338,16 @@ def run_bench(args):
             "best_cost_at_100ms_median": statistics.median(best100),
         }
         line.update(summarize(results, dev_ms, wall))
+        # "PAKR without AO-x": one replan, ends at the first solution.  first_solution_ms_host is
+        # SURVEY.md 8(d)'s definition -- host clock from pakr_plan entry to its return (memsets, cooperative launch, the
+        # loop, the result copy) -- beside the device figure, which starts at kernel start.
+        if not args.no_extras:
+            r0, dev0, wall0 = time_plans(torch, pl, cfg, list(range(100, 105)), flush, n_replans=1)
+            line["replan0"] = {"value": sum(r["children"] for r in r0) / (sum(dev0) * 1e-3), "unit": UNIT, "steps": 5,
+                               "ms_per_step": sum(dev0) / 5, "solved": sum(r["outcome"] for r in r0),
+                               "first_solution_ms_device_median": statistics.median(r["first_solution_ms"] for r in r0),
+                               "first_solution_ms_host_median": 1e3 * statistics.median(wall0),
+                               "iterations_per_step": float(np.mean([r["iterations"] for r in r0]))}
         pl.close()
         if not args.no_extras and world == 1:
             line["other_workloads"] = {}
@@ -346,18 +356,29 @@ def run_bench(args):
                 pl2 = pakr.Planner(p2, local)
                 pl2.plan(999, c2.B, c2.K, c2.tree_capacity, c2.n_replans)
                 res2, dev2, wall2 = time_plans(torch, pl2, c2, list(range(3)), flush)
-                row = {"B": c2.B, "K": c2.K, "n_replans": c2.n_replans, "steps": 3,
-                       "value": sum(r["children"] for r in res2) / (sum(dev2) * 1e-3), "unit": UNIT,
-                       "e2e": sum(r["children"] for r in res2) / sum(wall2), "ms_per_step": sum(dev2) / 3}
-                row.update(summarize(res2, dev2, wall2))
+                sm = summarize(res2, dev2, wall2)
                 rf = roofline_of(p2, res2, dev2, sm_max, measured)
-                row["roofline_frac"] = rf["frac"]  # executed lane-ops / peak
-                row["roofline_frac_vs_measured_ffma"] = rf.get("frac_vs_measured_ffma")
-                row["algorithmic_equiv_frac"] = rf["algorithmic_equiv_frac"]
+                # kept short on purpose: the driver records only the tail of this line
+                row = {"B": c2.B, "K": c2.K, "n_replans": c2.n_replans,
+                       "value": sum(r["children"] for r in res2) / (sum(dev2) * 1e-3),
+                       "e2e": sum(r["children"] for r in res2) / sum(wall2), "ms_per_step": sum(dev2) / 3,
+                       "first_solution_ms_median": sm["first_solution_ms_median"], "final_cost_median": sm["final_cost_median"],
+                       "replans_solved_per_step": sm["replans_solved_per_step"],
+                       "roofline_frac": rf["frac"],  # executed lane-ops / peak
+                       "algorithmic_equiv_frac": rf["algorithmic_equiv_frac"]}
                 if not args.no_cpu_baseline:
-                    row["cpu_baseline"] = oracle_baseline(name, 4.0, fanout=False)
+                    row["cpu_value"] = oracle_baseline(name, 4.0, fanout=False)["value"]  # oracle, 1 pinned core, 4 s cap
                 line["other_workloads"]["C5 (B=%d, K=%d)" % C5_POINT if name == "C5" else name] = row
                 pl2.close()
+            # HBM-bound regime of the NN scan: B = 8 queries share one pass over n = 2^23 rows, D = 6
+            p6, _ = wl.config2()
+            pl6 = pakr.Planner(p6, local)
+            n6 = 1 << 23
+            ms6 = measure_phase(torch, pl6, p6, n6, 8, 1, 3, flush, nn_mode=pakr.NN_SCAN)[0]
+            hbm = measured_hbm_gbs()
+            line["stream_tier"] = {"D": 6, "B": 8, "n": n6, "ms": ms6, "algorithmic_GBps": 4 * 6 * n6 / (ms6 * 1e-3) / 1e9,
+                                   "hbm_peak_GBps": hbm, "hbm_frac": 4 * 6 * n6 / (ms6 * 1e-3) / (hbm * 1e9)}
+            pl6.close()
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = oracle_baseline(args.workload, 12.0, fanout=True)
         print(json.dumps(line), flush=True)
@@ -404,17 +425,21 @@ def measure_phase(torch, pl, problem, n, B, K, reps, flush, nn_mode=0):
     return np.median(np.array(out), axis=0)
 
 
+def measured_hbm_gbs() -> float:
+    """Measured HBM copy bandwidth of this pool's B200s (driver-written MEASURED_PEAKS.json), else round 1's figure."""
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
+    except Exception:
+        return 6446.3
+
+
 def run_phases(args):
     import torch
     from paper_2607_03987_b200 import pakr
     pakr.lib()
     peak = NOMINAL_LANES * 1.965e9
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
-    hbm_peak_gbs = 6446.3  # fallback: the copy bandwidth measured on this pool in round 1
-    try:
-        hbm_peak_gbs = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
-    except Exception:
-        pass
+    hbm_peak_gbs = measured_hbm_gbs()
     reps = 3 if args.quick else 7
     nn_points = [("C2", 1 << 16, 1024), ("C2", 1 << 20, 1024), ("C5", 1 << 20, 16384), ("C3", 1 << 20, 2048),
                  ("C4", 1 << 18, 4096), ("C4", 1 << 22, 4096)]
