@@ -11,6 +11,7 @@ planner seed = step index.  metric = expanded nodes/s = children propagated and 
   python bench.py --what peak                 measured FFMA / FFMA2 rates (the ALU roofline's denominators)
   python bench.py --what phases [--only nn|filter|stream|prop] [--quick]   single phases through pakr_expand_step
   python bench.py --what sweep|c5|pathlen [--seeds N]                  BASELINE metrics over seeds, config 5 sweep
+  python bench.py --what oracle-c5            the oracle on config 5's small points: ns per (query, node) pair / child step
 
 With --gpus N > 1 and no RANK in the environment it starts the N ranks itself (torch.distributed.run, one
 planner replica per GPU, NCCL only for the timing harness' scalar reductions).
@@ -169,6 +170,69 @@ def oracle_baseline(name: str, budget_s: float, fanout: bool, seed: int = 0) -> 
                             "unit": UNIT, "sample": f"{len(cores)} pinned single-thread replicas, planner seeds "
                                                     f"{seed + 1}..{seed + len(cores)}, same cap; wall {wall:.1f} s"}
     return out
+
+
+def _oracle_c5_worker(job):
+    """Replan 0 of config 5 at (B, K) driven iteration by iteration, so the (query, node) pairs each NN call really
+    scored are known: -> oracle ns per pair and per child step.  Stops at the first solution or the wall-clock cap."""
+    B, K, seed, budget_s, core = job
+    if core is not None:
+        try:
+            os.sched_setaffinity(0, {core})
+        except OSError:
+            pass
+    from oracle import pakr_oracle as orc
+    problem, cfg = wl.config5(B=B, K=K)
+    op = orc.OracleProblem(problem)
+    tree = orc.OracleTree(op, cfg.tree_capacity)
+    tree.reset()
+    pairs = children = it = 0
+    ph = [0.0, 0.0, 0.0]
+    solved = False
+    t0 = time.perf_counter()
+    while time.perf_counter() - t0 < budget_s and tree.n < cfg.tree_capacity:
+        pairs += B * tree.n
+        out = orc.expand_iteration(op, tree, seed, 0, it, B, K)
+        children += B * K
+        it += 1
+        for i in range(3):
+            ph[i] += out["phase_ms"][i]
+        if out["goal"]:
+            solved = True
+            break
+    return dict(B=B, K=K, seed=seed, seconds=time.perf_counter() - t0, iterations=it, nodes=tree.n, solved=solved,
+                pairs=pairs, children=children, nn_ms=ph[0], prop_ms=ph[1], insert_ms=ph[2],
+                steps_per_edge=problem.steps_per_edge, D=problem.state_dim)
+
+
+def run_oracle_c5(args):
+    """--what oracle-c5: SURVEY.md 8(d) / BASELINE.md's CPU plan for config 5 -- the oracle as it stands on B in {256,
+    1024} x K in {1, 4}, 3 planner seeds, one pinned core, with its cost per (query, node) pair and per child step, so
+    the figures for C4 / the large C5 points are stated extrapolations instead of implied ones."""
+    from oracle import pakr_oracle as orc
+    orc.build()
+    core = sorted(os.sched_getaffinity(0))[0]
+    ctx = mp.get_context("spawn")
+    rows = []
+    with ctx.Pool(1) as pool:
+        for B in (256, 1024):
+            for K in (1, 4):
+                for seed in range(3):
+                    r = pool.map(_oracle_c5_worker, [(B, K, seed, 10.0, core)])[0]
+                    r["ns_per_pair"] = 1e6 * r["nn_ms"] / max(1, r["pairs"])
+                    r["ns_per_child_step"] = 1e6 * r["prop_ms"] / max(1, r["children"] * r["steps_per_edge"])
+                    r["nodes_per_s"] = r["children"] / r["seconds"]
+                    rows.append(r)
+                    print(json.dumps({"what": "oracle-c5", **r}), flush=True)
+    pp = statistics.median(r["ns_per_pair"] for r in rows if r["pairs"] > 1e6)
+    pc = statistics.median(r["ns_per_child_step"] for r in rows)
+    # extrapolation to the headline: per-plan totals of C4 from the GPU's own counters are not available here, so the
+    # statement is per unit: a (query, node) pair of D = 6 costs pp ns, a child step pc ns; C4 (D = 12, RK4) scales the
+    # pair cost by ~2 and is measured directly by the cpu_baseline leg.
+    print(json.dumps({"what": "oracle-c5-summary", "median_ns_per_pair_D6": pp, "median_ns_per_child_step": pc,
+                      "cores": 1, "cap_s_per_run": 10.0, "runs": len(rows),
+                      "example": "C5 B=4096 K=16 iteration on a 100 k-node tree = 4.1e8 pairs -> %.1f s of NN alone" % (4.096e8 * pp * 1e-9)}),
+          flush=True)
 
 
 def run_reference(args):
@@ -600,7 +664,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--what", default="bench", choices=["bench", "peak", "phases", "sweep", "c5", "pathlen"])
+    ap.add_argument("--what", default="bench", choices=["bench", "peak", "phases", "sweep", "c5", "pathlen", "oracle-c5"])
     ap.add_argument("--workload", default=WORKLOAD, choices=["C1", "C2", "C3", "C4", "C5"],
                     help="headline workload of --what bench (default: the largest single-GPU config)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -611,6 +675,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.what == "oracle-c5":
+        return run_oracle_c5(args)
     if args.what == "peak":
         return run_peak(args)
     if args.what == "phases":

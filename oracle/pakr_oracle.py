@@ -266,7 +266,7 @@ def expand_iteration(op: OracleProblem, tree: OracleTree, seed: int, r: int, it:
     goal = lib().orc_expand_iteration(op.ref, tree.ref, C.c_uint64(seed), C.c_uint32(r), C.c_uint32(it),
                                       C.c_int32(B), C.c_int32(K), C.c_double(c_best), C.byref(dbg))
     out.update(goal=bool(goal), n_inserted=int(dbg.n_inserted), goal_node=int(dbg.goal_node),
-               new_c_best=float(dbg.new_c_best))
+               new_c_best=float(dbg.new_c_best), phase_ms=[float(v) for v in dbg.phase_ms])  # NN / propagate / insert
     return out
 
 
