@@ -35,7 +35,7 @@ sys.path.insert(0, ROOT)
 
 import numpy as np  # noqa: E402
 
-from paper_2607_03987_b200 import replicas, workloads as wl  # noqa: E402
+from paper_2607_03987_b200 import peak, replicas, workloads as wl  # noqa: E402
 
 WORKLOAD = "C4"
 METRIC = "expanded nodes/s"
@@ -375,7 +375,7 @@ def run_bench(args):
 
     if rank == 0:
         sm_max = clocks["sm_max_mhz"] or 1965.0
-        measured = pakr.measure_fp32_peak(local)
+        measured = peak.measure_fp32_peak(local)
         roof = roofline_of(problem, results, dev_ms, sm_max, measured)
         roof["traffic"] = NCU_TRAFFIC_BYTES_PER_LAUNCH
         roof["traffic_source"] = ("constant: dram read + written bytes of one launch in the ncu --set full capture "
@@ -455,7 +455,7 @@ def run_bench(args):
 def run_peak(args):
     """Measured fp32 peaks: the denominators beside the nominal one in `roofline`."""
     from paper_2607_03987_b200 import pakr
-    m = pakr.measure_fp32_peak(0)
+    m = peak.measure_fp32_peak(0)
     nominal = NOMINAL_LANES * m["sm_clock_mhz"] * 1e6
     print(json.dumps({"what": "peak", "nominal_lane_ops_per_s": nominal, **m,
                       "ffma_frac_of_nominal": m["ffma_lane_ops_per_s"] / nominal,

@@ -6,11 +6,12 @@
 //   FADD2 + FFMA2   the scan's own mix: one packed subtract per packed fma
 //   HMMA            mma.sync.m16n8k16 f16 x f16 -> f32, the tensor-core NN filter's instruction (pakr_nn_filter.cuh),
 //                   alone (accumulating) and with the filter's epilogue: fresh accumulators folded into running minima
-// A lane-op is one fp32 add, multiply or fused multiply-add on one lane.  Not on the planning path.
+// A lane-op is one fp32 add, multiply or fused multiply-add on one lane.  Not on the planning path and not in libpakr.so:
+// this file is libpakr_peak.so, loaded by bench.py alone (paper_2607_03987_b200/peak.py).
 #include <algorithm>
 #include <cuda_runtime.h>
 
-#include "../../include/pakr.h"
+#include "pakr_peak.h"
 
 namespace {
 
@@ -125,8 +126,8 @@ cudaError_t time_kernel(K kernel, int sms, float* out, int reps, double lane_ops
 
 }  // namespace
 
-extern "C" pakr_status pakr_measure_fp32_peak(int cuda_device, pakr_fp32_peak* out) {
-  if (!out) return PAKR_ERR_INVALID_ARG;
+extern "C" int pakr_measure_fp32_peak(int cuda_device, pakr_fp32_peak* out) {
+  if (!out) return 1;
   int prev = -1;
   if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
   cudaError_t e = cudaSetDevice(cuda_device);
@@ -150,5 +151,5 @@ extern "C" pakr_status pakr_measure_fp32_peak(int cuda_device, pakr_fp32_peak* o
   }
   if (buf) cudaFree(buf);
   if (prev >= 0) cudaSetDevice(prev);
-  return e == cudaSuccess ? PAKR_OK : PAKR_ERR_CUDA;
+  return e == cudaSuccess ? 0 : 5;
 }

@@ -16,8 +16,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "libpakr.so")
 _CSRC = os.path.join(_HERE, "csrc")
-_SOURCES = ["pakr_api.cu", "pakr_kernel_inst.cu", "pakr_peak.cu", "pakr_kernel.cuh", "pakr_device.cuh",
-            "pakr_nn_filter.cuh"]
+_SOURCES = ["pakr_api.cu", "pakr_kernel_inst.cu", "pakr_kernel.cuh", "pakr_device.cuh", "pakr_nn_filter.cuh"]
 
 F_VALID, F_INBOUNDS, F_COLLFREE, F_NOTPRUNED, F_GOAL, F_INSERTED = 1, 2, 4, 8, 16, 32
 NN_AUTO, NN_SCAN, NN_INDEX, NN_FILTER = 0, 1, 2, 3
@@ -37,7 +36,8 @@ class PakrError(RuntimeError):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """nvcc -gencode arch=compute_100a,code=sm_100a -> paper_2607_03987_b200/libpakr.so (in-tree).
-    Ten translation units (host API; peak microbenchmark; kernels per NN tier and model group) compile in parallel."""
+    Nine translation units (host API; kernels per NN tier and model group) compile in parallel.  The roofline
+    microbenchmark is a library of its own (peak.py)."""
     srcs = [os.path.join(_CSRC, s) for s in _SOURCES] + [os.path.join(_HERE, "..", "include", "pakr.h")]
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     flags = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
@@ -53,7 +53,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             stale = True
     if force or stale:
         tag = f".{os.getpid()}.tmp"
-        units = [("pakr_api.cu", [], "api"), ("pakr_peak.cu", [], "peak")]
+        units = [("pakr_api.cu", [], "api")]
         for tier, part in ((0, 0), (0, 1), (1, 0), (1, 1), (2, 0), (2, 1), (3, 0), (3, 1)):
             units.append(("pakr_kernel_inst.cu", [f"-DPAKR_STREAM_TIER={tier}", f"-DPAKR_PART={part}"], f"t{tier}p{part}"))
         objs, procs = [], []
@@ -139,15 +139,9 @@ class _StepArgs(C.Structure):
                 ("n_inserted", C.c_void_p), ("goal_node", C.c_void_p), ("new_c_best", C.c_void_p)]
 
 
-class _Fp32Peak(C.Structure):
-    _fields_ = [("ffma_lane_ops_per_s", C.c_double), ("ffma2_lane_ops_per_s", C.c_double),
-                ("scan_mix_lane_ops_per_s", C.c_double), ("sm_clock_mhz", C.c_double), ("sm_count", C.c_int32),
-                ("mma_f16_mac_per_s", C.c_double), ("mma_f16_minfold_mac_per_s", C.c_double)]
-
-
 EXPORTS = ["pakr_create", "pakr_destroy", "pakr_last_error", "pakr_workspace_bytes", "pakr_workspace_bytes_for",
            "pakr_get_tree_layout",
-           "pakr_plan", "pakr_expand_step", "pakr_expand_step_static", "pakr_read_stats", "pakr_measure_fp32_peak"]
+           "pakr_plan", "pakr_expand_step", "pakr_expand_step_static", "pakr_read_stats"]
 
 _lib = None
 
@@ -179,19 +173,8 @@ def lib():
         L.pakr_read_stats.restype = C.c_int
         L.pakr_read_stats.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.c_size_t, C.c_void_p,
                                       C.POINTER(_Stats)]
-        L.pakr_measure_fp32_peak.restype = C.c_int
-        L.pakr_measure_fp32_peak.argtypes = [C.c_int, C.POINTER(_Fp32Peak)]
         _lib = L
     return _lib
-
-
-def measure_fp32_peak(device: int = 0) -> dict:
-    """pakr_measure_fp32_peak: sustained FFMA / FFMA2 / scan-mix lane-ops per second of the device."""
-    out = _Fp32Peak()
-    st = lib().pakr_measure_fp32_peak(device, C.byref(out))
-    if st != 0:
-        raise PakrError(st, "pakr_measure_fp32_peak failed")
-    return {k: getattr(out, k) for k, _ in _Fp32Peak._fields_}
 
 
 def _f32(a) -> np.ndarray:

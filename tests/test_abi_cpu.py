@@ -28,6 +28,14 @@ def test_library_exports_every_declared_symbol():
         assert hasattr(L, n), n
 
 
+def test_measurement_support_is_a_library_of_its_own():
+    """The roofline microbenchmark is not part of the product ABI: libpakr.so does not export it, libpakr_peak.so does."""
+    from paper_2607_03987_b200 import pakr, peak
+    assert not hasattr(ctypes.CDLL(pakr.build()), "pakr_measure_fp32_peak")
+    assert hasattr(ctypes.CDLL(peak.build()), "pakr_measure_fp32_peak")
+    assert "pakr_measure_fp32_peak" not in open(os.path.join(ROOT, "include", "pakr.h")).read()
+
+
 def test_sass_is_sm100a_with_tma():
     """The built library carries sm_100a SASS and the NN scan's bulk copies are TMA (UBLKCP)."""
     from paper_2607_03987_b200 import pakr
@@ -39,8 +47,7 @@ def test_sass_is_sm100a_with_tma():
 
 
 _STRUCTS = {"pakr_problem": "_Problem", "pakr_tree_layout": "_TreeLayout", "pakr_plan_opts": "_PlanOpts",
-            "pakr_stats": "_Stats", "pakr_result": "_Result", "pakr_step_args": "_StepArgs",
-            "pakr_fp32_peak": "_Fp32Peak"}
+            "pakr_stats": "_Stats", "pakr_result": "_Result", "pakr_step_args": "_StepArgs"}
 
 
 def _header_fields(name):
